@@ -1,0 +1,209 @@
+/*
+ * gradsim.h -- C ABI of the B200-native gradSim hot path: the differentiable multiphysics
+ * substep (tet Neo-Hookean FEM + triangle membrane + dihedral bending -> scatter-add ->
+ * penalty ground contact with friction -> semi-implicit Euler) and its hand-written adjoint,
+ * with an on-device state tape for backpropagation through time.
+ *
+ * Paper: arXiv 2104.02646 (gradSim).  Citations are "PAPER.md:<line>" = the paper's LaTeX as
+ * mounted at build time, plus the section; "DESIGN.md Ax" = a documented reading where the
+ * paper is silent.
+ *
+ * Conventions (all entry points)
+ *  - Every function returns an int status (GS_OK = 0, negative = error); nothing throws or exits.
+ *    gs_last_error() gives a thread-local message for the last failure.
+ *  - "HOST" pointers are plain host memory, read during the call only (caller may free after).
+ *    "DEVICE" pointers are CUDA device memory owned by the caller (e.g. a torch tensor's
+ *    data_ptr()); the library never allocates or frees device memory: it works inside the
+ *    workspace / tape blocks the caller hands over, which must outlive the model / tape and be
+ *    256-byte aligned.
+ *  - All device work is enqueued on the caller's stream (a cudaStream_t passed as void*) and is
+ *    asynchronous; only gs_model_create, gs_tape_create, gs_check_finite and the *_host entry
+ *    points synchronise.  One model is used from one stream at a time.
+ *  - State arrays crossing the ABI are fp32, CALLER'S particle order, [E][N][3] (env-major).
+ *    Per-element / per-particle parameter and gradient arrays are [E][count], caller's element order.
+ *    Internally particles and elements are reordered (Morton) and tiled; the permutation is applied
+ *    on the way in and out, off the hot path (a rollout stays in the internal order).
+ *  - Arithmetic is fp32 (parameter gradients are accumulated across substeps in fp64).
+ */
+#ifndef GRADSIM_H
+#define GRADSIM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gs_model gs_model; /* opaque: one scene (mesh shared by all E environments) */
+typedef struct gs_tape gs_tape;   /* opaque: on-device state tape of one rollout            */
+typedef void *gs_stream;          /* cudaStream_t                                           */
+
+enum gs_status {
+    GS_OK = 0,
+    GS_EINVAL = -1,     /* bad argument (null pointer, negative size, misaligned / too small block) */
+    GS_EMESH = -2,      /* invalid mesh: index out of range, V_e <= 0, degenerate triangle / hinge   */
+    GS_ENOMEM = -3,     /* host allocation failed                                                    */
+    GS_ECUDA = -4,      /* a CUDA runtime call failed (message has the CUDA error string)            */
+    GS_ENONFINITE = -5, /* a non-finite state was produced; see gs_check_finite                      */
+    GS_ESTATE = -6      /* call order violated (e.g. backward on a tape that holds no rollout)       */
+};
+
+/* parameter groups of gs_set_params / gs_param_grads (Table 5: the optimisable
+   parameters this path carries: Lame parameters and damping per element, mass per particle) */
+enum gs_param_group {
+    GS_TET_MU = 0, GS_TET_LAMBDA = 1, GS_TET_DAMP = 2,
+    GS_TRI_MU = 3, GS_TRI_LAMBDA = 4, GS_TRI_DAMP = 5,
+    GS_MASS = 6,
+    GS_NUM_GROUPS = 7
+};
+
+/* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */
+enum gs_param_layout {
+    GS_ELEM_PER_ENV = 1,    /* tet_* and tri_* arrays are [E][M] / [E][Mt]; else [M] / [Mt] broadcast */
+    GS_MASS_PER_ENV = 2,    /* mass is [E][N]; else [N] broadcast                                       */
+    GS_CONTACT_PER_ENV = 4  /* ke, kd, kf, mu_c are [E]; else [1] broadcast                             */
+};
+
+/* execution plans (gs_model_desc.plan) */
+enum gs_plan {
+    GS_PLAN_AUTO = 0,     /* resident when the mesh fits one CTA's shared memory, else streaming         */
+    GS_PLAN_STREAMING = 1,/* two grid-wide kernels per substep over Morton-ordered element tiles          */
+    GS_PLAN_RESIDENT = 2  /* one persistent CTA per environment, state in shared memory across substeps   */
+};
+
+/*
+ * Scene description.  All pointers HOST; copied during gs_model_create.
+ *   x_rest defines the rest shape: tets  B = D_m^-1, V = det(D_m)/6       (App. A.1)
+ *                                  tris  2x2 B in the triangle's rest frame, A = det(D_m)/2 (A4)
+ *                                  hinges rest angle theta0 and rest edge length l0        (A5, A6)
+ *   tets must be positively oriented (det D_m > 0), else GS_EMESH.
+ *   hinges[h] = (wing1, wing2, edge_a, edge_b): the two vertices opposite the shared edge, then the edge.
+ *   pinned[i] != 0 => inverse mass 0 (step(inv_mass)).
+ *   Contact: plane n.x = d, threshold particle_radius, stiffness ke, damping kd,
+ *   friction stiffness kf, friction coefficient mu_c (A7-A9).
+ */
+typedef struct {
+    int32_t n_particles, n_tets, n_tris, n_hinges, n_envs;
+    const float *x_rest;   /* [N][3] */
+    const float *mass;     /* [E][N] or [N], > 0 */
+    const uint8_t *pinned; /* [N] or NULL */
+    const int32_t *tets;   /* [M][4] */
+    const float *tet_mu, *tet_lambda, *tet_damp;
+    const int32_t *tris;   /* [Mt][3] */
+    const float *tri_mu, *tri_lambda, *tri_damp;
+    const int32_t *hinges; /* [Mh][4] */
+    const float *hinge_kb; /* [Mh] bending stiffness (units of force, A6) */
+    uint32_t param_layout; /* gs_param_layout flags */
+    float gravity[3];      /* acceleration added to every non-pinned particle (A10), e.g. (0,-9.8,0) */
+    float dt;              /* substep */
+    float plane_n[3];      /* unit normal */
+    float plane_d;
+    float particle_radius;
+    const float *ke, *kd, *kf, *mu_c; /* [E] or [1] */
+    int32_t plan;          /* gs_plan */
+} gs_model_desc;
+
+/* Upper bound of the device workspace a model of this description needs (bytes).  0 on a bad desc. */
+size_t gs_model_workspace_bytes(const gs_model_desc *desc);
+
+/* Validates the mesh, computes rest quantities, reorders and tiles it, uploads everything into
+   d_workspace (DEVICE, >= gs_model_workspace_bytes, 256-byte aligned).  Synchronises the stream.
+   Errors: GS_EINVAL, GS_EMESH (message names the element), GS_ENOMEM, GS_ECUDA. */
+int gs_model_create(const gs_model_desc *desc, void *d_workspace, size_t bytes, gs_stream stream, gs_model **out);
+void gs_model_destroy(gs_model *m);
+
+/* Which plan the model runs (gs_plan value), and basic sizes. */
+int gs_model_plan(const gs_model *m);
+int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, int32_t *n_envs);
+
+/* Replace one parameter group from DEVICE values [E][count] in caller order (count = M, Mt or N). */
+int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream stream);
+
+/*
+ * One forward substep (PAPER.md:618-619 semi-implicit Euler; 763-764 Listing 1):
+ *   f = tets + triangles + hinges + contact, all at the start-of-step state;
+ *   v+ = v + (f w + g [w>0]) dt;  x+ = x + v+ dt.
+ * d_x, d_v: DEVICE [E][N][3] in; d_x_out, d_v_out: DEVICE [E][N][3] out (may alias the inputs).
+ */
+int gs_step_forward(gs_model *m, const float *d_x, const float *d_v, float *d_x_out, float *d_v_out, gs_stream stream);
+
+/*
+ * Adjoint of one substep (PAPER.md:561-563 implicit-function adjoint; 622-631 Jacobians of g, solved
+ * explicitly thanks to their triangular structure).  d_x, d_v: state BEFORE the step.  d_adj_x_out,
+ * d_adj_v_out: dL/d(state after).  Writes dL/d(state before) to d_adj_x_in, d_adj_v_in (may alias the
+ * cotangent inputs).  Parameter gradients ACCUMULATE in the model until gs_zero_grads.
+ */
+int gs_step_backward(gs_model *m, const float *d_x, const float *d_v, const float *d_adj_x_out, const float *d_adj_v_out,
+                     float *d_adj_x_in, float *d_adj_v_in, gs_stream stream);
+
+/*
+ * State tape (reverse mode must store the input state of every step).
+ * checkpoint_every = 1 keeps every substep; K > 1 keeps states 0, K, 2K, ... and the final state, and
+ * the backward pass regenerates each segment by forward replay (BASELINE.json configs[2]).
+ * d_mem: DEVICE block of >= gs_tape_bytes, 256-byte aligned.
+ */
+size_t gs_tape_bytes(const gs_model *m, int n_substeps, int checkpoint_every);
+int gs_tape_create(gs_model *m, int n_substeps, int checkpoint_every, void *d_mem, size_t bytes, gs_tape **out);
+void gs_tape_destroy(gs_tape *t);
+
+/* Forward rollout of the tape's n_substeps from (d_x0, d_v0) [E][N][3]; optional final state out (may be NULL). */
+int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const float *d_v0, float *d_x_T, float *d_v_T, gs_stream stream);
+
+/* Copy the stored state after `substep` substeps to caller order.  GS_ESTATE if the tape does not hold
+   that substep (checkpointed tapes hold multiples of K and the final state).  Either output may be NULL. */
+int gs_tape_read(gs_model *m, gs_tape *t, int substep, float *d_x, float *d_v, gs_stream stream);
+
+/*
+ * Backward through the tape's rollout.  Loss cotangents enter at frame boundaries: frame k (0-based) is
+ * the state after (k+1)*frame_stride substeps, d_adj_x_frames is DEVICE [n_frames][E][N][3] (NULL / 0 for
+ * none); d_adj_x_T, d_adj_v_T are the cotangents of the final state (NULL = zero).  Outputs dL/dx0,
+ * dL/dv0 (either may be NULL).  Parameter gradients accumulate in the model.
+ */
+int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames,
+                        const float *d_adj_x_T, const float *d_adj_v_T, float *d_adj_x0, float *d_adj_v0, gs_stream stream);
+
+int gs_zero_grads(gs_model *m, gs_stream stream);
+/* Accumulated dL/d(parameter) of one group, DEVICE out [E][count] fp32 in caller order.  For GS_MASS the
+   gradient of a pinned particle is 0 (A11). */
+int gs_param_grads(gs_model *m, int group, float *d_out, gs_stream stream);
+
+/* Synchronises the stream; *first_bad_substep = index of the first substep (since the last rollout /
+   step call began) that produced a non-finite position or velocity, or -1.  Returns GS_ENONFINITE if any. */
+int gs_check_finite(gs_model *m, gs_stream stream, int *first_bad_substep);
+
+/*
+ * Loss helpers on caller-order DEVICE arrays, so that a whole optimisation iteration can stay on the
+ * device (centre-of-mass based loss; BASELINE.json configs).
+ *   gs_loss_centroid: L_e (+)= scale * || mean_i x_i - target_e ||^2 ; adj_x_i = 2 scale (c - c*) / N
+ *   gs_loss_pos:      L_e (+)= scale * sum_i || x_i - ref_i ||^2     ; adj_x_i = 2 scale (x_i - ref_i)
+ * d_x [E][N][3], d_target [E][3], d_ref [E][N][3], d_loss [E] (overwritten unless accumulate != 0),
+ * d_adj_x [E][N][3] overwritten (may be NULL).
+ */
+int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, const float *d_target, float scale, int accumulate,
+                     float *d_loss, float *d_adj_x, gs_stream stream);
+int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate,
+                float *d_loss, float *d_adj_x, gs_stream stream);
+
+/*
+ * End-to-end convenience with HOST buffers (used by bench.py's e2e leg): uploads x0, v0 [E][N][3] and
+ * the final-centroid targets [E][3], runs gs_rollout, the loss L_e = ||c(x_T) - target_e||^2,
+ * gs_rollout_backward, and downloads loss [E], dL/dx0, dL/dv0 [E][N][3] (either may be NULL) and the
+ * parameter gradients listed in groups[] into h_grads[k] ([E][count] each).  d_scratch: DEVICE block of
+ * >= gs_host_scratch_bytes.  Zeroes the model's gradients first.  Synchronises.
+ */
+size_t gs_host_scratch_bytes(const gs_model *m);
+int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, const float *h_target,
+                                  float *h_loss, float *h_adj_x0, float *h_adj_v0, int n_groups, const int *groups,
+                                  float *const *h_grads, void *d_scratch, size_t scratch_bytes, gs_stream stream);
+
+/* Number of kernel launches the library has enqueued since the process started (bench.py's gpu_launches). */
+uint64_t gs_launch_count(void);
+
+const char *gs_last_error(void);
+const char *gs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRADSIM_H */

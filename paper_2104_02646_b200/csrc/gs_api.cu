@@ -1,0 +1,354 @@
+// gs_api.cu -- extern "C" entry points of include/gradsim.h: argument checks, tape bookkeeping, rollout /
+// backward drivers (streaming or resident plan), loss helpers, host-buffer end-to-end call.
+#include <climits>
+#include <cstring>
+#include <new>
+
+#include "gs_internal.h"
+
+using namespace gs;
+
+namespace gs {
+const char *last_error();
+}
+
+#define GS_REQUIRE(cond, code, ...)      \
+    do {                                 \
+        if (!(cond)) {                   \
+            set_error(__VA_ARGS__);      \
+            return code;                 \
+        }                                \
+    } while (0)
+#define GS_TRY(expr)                     \
+    do {                                 \
+        int rc_ = (expr);                \
+        if (rc_ != GS_OK) return rc_;    \
+    } while (0)
+#define GS_CUDA(expr, what)                                   \
+    do {                                                      \
+        cudaError_t e_ = (expr);                              \
+        if (e_ != cudaSuccess) return cuda_fail(e_, what);    \
+    } while (0)
+
+static int check_desc(const gs_model_desc *d) {
+    GS_REQUIRE(d, GS_EINVAL, "desc is null");
+    GS_REQUIRE(d->n_particles > 0 && d->n_envs > 0, GS_EINVAL, "n_particles and n_envs must be > 0");
+    GS_REQUIRE(d->n_tets >= 0 && d->n_tris >= 0 && d->n_hinges >= 0, GS_EINVAL, "negative element count");
+    GS_REQUIRE(d->x_rest && d->mass, GS_EINVAL, "x_rest and mass are required");
+    GS_REQUIRE(d->n_tets == 0 || (d->tets && d->tet_mu && d->tet_lambda && d->tet_damp), GS_EINVAL, "tet arrays missing");
+    GS_REQUIRE(d->n_tris == 0 || (d->tris && d->tri_mu && d->tri_lambda && d->tri_damp), GS_EINVAL, "triangle arrays missing");
+    GS_REQUIRE(d->n_hinges == 0 || (d->hinges && d->hinge_kb), GS_EINVAL, "hinge arrays missing");
+    GS_REQUIRE(d->ke && d->kd && d->kf && d->mu_c, GS_EINVAL, "contact parameters missing");
+    GS_REQUIRE(d->dt > 0.0f, GS_EINVAL, "dt must be > 0");
+    GS_REQUIRE(d->plan >= GS_PLAN_AUTO && d->plan <= GS_PLAN_RESIDENT, GS_EINVAL, "unknown plan %d", d->plan);
+    GS_REQUIRE((size_t)d->n_particles * (size_t)d->n_envs < ((size_t)1 << 31), GS_EINVAL, "E*N must be < 2^31");
+    return GS_OK;
+}
+
+extern "C" size_t gs_model_workspace_bytes(const gs_model_desc *d) {
+    if (check_desc(d) != GS_OK) return 0;
+    const int counts[N_TYPES] = {d->n_tets, d->n_tris, d->n_hinges};
+    return workspace_bytes_upper(d->n_particles, d->n_envs, counts) + resident_blob_bytes(d);
+}
+
+extern "C" int gs_model_create(const gs_model_desc *d, void *d_workspace, size_t bytes, gs_stream stream, gs_model **out) {
+    GS_REQUIRE(out, GS_EINVAL, "out is null");
+    *out = nullptr;
+    GS_TRY(check_desc(d));
+    GS_REQUIRE(d_workspace, GS_EINVAL, "workspace is null");
+    gs_model *m = new (std::nothrow) gs_model();
+    GS_REQUIRE(m, GS_ENOMEM, "out of host memory");
+    int rc = GS_OK;
+    try {
+        rc = build_model(d, d_workspace, bytes, (cudaStream_t)stream, m);
+        if (rc == GS_OK) rc = configure_stream_kernels(m);
+        if (rc == GS_OK) rc = resident_prepare(m, d, d_workspace, bytes, (cudaStream_t)stream);
+    } catch (const std::bad_alloc &) {
+        set_error("out of host memory while planning the model");
+        rc = GS_ENOMEM;
+    }
+    if (rc != GS_OK) { delete m; return rc; }
+    *out = m;
+    return GS_OK;
+}
+
+extern "C" void gs_model_destroy(gs_model *m) { delete m; }
+extern "C" int gs_model_plan(const gs_model *m) { return m ? m->plan : GS_EINVAL; }
+extern "C" int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, int32_t *n_envs) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    if (n_particles) *n_particles = m->N;
+    if (n_elements) *n_elements = m->counts[0] + m->counts[1] + m->counts[2];
+    if (n_envs) *n_envs = m->E;
+    return GS_OK;
+}
+
+extern "C" int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream stream) {
+    GS_REQUIRE(m && d_values, GS_EINVAL, "null argument");
+    GS_REQUIRE(group >= 0 && group < GS_NUM_GROUPS, GS_EINVAL, "unknown parameter group %d", group);
+    return launch_set_params(m, group, d_values, (cudaStream_t)stream);
+}
+
+static int reset_bad(gs_model *m, cudaStream_t st) {
+    GS_CUDA(cudaMemsetAsync(m->dev.bad, 0x7f, sizeof(int), st), "reset non-finite flag");
+    return GS_OK;
+}
+
+extern "C" int gs_step_forward(gs_model *m, const float *d_x, const float *d_v, float *d_x_out, float *d_v_out, gs_stream stream) {
+    GS_REQUIRE(m && d_x && d_v && d_x_out && d_v_out, GS_EINVAL, "null argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    GS_TRY(reset_bad(m, st));
+    GS_TRY(launch_pack(m, d_x, d_v, m->d_xs[0], m->d_vs[0], true, st));
+    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], 0, st));
+    return launch_unpack(m, m->d_xs[1], m->d_vs[1], d_x_out, d_v_out, st);
+}
+
+extern "C" int gs_step_backward(gs_model *m, const float *d_x, const float *d_v, const float *d_adj_x_out, const float *d_adj_v_out,
+                                float *d_adj_x_in, float *d_adj_v_in, gs_stream stream) {
+    GS_REQUIRE(m && d_x && d_v && d_adj_x_out && d_adj_v_out && d_adj_x_in && d_adj_v_in, GS_EINVAL, "null argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    GS_TRY(reset_bad(m, st));
+    GS_TRY(launch_pack(m, d_x, d_v, m->d_xs[0], m->d_vs[0], true, st));
+    // the end-of-step velocity enters the mass gradient: recompute the forward step
+    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], 0, st));
+    GS_TRY(launch_pack(m, d_adj_x_out, d_adj_v_out, m->d_adjx, m->d_adjv, false, st));
+    GS_TRY(stream_step_adjoint(m, m->d_xs[0], m->d_vs[0], m->d_vs[1], nullptr, st));
+    return launch_unpack(m, m->d_adjx, m->d_adjv, d_adj_x_in, d_adj_v_in, st);
+}
+
+// ------------------------------------------------------------------------------------------ tape
+static int tape_slots(int T, int K) {
+    if (K == 1) return T + 1;
+    const int n_ck = (T + K - 1) / K;
+    return n_ck + 1 + (K - 1 > 2 ? K - 1 : 2);
+}
+
+extern "C" size_t gs_tape_bytes(const gs_model *m, int n_substeps, int checkpoint_every) {
+    if (!m || n_substeps < 1 || checkpoint_every < 1) return 0;
+    const int K = checkpoint_every > n_substeps ? n_substeps : checkpoint_every;
+    return (size_t)tape_slots(n_substeps, K) * 2 * (size_t)m->E * m->N * sizeof(float4) + 256;
+}
+
+extern "C" int gs_tape_create(gs_model *m, int n_substeps, int checkpoint_every, void *d_mem, size_t bytes, gs_tape **out) {
+    GS_REQUIRE(out, GS_EINVAL, "out is null");
+    *out = nullptr;
+    GS_REQUIRE(m && d_mem, GS_EINVAL, "null argument");
+    GS_REQUIRE(n_substeps >= 1 && checkpoint_every >= 1, GS_EINVAL, "n_substeps and checkpoint_every must be >= 1");
+    GS_REQUIRE(((uintptr_t)d_mem & 255) == 0, GS_EINVAL, "tape memory must be 256-byte aligned");
+    GS_REQUIRE(bytes >= gs_tape_bytes(m, n_substeps, checkpoint_every), GS_EINVAL, "tape memory too small: %zu < %zu", bytes,
+               gs_tape_bytes(m, n_substeps, checkpoint_every));
+    gs_tape *t = new (std::nothrow) gs_tape();
+    GS_REQUIRE(t, GS_ENOMEM, "out of host memory");
+    t->m = m; t->T = n_substeps;
+    t->K = checkpoint_every > n_substeps ? n_substeps : checkpoint_every;
+    if (m->plan == GS_PLAN_RESIDENT && t->K != 1) {
+        // the resident plan keeps the full tape (a full tape of a mesh that fits one CTA is small)
+        delete t;
+        set_error("the resident plan supports checkpoint_every = 1 only; create the model with GS_PLAN_STREAMING for checkpointing");
+        return GS_EINVAL;
+    }
+    t->n_ck = (t->T + t->K - 1) / t->K;
+    t->S = (size_t)m->E * m->N;
+    t->base = (float4 *)d_mem;
+    *out = t;
+    return GS_OK;
+}
+extern "C" void gs_tape_destroy(gs_tape *t) { delete t; }
+
+extern "C" int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const float *d_v0, float *d_x_T, float *d_v_T, gs_stream stream) {
+    GS_REQUIRE(m && t && d_x0 && d_v0, GS_EINVAL, "null argument");
+    GS_REQUIRE(t->m == m, GS_EINVAL, "tape belongs to another model");
+    cudaStream_t st = (cudaStream_t)stream;
+    GS_TRY(reset_bad(m, st));
+    GS_TRY(launch_pack(m, d_x0, d_v0, t->slot_x(t->slot_fwd(0)), t->slot_v(t->slot_fwd(0)), true, st));
+    if (m->plan == GS_PLAN_RESIDENT) {
+        GS_TRY(resident_rollout(m, t, st));
+    } else {
+        for (int s = 0; s < t->T; s++) {
+            const int a = t->slot_fwd(s), b = t->slot_fwd(s + 1);
+            GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, st));
+        }
+    }
+    t->has_rollout = true;
+    return launch_unpack(m, t->slot_x(t->slot_final()), t->slot_v(t->slot_final()), d_x_T, d_v_T, st);
+}
+
+extern "C" int gs_tape_read(gs_model *m, gs_tape *t, int substep, float *d_x, float *d_v, gs_stream stream) {
+    GS_REQUIRE(m && t && t->m == m, GS_EINVAL, "bad model / tape");
+    GS_REQUIRE(t->has_rollout, GS_ESTATE, "the tape holds no rollout yet");
+    GS_REQUIRE(t->holds(substep), GS_ESTATE, "the tape does not hold substep %d (T = %d, checkpoint_every = %d)", substep, t->T, t->K);
+    const int s = t->slot_bwd(substep);
+    return launch_unpack(m, t->slot_x(s), t->slot_v(s), d_x, d_v, (cudaStream_t)stream);
+}
+
+extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames,
+                                   const float *d_adj_x_T, const float *d_adj_v_T, float *d_adj_x0, float *d_adj_v0, gs_stream stream) {
+    GS_REQUIRE(m && t && t->m == m, GS_EINVAL, "bad model / tape");
+    GS_REQUIRE(t->has_rollout, GS_ESTATE, "gs_rollout_backward needs a gs_rollout on this tape first");
+    GS_REQUIRE(n_frames >= 0 && (n_frames == 0 || (d_adj_x_frames && frame_stride >= 1)), GS_EINVAL, "bad frame arguments");
+    GS_REQUIRE(n_frames == 0 || (long long)n_frames * frame_stride <= t->T, GS_EINVAL, "frames reach beyond the rollout: %d * %d > %d", n_frames,
+               frame_stride, t->T);
+    cudaStream_t st = (cudaStream_t)stream;
+    GS_TRY(launch_pack(m, d_adj_x_T, d_adj_v_T, m->d_adjx, m->d_adjv, false, st));
+    const size_t frame_elems = (size_t)m->E * m->N * 3;
+    if (m->plan == GS_PLAN_RESIDENT) {
+        GS_TRY(resident_rollout_backward(m, t, n_frames, frame_stride, d_adj_x_frames, st));
+    } else {
+        for (int c = t->n_ck - 1; c >= 0; c--) {
+            const int t0 = c * t->K, t1 = t0 + t->K < t->T ? t0 + t->K : t->T;
+            for (int s = t0; s + 1 < t1; s++) {  // regenerate the segment's states from its checkpoint
+                const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
+                GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, st));
+            }
+            for (int s = t1 - 1; s >= t0; s--) {
+                const float *cot = nullptr;
+                if (n_frames > 0 && (s + 1) % frame_stride == 0 && (s + 1) / frame_stride <= n_frames)
+                    cot = d_adj_x_frames + (size_t)((s + 1) / frame_stride - 1) * frame_elems;
+                const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
+                GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, st));
+            }
+        }
+    }
+    GS_TRY(launch_flush_grads(m, st));
+    return launch_unpack(m, m->d_adjx, m->d_adjv, d_adj_x0, d_adj_v0, st);
+}
+
+extern "C" int gs_zero_grads(gs_model *m, gs_stream stream) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    return launch_zero_grads(m, (cudaStream_t)stream);
+}
+extern "C" int gs_param_grads(gs_model *m, int group, float *d_out, gs_stream stream) {
+    GS_REQUIRE(m && d_out, GS_EINVAL, "null argument");
+    GS_REQUIRE(group >= 0 && group < GS_NUM_GROUPS, GS_EINVAL, "unknown parameter group %d", group);
+    return launch_get_grads(m, group, d_out, (cudaStream_t)stream);
+}
+
+extern "C" int gs_check_finite(gs_model *m, gs_stream stream, int *first_bad_substep) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    int bad = 0;
+    GS_CUDA(cudaMemcpyAsync(&bad, m->dev.bad, sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)stream), "read non-finite flag");
+    GS_CUDA(cudaStreamSynchronize((cudaStream_t)stream), "synchronize");
+    const bool is_bad = bad >= 0 && bad < 0x7f000000;
+    if (first_bad_substep) *first_bad_substep = is_bad ? bad : -1;
+    if (is_bad) { set_error("non-finite state first produced by substep %d", bad); return GS_ENONFINITE; }
+    return GS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ losses
+// one CTA per environment
+__global__ void __launch_bounds__(256) k_loss_centroid(int N, const float *__restrict__ x, const float *__restrict__ target, float scale, int accumulate,
+                                                       float *__restrict__ loss, float *__restrict__ adj) {
+    __shared__ float red[3][8];
+    __shared__ float cen[3];
+    const int env = blockIdx.x, tid = threadIdx.x;
+    const float *xe = x + (size_t)env * N * 3;
+    float sx = 0.f, sy = 0.f, sz = 0.f;
+    for (int i = tid; i < N; i += blockDim.x) { sx += xe[3 * i]; sy += xe[3 * i + 1]; sz += xe[3 * i + 2]; }
+    for (int o = 16; o > 0; o >>= 1) { sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o); }
+    if ((tid & 31) == 0) { red[0][tid >> 5] = sx; red[1][tid >> 5] = sy; red[2][tid >> 5] = sz; }
+    __syncthreads();
+    if (tid < 3) {
+        float s = 0.f;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) s += red[tid][w];
+        cen[tid] = s / (float)N - target[env * 3 + tid];
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const float L = scale * (cen[0] * cen[0] + cen[1] * cen[1] + cen[2] * cen[2]);
+        loss[env] = accumulate ? loss[env] + L : L;
+    }
+    if (adj) {
+        const float k = 2.0f * scale / (float)N;
+        float *ae = adj + (size_t)env * N * 3;
+        for (int i = tid; i < 3 * N; i += blockDim.x) ae[i] = k * cen[i % 3];
+    }
+}
+__global__ void __launch_bounds__(256) k_loss_pos(int N, const float *__restrict__ x, const float *__restrict__ ref, float scale, int accumulate,
+                                                  float *__restrict__ loss, float *__restrict__ adj) {
+    __shared__ float red[8];
+    const int env = blockIdx.x, tid = threadIdx.x;
+    const size_t o = (size_t)env * N * 3;
+    float s = 0.f;
+    for (int i = tid; i < 3 * N; i += blockDim.x) {
+        const float dlt = x[o + i] - ref[o + i];
+        s = fmaf(dlt, dlt, s);
+        if (adj) adj[o + i] = 2.0f * scale * dlt;
+    }
+    for (int k = 16; k > 0; k >>= 1) s += __shfl_xor_sync(0xffffffffu, s, k);
+    if ((tid & 31) == 0) red[tid >> 5] = s;
+    __syncthreads();
+    if (tid == 0) {
+        float tot = 0.f;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) tot += red[w];
+        tot *= scale;
+        loss[env] = accumulate ? loss[env] + tot : tot;
+    }
+}
+
+extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, const float *d_target, float scale, int accumulate, float *d_loss,
+                                float *d_adj_x, gs_stream stream) {
+    GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_target && d_loss, GS_EINVAL, "bad argument");
+    k_loss_centroid<<<n_envs, 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_target, scale, accumulate, d_loss, d_adj_x);
+    GS_CUDA(cudaGetLastError(), "k_loss_centroid");
+    g_launches++;
+    return GS_OK;
+}
+extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate, float *d_loss, float *d_adj_x,
+                           gs_stream stream) {
+    GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_ref && d_loss, GS_EINVAL, "bad argument");
+    k_loss_pos<<<n_envs, 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_ref, scale, accumulate, d_loss, d_adj_x);
+    GS_CUDA(cudaGetLastError(), "k_loss_pos");
+    g_launches++;
+    return GS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ host-buffer end-to-end
+static size_t al256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+extern "C" size_t gs_host_scratch_bytes(const gs_model *m) {
+    if (!m) return 0;
+    const size_t st = al256((size_t)m->E * m->N * 3 * sizeof(float));
+    int cmax = m->N;
+    for (int t = 0; t < 2; t++) cmax = cmax > m->counts[t] ? cmax : m->counts[t];
+    return 6 * st + al256((size_t)m->E * 3 * sizeof(float)) + al256((size_t)m->E * sizeof(float)) + al256((size_t)m->E * cmax * sizeof(float)) + 256;
+}
+
+extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, const float *h_target, float *h_loss,
+                                             float *h_adj_x0, float *h_adj_v0, int n_groups, const int *groups, float *const *h_grads, void *d_scratch,
+                                             size_t scratch_bytes, gs_stream stream) {
+    GS_REQUIRE(m && t && h_x0 && h_v0 && h_target && d_scratch, GS_EINVAL, "null argument");
+    GS_REQUIRE(n_groups >= 0 && (n_groups == 0 || (groups && h_grads)), GS_EINVAL, "bad groups");
+    GS_REQUIRE(scratch_bytes >= gs_host_scratch_bytes(m) && ((uintptr_t)d_scratch & 255) == 0, GS_EINVAL, "scratch too small or misaligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t sb = (size_t)m->E * m->N * 3 * sizeof(float), sa = al256(sb);
+    char *p = (char *)d_scratch;
+    float *d_x0 = (float *)p, *d_v0 = (float *)(p + sa), *d_xT = (float *)(p + 2 * sa), *d_cot = (float *)(p + 3 * sa);
+    float *d_ax0 = (float *)(p + 4 * sa), *d_av0 = (float *)(p + 5 * sa);
+    float *d_tgt = (float *)(p + 6 * sa);
+    float *d_loss = (float *)((char *)d_tgt + al256((size_t)m->E * 3 * sizeof(float)));
+    float *d_g = (float *)((char *)d_loss + al256((size_t)m->E * sizeof(float)));
+    GS_CUDA(cudaMemcpyAsync(d_x0, h_x0, sb, cudaMemcpyHostToDevice, st), "H2D x0");
+    GS_CUDA(cudaMemcpyAsync(d_v0, h_v0, sb, cudaMemcpyHostToDevice, st), "H2D v0");
+    GS_CUDA(cudaMemcpyAsync(d_tgt, h_target, (size_t)m->E * 3 * sizeof(float), cudaMemcpyHostToDevice, st), "H2D target");
+    GS_TRY(gs_zero_grads(m, stream));
+    GS_TRY(gs_rollout(m, t, d_x0, d_v0, d_xT, nullptr, stream));
+    GS_TRY(gs_loss_centroid(m->E, m->N, d_xT, d_tgt, 1.0f, 0, d_loss, d_cot, stream));
+    GS_TRY(gs_rollout_backward(m, t, 0, 1, nullptr, d_cot, nullptr, d_ax0, d_av0, stream));
+    if (h_loss) GS_CUDA(cudaMemcpyAsync(h_loss, d_loss, (size_t)m->E * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
+    if (h_adj_x0) GS_CUDA(cudaMemcpyAsync(h_adj_x0, d_ax0, sb, cudaMemcpyDeviceToHost, st), "D2H adj_x0");
+    if (h_adj_v0) GS_CUDA(cudaMemcpyAsync(h_adj_v0, d_av0, sb, cudaMemcpyDeviceToHost, st), "D2H adj_v0");
+    for (int k = 0; k < n_groups; k++) {
+        const int g = groups[k];
+        GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
+        const int c = g == GS_MASS ? m->N : m->counts[g / 3];
+        if (c == 0) continue;
+        GS_TRY(gs_param_grads(m, g, d_g, stream));
+        // the staging buffer is reused: order the copy before the next group's kernel on the same stream
+        GS_CUDA(cudaMemcpyAsync(h_grads[k], d_g, (size_t)m->E * c * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H grads");
+    }
+    GS_CUDA(cudaStreamSynchronize(st), "synchronize");
+    int bad = -1;
+    return gs_check_finite(m, stream, &bad);
+}
+
+extern "C" uint64_t gs_launch_count(void) { return g_launches; }
+extern "C" const char *gs_version(void) { return "gradsim-b200 0.1 (sm_100a)"; }

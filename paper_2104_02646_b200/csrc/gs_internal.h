@@ -1,0 +1,133 @@
+// gs_internal.h -- host-side model / tape objects and the POD views handed to kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/gradsim.h"
+
+namespace gs {
+
+enum { T_TET = 0, T_TRI = 1, T_HINGE = 2, N_TYPES = 3 };
+static const int kArity[N_TYPES] = {4, 3, 4};
+
+constexpr int kTileElems = 256;      // elements per tile = threads per CTA of the streaming element kernels
+constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
+
+// Device view of one element set (tets, triangles or hinges) in INTERNAL (Morton, tiled) order.
+struct ElemDev {
+    int count, n_tiles, max_tile_parts;
+    const ushort4 *lidx;        // [count] tile-local particle indices (w unused for triangles)
+    const int *tile_part_ptr;   // [n_tiles + 1]
+    const int *tile_parts;      // internal particle ids of each tile's particles (ascending)
+    const uint16_t *csr_end;    // per tile-particle: end offset into the tile's slot list
+    const uint16_t *csr_slots;  // [n_tiles][arity * kTileElems] slot = k * kTileElems + local element
+    const float4 *c0, *c1;      // tets: B[0..3], B[4..7]; tris: B[0..3], (A,-,-,-); hinges: (theta0, l0, kb, -)
+    const float2 *c2;           // tets: (B[8], V)
+    const float *mu, *lam, *damp;  // [E][count]
+    float *g32;                 // [3][E][count] per-substep fp32 accumulators (mu, lambda, damp)
+    double *g64;                // [3][E][count] fp64 masters
+    const int *perm;            // [count] internal -> caller element index
+};
+
+struct ModelDev {
+    int N, E;
+    ElemDev es[N_TYPES];
+    int tile_begin[N_TYPES + 1];  // blockIdx.x ranges of the fused element kernels
+    float gx, gy, gz, dt;
+    float nx, ny, nz, pd, pr;
+    const float *ke, *kd, *kf, *muc;  // [E]
+    const int *perm_p;                // [N] internal -> caller particle index
+    const float *inv_mass;            // [E][N] internal order (0 = pinned)
+    float *gmass32;                   // [E][N]
+    double *gmass64;                  // [E][N]
+    int *bad;                         // first non-finite substep (INT_MAX = none)
+};
+
+struct HostElemSet {
+    int count = 0, n_tiles = 0, max_tile_parts = 0;
+    std::vector<int> perm;  // internal -> caller
+};
+
+}  // namespace gs
+
+struct gs_model {
+    gs::ModelDev dev;
+    int N = 0, E = 0, plan = GS_PLAN_STREAMING;
+    int counts[gs::N_TYPES] = {0, 0, 0};
+    gs::HostElemSet hes[gs::N_TYPES];
+    std::vector<int> perm_p;  // internal -> caller
+    // scratch device buffers (inside the workspace)
+    float4 *d_f = nullptr;                 // [E][N] force accumulators (zero between substeps)
+    float4 *d_xs[2] = {nullptr, nullptr};  // single-step state scratch
+    float4 *d_vs[2] = {nullptr, nullptr};
+    float4 *d_adjx = nullptr, *d_adjv = nullptr, *d_adjf = nullptr;
+    // mutable copies of device pointers the API writes
+    float *d_inv_mass = nullptr;
+    float *d_param[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int steps_since_flush = 0;
+    int fwd_smem = 0, adj_smem = 0;
+    int step_counter = 0;  // substep index written to dev.bad on a non-finite state
+    // resident plan
+    int res_threads = 0, res_smem_fwd = 0, res_smem_adj = 0;
+    void *res_blob = nullptr;  // device: packed connectivity + constants for the resident kernels
+};
+
+struct gs_tape {
+    gs_model *m = nullptr;
+    int T = 0, K = 1, n_ck = 0;
+    size_t S = 0;  // float4 elements per array per slot = E * N
+    float4 *base = nullptr;
+    bool has_rollout = false;
+    // slot index helpers (each slot = x4[S] then v4[S])
+    float4 *slot_x(int s) const { return base + (size_t)(2 * s) * S; }
+    float4 *slot_v(int s) const { return base + (size_t)(2 * s + 1) * S; }
+    int n_slots() const { return K == 1 ? T + 1 : n_ck + 1 + (K - 1 > 2 ? K - 1 : 2); }
+    int slot_final() const { return K == 1 ? T : n_ck; }
+    int slot_work(int j) const { return n_ck + 1 + j; }  // K > 1 only
+    // slot holding state t during the forward pass
+    int slot_fwd(int t) const {
+        if (K == 1) return t;
+        if (t == T) return slot_final();
+        if (t % K == 0) return t / K;
+        return slot_work(t & 1);
+    }
+    // slot holding state t while segment c = t0/K is being processed backward (t in [t0, t1])
+    int slot_bwd(int t) const {
+        if (K == 1) return t;
+        if (t == T) return slot_final();
+        if (t % K == 0) return t / K;
+        return slot_work(t % K - 1);
+    }
+    bool holds(int t) const { return t >= 0 && t <= T && (K == 1 || t == T || t % K == 0); }
+};
+
+namespace gs {
+void set_error(const char *fmt, ...);
+int cuda_fail(cudaError_t e, const char *what);
+extern uint64_t g_launches;
+
+// gs_plan.cpp: host preprocessing.  Fills a byte image of the workspace (static part) and the model's host fields.
+struct WorkspaceLayout;
+size_t workspace_bytes_upper(int N, int E, const int counts[N_TYPES]);
+int build_model(const gs_model_desc *desc, void *d_workspace, size_t bytes, cudaStream_t stream, gs_model *m);
+
+// gs_stream.cu: streaming plan launches
+int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st);
+int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st);
+int launch_pack(gs_model *m, const float *x, const float *v, float4 *x4, float4 *v4, bool x_is_state, cudaStream_t st);
+int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, float *v, cudaStream_t st);
+int launch_flush_grads(gs_model *m, cudaStream_t st);
+int launch_zero_grads(gs_model *m, cudaStream_t st);
+int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st);
+int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st);
+int configure_stream_kernels(gs_model *m);
+
+// gs_resident.cu: resident plan
+size_t resident_blob_bytes(const gs_model_desc *desc);
+int resident_prepare(gs_model *m, const gs_model_desc *desc, void *d_workspace, size_t bytes, cudaStream_t st);
+int resident_rollout(gs_model *m, gs_tape *t, cudaStream_t st);
+int resident_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames, cudaStream_t st);
+}  // namespace gs

@@ -1,0 +1,355 @@
+// gs_plan.cu -- host preprocessing of a scene: validation, rest-shape quantities, Morton reordering of
+// particles and elements, tiling with tile-local indices and per-tile gather lists, upload into the
+// caller's workspace.  Off the hot path (runs once per model).
+//
+// Rest quantities (fp64 on the host, stored fp32):
+//   tets      B = D_m^-1, V = det(D_m)/6                         PAPER.md:575-581 (V_e, constant-strain tets)
+//   triangles 2x2 B in the rest frame (t1, t2), A = det(D_m)/2   PAPER.md:584; A4
+//   hinges    theta0 (signed rest dihedral), l0 (rest edge)      PAPER.md:585-586; A5, A6
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+
+#include "gs_internal.h"
+
+namespace gs {
+
+static thread_local char t_err[512] = "";
+uint64_t g_launches = 0;
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof t_err, fmt, ap);
+    va_end(ap);
+}
+const char *last_error() { return t_err; }
+int cuda_fail(cudaError_t e, const char *what) {
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return GS_ECUDA;
+}
+
+// ---------------------------------------------------------------------------------- workspace layout
+struct Bump {
+    char *base;
+    size_t off = 0;
+    explicit Bump(void *b) : base((char *)b) {}
+    template <class T>
+    T *take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? (T *)(base + off) : nullptr;
+        off += (n ? n : 1) * sizeof(T);
+        return p;
+    }
+};
+
+struct Layout {
+    // per type
+    ushort4 *lidx[N_TYPES];
+    int *tile_part_ptr[N_TYPES], *tile_parts[N_TYPES], *perm[N_TYPES];
+    uint16_t *csr_end[N_TYPES], *csr_slots[N_TYPES];
+    float4 *c0[N_TYPES], *c1[N_TYPES];
+    float2 *c2[N_TYPES];
+    float *mu[N_TYPES], *lam[N_TYPES], *damp[N_TYPES], *g32[N_TYPES];
+    double *g64[N_TYPES];
+    int *perm_p, *bad;
+    float *inv_mass, *gmass32, *ke, *kd, *kf, *muc;
+    double *gmass64;
+    float4 *f, *xs[2], *vs[2], *adjx, *adjv, *adjf;
+    size_t bytes;
+};
+
+static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
+    Layout L;
+    Bump b(base);
+    const size_t EN = (size_t)E * N;
+    for (int t = 0; t < N_TYPES; t++) {
+        const size_t c = counts[t], a = kArity[t], nt = (c + kTileElems - 1) / kTileElems;
+        L.lidx[t] = b.take<ushort4>(c);
+        L.tile_part_ptr[t] = b.take<int>(nt + 1);
+        L.tile_parts[t] = b.take<int>(a * c);
+        L.csr_end[t] = b.take<uint16_t>(a * c);
+        L.csr_slots[t] = b.take<uint16_t>(nt * a * kTileElems);
+        L.c0[t] = b.take<float4>(c);
+        L.c1[t] = t == T_HINGE ? nullptr : b.take<float4>(c);
+        L.c2[t] = t == T_TET ? b.take<float2>(c) : nullptr;
+        if (t != T_HINGE) {
+            L.mu[t] = b.take<float>(E * c);
+            L.lam[t] = b.take<float>(E * c);
+            L.damp[t] = b.take<float>(E * c);
+            L.g32[t] = b.take<float>(3 * E * c);
+            L.g64[t] = b.take<double>(3 * E * c);
+        } else {
+            L.mu[t] = L.lam[t] = L.damp[t] = L.g32[t] = nullptr;
+            L.g64[t] = nullptr;
+        }
+        L.perm[t] = b.take<int>(c);
+    }
+    L.perm_p = b.take<int>(N);
+    L.inv_mass = b.take<float>(EN);
+    L.gmass32 = b.take<float>(EN);
+    L.gmass64 = b.take<double>(EN);
+    L.ke = b.take<float>(E); L.kd = b.take<float>(E); L.kf = b.take<float>(E); L.muc = b.take<float>(E);
+    L.bad = b.take<int>(1);
+    L.f = b.take<float4>(EN);
+    for (int i = 0; i < 2; i++) { L.xs[i] = b.take<float4>(EN); L.vs[i] = b.take<float4>(EN); }
+    L.adjx = b.take<float4>(EN); L.adjv = b.take<float4>(EN); L.adjf = b.take<float4>(EN);
+    L.bytes = ((b.off + 255) & ~(size_t)255) + 256;
+    return L;
+}
+
+size_t workspace_bytes_upper(int N, int E, const int counts[N_TYPES]) { return make_layout(nullptr, N, E, counts).bytes; }
+
+// ---------------------------------------------------------------------------------- geometry helpers (fp64)
+struct d3 { double x, y, z; };
+static inline d3 sub(d3 a, d3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+static inline d3 crs(d3 a, d3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+static inline double dt3(d3 a, d3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+static inline d3 scl(double s, d3 a) { return {s * a.x, s * a.y, s * a.z}; }
+static inline d3 P(const float *x, int i) { return {x[3 * i], x[3 * i + 1], x[3 * i + 2]}; }
+
+static inline uint64_t spread21(uint64_t v) {
+    v &= 0x1fffff;
+    v = (v | v << 32) & 0x1f00000000ffffULL;
+    v = (v | v << 16) & 0x1f0000ff0000ffULL;
+    v = (v | v << 8) & 0x100f00f00f00f00fULL;
+    v = (v | v << 4) & 0x10c30c30c30c30c3ULL;
+    v = (v | v << 2) & 0x1249249249249249ULL;
+    return v;
+}
+
+template <class T>
+static int upload(T *dst, const std::vector<T> &src, cudaStream_t st) {
+    if (src.empty()) return GS_OK;
+    cudaError_t e = cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+    return e == cudaSuccess ? GS_OK : cuda_fail(e, "upload");
+}
+#define UP(dst, vec) do { int rc_ = upload(dst, vec, stream); if (rc_ != GS_OK) return rc_; } while (0)
+
+// ---------------------------------------------------------------------------------- build
+int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStream_t stream, gs_model *m) {
+    const int N = d->n_particles, E = d->n_envs;
+    const int counts[N_TYPES] = {d->n_tets, d->n_tris, d->n_hinges};
+    Layout L = make_layout(d_workspace, N, E, counts);
+    if (bytes < L.bytes) { set_error("workspace too small: %zu < %zu bytes", bytes, L.bytes); return GS_EINVAL; }
+    if (((uintptr_t)d_workspace & 255) != 0) { set_error("workspace must be 256-byte aligned"); return GS_EINVAL; }
+    const float *X = d->x_rest;
+
+    // ---- validation of indices and masses
+    const int32_t *conn[N_TYPES] = {d->tets, d->tris, d->hinges};
+    static const char *tname[N_TYPES] = {"tet", "triangle", "hinge"};
+    for (int t = 0; t < N_TYPES; t++)
+        for (int e = 0; e < counts[t]; e++)
+            for (int k = 0; k < kArity[t]; k++) {
+                int i = conn[t][(size_t)e * kArity[t] + k];
+                if (i < 0 || i >= N) { set_error("%s %d: particle index %d out of range [0, %d)", tname[t], e, i, N); return GS_EMESH; }
+                for (int q = 0; q < k; q++)
+                    if (conn[t][(size_t)e * kArity[t] + q] == i) { set_error("%s %d: repeated particle index %d", tname[t], e, i); return GS_EMESH; }
+            }
+    const size_t n_mass = (d->param_layout & GS_MASS_PER_ENV) ? (size_t)E * N : (size_t)N;
+    for (size_t i = 0; i < n_mass; i++)
+        if (!(d->mass[i] > 0.0f) || !std::isfinite(d->mass[i])) { set_error("mass[%zu] must be finite and > 0", i); return GS_EINVAL; }
+    for (int i = 0; i < 3 * N; i++)
+        if (!std::isfinite(X[i])) { set_error("x_rest has a non-finite entry at particle %d", i / 3); return GS_EINVAL; }
+
+    // ---- particle Morton order
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int i = 0; i < N; i++)
+        for (int r = 0; r < 3; r++) { lo[r] = std::min(lo[r], (double)X[3 * i + r]); hi[r] = std::max(hi[r], (double)X[3 * i + r]); }
+    double span = 1e-30;
+    for (int r = 0; r < 3; r++) span = std::max(span, hi[r] - lo[r]);
+    auto morton = [&](double x, double y, double z) -> uint64_t {
+        const double s = 2097151.0 / span;
+        uint64_t ix = (uint64_t)std::min(2097151.0, std::max(0.0, (x - lo[0]) * s));
+        uint64_t iy = (uint64_t)std::min(2097151.0, std::max(0.0, (y - lo[1]) * s));
+        uint64_t iz = (uint64_t)std::min(2097151.0, std::max(0.0, (z - lo[2]) * s));
+        return spread21(ix) | (spread21(iy) << 1) | (spread21(iz) << 2);
+    };
+    std::vector<uint64_t> key(N);
+    for (int i = 0; i < N; i++) key[i] = morton(X[3 * i], X[3 * i + 1], X[3 * i + 2]);
+    m->perm_p.resize(N);
+    std::iota(m->perm_p.begin(), m->perm_p.end(), 0);
+    std::stable_sort(m->perm_p.begin(), m->perm_p.end(), [&](int a, int b) { return key[a] < key[b]; });
+    std::vector<int> inv_p(N);  // caller -> internal
+    for (int i = 0; i < N; i++) inv_p[m->perm_p[i]] = i;
+    UP(L.perm_p, m->perm_p);
+
+    // ---- per-particle parameters
+    {
+        std::vector<float> w((size_t)E * N);
+        for (int env = 0; env < E; env++)
+            for (int i = 0; i < N; i++) {
+                int c = m->perm_p[i];
+                float mass = (d->param_layout & GS_MASS_PER_ENV) ? d->mass[(size_t)env * N + c] : d->mass[c];
+                w[(size_t)env * N + i] = (d->pinned && d->pinned[c]) ? 0.0f : 1.0f / mass;
+            }
+        UP(L.inv_mass, w);
+        std::vector<float> s(E);
+        const float *src[4] = {d->ke, d->kd, d->kf, d->mu_c};
+        float *dst[4] = {L.ke, L.kd, L.kf, L.muc};
+        for (int q = 0; q < 4; q++) {
+            for (int env = 0; env < E; env++) s[env] = (d->param_layout & GS_CONTACT_PER_ENV) ? src[q][env] : src[q][0];
+            UP(dst[q], s);
+        }
+    }
+
+    // ---- elements: rest quantities, Morton order, tiles
+    ModelDev &dev = m->dev;
+    memset(&dev, 0, sizeof dev);
+    int tile_cursor = 0;
+    for (int t = 0; t < N_TYPES; t++) {
+        const int c = counts[t], a = kArity[t];
+        const int nt = (c + kTileElems - 1) / kTileElems;
+        HostElemSet &hs = m->hes[t];
+        hs.count = c; hs.n_tiles = nt; hs.max_tile_parts = 0;
+        hs.perm.resize(c);
+        std::vector<uint64_t> ekey(c);
+        std::vector<float4> c0(c), c1(t == T_HINGE ? 0 : c);
+        std::vector<float2> c2(t == T_TET ? c : 0);
+        // rest quantities in caller order first
+        std::vector<float4> r0(c), r1(c);
+        std::vector<float2> r2(c);
+        for (int e = 0; e < c; e++) {
+            const int32_t *ix = conn[t] + (size_t)e * a;
+            d3 cen = {0, 0, 0};
+            for (int k = 0; k < a; k++) { d3 p = P(X, ix[k]); cen.x += p.x / a; cen.y += p.y / a; cen.z += p.z / a; }
+            ekey[e] = morton(cen.x, cen.y, cen.z);
+            if (t == T_TET) {
+                d3 x0 = P(X, ix[0]), e1 = sub(P(X, ix[1]), x0), e2 = sub(P(X, ix[2]), x0), e3 = sub(P(X, ix[3]), x0);
+                // D_m columns e1 e2 e3; inverse rows = (e2 x e3, e3 x e1, e1 x e2) / det
+                d3 r_0 = crs(e2, e3), r_1 = crs(e3, e1), r_2 = crs(e1, e2);
+                double det = dt3(e1, r_0);
+                if (!(det > 0.0) || !std::isfinite(det)) { set_error("tet %d: non-positive rest volume (det D_m = %g)", e, det); return GS_EMESH; }
+                r_0 = scl(1.0 / det, r_0); r_1 = scl(1.0 / det, r_1); r_2 = scl(1.0 / det, r_2);
+                r0[e] = make_float4((float)r_0.x, (float)r_0.y, (float)r_0.z, (float)r_1.x);
+                r1[e] = make_float4((float)r_1.y, (float)r_1.z, (float)r_2.x, (float)r_2.y);
+                r2[e] = make_float2((float)r_2.z, (float)(det / 6.0));
+            } else if (t == T_TRI) {
+                d3 x0 = P(X, ix[0]), e1 = sub(P(X, ix[1]), x0), e2 = sub(P(X, ix[2]), x0), nn = crs(e1, e2);
+                double l1 = std::sqrt(dt3(e1, e1)), ln = std::sqrt(dt3(nn, nn));
+                if (!(0.5 * ln > 1e-12) || !(l1 > 0)) { set_error("triangle %d: degenerate rest shape (area %g)", e, 0.5 * ln); return GS_EMESH; }
+                d3 t1 = scl(1.0 / l1, e1), t2 = crs(scl(1.0 / ln, nn), t1);
+                double A = dt3(t1, e1), B = dt3(t1, e2), C = dt3(t2, e1), D = dt3(t2, e2), det = A * D - B * C;
+                r0[e] = make_float4((float)(D / det), (float)(-B / det), (float)(-C / det), (float)(A / det));
+                r1[e] = make_float4((float)(det / 2.0), 0.f, 0.f, 0.f);
+            } else {
+                d3 x1 = P(X, ix[0]), x2 = P(X, ix[1]), x3 = P(X, ix[2]), x4 = P(X, ix[3]);
+                d3 n1 = crs(sub(x1, x3), sub(x1, x4)), n2 = crs(sub(x2, x4), sub(x2, x3)), ed = sub(x4, x3);
+                double l0 = std::sqrt(dt3(ed, ed)), a1 = std::sqrt(dt3(n1, n1)), a2 = std::sqrt(dt3(n2, n2));
+                if (!(l0 > 0) || !(a1 > 1e-12) || !(a2 > 1e-12)) { set_error("hinge %d: degenerate rest shape", e); return GS_EMESH; }
+                d3 eh = scl(1.0 / l0, ed);
+                double th = std::atan2(dt3(crs(scl(1 / a1, n1), scl(1 / a2, n2)), eh), dt3(n1, n2) / (a1 * a2));
+                r0[e] = make_float4((float)th, (float)l0, d->hinge_kb[e], 0.f);
+            }
+        }
+        std::iota(hs.perm.begin(), hs.perm.end(), 0);
+        std::stable_sort(hs.perm.begin(), hs.perm.end(), [&](int x, int y) { return ekey[x] < ekey[y]; });
+        for (int e = 0; e < c; e++) {
+            c0[e] = r0[hs.perm[e]];
+            if (t != T_HINGE) c1[e] = r1[hs.perm[e]];
+            if (t == T_TET) c2[e] = r2[hs.perm[e]];
+        }
+        // tiles
+        std::vector<ushort4> lidx(c);
+        std::vector<int> tpp(nt + 1, 0), tparts;
+        std::vector<uint16_t> csr_end, csr_slots((size_t)nt * a * kTileElems, 0);
+        tparts.reserve((size_t)c * 2);
+        std::vector<int> ids, cnt, pos;
+        for (int j = 0; j < nt; j++) {
+            const int e0 = j * kTileElems, e1 = std::min(c, e0 + kTileElems);
+            ids.clear();
+            for (int e = e0; e < e1; e++)
+                for (int k = 0; k < a; k++) ids.push_back(inv_p[conn[t][(size_t)hs.perm[e] * a + k]]);
+            std::sort(ids.begin(), ids.end());
+            ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
+            const int P_ = (int)ids.size();
+            hs.max_tile_parts = std::max(hs.max_tile_parts, P_);
+            cnt.assign(P_ + 1, 0);
+            for (int e = e0; e < e1; e++) {
+                unsigned short li[4] = {0, 0, 0, 0};
+                for (int k = 0; k < a; k++) {
+                    int gi = inv_p[conn[t][(size_t)hs.perm[e] * a + k]];
+                    int lp = (int)(std::lower_bound(ids.begin(), ids.end(), gi) - ids.begin());
+                    li[k] = (unsigned short)lp;
+                    cnt[lp + 1]++;
+                }
+                lidx[e] = make_ushort4(li[0], li[1], li[2], li[3]);
+            }
+            for (int p = 0; p < P_; p++) cnt[p + 1] += cnt[p];
+            pos.assign(cnt.begin(), cnt.end() - 1);
+            uint16_t *slots = csr_slots.data() + (size_t)j * a * kTileElems;
+            for (int e = e0; e < e1; e++) {
+                const unsigned short li[4] = {lidx[e].x, lidx[e].y, lidx[e].z, lidx[e].w};
+                for (int k = 0; k < a; k++) slots[pos[li[k]]++] = (uint16_t)(k * kTileElems + (e - e0));
+            }
+            for (int p = 0; p < P_; p++) { tparts.push_back(ids[p]); csr_end.push_back((uint16_t)cnt[p + 1]); }
+            tpp[j + 1] = (int)tparts.size();
+        }
+        UP(L.lidx[t], lidx); UP(L.tile_part_ptr[t], tpp); UP(L.tile_parts[t], tparts); UP(L.csr_end[t], csr_end);
+        UP(L.csr_slots[t], csr_slots); UP(L.c0[t], c0);
+        if (t != T_HINGE) UP(L.c1[t], c1);
+        if (t == T_TET) UP(L.c2[t], c2);
+        UP(L.perm[t], hs.perm);
+        // per-env element parameters in internal order
+        if (t != T_HINGE) {
+            const float *src[3] = {t == T_TET ? d->tet_mu : d->tri_mu, t == T_TET ? d->tet_lambda : d->tri_lambda, t == T_TET ? d->tet_damp : d->tri_damp};
+            float *dst[3] = {L.mu[t], L.lam[t], L.damp[t]};
+            std::vector<float> v((size_t)E * c);
+            for (int q = 0; q < 3; q++) {
+                for (int env = 0; env < E; env++)
+                    for (int e = 0; e < c; e++) {
+                        float val = (d->param_layout & GS_ELEM_PER_ENV) ? src[q][(size_t)env * c + hs.perm[e]] : src[q][hs.perm[e]];
+                        if (!std::isfinite(val)) { set_error("%s parameter %d of element %d is not finite", tname[t], q, hs.perm[e]); return GS_EINVAL; }
+                        if (q == 1 && !(val > 0.0f)) { set_error("%s %d: lambda must be > 0", tname[t], hs.perm[e]); return GS_EINVAL; }
+                        v[(size_t)env * c + e] = val;
+                    }
+                UP(dst[q], v);
+            }
+            cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * std::max(c, 1), stream);
+            if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * std::max(c, 1), stream);
+            if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
+        }
+        ElemDev &ed = dev.es[t];
+        ed.count = c; ed.n_tiles = nt; ed.max_tile_parts = hs.max_tile_parts;
+        ed.lidx = L.lidx[t]; ed.tile_part_ptr = L.tile_part_ptr[t]; ed.tile_parts = L.tile_parts[t];
+        ed.csr_end = L.csr_end[t]; ed.csr_slots = L.csr_slots[t];
+        ed.c0 = L.c0[t]; ed.c1 = L.c1[t]; ed.c2 = L.c2[t];
+        ed.mu = L.mu[t]; ed.lam = L.lam[t]; ed.damp = L.damp[t]; ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
+        ed.perm = L.perm[t];
+        dev.tile_begin[t] = tile_cursor;
+        tile_cursor += nt;
+        m->counts[t] = c;
+        if (t != T_HINGE) { m->d_param[3 * t] = L.mu[t]; m->d_param[3 * t + 1] = L.lam[t]; m->d_param[3 * t + 2] = L.damp[t]; }
+    }
+    dev.tile_begin[N_TYPES] = tile_cursor;
+    dev.N = N; dev.E = E;
+    dev.gx = d->gravity[0]; dev.gy = d->gravity[1]; dev.gz = d->gravity[2]; dev.dt = d->dt;
+    {
+        double nl = std::sqrt((double)d->plane_n[0] * d->plane_n[0] + (double)d->plane_n[1] * d->plane_n[1] + (double)d->plane_n[2] * d->plane_n[2]);
+        if (!(nl > 0)) { set_error("plane_n must be non-zero"); return GS_EINVAL; }
+        dev.nx = (float)(d->plane_n[0] / nl); dev.ny = (float)(d->plane_n[1] / nl); dev.nz = (float)(d->plane_n[2] / nl);
+    }
+    dev.pd = d->plane_d; dev.pr = d->particle_radius;
+    dev.ke = L.ke; dev.kd = L.kd; dev.kf = L.kf; dev.muc = L.muc;
+    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.bad = L.bad;
+    m->N = N; m->E = E;
+    m->d_f = L.f; m->d_xs[0] = L.xs[0]; m->d_xs[1] = L.xs[1]; m->d_vs[0] = L.vs[0]; m->d_vs[1] = L.vs[1];
+    m->d_adjx = L.adjx; m->d_adjv = L.adjv; m->d_adjf = L.adjf;
+    m->d_inv_mass = L.inv_mass;
+    const size_t EN = (size_t)E * N;
+    cudaError_t ce = cudaMemsetAsync(L.f, 0, sizeof(float4) * EN, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gmass32, 0, sizeof(float) * EN, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gmass64, 0, sizeof(double) * EN, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.bad, 0x7f, sizeof(int), stream);
+    if (ce != cudaSuccess) return cuda_fail(ce, "memset workspace");
+    ce = cudaStreamSynchronize(stream);
+    if (ce != cudaSuccess) return cuda_fail(ce, "model upload");
+    return GS_OK;
+}
+
+}  // namespace gs
+
+extern "C" const char *gs_last_error(void) { return gs::last_error(); }
