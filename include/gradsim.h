@@ -151,7 +151,8 @@ void gs_tape_destroy(gs_tape *t);
 int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const float *d_v0, float *d_x_T, float *d_v_T, gs_stream stream);
 
 /* Copy the stored state after `substep` substeps to caller order.  GS_ESTATE if the tape does not hold
-   that substep (checkpointed tapes hold multiples of K and the final state).  Either output may be NULL. */
+   that substep (checkpointed tapes hold multiples of K and the final state, so a loss that reads frames
+   every frame_stride substeps needs K | frame_stride).  Either output may be NULL. */
 int gs_tape_read(gs_model *m, gs_tape *t, int substep, float *d_x, float *d_v, gs_stream stream);
 
 /*
@@ -199,6 +200,19 @@ int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, co
 
 /* Number of kernel launches the library has enqueued since the process started (bench.py's gpu_launches). */
 uint64_t gs_launch_count(void);
+
+/*
+ * Per-kernel device timing (bench.py's roofline leg).  While enabled, every hot-path kernel launch of this
+ * model is bracketed by CUDA events recorded on the caller's stream.  gs_kernel_times synchronises the
+ * stream, adds the elapsed time of every recorded launch to ms_total[kernel] and its count to
+ * launches[kernel] (arrays of n >= GS_K_COUNT entries, overwritten), and clears the record.
+ * Off by default; the events cost a few microseconds of host time per launch, so timed throughput runs
+ * keep it off.  Kernel ids: elements_fwd = a1-a4, particles_fwd = a5-a7,
+ * particles_adj = a8, elements_adj = a9-a10, other = layout conversion / gradient flush / losses.
+ */
+enum gs_kernel_id { GS_K_ELEMENTS_FWD = 0, GS_K_PARTICLES_FWD = 1, GS_K_PARTICLES_ADJ = 2, GS_K_ELEMENTS_ADJ = 3, GS_K_OTHER = 4, GS_K_COUNT = 5 };
+int gs_kernel_timing(gs_model *m, int enable);
+int gs_kernel_times(gs_model *m, gs_stream stream, int n, double *ms_total, uint64_t *launches);
 
 const char *gs_last_error(void);
 const char *gs_version(void);

@@ -224,7 +224,7 @@ def truth_targets(sc):
     (guess -> unroll -> compare with the observed trajectory)."""
     import copy
 
-    if sc.loss == "final_centroid":
+    if sc.target is not None:  # seeded targets (final_centroid [E,3]; final-state position loss [1,E,N,3])
         return _d(sc.target)
     tsc = copy.copy(sc)
     for k, val in sc.truth.items():

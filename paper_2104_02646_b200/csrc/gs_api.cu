@@ -350,5 +350,51 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
     return gs_check_finite(m, stream, &bad);
 }
 
+// ------------------------------------------------------------------------------------------ kernel timing
+gs_model::~gs_model() {
+    for (cudaEvent_t e : ev_pool) cudaEventDestroy(e);
+}
+namespace gs {
+static cudaEvent_t next_event(gs_model *m) {
+    if (m->ev_used == m->ev_pool.size()) {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        m->ev_pool.push_back(e);
+    }
+    return m->ev_pool[m->ev_used++];
+}
+cudaEvent_t timing_begin(gs_model *m, cudaStream_t st) {
+    cudaEvent_t a = next_event(m);
+    if (a) cudaEventRecord(a, st);
+    return a;
+}
+void timing_end(gs_model *m, int id, cudaEvent_t a, cudaStream_t st) {
+    cudaEvent_t b = next_event(m);
+    if (!b) return;
+    cudaEventRecord(b, st);
+    m->timed.push_back({id, a, b});
+}
+}  // namespace gs
+
+extern "C" int gs_kernel_timing(gs_model *m, int enable) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    m->timing = enable != 0;
+    return GS_OK;
+}
+extern "C" int gs_kernel_times(gs_model *m, gs_stream stream, int n, double *ms_total, uint64_t *launches) {
+    GS_REQUIRE(m && ms_total && launches && n >= GS_K_COUNT, GS_EINVAL, "bad argument");
+    GS_CUDA(cudaStreamSynchronize((cudaStream_t)stream), "synchronize");
+    for (int k = 0; k < n; k++) { ms_total[k] = 0.0; launches[k] = 0; }
+    for (const gs_model::TimedLaunch &t : m->timed) {
+        float ms = 0.f;
+        GS_CUDA(cudaEventElapsedTime(&ms, t.a, t.b), "cudaEventElapsedTime");
+        ms_total[t.id] += ms;
+        launches[t.id]++;
+    }
+    m->timed.clear();
+    m->ev_used = 0;
+    return GS_OK;
+}
+
 extern "C" uint64_t gs_launch_count(void) { return g_launches; }
 extern "C" const char *gs_version(void) { return "gradsim-b200 0.1 (sm_100a)"; }

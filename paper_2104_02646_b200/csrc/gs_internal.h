@@ -73,6 +73,13 @@ struct gs_model {
     // resident plan
     int res_threads = 0, res_smem_fwd = 0, res_smem_adj = 0;
     void *res_blob = nullptr;  // device: packed connectivity + constants for the resident kernels
+    // per-kernel event timing (gs_kernel_timing)
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;  // all events ever created for this model
+    size_t ev_used = 0;
+    struct TimedLaunch { int id; cudaEvent_t a, b; };
+    std::vector<TimedLaunch> timed;
+    ~gs_model();
 };
 
 struct gs_tape {
@@ -106,6 +113,9 @@ struct gs_tape {
 
 namespace gs {
 void set_error(const char *fmt, ...);
+// event bracket around one launch when m->timing is on (gs_api.cu)
+cudaEvent_t timing_begin(gs_model *m, cudaStream_t st);
+void timing_end(gs_model *m, int id, cudaEvent_t a, cudaStream_t st);
 int cuda_fail(cudaError_t e, const char *what);
 extern uint64_t g_launches;
 

@@ -25,6 +25,14 @@ namespace gs {
         if (e_ != cudaSuccess) return cuda_fail(e_, what);           \
         g_launches++;                                                \
     } while (0)
+// GS_TIMED(m, id, st, what, launch): the launch, bracketed by events when the model's kernel timing is on
+#define GS_TIMED(m, id, st, what, ...)                                 \
+    do {                                                               \
+        cudaEvent_t ta_ = (m)->timing ? timing_begin(m, st) : nullptr; \
+        __VA_ARGS__;                                                   \
+        GS_LAUNCH_CHECK(what);                                         \
+        if (ta_) timing_end(m, id, ta_, st);                           \
+    } while (0)
 
 __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float c) {
     // one vector reduction per particle instead of three scalar ones (REDG.E.ADD.F32x4)
@@ -327,37 +335,33 @@ static inline int pmax_of(const gs_model *m) {
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
     const int tiles = m->dev.tile_begin[N_TYPES];
     if (tiles > 0) {
-        k_elements_fwd<<<dim3(tiles, m->E), kTileElems, m->fwd_smem, st>>>(m->dev, x, v, m->d_f, pmax_of(m));
-        GS_LAUNCH_CHECK("k_elements_fwd");
+        GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", k_elements_fwd<<<dim3(tiles, m->E), kTileElems, m->fwd_smem, st>>>(m->dev, x, v, m->d_f, pmax_of(m)));
     }
-    k_particles_fwd<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, m->d_f, xo, vo, substep);
-    GS_LAUNCH_CHECK("k_particles_fwd");
+    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", k_particles_fwd<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, m->d_f, xo, vo, substep));
     return GS_OK;
 }
 
 // adjoint of the substep whose start state is (x, v) and whose end velocity is v_next; cotangents live in
 // m->d_adjx / m->d_adjv (updated in place); frame_cot (caller order, may be null) is added to adj_x first.
 int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st) {
-    k_particles_adj<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf);
-    GS_LAUNCH_CHECK("k_particles_adj");
+    GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
+             k_particles_adj<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
     const int tiles = m->dev.tile_begin[N_TYPES];
     if (tiles > 0) {
-        k_elements_adj<<<dim3(tiles, m->E), kTileElems, m->adj_smem, st>>>(m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv, pmax_of(m));
-        GS_LAUNCH_CHECK("k_elements_adj");
+        GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
+                 k_elements_adj<<<dim3(tiles, m->E), kTileElems, m->adj_smem, st>>>(m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv, pmax_of(m)));
     }
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
     return GS_OK;
 }
 
 int launch_pack(gs_model *m, const float *x, const float *v, float4 *x4, float4 *v4, bool x_is_state, cudaStream_t st) {
-    k_pack<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, x4, v4, x_is_state ? 1 : 0);
-    GS_LAUNCH_CHECK("k_pack");
+    GS_TIMED(m, GS_K_OTHER, st, "k_pack", k_pack<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, x4, v4, x_is_state ? 1 : 0));
     return GS_OK;
 }
 int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, float *v, cudaStream_t st) {
     if (!x && !v) return GS_OK;
-    k_unpack<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x4, v4, x, v);
-    GS_LAUNCH_CHECK("k_unpack");
+    GS_TIMED(m, GS_K_OTHER, st, "k_unpack", k_unpack<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x4, v4, x, v));
     return GS_OK;
 }
 
@@ -366,11 +370,9 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
     for (int t = 0; t < 2; t++) {
         const size_t n = 3 * (size_t)m->E * m->counts[t];
         if (!n) continue;
-        k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n);
-        GS_LAUNCH_CHECK("k_flush");
+        GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
-    k_flush<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N);
-    GS_LAUNCH_CHECK("k_flush");
+    GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
     return GS_OK;
 }
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
@@ -378,11 +380,9 @@ int launch_zero_grads(gs_model *m, cudaStream_t st) {
     for (int t = 0; t < 2; t++) {
         const size_t n = 3 * (size_t)m->E * m->counts[t];
         if (!n) continue;
-        k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n);
-        GS_LAUNCH_CHECK("k_zero");
+        GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
-    k_zero<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N);
-    GS_LAUNCH_CHECK("k_zero");
+    GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
     return GS_OK;
 }
 int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {

@@ -1,0 +1,82 @@
+"""The C-ABI library builds for sm_100a without a GPU, loads, and exports every symbol include/gradsim.h
+declares; the Python binding declares a signature for each of them.  No compute calls here."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2104_02646_b200 import build as gs_build
+from paper_2104_02646_b200 import gradsim as gs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "gradsim.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gs_[a-z_0-9]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def lib_path():
+    return gs_build.build()
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = _declared()
+    for need in ("gs_model_create", "gs_step_forward", "gs_step_backward", "gs_rollout", "gs_rollout_backward", "gs_param_grads"):
+        assert need in names
+
+
+def test_library_exports_every_declared_symbol(lib_path):
+    L = C.CDLL(lib_path)
+    for name in _declared():
+        assert hasattr(L, name), f"{name} declared in gradsim.h but not exported"
+
+
+def test_binding_covers_every_declared_symbol(lib_path):
+    assert sorted(gs.SIGNATURES) == _declared()
+    L = gs.lib()
+    assert L.gs_version().decode().startswith("gradsim-b200")
+    assert L.gs_launch_count() >= 0
+
+
+def test_desc_struct_matches_header_field_order():
+    src = open(os.path.join(ROOT, "include", "gradsim.h")).read()
+    body = re.search(r"typedef struct \{(.*?)\} gs_model_desc;", src, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if not decl:
+            continue
+        decl = re.sub(r"^(const\s+)?(int32_t|uint32_t|uint8_t|float)\s*", "", decl)
+        for part in decl.split(","):
+            fields.append(re.sub(r"[\*\s]|\[\d+\]", "", part))
+    assert fields == [f[0] for f in gs.gs_model_desc._fields_]
+
+
+def test_argument_errors_without_a_device(lib_path):
+    """Pure host-side argument checks return codes instead of crashing (no CUDA call is reached)."""
+    L = gs.lib()
+    assert L.gs_model_workspace_bytes(None) == 0
+    out = C.c_void_p()
+    assert L.gs_model_create(None, None, 0, None, C.byref(out)) == gs.GS_EINVAL
+    assert b"desc" in L.gs_last_error()
+    assert L.gs_tape_bytes(None, 10, 1) == 0
+    assert L.gs_zero_grads(None, None) == gs.GS_EINVAL
+    assert L.gs_step_forward(None, None, None, None, None, None) == gs.GS_EINVAL
+    d = gs.gs_model_desc()
+    d.n_particles, d.n_envs = 0, 1
+    assert L.gs_model_workspace_bytes(C.byref(d)) == 0
+
+
+def test_product_path_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2104_02646_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", txt, flags=re.M), f
+                assert "gs_oracle" not in txt and "libgs_oracle" not in txt, f

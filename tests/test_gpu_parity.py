@@ -1,0 +1,205 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 oracle, element by element, on the same
+seeded inputs (north_star tolerances; "relative" as in DESIGN.md reading A18):
+
+  one substep      max_i |dx_i|_inf <= 1e-5 * scene extent
+  full rollout     max_i |dx_i|_inf <= 1e-3 * scene extent
+  every gradient   ||dg||_inf / ||g_oracle||_inf <= 2e-3 per array
+
+Small variants of the five configs (several tiles + a ragged tail, seconds in the oracle) run
+element-by-element; the full-size configs are compared in test_gpu_full_size.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2104_02646_b200 import gradsim as gs
+from paper_2104_02646_b200 import scenes
+
+from gpu_util import dev, gpu_run_scene, host, rel_inf
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP, TOL_ROLLOUT, TOL_GRAD = 1e-5, 1e-3, 2e-3
+PLANS = [gs.GS_PLAN_STREAMING]
+
+
+def _grad_groups(sc):
+    g = ["mass"]
+    if sc.tets.shape[0]:
+        g += ["tet_mu", "tet_lambda", "tet_damp"]
+    if sc.tris.shape[0]:
+        g += ["tri_mu", "tri_lambda", "tri_damp"]
+    return g
+
+
+@pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("plan", PLANS)
+def test_one_substep_forward_and_adjoint(config, plan):
+    sc = scenes.make_scene(config, small=True)
+    x, v = scenes.perturbed_state(sc)
+    o = orc.Oracle(sc)
+    xo, vo = o.step(x, v)
+    assert (x[..., 1] < 0).any() and (x[..., 1] > 0).any()  # both contact branches
+    m = gs.Model(sc, plan=plan)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert m.check_finite() == -1
+    ext = sc.extent()
+    assert np.abs(host(xg) - xo).max() <= TOL_STEP * ext
+    assert rel_inf(host(vg), vo) <= 2e-5
+    # adjoint of the same substep with seeded cotangents
+    r = scenes.rng_for(config, "misc", 77)
+    bx, bv = r.normal(size=x.shape).astype(np.float32), r.normal(size=x.shape).astype(np.float32)
+    o.zero_grads()
+    ax, av = o.step_adjoint(x, v, bx, bv)
+    m.zero_grads()
+    axg, avg = m.step_backward(dev(x), dev(v), dev(bx), dev(bv))
+    assert rel_inf(host(axg), ax) <= TOL_GRAD
+    assert rel_inf(host(avg), av) <= TOL_GRAD
+    for g in _grad_groups(sc):
+        assert rel_inf(host(m.param_grads(g)), o.grads(g)) <= TOL_GRAD, g
+    # the fp32 path is far inside the budget on a single substep: keep it that way
+    assert rel_inf(host(axg), ax) <= 1e-4 and rel_inf(host(avg), av) <= 1e-4
+
+
+@pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("plan", PLANS)
+def test_small_rollout_and_gradients(config, plan):
+    sc = scenes.make_scene(config, small=True)
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"], plan=plan)
+    assert got["bad"] == -1
+    ext = sc.extent()
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
+    assert np.abs(got["rec_x"] - ref["rec_x"]).max() <= TOL_ROLLOUT * ext
+    assert rel_inf(got["loss"], ref["loss"]) <= 5e-3
+    assert rel_inf(got["adj_x0"], ref["adj_x0"]) <= TOL_GRAD
+    assert rel_inf(got["adj_v0"], ref["adj_v0"]) <= TOL_GRAD
+    for g in _grad_groups(sc):
+        if config == 3:  # per-environment totals (BASELINE.json configs[3])
+            a, b = got["g_" + g].sum(1), ref["g_" + g].sum(1)
+            assert np.abs(a - b).max() <= TOL_GRAD * np.abs(b).max(), g
+        assert rel_inf(got["g_" + g], ref["g_" + g]) <= TOL_GRAD, g
+
+
+def test_checkpointed_backward_matches_full_tape():
+    """Segment replay regenerates the same states, so K only changes which fp32 sums are flushed when."""
+    sc = scenes.make_scene(2, small=True)
+    ref = orc.run_scene(sc)
+    full = gpu_run_scene(sc, ref["target"], K=1, plan=gs.GS_PLAN_STREAMING)
+    for K in (4, 16, 32):  # frame losses need K | frame_stride (gradsim.h, gs_tape_read)
+        ck = gpu_run_scene(sc, ref["target"], K=K, plan=gs.GS_PLAN_STREAMING)
+        assert np.abs(ck["xT"] - full["xT"]).max() <= 1e-6 * sc.extent()
+        for k in ("adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_mass"):
+            assert rel_inf(ck[k], full[k]) <= 1e-4, (K, k)
+            assert rel_inf(ck[k], ref[k]) <= TOL_GRAD, (K, k)
+
+
+def test_tape_read_and_intermediate_states():
+    sc = scenes.make_scene(0, small=True)
+    o = orc.Oracle(sc)
+    ro = o.rollout(sc.x0, sc.v0, 40, rec_times=[1, 17, 40], want_rec_v=True)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    tape = m.tape(40, 1)
+    tape.rollout(dev(sc.x0), dev(sc.v0))
+    for k, t in enumerate([1, 17, 40]):
+        x, v = tape.read(t)
+        assert np.abs(host(x) - ro["rec_x"][k]).max() <= 1e-5 * sc.extent()
+        assert rel_inf(host(v), ro["rec_v"][k]) <= 1e-4
+    x, v = tape.read(0)
+    assert np.array_equal(host(x), sc.x0.astype(np.float64))
+
+
+def test_set_params_changes_the_result_like_the_oracle():
+    sc = scenes.make_scene(0, small=True)
+    x, v = scenes.perturbed_state(sc)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    r = scenes.rng_for(0, "misc", 5)
+    new_mu = r.uniform(5e3, 3e4, sc.tet_mu.shape).astype(np.float32)
+    new_m = r.uniform(0.05, 0.2, sc.mass.shape).astype(np.float32)
+    m.set_params("tet_mu", dev(new_mu))
+    m.set_params("mass", dev(new_m))
+    sc.tet_mu, sc.mass = new_mu, new_m
+    xo, vo = orc.Oracle(sc).step(x, v)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
+    assert rel_inf(host(vg), vo) <= 2e-5
+
+
+# ------------------------------------------------------------------------------------------ edge cases
+def test_particles_only_free_fall_closed_form():
+    """No elements at all (empty element sets): Listing 1 alone; closed form of P1."""
+    T, dt = 64, 1.0 / 1920.0
+    x0 = np.array([[0.3, 5.0, -0.2], [1.0, 7.0, 2.0], [0.0, 9.0, 0.0]])
+    v0 = np.array([[0.1, 0.4, -0.3], [0.0, -0.2, 0.5], [0.0, 0.0, 0.0]])
+    sc = scenes.custom_scene(x0, v0=v0, dt=dt, pinned=[0, 0, 1], n_substeps=T)
+    m = gs.Model(sc)
+    tape = m.tape(T)
+    xT, vT = tape.rollout(dev(sc.x0), dev(sc.v0))
+    g = np.array([0.0, -9.8, 0.0])
+    exp = x0 + v0 * T * dt + g * dt * dt * T * (T + 1) / 2
+    exp[2] = x0[2]
+    assert np.abs(host(xT)[0] - exp).max() <= 1e-5
+    bx = torch.zeros((1, 3, 3), device="cuda:0")
+    bx[0, 0, 1] = 1.0
+    ax0, av0 = tape.backward(adj_x_T=bx)
+    assert abs(host(av0)[0, 0, 1] - T * dt) <= 1e-6 * T * dt * 10  # d(final height)/d(v0_y) = T dt
+    assert host(ax0)[0, 0, 1] == 1.0
+
+
+def test_single_element_meshes_and_ragged_tiles():
+    r = np.random.default_rng(3)
+    # 1 tet; 1 triangle; 2 triangles + 1 hinge; 257 tets (one full tile + a tail of one)
+    cases = []
+    cases.append(scenes.custom_scene(np.array([[0, 0.01, 0], [0.1, 0.01, 0], [0, 0.11, 0], [0, 0.01, 0.1]], float), tets=[[0, 1, 2, 3]]))
+    cases.append(scenes.custom_scene(np.array([[0, 0.01, 0], [0, 0.01, 0.1], [0.1, 0.01, 0]], float), tris=[[0, 1, 2]]))
+    xc, tris, hinges = scenes.cloth_grid(2, 2, 0.05, origin=(0, 0.01, 0))
+    cases.append(scenes.custom_scene(xc, tris=tris, hinges=hinges))
+    xs, tets = scenes.hex_grid_tets(13, 2, 2, 0.1, origin=(0, 0.02, 0))
+    cases.append(scenes.custom_scene(xs, tets=tets[:257]))
+    for sc in cases:
+        x = (sc.x0 + 0.01 * r.uniform(-1, 1, sc.x0.shape)).astype(np.float32)
+        v = r.uniform(-0.5, 0.5, sc.x0.shape).astype(np.float32)
+        xo, vo = orc.Oracle(sc).step(x, v)
+        m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+        xg, vg = m.step_forward(dev(x), dev(v))
+        assert np.abs(host(xg) - xo).max() <= TOL_STEP * max(sc.extent(), 0.1), sc.tets.shape
+        assert rel_inf(host(vg), vo) <= 2e-5
+
+
+def test_pinned_particles_do_not_move_and_have_zero_mass_gradient():
+    sc = scenes.make_scene(1, small=True)
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"])
+    pin = sc.pinned.astype(bool)
+    assert pin.sum() == 2
+    assert np.array_equal(got["xT"][:, pin], sc.x0[:, pin].astype(np.float64))
+    assert (got["g_mass"][:, pin] == 0).all()
+
+
+def test_error_paths():
+    x = np.array([[0, 0.01, 0], [0.1, 0.01, 0], [0, 0.11, 0], [0, 0.01, 0.1]], float)
+    with pytest.raises(gs.GradSimError) as e:  # inverted tet
+        gs.Model(scenes.custom_scene(x, tets=[[0, 1, 3, 2]]))
+    assert e.value.code == gs.GS_EMESH and "tet 0" in str(e.value)
+    with pytest.raises(gs.GradSimError) as e:  # index out of range
+        gs.Model(scenes.custom_scene(x, tets=[[0, 1, 2, 4]]))
+    assert e.value.code == gs.GS_EMESH
+    with pytest.raises(gs.GradSimError) as e:  # degenerate triangle
+        gs.Model(scenes.custom_scene(np.array([[0, 0, 0], [1, 0, 0], [2, 0, 0]], float), tris=[[0, 1, 2]], hinges=np.zeros((0, 4), np.int32)))
+    assert e.value.code == gs.GS_EMESH
+    sc = scenes.custom_scene(x, tets=[[0, 1, 2, 3]])
+    m = gs.Model(sc)
+    tape = m.tape(4)
+    with pytest.raises(gs.GradSimError) as e:  # backward before any rollout
+        tape.backward()
+    assert e.value.code == gs.GS_ESTATE
+    # workspace too small
+    import ctypes as C
+    desc, keep = gs.fill_desc(sc)
+    out = C.c_void_p()
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda:0")
+    assert gs.lib().gs_model_create(C.byref(desc), C.c_void_p(ws.data_ptr()), 1024, None, C.byref(out)) == gs.GS_EINVAL
+    # non-finite state is reported with its substep
+    tape.rollout(dev(sc.x0), dev(np.full(sc.x0.shape, 3e38, np.float32)))
+    assert m.check_finite() == 0

@@ -531,7 +531,7 @@ def test_openmp_thread_count_does_not_change_results():
     sc = scenes.make_scene(3, small=True)
     sc.n_substeps = 20
     a = orc.Oracle(sc).rollout(sc.x0, sc.v0, 20)["xT"]
-    sc1 = scenes.batched_sysid_scene(n_envs=1, n_substeps=20)
+    sc1 = scenes.batched_sysid_scene(n_envs=1, n_substeps=20, y0=0.02)
     for k in ("tet_mu", "tet_lambda", "mass", "mu_c"):
         setattr(sc1, k, getattr(sc, k)[2:3])
     b = orc.Oracle(sc1).rollout(sc1.x0, sc1.v0, 20)["xT"]
