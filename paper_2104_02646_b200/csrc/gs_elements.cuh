@@ -229,7 +229,9 @@ __device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], 
     const vec3 dm2 = i2 * (dn2 - (2.0f * dot(h.n2, dn2) * i2) * h.n2);
     const float dc13 = dot(q13, h.eh) + dot(h.p13, deh), dc14 = dot(q14, h.eh) + dot(h.p14, deh);
     const float dc23 = dot(q23, h.eh) + dot(h.p23, deh), dc24 = dot(q24, h.eh) + dot(h.p24, deh);
-    const float s = dot(d[0], a[0]) + dot(d[1], a[1]) + dot(d[2], a[2]) + dot(d[3], a[3]);
+    // s = sum_i d_i . a_i written with cotangent differences only (sum_i d_i = 0): the adjoint field is smooth,
+    // so the plain sum cancels to ~1e-4 of its terms and would lose that many digits in fp32
+    const float s = dot(h.m1, h.c13 * q14 - h.c14 * q13) + dot(h.m2, h.c23 * q24 - h.c24 * q23);
     float sn, cs;
     sincosf(0.5f * (h.theta - theta0), &sn, &cs);
     const float E1 = kb * l0 * sn, E2s = 0.5f * kb * l0 * cs * s;

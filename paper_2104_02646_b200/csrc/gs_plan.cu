@@ -308,9 +308,11 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                     }
                 UP(dst[q], v);
             }
-            cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * std::max(c, 1), stream);
-            if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * std::max(c, 1), stream);
-            if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
+            if (c > 0) {  // an empty set owns one placeholder element only: clearing E * 1 entries would run into its neighbours
+                cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * c, stream);
+                if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * c, stream);
+                if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
+            }
         }
         ElemDev &ed = dev.es[t];
         ed.count = c; ed.n_tiles = nt; ed.max_tile_parts = hs.max_tile_parts;
