@@ -69,7 +69,9 @@ enum gs_param_layout {
 enum gs_plan {
     GS_PLAN_AUTO = 0,     /* resident when the mesh fits one CTA's shared memory, else streaming         */
     GS_PLAN_STREAMING = 1,/* two grid-wide kernels per substep over Morton-ordered element tiles          */
-    GS_PLAN_RESIDENT = 2  /* one persistent CTA per environment, state in shared memory across substeps   */
+    GS_PLAN_RESIDENT = 2  /* one persistent CTA per environment, state on-chip across ALL substeps of a rollout
+                             (tets-only meshes of <= 2048 tets; gs_step_* and checkpointed tapes of such a model
+                             still run the streaming kernels) */
 };
 
 /*
@@ -210,7 +212,12 @@ uint64_t gs_launch_count(void);
  * keep it off.  Kernel ids: elements_fwd = a1-a4, particles_fwd = a5-a7,
  * particles_adj = a8, elements_adj = a9-a10, other = layout conversion / gradient flush / losses.
  */
-enum gs_kernel_id { GS_K_ELEMENTS_FWD = 0, GS_K_PARTICLES_FWD = 1, GS_K_PARTICLES_ADJ = 2, GS_K_ELEMENTS_ADJ = 3, GS_K_OTHER = 4, GS_K_COUNT = 5 };
+enum gs_kernel_id {
+    GS_K_ELEMENTS_FWD = 0, GS_K_PARTICLES_FWD = 1, GS_K_PARTICLES_ADJ = 2, GS_K_ELEMENTS_ADJ = 3, GS_K_OTHER = 4,
+    GS_K_RESIDENT_FWD = 5, /* resident plan: a1-a7 of all T substeps in one launch */
+    GS_K_RESIDENT_ADJ = 6, /* resident plan: a8-a10 of all T substeps in one launch */
+    GS_K_COUNT = 7
+};
 int gs_kernel_timing(gs_model *m, int enable);
 int gs_kernel_times(gs_model *m, gs_stream stream, int n, double *ms_total, uint64_t *launches);
 

@@ -140,12 +140,6 @@ extern "C" int gs_tape_create(gs_model *m, int n_substeps, int checkpoint_every,
     GS_REQUIRE(t, GS_ENOMEM, "out of host memory");
     t->m = m; t->T = n_substeps;
     t->K = checkpoint_every > n_substeps ? n_substeps : checkpoint_every;
-    if (m->plan == GS_PLAN_RESIDENT && t->K != 1) {
-        // the resident plan keeps the full tape (a full tape of a mesh that fits one CTA is small)
-        delete t;
-        set_error("the resident plan supports checkpoint_every = 1 only; create the model with GS_PLAN_STREAMING for checkpointing");
-        return GS_EINVAL;
-    }
     t->n_ck = (t->T + t->K - 1) / t->K;
     t->S = (size_t)m->E * m->N;
     t->base = (float4 *)d_mem;
@@ -160,7 +154,7 @@ extern "C" int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const floa
     cudaStream_t st = (cudaStream_t)stream;
     GS_TRY(reset_bad(m, st));
     GS_TRY(launch_pack(m, d_x0, d_v0, t->slot_x(t->slot_fwd(0)), t->slot_v(t->slot_fwd(0)), true, st));
-    if (m->plan == GS_PLAN_RESIDENT) {
+    if (m->plan == GS_PLAN_RESIDENT && t->K == 1) {  // a checkpointed tape of a resident model runs the streaming loop
         GS_TRY(resident_rollout(m, t, st));
     } else {
         for (int s = 0; s < t->T; s++) {
@@ -190,7 +184,7 @@ extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int fr
     cudaStream_t st = (cudaStream_t)stream;
     GS_TRY(launch_pack(m, d_adj_x_T, d_adj_v_T, m->d_adjx, m->d_adjv, false, st));
     const size_t frame_elems = (size_t)m->E * m->N * 3;
-    if (m->plan == GS_PLAN_RESIDENT) {
+    if (m->plan == GS_PLAN_RESIDENT && t->K == 1) {
         GS_TRY(resident_rollout_backward(m, t, n_frames, frame_stride, d_adj_x_frames, st));
     } else {
         for (int c = t->n_ck - 1; c >= 0; c--) {
@@ -352,6 +346,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
 
 // ------------------------------------------------------------------------------------------ kernel timing
 gs_model::~gs_model() {
+    gs::resident_release(this);
     for (cudaEvent_t e : ev_pool) cudaEventDestroy(e);
 }
 namespace gs {

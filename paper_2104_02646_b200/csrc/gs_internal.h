@@ -70,9 +70,8 @@ struct gs_model {
     int steps_since_flush = 0;
     int fwd_smem = 0, adj_smem = 0;
     int step_counter = 0;  // substep index written to dev.bad on a non-finite state
-    // resident plan
-    int res_threads = 0, res_smem_fwd = 0, res_smem_adj = 0;
-    void *res_blob = nullptr;  // device: packed connectivity + constants for the resident kernels
+    // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
+    void *res_host = nullptr;
     // per-kernel event timing (gs_kernel_timing)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;  // all events ever created for this model
@@ -138,6 +137,7 @@ int configure_stream_kernels(gs_model *m);
 // gs_resident.cu: resident plan
 size_t resident_blob_bytes(const gs_model_desc *desc);
 int resident_prepare(gs_model *m, const gs_model_desc *desc, void *d_workspace, size_t bytes, cudaStream_t st);
+void resident_release(gs_model *m);
 int resident_rollout(gs_model *m, gs_tape *t, cudaStream_t st);
 int resident_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames, cudaStream_t st);
 }  // namespace gs

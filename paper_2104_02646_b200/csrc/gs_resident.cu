@@ -1,14 +1,406 @@
-// gs_resident.cu -- the RESIDENT plan (one persistent CTA per environment).  Placeholder: not built yet,
-// every model runs the streaming plan.
+// gs_resident.cu -- the RESIDENT plan: one persistent CTA per environment runs ALL substeps of a rollout
+// (k_resident_fwd) or of its adjoint (k_resident_adj) in one launch.
+//
+// For meshes that fit one CTA (BASELINE.json configs[0] and the 1024-environment configs[3]: 125 particles,
+// 320 tets) two grid-wide launches per substep are pure launch latency, and streaming the state through HBM
+// every substep is wasted traffic.  Here
+//   - each thread owns EPT tets for the whole rollout: connectivity, B, V, mu, lambda, k_damp stay in registers;
+//   - each of the first N threads owns one particle: x, v (forward) or adj_x, adj_v (adjoint) stay in
+//     registers across substeps and are mirrored to shared memory for the element phase;
+//   - scatter is a shared-memory gather list: element threads write per-vertex
+//     contributions to conflict-free slots, the particle thread sums its slots -- no atomics, deterministic;
+//   - the only HBM traffic is the tape: one coalesced float4 store of (x, v) per particle per substep in the
+//     forward pass, one prefetched load per substep in the adjoint;
+//   - parameter gradients (a10) accumulate in registers over the whole rollout (fp32 chunks of 32 substeps
+//     folded into fp64, hazard H4) and are written once.
+// Two __syncthreads per substep.  Bound: plain fp32 ALU + barrier latency, not HBM.
+//
+// Tets only (the element functions are those of gs_elements.cuh, shared with the streaming plan); meshes with
+// triangles / hinges, more than kResMaxTets tets or more particles than threads run the streaming plan.
+#include <algorithm>
+#include <climits>
+#include <vector>
+
+#include "gs_elements.cuh"
 #include "gs_internal.h"
 
 namespace gs {
-size_t resident_blob_bytes(const gs_model_desc *) { return 0; }
-int resident_prepare(gs_model *m, const gs_model_desc *desc, void *, size_t, cudaStream_t) {
-    if (desc->plan == GS_PLAN_RESIDENT) { set_error("the resident plan is not available in this build"); return GS_EINVAL; }
-    m->plan = GS_PLAN_STREAMING;
+
+constexpr int kResMaxTets = 2048;
+constexpr int kResMaxThreads = 1024;
+
+struct ResDev {
+    int M, N, nthreads;
+    const ushort4 *idx;        // [M] internal particle ids of each tet (internal element order)
+    const uint16_t *csr_ptr;   // [N + 1]
+    const uint16_t *csr_slots; // [4 M] slot = k * M + e
+};
+
+struct ResHost {
+    ResDev rd;
+    int ept;
+    size_t smem_fwd, smem_adj;
+};
+
+static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
+
+// shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float, csr_ptr, csr_slots
+static size_t res_smem(int N, int M, int planes, bool adj) {
+    return (size_t)(adj ? 3 : 2) * N * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float) + al16((size_t)(N + 1) * 2) + al16((size_t)4 * M * 2);
+}
+
+static bool resident_fits(const gs_model_desc *d) {
+    if (d->n_tris > 0 || d->n_hinges > 0 || d->n_tets < 1 || d->n_tets > kResMaxTets) return false;
+    const int ept = d->n_tets > kResMaxThreads ? 2 : 1;
+    const int nthreads = ((d->n_tets + ept - 1) / ept + 31) / 32 * 32;
+    if (d->n_particles > nthreads) return false;
+    return res_smem(d->n_particles, d->n_tets, 6, true) <= 200 * 1024;
+}
+
+size_t resident_blob_bytes(const gs_model_desc *d) {
+    if (!resident_fits(d)) return 0;
+    return 256 * 4 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
+}
+
+// ------------------------------------------------------------------------------------------ kernels
+struct TetReg {
+    float b[9], V, mu, lam, kd;
+    ushort4 li;
+    bool on;
+};
+
+template <int EPT>
+__device__ __forceinline__ void load_tets(const ModelDev &md, const ResDev &rd, int env, TetReg tr[EPT]) {
+    const ElemDev &es = md.es[T_TET];
+#pragma unroll
+    for (int j = 0; j < EPT; j++) {
+        const int e = threadIdx.x + j * blockDim.x;
+        tr[j].on = e < rd.M;
+        const int ee = tr[j].on ? e : 0;
+        const float4 c0 = es.c0[ee], c1 = es.c1[ee];
+        const float2 c2 = es.c2[ee];
+        tr[j].b[0] = c0.x; tr[j].b[1] = c0.y; tr[j].b[2] = c0.z; tr[j].b[3] = c0.w;
+        tr[j].b[4] = c1.x; tr[j].b[5] = c1.y; tr[j].b[6] = c1.z; tr[j].b[7] = c1.w; tr[j].b[8] = c2.x;
+        tr[j].V = c2.y;
+        const size_t pe = (size_t)env * es.count + ee;
+        tr[j].mu = es.mu[pe]; tr[j].lam = es.lam[pe]; tr[j].kd = es.damp[pe];
+        tr[j].li = rd.idx[ee];
+    }
+}
+
+__device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint16_t *s_slots) {
+    for (int i = threadIdx.x; i <= rd.N; i += blockDim.x) s_ptr[i] = rd.csr_ptr[i];
+    for (int i = threadIdx.x; i < 4 * rd.M; i += blockDim.x) s_slots[i] = rd.csr_slots[i];
+}
+
+// forward: substeps [0, T), tape slot s = (x4, v4) at base + 2 s S (+ S for v), S = E N
+template <int EPT, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, const ResDev rd, float4 *__restrict__ tape, size_t S, int T) {
+    extern __shared__ float4 smem4[];
+    const int N = rd.N, M = rd.M, PL = 4 * M;
+    float4 *sx = smem4, *sv = smem4 + N;
+    float *sf = reinterpret_cast<float *>(smem4 + 2 * N);  // [3][4 M]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 3 * PL);
+    uint16_t *s_slots = s_ptr + (((N + 1) + 7) & ~7);
+    const int tid = threadIdx.x, env = blockIdx.x;
+    const size_t poff = (size_t)env * N + tid;
+    TetReg tr[EPT];
+    load_tets<EPT>(md, rd, env, tr);
+    load_csr(rd, s_ptr, s_slots);
+    const bool is_p = tid < N;
+    float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq;
+    if (is_p) { xq = tape[poff]; vq = tape[S + poff]; sx[tid] = xq; sv[tid] = vq; }
+    ContactParams cp;
+    cp.n = vec3(md.nx, md.ny, md.nz); cp.d = md.pd; cp.r = md.pr;
+    cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
+    const vec3 g(md.gx, md.gy, md.gz);
+    __syncthreads();
+    int beg = 0, end = 0;
+    if (is_p) { beg = s_ptr[tid]; end = s_ptr[tid + 1]; }
+    int bad = INT_MAX;
+    for (int s = 0; s < T; s++) {
+#pragma unroll
+        for (int j = 0; j < EPT; j++) {
+            if (tr[j].on) {
+                const ushort4 li = tr[j].li;
+                const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
+                const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
+                vec3 f[4];
+                tet_force(x, v, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, f);
+                const int e = tid + j * blockDim.x;
+#pragma unroll
+                for (int k = 0; k < 4; k++) { sf[k * M + e] = f[k].x; sf[PL + k * M + e] = f[k].y; sf[2 * PL + k * M + e] = f[k].z; }
+            }
+        }
+        __syncthreads();
+        if (is_p) {
+            float ax = 0.f, ay = 0.f, az = 0.f;
+            for (int q = beg; q < end; q++) {
+                const int sl = s_slots[q];
+                ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
+            }
+            const vec3 x(xq), v(vq);
+            const vec3 f = vec3(ax, ay, az) + contact_force(cp, x, v);
+            vec3 x1, v1;
+            integrate(x, v, f, xq.w, g, md.dt, x1, v1);
+            xq = make_float4(x1.x, x1.y, x1.z, xq.w);
+            vq = make_float4(v1.x, v1.y, v1.z, 0.f);
+            sx[tid] = xq; sv[tid] = vq;
+            float4 *slot = tape + (size_t)(2 * (s + 1)) * S;
+            slot[poff] = xq; slot[S + poff] = vq;
+            const float chk = x1.x + x1.y + x1.z + v1.x + v1.y + v1.z;
+            if (!(fabsf(chk) <= 3.0e38f) && bad == INT_MAX) bad = s;
+        }
+        __syncthreads();
+    }
+    if (bad != INT_MAX) atomicMin(md.bad, bad);
+}
+
+// adjoint: substeps T-1 .. 0.  adjx / adjv: [E][N] float4 in/out (dL/d(final state) -> dL/d(initial state)).
+// frames: caller-order [n_frames][E][N][3] cotangents of the states after (k+1) * stride substeps, or nullptr.
+template <int EPT, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, const ResDev rd, const float4 *__restrict__ tape, size_t S, int T,
+                                                              float4 *__restrict__ adjx, float4 *__restrict__ adjv, const float *__restrict__ frames,
+                                                              int n_frames, int stride) {
+    extern __shared__ float4 smem4[];
+    const int N = rd.N, M = rd.M, PL = 4 * M;
+    float4 *sx = smem4, *sv = smem4 + N, *sa = smem4 + 2 * N;
+    float *sf = reinterpret_cast<float *>(smem4 + 3 * N);  // [6][4 M]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 6 * PL);
+    uint16_t *s_slots = s_ptr + (((N + 1) + 7) & ~7);
+    const int tid = threadIdx.x, env = blockIdx.x;
+    const size_t poff = (size_t)env * N + tid;
+    TetReg tr[EPT];
+    load_tets<EPT>(md, rd, env, tr);
+    load_csr(rd, s_ptr, s_slots);
+    const bool is_p = tid < N;
+    ContactParams cp;
+    cp.n = vec3(md.nx, md.ny, md.nz); cp.d = md.pd; cp.r = md.pr;
+    cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
+    const vec3 g(md.gx, md.gy, md.gz);
+    const float dt = md.dt;
+    vec3 bx = zero3(), bv = zero3();       // running cotangents of this thread's particle
+    float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq, vnext = xq;
+    const float *cot = nullptr;
+    if (is_p) {
+        bx = vec3(adjx[poff]); bv = vec3(adjv[poff]);
+        vnext = tape[(size_t)(2 * T + 1) * S + poff];
+        xq = tape[(size_t)(2 * (T - 1)) * S + poff]; vq = tape[(size_t)(2 * (T - 1) + 1) * S + poff];
+        if (frames) cot = frames + ((size_t)env * N + md.perm_p[tid]) * 3;
+    }
+    const size_t frame_elems = (size_t)md.E * N * 3;
+    float gm32 = 0.f;
+    double gm64 = 0.0;
+    float g32[EPT][3];
+    double g64[EPT][3];
+#pragma unroll
+    for (int j = 0; j < EPT; j++)
+#pragma unroll
+        for (int q = 0; q < 3; q++) { g32[j][q] = 0.f; g64[j][q] = 0.0; }
+    __syncthreads();
+    int beg = 0, end = 0;
+    if (is_p) { beg = s_ptr[tid]; end = s_ptr[tid + 1]; }
+    for (int s = T - 1; s >= 0; s--) {
+        if (is_p) {
+            // prefetch the start state of the previous substep while this one is processed
+            float4 xp = xq, vp = vq;
+            if (s > 0) { xp = tape[(size_t)(2 * (s - 1)) * S + poff]; vp = tape[(size_t)(2 * (s - 1) + 1) * S + poff]; }
+            if (s != T - 1) {  // contributions of the element phase of substep s + 1
+                float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
+                for (int q = beg; q < end; q++) {
+                    const int sl = s_slots[q];
+                    ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
+                    cx += sf[3 * PL + sl]; cy += sf[4 * PL + sl]; cz += sf[5 * PL + sl];
+                }
+                bx += vec3(ax, ay, az); bv += vec3(cx, cy, cz);
+            }
+            if (cot && (s + 1) % stride == 0 && (s + 1) / stride <= n_frames) {
+                const float *c = cot + (size_t)((s + 1) / stride - 1) * frame_elems;
+                bx += vec3(c[0], c[1], c[2]);
+            }
+            const float w = xq.w;
+            const vec3 x(xq), v(vq);
+            const vec3 lv = madd(bv, dt, bx);
+            const vec3 af = (dt * w) * lv;
+            vec3 ax = bx, av = lv;
+            if (w > 0.0f) {
+                const vec3 dvf = (vec3(vnext) - v) - dt * g;
+                gm32 += -w * dot(dvf, lv);
+            }
+            contact_adjoint(cp, x, v, af, ax, av);
+            bx = ax; bv = av;
+            sx[tid] = xq; sv[tid] = vq; sa[tid] = make_float4(af.x, af.y, af.z, 0.f);
+            vnext = vq; xq = xp; vq = vp;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < EPT; j++) {
+            if (tr[j].on) {
+                const ushort4 li = tr[j].li;
+                const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
+                const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
+                const vec3 a[4] = {vec3(sa[li.x]), vec3(sa[li.y]), vec3(sa[li.z]), vec3(sa[li.w])};
+                vec3 ax[4], av[4];
+                float gmu, glam, gk;
+                tet_adjoint(x, v, a, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, ax, av, gmu, glam, gk);
+                g32[j][0] += gmu; g32[j][1] += glam; g32[j][2] += gk;
+                const int e = tid + j * blockDim.x;
+#pragma unroll
+                for (int k = 0; k < 4; k++) {
+                    sf[k * M + e] = ax[k].x; sf[PL + k * M + e] = ax[k].y; sf[2 * PL + k * M + e] = ax[k].z;
+                    sf[3 * PL + k * M + e] = av[k].x; sf[4 * PL + k * M + e] = av[k].y; sf[5 * PL + k * M + e] = av[k].z;
+                }
+            }
+        }
+        if ((s & (kFlushEvery - 1)) == 0) {  // fold the fp32 chunk into fp64 (hazard H4)
+            gm64 += (double)gm32; gm32 = 0.f;
+#pragma unroll
+            for (int j = 0; j < EPT; j++)
+#pragma unroll
+                for (int q = 0; q < 3; q++) { g64[j][q] += (double)g32[j][q]; g32[j][q] = 0.f; }
+        }
+        __syncthreads();
+    }
+    if (is_p) {
+        float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
+        for (int q = beg; q < end; q++) {
+            const int sl = s_slots[q];
+            ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
+            cx += sf[3 * PL + sl]; cy += sf[4 * PL + sl]; cz += sf[5 * PL + sl];
+        }
+        bx += vec3(ax, ay, az); bv += vec3(cx, cy, cz);
+        adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
+        adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
+        md.gmass64[poff] += gm64;
+    }
+    const ElemDev &es = md.es[T_TET];
+    const size_t gstride = (size_t)md.E * es.count;
+#pragma unroll
+    for (int j = 0; j < EPT; j++) {
+        if (tr[j].on) {
+            const size_t pe = (size_t)env * es.count + tid + j * blockDim.x;
+#pragma unroll
+            for (int q = 0; q < 3; q++) es.g64[q * gstride + pe] += g64[j][q];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host
+#define GS_RES_CHECK(what)                                           \
+    do {                                                             \
+        cudaError_t e_ = cudaGetLastError();                         \
+        if (e_ != cudaSuccess) return cuda_fail(e_, what);           \
+        g_launches++;                                                \
+    } while (0)
+
+static ResHost *res_of(gs_model *m) { return (ResHost *)m->res_host; }
+
+template <class K>
+static int set_smem(K kern, size_t bytes) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    return e == cudaSuccess ? GS_OK : cuda_fail(e, "cudaFuncSetAttribute (resident)");
+}
+
+int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStream_t st) {
+    const bool fits = resident_fits(d);
+    if (d->plan == GS_PLAN_RESIDENT && !fits) {
+        set_error("the resident plan needs a tets-only mesh with <= %d tets and no more particles than threads", kResMaxTets);
+        return GS_EINVAL;
+    }
+    if (d->plan == GS_PLAN_STREAMING || !fits) { m->plan = GS_PLAN_STREAMING; return GS_OK; }
+    const int N = d->n_particles, M = d->n_tets;
+    const int counts[N_TYPES] = {d->n_tets, d->n_tris, d->n_hinges};
+    const size_t off = workspace_bytes_upper(N, d->n_envs, counts);
+    if (off + resident_blob_bytes(d) > bytes) { set_error("workspace too small for the resident plan"); return GS_EINVAL; }
+    std::vector<int> inv_p(N);
+    for (int i = 0; i < N; i++) inv_p[m->perm_p[i]] = i;
+    std::vector<ushort4> idx(M);
+    std::vector<uint16_t> ptr(N + 1, 0), slots((size_t)4 * M);
+    std::vector<int> cnt(N + 1, 0);
+    for (int e = 0; e < M; e++) {
+        const int32_t *ix = d->tets + (size_t)m->hes[T_TET].perm[e] * 4;
+        const int li[4] = {inv_p[ix[0]], inv_p[ix[1]], inv_p[ix[2]], inv_p[ix[3]]};
+        idx[e] = make_ushort4((unsigned short)li[0], (unsigned short)li[1], (unsigned short)li[2], (unsigned short)li[3]);
+        for (int k = 0; k < 4; k++) cnt[li[k] + 1]++;
+    }
+    for (int p = 0; p < N; p++) cnt[p + 1] += cnt[p];
+    for (int p = 0; p <= N; p++) ptr[p] = (uint16_t)cnt[p];
+    std::vector<int> pos(cnt.begin(), cnt.end() - 1);
+    for (int e = 0; e < M; e++) {
+        const unsigned short li[4] = {idx[e].x, idx[e].y, idx[e].z, idx[e].w};
+        for (int k = 0; k < 4; k++) slots[pos[li[k]]++] = (uint16_t)(k * M + e);
+    }
+    char *p = (char *)d_workspace + off;
+    auto take = [&](size_t n) { char *q = p; p += (n + 255) & ~(size_t)255; return q; };
+    ushort4 *d_idx = (ushort4 *)take(idx.size() * sizeof(ushort4));
+    uint16_t *d_ptr = (uint16_t *)take(ptr.size() * 2);
+    uint16_t *d_slots = (uint16_t *)take(slots.size() * 2);
+    cudaError_t ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * 2, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_slots, slots.data(), slots.size() * 2, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) return cuda_fail(ce, "resident upload");
+    ResHost *rh = new ResHost();
+    rh->ept = M > kResMaxThreads ? 2 : 1;
+    rh->rd.M = M; rh->rd.N = N;
+    rh->rd.nthreads = ((M + rh->ept - 1) / rh->ept + 31) / 32 * 32;
+    rh->rd.idx = d_idx; rh->rd.csr_ptr = d_ptr; rh->rd.csr_slots = d_slots;
+    rh->smem_fwd = res_smem(N, M, 3, false);
+    rh->smem_adj = res_smem(N, M, 6, true);
+    m->res_host = rh;
+    int rc = GS_OK;
+    if (rh->ept == 1 && rh->rd.nthreads <= 320) {
+        rc = set_smem(k_resident_fwd<1, 320, 3>, rh->smem_fwd);
+        if (rc == GS_OK) rc = set_smem(k_resident_adj<1, 320, 2>, rh->smem_adj);
+    } else if (rh->ept == 1) {
+        rc = set_smem(k_resident_fwd<1, 1024, 1>, rh->smem_fwd);
+        if (rc == GS_OK) rc = set_smem(k_resident_adj<1, 1024, 1>, rh->smem_adj);
+    } else {
+        rc = set_smem(k_resident_fwd<2, 1024, 1>, rh->smem_fwd);
+        if (rc == GS_OK) rc = set_smem(k_resident_adj<2, 1024, 1>, rh->smem_adj);
+    }
+    if (rc != GS_OK) return rc;
+    m->plan = GS_PLAN_RESIDENT;
     return GS_OK;
 }
-int resident_rollout(gs_model *, gs_tape *, cudaStream_t) { set_error("resident plan unavailable"); return GS_ESTATE; }
-int resident_rollout_backward(gs_model *, gs_tape *, int, int, const float *, cudaStream_t) { set_error("resident plan unavailable"); return GS_ESTATE; }
+
+void resident_release(gs_model *m) {
+    delete res_of(m);
+    m->res_host = nullptr;
+}
+
+int resident_rollout(gs_model *m, gs_tape *t, cudaStream_t st) {
+    ResHost *rh = res_of(m);
+    if (!rh) { set_error("resident plan unavailable"); return GS_ESTATE; }
+    const dim3 grid(m->E), block(rh->rd.nthreads);
+    cudaEvent_t ta = m->timing ? timing_begin(m, st) : nullptr;
+    if (rh->ept == 1 && rh->rd.nthreads <= 320)
+        k_resident_fwd<1, 320, 3><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
+    else if (rh->ept == 1)
+        k_resident_fwd<1, 1024, 1><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
+    else
+        k_resident_fwd<2, 1024, 1><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
+    GS_RES_CHECK("k_resident_fwd");
+    if (ta) timing_end(m, GS_K_RESIDENT_FWD, ta, st);
+    return GS_OK;
+}
+
+int resident_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames, cudaStream_t st) {
+    ResHost *rh = res_of(m);
+    if (!rh) { set_error("resident plan unavailable"); return GS_ESTATE; }
+    const dim3 grid(m->E), block(rh->rd.nthreads);
+    const float *fr = n_frames > 0 ? d_adj_x_frames : nullptr;
+    const int stride = frame_stride > 0 ? frame_stride : 1;
+    cudaEvent_t ta = m->timing ? timing_begin(m, st) : nullptr;
+    if (rh->ept == 1 && rh->rd.nthreads <= 320)
+        k_resident_adj<1, 320, 2><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
+    else if (rh->ept == 1)
+        k_resident_adj<1, 1024, 1><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
+    else
+        k_resident_adj<2, 1024, 1><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
+    GS_RES_CHECK("k_resident_adj");
+    if (ta) timing_end(m, GS_K_RESIDENT_ADJ, ta, st);
+    return GS_OK;
+}
+
 }  // namespace gs

@@ -82,6 +82,60 @@ def test_small_rollout_and_gradients(config, plan):
         assert rel_inf(got["g_" + g], ref["g_" + g]) <= TOL_GRAD, g
 
 
+@pytest.mark.parametrize("config", [0, 3])
+def test_resident_plan_rollout_and_gradients(config):
+    """The persistent one-CTA-per-environment plan (tets-only meshes that fit a CTA): same parity bar, plan AUTO
+    must pick it, and it must agree with the streaming plan far inside the tolerance (same arithmetic, other
+    summation order)."""
+    sc = scenes.make_scene(config, small=True)
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"], plan=gs.GS_PLAN_RESIDENT)
+    assert got["model"].plan == gs.GS_PLAN_RESIDENT and got["bad"] == -1
+    assert gs.Model(sc).plan == gs.GS_PLAN_RESIDENT
+    ext = sc.extent()
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
+    assert np.abs(got["rec_x"] - ref["rec_x"]).max() <= TOL_ROLLOUT * ext
+    assert rel_inf(got["loss"], ref["loss"]) <= 5e-3
+    stream = gpu_run_scene(sc, ref["target"], plan=gs.GS_PLAN_STREAMING)
+    assert np.abs(got["xT"] - stream["xT"]).max() <= 1e-4 * ext
+    for k in ["adj_x0", "adj_v0"] + ["g_" + g for g in _grad_groups(sc)]:
+        if config == 3 and k.startswith("g_"):
+            a, b = got[k].sum(1), ref[k].sum(1)
+            assert np.abs(a - b).max() <= TOL_GRAD * np.abs(b).max(), k
+        assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
+
+
+def test_resident_plan_edge_cases():
+    x = np.array([[0, 0.01, 0], [0.1, 0.01, 0], [0, 0.11, 0], [0, 0.01, 0.1]], float)
+    # a single tet (4 particles, one warp) rolls out resident and matches the oracle
+    sc = scenes.custom_scene(x, tets=[[0, 1, 2, 3]], n_substeps=96)
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"], plan=gs.GS_PLAN_RESIDENT)
+    assert got["model"].plan == gs.GS_PLAN_RESIDENT
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * max(sc.extent(), 0.1)
+    for k in ("adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_mass"):
+        assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
+    # a mesh with triangles cannot run resident: explicit request fails, AUTO falls back to streaming
+    sc1 = scenes.make_scene(1, small=True)
+    with pytest.raises(gs.GradSimError) as e:
+        gs.Model(sc1, plan=gs.GS_PLAN_RESIDENT)
+    assert e.value.code == gs.GS_EINVAL
+    assert gs.Model(sc1).plan == gs.GS_PLAN_STREAMING
+    # a checkpointed tape of a resident model runs the streaming loop and gives the same answer
+    sc0 = scenes.make_scene(0, small=True)
+    ref0 = orc.run_scene(sc0)
+    a = gpu_run_scene(sc0, ref0["target"], K=1, plan=gs.GS_PLAN_RESIDENT)
+    b = gpu_run_scene(sc0, ref0["target"], K=16, plan=gs.GS_PLAN_RESIDENT)
+    assert np.abs(a["xT"] - b["xT"]).max() <= 1e-4 * sc0.extent()
+    for k in ("adj_x0", "g_tet_mu", "g_mass"):
+        assert rel_inf(b[k], ref0[k]) <= TOL_GRAD, k
+    # non-finite states are reported with their substep by the resident kernel too
+    m = a["model"]
+    tape = m.tape(8)
+    tape.rollout(dev(sc0.x0), dev(np.full(sc0.x0.shape, 3e38, np.float32)))
+    assert m.check_finite() == 0
+
+
 def test_checkpointed_backward_matches_full_tape():
     """Segment replay regenerates the same states, so K only changes which fp32 sums are flushed when."""
     sc = scenes.make_scene(2, small=True)
