@@ -194,6 +194,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--plan", type=int, default=0)
+    ap.add_argument("--substeps", type=int, default=0, help="override the rollout length (profiling runs only; recorded in config)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -220,6 +221,8 @@ def main():
         torch.cuda.synchronize()
 
     sc = make_workload(args.config, args.small)
+    if args.substeps > 0:
+        sc.n_substeps = args.substeps
     E, N, T, K = sc.n_envs, sc.n_particles, sc.n_substeps, sc.checkpoint_every
     m = gs.Model(sc, plan=args.plan, device=devs)
     tape = m.tape(T, K)
@@ -296,8 +299,14 @@ def main():
         gs._check(L.gs_kernel_times(m.h, gs._stream(), len(KERNELS), ms_k, n_k))
         L.gs_kernel_timing(m.h, 0)
         tot = sum(ms_k)
+        # the streaming plan launches one element kernel per non-empty element type: "us_avg" of the element rows is
+        # per SUBSTEP (all types together), so that it pairs with the whole element stream's algorithmic bytes
+        n_types = 1  # all element types of a substep share one persistent launch
         for name, a, b in zip(KERNELS, ms_k, n_k):
-            kernels[name] = {"launches": int(b), "ms_total": a, "us_avg": (1e3 * a / b) if b else None, "share": a / tot if tot else None}
+            per = n_types if name in ("k_elements_fwd", "k_elements_adj") else 1
+            kernels[name] = {"launches": int(b), "ms_total": a, "us_avg": (1e3 * a * per / b) if b else None, "share": a / tot if tot else None}
+            if per > 1:
+                kernels[name]["launches_per_substep"] = per
         alg = {"k_elements_fwd": element_stream_bytes(sc, BYTES_FWD), "k_elements_adj": element_stream_bytes(sc, BYTES_ADJ),
                "k_particles_fwd": E * N * BYTES_FWD["particle"], "k_particles_adj": E * N * BYTES_ADJ["particle"]}
         # resident plan: one launch covers all T substeps; streaming byte model (state in and out every substep) and flops
@@ -348,7 +357,7 @@ def main():
         "metric": METRIC, "value": units_per_step * world / step_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * step_s, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": sc.name, "config_index": args.config, "particles": N, "tets": int(sc.tets.shape[0]), "tris": int(sc.tris.shape[0]),
-                   "hinges": int(sc.hinges.shape[0]), "envs": E, "substeps": T, "checkpoint_every": K, "plan": m.plan,
+                   "hinges": int(sc.hinges.shape[0]), "envs": E, "substeps": T, "substeps_overridden": bool(args.substeps), "checkpoint_every": K, "plan": m.plan,
                    "l2": "inputs larger than L2 (state tape + element streams stream from HBM every step)" if tape.nbytes > 3e8 else "working set may sit in L2",
                    "friction_reading": "BASELINE kf -> mu_c, k_f = 50 (DESIGN.md A9)", "parallelism": f"replicas x{world}"},
         "forward": {"value": units_per_step * world / fwd_s, "unit": UNIT, "ms_per_step": 1e3 * fwd_s,

@@ -50,21 +50,20 @@ __device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], cons
     tet_kin(x[0], x[1], x[2], x[3], b, k);
     vec3 g1, g2, g3;
     mat_cols_times_B(v[1] - v[0], v[2] - v[0], v[3] - v[0], b, g1, g2, g3);
+    // -V is folded into the three scalar coefficients, so the columns below are those of -V P
     const float s1 = k.Ic / (k.Ic + 1.0f);
-    const float ce = lam * (k.J - 1.0f) - 0.75f * mu;  // = lambda (J - alpha), alpha = 1 + 3mu/(4 lambda)  (A1)
-    const float ms = mu * s1;
-    // S = sym(F^T Fdot)
-    const float s11 = dot(k.f1, g1), s22 = dot(k.f2, g2), s33 = dot(k.f3, g3);
-    const float s12 = 0.5f * (dot(k.f1, g2) + dot(k.f2, g1));
-    const float s13 = 0.5f * (dot(k.f1, g3) + dot(k.f3, g1));
-    const float s23 = 0.5f * (dot(k.f2, g3) + dot(k.f3, g2));
-    vec3 p1 = madd(ms * k.f1, ce, k.c1), p2 = madd(ms * k.f2, ce, k.c2), p3 = madd(ms * k.f3, ce, k.c3);
-    p1 += kd * madd(madd(s11 * k.f1, s12, k.f2), s13, k.f3);
-    p2 += kd * madd(madd(s12 * k.f1, s22, k.f2), s23, k.f3);
-    p3 += kd * madd(madd(s13 * k.f1, s23, k.f2), s33, k.f3);
-    vec3 h1, h2, h3;
-    mat_cols_times_Bt(p1, p2, p3, b, h1, h2, h3);
-    f[1] = -V * h1; f[2] = -V * h2; f[3] = -V * h3;
+    const float ce = -V * (lam * (k.J - 1.0f) - 0.75f * mu);  // lambda (J - alpha), alpha = 1 + 3mu/(4 lambda)  (A1)
+    const float ms = -V * mu * s1;
+    const float kv = -V * kd, kh = 0.5f * kv;
+    // kv S, S = sym(F^T Fdot)
+    const float s11 = kv * dot(k.f1, g1), s22 = kv * dot(k.f2, g2), s33 = kv * dot(k.f3, g3);
+    const float s12 = kh * (dot(k.f1, g2) + dot(k.f2, g1));
+    const float s13 = kh * (dot(k.f1, g3) + dot(k.f3, g1));
+    const float s23 = kh * (dot(k.f2, g3) + dot(k.f3, g2));
+    const vec3 p1 = madd(madd(madd(madd(ms * k.f1, ce, k.c1), s11, k.f1), s12, k.f2), s13, k.f3);
+    const vec3 p2 = madd(madd(madd(madd(ms * k.f2, ce, k.c2), s12, k.f1), s22, k.f2), s23, k.f3);
+    const vec3 p3 = madd(madd(madd(madd(ms * k.f3, ce, k.c3), s13, k.f1), s23, k.f2), s33, k.f3);
+    mat_cols_times_Bt(p1, p2, p3, b, f[1], f[2], f[3]);
     f[0] = -(f[1] + f[2] + f[3]);
 }
 
@@ -180,23 +179,43 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
 // ------------------------------------------------------------------------------------------ hinges
 // vertices: x[0], x[1] wings; x[2], x[3] the shared edge.  theta = signed dihedral (0 when flat);
 // f_i = k_b l0 sin((theta - theta0)/2) d_i, d_i = -d(theta)/dx_i (Bridson directions).
+// Rest constants per hinge: s0h = sin(theta0/2), c0h = cos(theta0/2), kl = k_b * l0 (fp64 on the host).
+__device__ __forceinline__ float rcp_fast(float x) {  // MUFU.RCP, <= 1 ulp: geometry of well-shaped hinges only (not contact, hazard H3)
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 struct HingeGeo {
     vec3 p13, p14, p23, p24, n1, n2, eh, m1, m2;
-    float L, n1s, n2s, c13, c14, c23, c24, theta;
+    float L, iL, i1, i2, c13, c14, c23, c24, sh, ch;  // sh, ch = sin, cos of (theta - theta0)/2
 };
-__device__ __forceinline__ void hinge_geo(const vec3 x[4], HingeGeo &h) {
+__device__ __forceinline__ void hinge_geo(const vec3 x[4], float s0h, float c0h, HingeGeo &h) {
     h.p13 = x[0] - x[2]; h.p14 = x[0] - x[3]; h.p23 = x[1] - x[2]; h.p24 = x[1] - x[3];
     h.n1 = cross(h.p13, h.p14); h.n2 = cross(h.p24, h.p23);
     const vec3 e = x[3] - x[2];
-    h.L = sqrtf(dot(e, e));
-    h.eh = (1.0f / h.L) * e;
-    h.n1s = dot(h.n1, h.n1); h.n2s = dot(h.n2, h.n2);
-    h.m1 = (1.0f / h.n1s) * h.n1; h.m2 = (1.0f / h.n2s) * h.n2;
+    const float L2 = dot(e, e);
+    h.iL = rsqrtf(L2);
+    h.L = L2 * h.iL;
+    h.eh = h.iL * e;
+    const float n1s = dot(h.n1, h.n1), n2s = dot(h.n2, h.n2);
+    h.i1 = rcp_fast(n1s); h.i2 = rcp_fast(n2s);
+    h.m1 = h.i1 * h.n1; h.m2 = h.i2 * h.n2;
     h.c13 = dot(h.p13, h.eh); h.c14 = dot(h.p14, h.eh); h.c23 = dot(h.p23, h.eh); h.c24 = dot(h.p24, h.eh);
-    // atan2 then sin of the half angle: no 1 - cos(theta) cancellation on flat cloth (hazard H1)
-    const float inv = rsqrtf(h.n1s * h.n2s);
+    // (sin, cos) of theta, then the half angle by the branch that does not cancel (hazard H1: never
+    // sqrt((1 - cos theta)/2) near theta = 0, where flat cloth lives), then the rest-angle shift -- no atan2 / sin
+    const float inv = rsqrtf(n1s * n2s);
     const float sn = dot(cross(h.n1, h.n2), h.eh) * inv, cs = dot(h.n1, h.n2) * inv;
-    h.theta = atan2f(sn, cs);
+    float sht, cht;
+    if (cs >= 0.0f) {
+        cht = sqrtf(0.5f * (1.0f + cs));
+        sht = 0.5f * sn * rcp_fast(cht);
+    } else {
+        const float a = sqrtf(0.5f * (1.0f - cs));
+        sht = copysignf(a, sn);
+        cht = 0.5f * fabsf(sn) * rcp_fast(a);
+    }
+    h.sh = sht * c0h - cht * s0h;
+    h.ch = cht * c0h + sht * s0h;
 }
 __device__ __forceinline__ void hinge_dirs(const HingeGeo &h, vec3 d[4]) {
     d[0] = h.L * h.m1;
@@ -204,18 +223,18 @@ __device__ __forceinline__ void hinge_dirs(const HingeGeo &h, vec3 d[4]) {
     d[2] = madd(h.c14 * h.m1, h.c24, h.m2);
     d[3] = -madd(h.c13 * h.m1, h.c23, h.m2);
 }
-__device__ __forceinline__ void hinge_force(const vec3 x[4], float theta0, float l0, float kb, vec3 f[4]) {
+__device__ __forceinline__ void hinge_force(const vec3 x[4], float s0h, float c0h, float kl, vec3 f[4]) {
     HingeGeo h;
-    hinge_geo(x, h);
+    hinge_geo(x, s0h, c0h, h);
     vec3 d[4];
     hinge_dirs(h, d);
-    const float s = kb * l0 * sinf(0.5f * (h.theta - theta0));
+    const float s = kl * h.sh;
     f[0] = s * d[0]; f[1] = s * d[1]; f[2] = s * d[2]; f[3] = s * d[3];
 }
 // VJP = JVP (the force is conservative): ax_j = -E'' s d_j + E' Dd_j[a], s = sum_i d_i . a_i
-__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float theta0, float l0, float kb, vec3 ax[4]) {
+__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float s0h, float c0h, float kl, vec3 ax[4]) {
     HingeGeo h;
-    hinge_geo(x, h);
+    hinge_geo(x, s0h, c0h, h);
     vec3 d[4];
     hinge_dirs(h, d);
     const vec3 q13 = a[0] - a[2], q14 = a[0] - a[3], q23 = a[1] - a[2], q24 = a[1] - a[3];
@@ -223,18 +242,15 @@ __device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], 
     const vec3 dn2 = cross(q24, h.p23) + cross(h.p24, q23);
     const vec3 de = a[3] - a[2];
     const float dL = dot(h.eh, de);
-    const vec3 deh = (1.0f / h.L) * (de - dL * h.eh);
-    const float i1 = 1.0f / h.n1s, i2 = 1.0f / h.n2s;
-    const vec3 dm1 = i1 * (dn1 - (2.0f * dot(h.n1, dn1) * i1) * h.n1);
-    const vec3 dm2 = i2 * (dn2 - (2.0f * dot(h.n2, dn2) * i2) * h.n2);
+    const vec3 deh = h.iL * (de - dL * h.eh);
+    const vec3 dm1 = h.i1 * (dn1 - (2.0f * dot(h.n1, dn1) * h.i1) * h.n1);
+    const vec3 dm2 = h.i2 * (dn2 - (2.0f * dot(h.n2, dn2) * h.i2) * h.n2);
     const float dc13 = dot(q13, h.eh) + dot(h.p13, deh), dc14 = dot(q14, h.eh) + dot(h.p14, deh);
     const float dc23 = dot(q23, h.eh) + dot(h.p23, deh), dc24 = dot(q24, h.eh) + dot(h.p24, deh);
     // s = sum_i d_i . a_i written with cotangent differences only (sum_i d_i = 0): the adjoint field is smooth,
     // so the plain sum cancels to ~1e-4 of its terms and would lose that many digits in fp32
     const float s = dot(h.m1, h.c13 * q14 - h.c14 * q13) + dot(h.m2, h.c23 * q24 - h.c24 * q23);
-    float sn, cs;
-    sincosf(0.5f * (h.theta - theta0), &sn, &cs);
-    const float E1 = kb * l0 * sn, E2s = 0.5f * kb * l0 * cs * s;
+    const float E1 = kl * h.sh, E2s = 0.5f * kl * h.ch * s;
     ax[0] = madd(-E2s * d[0], E1, madd(dL * h.m1, h.L, dm1));
     ax[1] = madd(-E2s * d[1], E1, madd(dL * h.m2, h.L, dm2));
     ax[2] = madd(-E2s * d[2], E1, madd(madd(madd(dc14 * h.m1, h.c14, dm1), dc24, h.m2), h.c24, dm2));

@@ -13,24 +13,55 @@ namespace gs {
 enum { T_TET = 0, T_TRI = 1, T_HINGE = 2, N_TYPES = 3 };
 static const int kArity[N_TYPES] = {4, 3, 4};
 
-constexpr int kTileElems = 256;      // elements per tile = threads per CTA of the streaming element kernels
+constexpr int kTileElems = 128;      // elements per tile = threads per CTA of the streaming element kernels
 constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
+
+// Byte layout of one tile's RECORD: everything static a tile of kTileElems elements needs, packed contiguously so
+// that ONE bulk copy (cp.async.bulk, TMA) brings it into shared memory:
+//   lidx   ushort4[256]  tile-local particle indices (w unused for triangles)
+//   c0     float4[256]   tets: B[0..3]; tris: 2x2 B; hinges: (sin(theta0/2), cos(theta0/2), kb * l0, -)
+//   c1     float4[256]   tets: B[4..7]
+//   c2     float2[256]   tets: (B[8], V)
+//   area   float[256]    tris: rest area
+//   slots  u16[arity*256] gather list: slot = k * 256 + local element, grouped by CHUNK: the element-vertices of one
+//                        tile-particle, cut into runs of at most kChunk so that the summation is spread over all
+//                        threads of the CTA with near-uniform trip counts (longest runs first)
+//   chunk_end  u16[cmax] end of each chunk's run in `slots`
+//   chunk_part u16[cmax] tile-local particle index of each chunk (0xFFFF = padding)
+template <int TYPE>
+struct RecLayout {
+    static constexpr int kArityT = TYPE == 1 ? 3 : 4;
+    static constexpr int oLidx = 0;
+    static constexpr int oC0 = kTileElems * 8;
+    static constexpr int oC1 = oC0 + kTileElems * 16;
+    static constexpr int oC2 = oC1 + (TYPE == 0 ? kTileElems * 16 : 0);
+    static constexpr int oArea = oC2 + (TYPE == 0 ? kTileElems * 8 : 0);
+    static constexpr int oSlots = oArea + (TYPE == 1 ? kTileElems * 4 : 0);
+    static constexpr int oChunkEnd = oSlots + kArityT * kTileElems * 2;
+    __host__ __device__ static constexpr int bytes(int cmax) { return oChunkEnd + cmax * 4; }
+};
+inline int rec_bytes_of(int type, int cmax) {
+    return type == 0 ? RecLayout<0>::bytes(cmax) : (type == 1 ? RecLayout<1>::bytes(cmax) : RecLayout<2>::bytes(cmax));
+}
+constexpr int kChunk = 8;  // longest run of slots one thread sums
+constexpr int kParBytes = 3 * kTileElems * 4;  // one tile's (mu | lambda | k_damp) block of one environment
 
 // Device view of one element set (tets, triangles or hinges) in INTERNAL (Morton, tiled) order.
 struct ElemDev {
-    int count, n_tiles, max_tile_parts;
-    const ushort4 *lidx;        // [count] tile-local particle indices (w unused for triangles)
-    const int *tile_part_ptr;   // [n_tiles + 1]
-    const int *tile_parts;      // internal particle ids of each tile's particles (ascending)
-    const uint16_t *csr_end;    // per tile-particle: end offset into the tile's slot list
-    const uint16_t *csr_slots;  // [n_tiles][arity * kTileElems] slot = k * kTileElems + local element
-    const float4 *c0, *c1;      // tets: B[0..3], B[4..7]; tris: B[0..3], (A,-,-,-); hinges: (theta0, l0, kb, -)
-    const float2 *c2;           // tets: (B[8], V)
-    const float *mu, *lam, *damp;  // [E][count]
-    float *g32;                 // [3][E][count] per-substep fp32 accumulators (mu, lambda, damp)
-    double *g64;                // [3][E][count] fp64 masters
+    int count, cpad, n_tiles, pmax;  // cpad = n_tiles * kTileElems; pmax: particle slots per tile (multiple of 8)
+    int cmax;                   // chunks per tile (multiple of 8, >= the tile with most chunks)
+    int rec_bytes;              // RecLayout<type>::bytes(cmax)
+    const char *rec;            // [n_tiles][rec_bytes]
+    const int *tile_parts;      // [n_tiles][pmax] internal particle ids, most-referenced first, -1 padded
+    float *par;                 // [E][n_tiles][3][kTileElems]  mu, lambda, k_damp (tets, tris)
+    float *g32;                 // [3][E][cpad] per-substep fp32 accumulators (mu, lambda, damp)
+    double *g64;                // [3][E][cpad] fp64 masters
     const int *perm;            // [count] internal -> caller element index
 };
+// index of parameter q (0 mu, 1 lambda, 2 damp) of internal element e of environment env inside ElemDev::par
+__host__ __device__ inline size_t par_index(int n_tiles, int env, int e, int q) {
+    return (((size_t)env * n_tiles + (e / kTileElems)) * 3 + q) * kTileElems + (e % kTileElems);
+}
 
 struct ModelDev {
     int N, E;
@@ -47,7 +78,7 @@ struct ModelDev {
 };
 
 struct HostElemSet {
-    int count = 0, n_tiles = 0, max_tile_parts = 0;
+    int count = 0, cpad = 0, n_tiles = 0, max_tile_parts = 0, pmax = 0, cmax = 0;
     std::vector<int> perm;  // internal -> caller
 };
 
@@ -66,9 +97,11 @@ struct gs_model {
     float4 *d_adjx = nullptr, *d_adjv = nullptr, *d_adjf = nullptr;
     // mutable copies of device pointers the API writes
     float *d_inv_mass = nullptr;
-    float *d_param[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int steps_since_flush = 0;
-    int fwd_smem = 0, adj_smem = 0;
+    int n_sms = 148;
+    int smem_fwd = 0, smem_adj = 0;  // dynamic shared memory of the element kernels
+    int occ_fwd = 1, occ_adj = 1;    // co-resident CTAs per SM
+    long long elem_items = 0;        // work items (tile x environment) of the largest element type
     int step_counter = 0;  // substep index written to dev.bad on a non-finite state
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
     void *res_host = nullptr;

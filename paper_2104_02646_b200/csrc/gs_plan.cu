@@ -48,12 +48,9 @@ struct Bump {
 
 struct Layout {
     // per type
-    ushort4 *lidx[N_TYPES];
-    int *tile_part_ptr[N_TYPES], *tile_parts[N_TYPES], *perm[N_TYPES];
-    uint16_t *csr_end[N_TYPES], *csr_slots[N_TYPES];
-    float4 *c0[N_TYPES], *c1[N_TYPES];
-    float2 *c2[N_TYPES];
-    float *mu[N_TYPES], *lam[N_TYPES], *damp[N_TYPES], *g32[N_TYPES];
+    char *rec[N_TYPES];
+    int *tile_parts[N_TYPES], *perm[N_TYPES];
+    float *par[N_TYPES], *g32[N_TYPES];
     double *g64[N_TYPES];
     int *perm_p, *bad;
     float *inv_mass, *gmass32, *ke, *kd, *kf, *muc;
@@ -67,23 +64,16 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     Bump b(base);
     const size_t EN = (size_t)E * N;
     for (int t = 0; t < N_TYPES; t++) {
-        const size_t c = counts[t], a = kArity[t], nt = (c + kTileElems - 1) / kTileElems;
-        L.lidx[t] = b.take<ushort4>(c);
-        L.tile_part_ptr[t] = b.take<int>(nt + 1);
-        L.tile_parts[t] = b.take<int>(a * c);
-        L.csr_end[t] = b.take<uint16_t>(a * c);
-        L.csr_slots[t] = b.take<uint16_t>(nt * a * kTileElems);
-        L.c0[t] = b.take<float4>(c);
-        L.c1[t] = t == T_HINGE ? nullptr : b.take<float4>(c);
-        L.c2[t] = t == T_TET ? b.take<float2>(c) : nullptr;
+        const size_t c = counts[t], a = kArity[t], nt = (c + kTileElems - 1) / kTileElems, cp = nt * kTileElems;
+        // upper bounds (pmax <= arity * kTileElems is only known after the mesh has been tiled)
+        L.rec[t] = b.take<char>(nt * (size_t)rec_bytes_of(t, (int)a * kTileElems));
+        L.tile_parts[t] = b.take<int>(a * cp);
         if (t != T_HINGE) {
-            L.mu[t] = b.take<float>(E * c);
-            L.lam[t] = b.take<float>(E * c);
-            L.damp[t] = b.take<float>(E * c);
-            L.g32[t] = b.take<float>(3 * E * c);
-            L.g64[t] = b.take<double>(3 * E * c);
+            L.par[t] = b.take<float>(3 * E * cp);
+            L.g32[t] = b.take<float>(3 * E * cp);
+            L.g64[t] = b.take<double>(3 * E * cp);
         } else {
-            L.mu[t] = L.lam[t] = L.damp[t] = L.g32[t] = nullptr;
+            L.par[t] = L.g32[t] = nullptr;
             L.g64[t] = nullptr;
         }
         L.perm[t] = b.take<int>(c);
@@ -207,8 +197,6 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         hs.count = c; hs.n_tiles = nt; hs.max_tile_parts = 0;
         hs.perm.resize(c);
         std::vector<uint64_t> ekey(c);
-        std::vector<float4> c0(c), c1(t == T_HINGE ? 0 : c);
-        std::vector<float2> c2(t == T_TET ? c : 0);
         // rest quantities in caller order first
         std::vector<float4> r0(c), r1(c);
         std::vector<float2> r2(c);
@@ -242,89 +230,131 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                 if (!(l0 > 0) || !(a1 > 1e-12) || !(a2 > 1e-12)) { set_error("hinge %d: degenerate rest shape", e); return GS_EMESH; }
                 d3 eh = scl(1.0 / l0, ed);
                 double th = std::atan2(dt3(crs(scl(1 / a1, n1), scl(1 / a2, n2)), eh), dt3(n1, n2) / (a1 * a2));
-                r0[e] = make_float4((float)th, (float)l0, d->hinge_kb[e], 0.f);
+                r0[e] = make_float4((float)std::sin(0.5 * th), (float)std::cos(0.5 * th), (float)((double)d->hinge_kb[e] * l0), 0.f);
             }
         }
         std::iota(hs.perm.begin(), hs.perm.end(), 0);
         std::stable_sort(hs.perm.begin(), hs.perm.end(), [&](int x, int y) { return ekey[x] < ekey[y]; });
-        for (int e = 0; e < c; e++) {
-            c0[e] = r0[hs.perm[e]];
-            if (t != T_HINGE) c1[e] = r1[hs.perm[e]];
-            if (t == T_TET) c2[e] = r2[hs.perm[e]];
-        }
-        // tiles
-        std::vector<ushort4> lidx(c);
-        std::vector<int> tpp(nt + 1, 0), tparts;
-        std::vector<uint16_t> csr_end, csr_slots((size_t)nt * a * kTileElems, 0);
-        tparts.reserve((size_t)c * 2);
-        std::vector<int> ids, cnt, pos;
+        const int cp = nt * kTileElems;
+        hs.cpad = cp;
+        // tiles, pass 1: the particles of each tile, most-referenced first (near-uniform trip counts per warp in the
+        // kernels' gather loops), and the fullest tile
+        std::vector<std::vector<int>> tids(nt);
+        std::vector<std::vector<int>> tcnt(nt);
+        std::vector<int> ids, cnt, order;
         for (int j = 0; j < nt; j++) {
             const int e0 = j * kTileElems, e1 = std::min(c, e0 + kTileElems);
             ids.clear();
             for (int e = e0; e < e1; e++)
                 for (int k = 0; k < a; k++) ids.push_back(inv_p[conn[t][(size_t)hs.perm[e] * a + k]]);
             std::sort(ids.begin(), ids.end());
-            ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
-            const int P_ = (int)ids.size();
-            hs.max_tile_parts = std::max(hs.max_tile_parts, P_);
-            cnt.assign(P_ + 1, 0);
+            std::vector<int> uniq, ucnt;
+            for (size_t q = 0; q < ids.size();) {
+                size_t q1 = q;
+                while (q1 < ids.size() && ids[q1] == ids[q]) q1++;
+                uniq.push_back(ids[q]); ucnt.push_back((int)(q1 - q));
+                q = q1;
+            }
+            order.resize(uniq.size());
+            std::iota(order.begin(), order.end(), 0);
+            std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return ucnt[x] > ucnt[y]; });
+            tids[j].resize(uniq.size()); tcnt[j].resize(uniq.size());
+            for (size_t q = 0; q < uniq.size(); q++) { tids[j][q] = uniq[order[q]]; tcnt[j][q] = ucnt[order[q]]; }
+            hs.max_tile_parts = std::max(hs.max_tile_parts, (int)uniq.size());
+        }
+        const int pmax = std::max(8, (hs.max_tile_parts + 7) / 8 * 8);
+        hs.pmax = pmax;
+        int max_chunks = 0;
+        for (int j = 0; j < nt; j++) {
+            int nc = 0;
+            for (int v : tcnt[j]) nc += (v + kChunk - 1) / kChunk;
+            max_chunks = std::max(max_chunks, nc);
+        }
+        const int cmax = std::max(8, (max_chunks + 7) / 8 * 8);
+        hs.cmax = cmax;
+        // pass 2: one packed record per tile (RecLayout), fixed-stride particle lists
+        const int rb = rec_bytes_of(t, cmax);
+        const int oC0 = kTileElems * 8, oC1 = oC0 + kTileElems * 16, oC2 = oC1 + (t == T_TET ? kTileElems * 16 : 0);
+        const int oArea = oC2 + (t == T_TET ? kTileElems * 8 : 0), oSlots = oArea + (t == T_TRI ? kTileElems * 4 : 0);
+        const int oChunkEnd = oSlots + a * kTileElems * 2;
+        std::vector<char> rec((size_t)nt * rb, 0);
+        std::vector<int> tparts((size_t)nt * pmax, -1);
+        std::vector<int> pos;
+        for (int j = 0; j < nt; j++) {
+            const int e0 = j * kTileElems, e1 = std::min(c, e0 + kTileElems);
+            const int P_ = (int)tids[j].size();
+            char *R = rec.data() + (size_t)j * rb;
+            ushort4 *lidx = (ushort4 *)R;
+            float4 *q0 = (float4 *)(R + oC0), *q1 = (float4 *)(R + oC1);
+            float2 *q2 = (float2 *)(R + oC2);
+            float *qa = (float *)(R + oArea);
+            uint16_t *slots = (uint16_t *)(R + oSlots), *chunk_end = (uint16_t *)(R + oChunkEnd), *chunk_part = chunk_end + cmax;
+            // local index of a global id: sorted (id, local) pairs
+            std::vector<std::pair<int, int>> look(P_);
+            for (int q = 0; q < P_; q++) look[q] = {tids[j][q], q};
+            std::sort(look.begin(), look.end());
+            // chunks: full runs of kChunk first, then the remainders, longest first; pos[q] = next free slot of particle q
+            std::vector<std::pair<int, int>> chunks;  // (particle, length)
+            for (int q = 0; q < P_; q++)
+                for (int r = tcnt[j][q]; r > 0; r -= kChunk) chunks.push_back({q, std::min(r, kChunk)});
+            std::stable_sort(chunks.begin(), chunks.end(), [](const std::pair<int, int> &x, const std::pair<int, int> &y) { return x.second > y.second; });
+            // slot ranges of the chunks, in chunk order; a particle's chunks take consecutive pieces of its incidences
+            std::vector<int> cbeg(chunks.size());
+            int run = 0;
+            for (size_t k = 0; k < chunks.size(); k++) { cbeg[k] = run; run += chunks[k].second; }
+            for (int k = 0; k < cmax; k++) {
+                chunk_end[k] = (uint16_t)(k < (int)chunks.size() ? cbeg[k] + chunks[k].second : run);
+                chunk_part[k] = (uint16_t)(k < (int)chunks.size() ? chunks[k].first : 0xFFFF);
+            }
+            // per particle: queue of (next slot position, remaining in chunk) over its chunks
+            std::vector<std::vector<int>> pslots(P_);
+            for (size_t k = 0; k < chunks.size(); k++)
+                for (int r = 0; r < chunks[k].second; r++) pslots[chunks[k].first].push_back(cbeg[k] + r);
+            pos.assign(P_ + 1, 0);  // pos[q]: how many incidences of particle q have been placed
+            for (int q = 0; q < P_; q++) tparts[(size_t)j * pmax + q] = tids[j][q];
             for (int e = e0; e < e1; e++) {
                 unsigned short li[4] = {0, 0, 0, 0};
                 for (int k = 0; k < a; k++) {
-                    int gi = inv_p[conn[t][(size_t)hs.perm[e] * a + k]];
-                    int lp = (int)(std::lower_bound(ids.begin(), ids.end(), gi) - ids.begin());
+                    const int gi = inv_p[conn[t][(size_t)hs.perm[e] * a + k]];
+                    const int lp = std::lower_bound(look.begin(), look.end(), std::make_pair(gi, -1))->second;
                     li[k] = (unsigned short)lp;
-                    cnt[lp + 1]++;
+                    slots[pslots[lp][pos[lp]++]] = (uint16_t)(k * kTileElems + (e - e0));
                 }
-                lidx[e] = make_ushort4(li[0], li[1], li[2], li[3]);
+                lidx[e - e0] = make_ushort4(li[0], li[1], li[2], li[3]);
+                q0[e - e0] = r0[hs.perm[e]];
+                if (t == T_TET) { q1[e - e0] = r1[hs.perm[e]]; q2[e - e0] = r2[hs.perm[e]]; }
+                if (t == T_TRI) qa[e - e0] = r1[hs.perm[e]].x;
             }
-            for (int p = 0; p < P_; p++) cnt[p + 1] += cnt[p];
-            pos.assign(cnt.begin(), cnt.end() - 1);
-            uint16_t *slots = csr_slots.data() + (size_t)j * a * kTileElems;
-            for (int e = e0; e < e1; e++) {
-                const unsigned short li[4] = {lidx[e].x, lidx[e].y, lidx[e].z, lidx[e].w};
-                for (int k = 0; k < a; k++) slots[pos[li[k]]++] = (uint16_t)(k * kTileElems + (e - e0));
-            }
-            for (int p = 0; p < P_; p++) { tparts.push_back(ids[p]); csr_end.push_back((uint16_t)cnt[p + 1]); }
-            tpp[j + 1] = (int)tparts.size();
         }
-        UP(L.lidx[t], lidx); UP(L.tile_part_ptr[t], tpp); UP(L.tile_parts[t], tparts); UP(L.csr_end[t], csr_end);
-        UP(L.csr_slots[t], csr_slots); UP(L.c0[t], c0);
-        if (t != T_HINGE) UP(L.c1[t], c1);
-        if (t == T_TET) UP(L.c2[t], c2);
+        UP(L.rec[t], rec); UP(L.tile_parts[t], tparts);
         UP(L.perm[t], hs.perm);
-        // per-env element parameters in internal order
+        // per-env element parameters: [E][n_tiles][3][kTileElems] (padding holds harmless finite values)
         if (t != T_HINGE) {
             const float *src[3] = {t == T_TET ? d->tet_mu : d->tri_mu, t == T_TET ? d->tet_lambda : d->tri_lambda, t == T_TET ? d->tet_damp : d->tri_damp};
-            float *dst[3] = {L.mu[t], L.lam[t], L.damp[t]};
-            std::vector<float> v((size_t)E * c);
-            for (int q = 0; q < 3; q++) {
+            std::vector<float> v((size_t)3 * E * cp, 1.0f);
+            for (int q = 0; q < 3; q++)
                 for (int env = 0; env < E; env++)
                     for (int e = 0; e < c; e++) {
                         float val = (d->param_layout & GS_ELEM_PER_ENV) ? src[q][(size_t)env * c + hs.perm[e]] : src[q][hs.perm[e]];
                         if (!std::isfinite(val)) { set_error("%s parameter %d of element %d is not finite", tname[t], q, hs.perm[e]); return GS_EINVAL; }
                         if (q == 1 && !(val > 0.0f)) { set_error("%s %d: lambda must be > 0", tname[t], hs.perm[e]); return GS_EINVAL; }
-                        v[(size_t)env * c + e] = val;
+                        v[par_index(nt, env, e, q)] = val;
                     }
-                UP(dst[q], v);
-            }
-            if (c > 0) {  // an empty set owns one placeholder element only: clearing E * 1 entries would run into its neighbours
-                cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * c, stream);
-                if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * c, stream);
+            UP(L.par[t], v);
+            if (c > 0) {  // an empty set owns one placeholder element only
+                cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * cp, stream);
+                if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * cp, stream);
                 if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
             }
         }
         ElemDev &ed = dev.es[t];
-        ed.count = c; ed.n_tiles = nt; ed.max_tile_parts = hs.max_tile_parts;
-        ed.lidx = L.lidx[t]; ed.tile_part_ptr = L.tile_part_ptr[t]; ed.tile_parts = L.tile_parts[t];
-        ed.csr_end = L.csr_end[t]; ed.csr_slots = L.csr_slots[t];
-        ed.c0 = L.c0[t]; ed.c1 = L.c1[t]; ed.c2 = L.c2[t];
-        ed.mu = L.mu[t]; ed.lam = L.lam[t]; ed.damp = L.damp[t]; ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
+        ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.cmax = cmax; ed.rec_bytes = rb;
+        ed.rec = L.rec[t]; ed.tile_parts = L.tile_parts[t]; ed.par = L.par[t];
+        ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
         ed.perm = L.perm[t];
         dev.tile_begin[t] = tile_cursor;
         tile_cursor += nt;
         m->counts[t] = c;
-        if (t != T_HINGE) { m->d_param[3 * t] = L.mu[t]; m->d_param[3 * t + 1] = L.lam[t]; m->d_param[3 * t + 2] = L.damp[t]; }
     }
     dev.tile_begin[N_TYPES] = tile_cursor;
     dev.N = N; dev.E = E;

@@ -77,13 +77,17 @@ __device__ __forceinline__ void load_tets(const ModelDev &md, const ResDev &rd, 
         const int e = threadIdx.x + j * blockDim.x;
         tr[j].on = e < rd.M;
         const int ee = tr[j].on ? e : 0;
-        const float4 c0 = es.c0[ee], c1 = es.c1[ee];
-        const float2 c2 = es.c2[ee];
+        using R = RecLayout<T_TET>;
+        const char *rec = es.rec + (size_t)(ee / kTileElems) * es.rec_bytes;
+        const int el = ee % kTileElems;
+        const float4 c0 = ((const float4 *)(rec + R::oC0))[el], c1 = ((const float4 *)(rec + R::oC1))[el];
+        const float2 c2 = ((const float2 *)(rec + R::oC2))[el];
         tr[j].b[0] = c0.x; tr[j].b[1] = c0.y; tr[j].b[2] = c0.z; tr[j].b[3] = c0.w;
         tr[j].b[4] = c1.x; tr[j].b[5] = c1.y; tr[j].b[6] = c1.z; tr[j].b[7] = c1.w; tr[j].b[8] = c2.x;
         tr[j].V = c2.y;
-        const size_t pe = (size_t)env * es.count + ee;
-        tr[j].mu = es.mu[pe]; tr[j].lam = es.lam[pe]; tr[j].kd = es.damp[pe];
+        tr[j].mu = es.par[par_index(es.n_tiles, env, ee, 0)];
+        tr[j].lam = es.par[par_index(es.n_tiles, env, ee, 1)];
+        tr[j].kd = es.par[par_index(es.n_tiles, env, ee, 2)];
         tr[j].li = rd.idx[ee];
     }
 }
@@ -274,11 +278,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         md.gmass64[poff] += gm64;
     }
     const ElemDev &es = md.es[T_TET];
-    const size_t gstride = (size_t)md.E * es.count;
+    const size_t gstride = (size_t)md.E * es.cpad;
 #pragma unroll
     for (int j = 0; j < EPT; j++) {
         if (tr[j].on) {
-            const size_t pe = (size_t)env * es.count + tid + j * blockDim.x;
+            const size_t pe = (size_t)env * es.cpad + tid + j * blockDim.x;
 #pragma unroll
             for (int q = 0; q < 3; q++) es.g64[q * gstride + pe] += g64[j][q];
         }

@@ -1,17 +1,23 @@
-// gs_stream.cu -- the STREAMING plan: two grid-wide kernels per substep.
+// gs_stream.cu -- the STREAMING plan: per substep, one persistent element kernel per element type plus one
+// particle kernel, forward and adjoint.
 //
-//   k_elements_fwd   one CTA per tile of kTileElems Morton-ordered elements (tets, triangles and hinges in ONE
-//                    launch, CTA ranges per type).  The tile's particles are staged in shared memory (float4
-//                    gathers through a tile-local particle list), each thread evaluates one element with 16-bit
-//                    local indices, writes its per-vertex forces to conflict-free shared-memory slots, and a
-//                    per-tile-particle gather list sums them (no shared-memory atomics: fp32 smem atomics are CAS
-//                    loops on sm_100a).  One REDG.E.ADD.F32x4 per tile-particle goes to the global force array.
-//   k_particles_fwd  per particle: contact + friction from (x-, v-), semi-implicit Euler, writes the next tape
-//                    slot, re-zeroes the force accumulator, flags non-finite states.
-//   k_particles_adj  adjoint of integrate + contact; mass gradient; produces adj_f.
-//   k_elements_adj   gather-form VJP of the element forces with the same tiles; parameter gradients.
+//   k_tiles_fwd<TYPE>  persistent CTAs (a multiple of the SM count) walk the Morton-ordered tiles of kTileElems
+//                      elements of one type.  A tile's streams -- its particle list, the gathered particle states
+//                      (x, v as float4), tile-local 16-bit connectivity, rest constants, parameters and the
+//                      per-tile gather lists -- are prefetched into shared memory with cp.async, double-buffered:
+//                      the particle ids two tiles ahead, everything else one tile ahead, so no thread ever waits on
+//                      a dependent global load.  One thread evaluates one element from shared memory, writes its
+//                      per-vertex forces to conflict-free float4 slots, and each tile-particle sums its slots
+//                      (no shared-memory atomics: fp32 smem atomics are CAS loops on sm_100a) and issues ONE
+//                      red.global.add.v4.f32 to the global force array.
+//   k_particles_fwd    per particle: contact + friction from (x-, v-), semi-implicit Euler, writes the next tape
+//                      slot, re-zeroes the force accumulator, flags non-finite states.
+//   k_particles_adj    adjoint of integrate + contact; mass gradient; produces adj_f.
+//   k_tiles_adj<TYPE>  gather-form VJP of the element forces with the same tiles and pipeline; parameter gradients
+//                      leave as fire-and-forget red.global.add.f32.
 //
 // a1-a10 of SURVEY.md 8(a); citations of the formulas are in gs_elements.cuh.
+#include <algorithm>
 #include <climits>
 
 #include "gs_elements.cuh"
@@ -38,74 +44,257 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
     // one vector reduction per particle instead of three scalar ones (REDG.E.ADD.F32x4)
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(0.0f) : "memory");
 }
+__device__ __forceinline__ void red_add_f32(float *addr, float a) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
+}
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+// mbarrier + bulk async copy (TMA, 1-D): one thread arms the barrier with the byte count and issues the copy, the
+// copy engine signals the barrier when the bytes have landed; every consumer thread waits on the phase parity
+__device__ __forceinline__ void mbar_init(uint64_t *b, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)), "l"(gmem_src),
+                 "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(b)),
+        "r"(parity)
+        : "memory");
+}
 
-__device__ __forceinline__ int tile_type(const ModelDev &md, int tile) { return tile >= md.tile_begin[2] ? 2 : (tile >= md.tile_begin[1] ? 1 : 0); }
+// ------------------------------------------------------------------------------------------ tile pipeline
+// Shared memory of one CTA of a tile kernel (ADJ adds the gathered adj_f and a second output plane):
+//   ids   int[3][pmax]                      particle ids of tiles i, i+1, i+2      (bulk copy, two tiles ahead)
+//   buf   [2] { x, (v), (a) float4[pmax];   gathered particle states               (cp.async 16 B, one tile ahead)
+//               rec  RecLayout<TYPE>;       the tile's packed static record         (bulk copy, one tile ahead)
+//               par  float[3][256] }        mu | lambda | k_damp of (env, tile)     (bulk copy, one tile ahead)
+//   out   float4[arity][256] (x2 for ADJ with velocities)   per element-vertex contributions
+//   bars  uint64[5]                         full[2], idfull[3]
+template <int TYPE, bool ADJ>
+struct TileSmem {
+    using R = RecLayout<TYPE>;
+    static constexpr bool kHasV = TYPE != T_HINGE;
+    static constexpr int kGather = 1 + (kHasV ? 1 : 0) + (ADJ ? 1 : 0);
+    static constexpr int kPar = TYPE != T_HINGE ? kParBytes : 0;
+    __host__ __device__ static int buf_bytes(int pmax, int cmax) { return pmax * 16 * kGather + R::bytes(cmax) + kPar; }
+    __host__ __device__ static int out_bytes() { return R::kArityT * kTileElems * 16 * ((ADJ && kHasV) ? 2 : 1); }
+    __host__ __device__ static int total_bytes(int pmax, int cmax) { return 3 * pmax * 4 + 2 * buf_bytes(pmax, cmax) + out_bytes(); }
+};
+
+template <int TYPE, bool ADJ>
+struct TileView {
+    using R = RecLayout<TYPE>;
+    using S = TileSmem<TYPE, ADJ>;
+    float4 *x, *v, *a;
+    char *rec;
+    const ushort4 *lidx;
+    const float4 *c0, *c1;
+    const float2 *c2;
+    const float *area, *mu, *lam, *damp;
+    const uint16_t *slots, *chunk_end, *chunk_part;
+    __device__ __forceinline__ TileView(char *base, int pmax, int cmax) {
+        char *p = base;
+        x = (float4 *)p; p += pmax * 16;
+        v = (float4 *)p; if (S::kHasV) p += pmax * 16;
+        a = (float4 *)p; if (ADJ) p += pmax * 16;
+        rec = p;
+        lidx = (const ushort4 *)(p + R::oLidx);
+        c0 = (const float4 *)(p + R::oC0);
+        c1 = (const float4 *)(p + R::oC1);
+        c2 = (const float2 *)(p + R::oC2);
+        area = (const float *)(p + R::oArea);
+        slots = (const uint16_t *)(p + R::oSlots);
+        chunk_end = (const uint16_t *)(p + R::oChunkEnd);
+        chunk_part = chunk_end + cmax;
+        p += R::bytes(cmax);
+        mu = (const float *)p; lam = mu + kTileElems; damp = lam + kTileElems;
+    }
+};
+
+// The persistent tile loop shared by the forward and adjoint kernels.  `compute(tv, tile, env, e_local)` evaluates one
+// element into the output slots; `emit(id, env, sums...)` is called once per tile-particle with its summed slots.
+template <int TYPE, bool ADJ>
+struct TilePipe {
+    using S = TileSmem<TYPE, ADJ>;
+    const ElemDev &es;
+    const int N, E, pmax, cmax, bb;
+    int *idbuf;
+    char *bufs;
+    float4 *out;
+    uint64_t *bars;  // full[0..1], idfull[0..2]
+    const float4 *x4, *v4, *a4;
+    __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_)
+        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), cmax(md.es[TYPE].cmax), bb(S::buf_bytes(md.es[TYPE].pmax, md.es[TYPE].cmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
+        idbuf = (int *)smem;
+        bufs = smem + 3 * pmax * 4;
+        out = (float4 *)(bufs + 2 * bb);
+    }
+    // work item -> (tile, env); single-environment models (the large meshes) skip the division
+    __device__ __forceinline__ void split(int item, unsigned &tile, unsigned &env) const {
+        if (E == 1) { tile = (unsigned)item; env = 0u; }
+        else { env = (unsigned)item / (unsigned)es.n_tiles; tile = (unsigned)item - env * (unsigned)es.n_tiles; }
+    }
+    __device__ __forceinline__ void load_ids(int item, int slot) {  // one thread
+        unsigned tile, env;
+        split(item, tile, env);
+        mbar_expect_tx(bars + 2 + slot, pmax * 4);
+        bulk_g2s(idbuf + slot * pmax, es.tile_parts + (size_t)tile * pmax, pmax * 4, bars + 2 + slot);
+    }
+    __device__ __forceinline__ void load_static(int item, int b) {  // one thread
+        unsigned tile, env;
+        split(item, tile, env);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax, cmax);
+        mbar_expect_tx(bars + b, es.rec_bytes + S::kPar);
+        bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b);
+        if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b);
+    }
+    __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
+        unsigned tile, env;
+        split(item, tile, env);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax, cmax);
+        const int *ids = idbuf + slot * pmax;
+        const size_t eoff = (size_t)env * N;
+        for (int p = threadIdx.x; p < pmax; p += kTileElems) {
+            const int id = ids[p];
+            if (id >= 0) {
+                cp_async16(tv.x + p, x4 + eoff + id);
+                if (S::kHasV) cp_async16(tv.v + p, v4 + eoff + id);
+                if (ADJ) cp_async16(tv.a + p, a4 + eoff + id);
+            }
+        }
+        cp_async_commit();
+    }
+    // `rot` rotates which CTAs get the odd extra tile, so that the types of one launch do not pile their remainders
+    // onto the same CTAs
+    template <class Compute, class Emit>
+    __device__ __forceinline__ void run(int rot, Compute compute, Emit emit) {
+        const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
+        const int first = (int)((blockIdx.x + (unsigned)rot) % (unsigned)G);
+        if (first >= n_items) return;
+        const int cnt = (n_items - first + G - 1) / G;
+        if (tid == 0) {
+            load_ids(first, 0);
+            if (cnt > 1) load_ids(first + G, 1);
+            load_static(first, 0);
+        }
+        mbar_wait(bars + 2, 0);
+        gather(first, 0, 0);
+        int s3 = 0, q3 = 0;  // i % 3, i / 3: ids of the CTA's j-th item use id buffer j % 3 for the (j / 3)-th time
+        for (int i = 0; i < cnt; i++) {
+            const int item = first + i * G;
+            const int s3n = s3 == 2 ? 0 : s3 + 1, s3nn = s3n == 2 ? 0 : s3n + 1;
+            cp_async_wait_all();
+            mbar_wait(bars + (i & 1), (i >> 1) & 1);
+            if (i + 1 < cnt) mbar_wait(bars + 2 + s3n, (q3 + (s3n == 0 ? 1 : 0)) & 1);
+            __syncthreads();
+            if (tid == 0) {
+                if (i + 2 < cnt) load_ids(item + 2 * G, s3nn);
+                if (i + 1 < cnt) load_static(item + G, (i + 1) & 1);
+            }
+            if (i + 1 < cnt) gather(item + G, s3n, (i + 1) & 1);
+            unsigned tile, env;
+            split(item, tile, env);
+            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, pmax, cmax);
+            if ((int)(tile * kTileElems + tid) < es.count) compute(tv, (int)tile, (int)env, out);
+            __syncthreads();
+            const int *ids = idbuf + s3 * pmax;
+            for (int c = tid; c < cmax; c += kTileElems) {
+                const int part = tv.chunk_part[c];
+                if (part == 0xFFFF) continue;
+                emit(tv, ids[part], (int)env, c ? tv.chunk_end[c - 1] : 0, tv.chunk_end[c], out);
+            }
+            if (s3n == 0) q3++;
+            s3 = s3n;
+        }
+    }
+};
 
 // ------------------------------------------------------------------------------------------ forward elements
+constexpr int kBarBytes = 128;  // 15 mbarriers at the start of shared memory: 5 per element type
+
+__device__ __forceinline__ void init_barriers(uint64_t *bars) {
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < 15; k++) mbar_init(bars + k, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+}
+
+template <int TYPE>
+__device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64_t *bars, int rot, const float4 *__restrict__ x4,
+                                          const float4 *__restrict__ v4, float4 *__restrict__ f4) {
+    TilePipe<TYPE, false> pipe(md, smem, bars, x4, v4, nullptr);
+    const int N = md.N;
+    pipe.run(
+        rot,
+        [&](const TileView<TYPE, false> &tv, int, int, float4 *sf) {
+            const int tid = threadIdx.x;
+            const ushort4 li = tv.lidx[tid];
+            if (TYPE == T_TET) {
+                const float4 c0 = tv.c0[tid], c1 = tv.c1[tid];
+                const float2 c2 = tv.c2[tid];
+                const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
+                const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
+                const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
+                vec3 f[4];
+                tet_force(x, v, b, c2.y, tv.mu[tid], tv.lam[tid], tv.damp[tid], f);
+#pragma unroll
+                for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
+            } else if (TYPE == T_TRI) {
+                const float4 c0 = tv.c0[tid];
+                const float b[4] = {c0.x, c0.y, c0.z, c0.w};
+                const vec3 x[3] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z])};
+                const vec3 v[3] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z])};
+                vec3 f[3];
+                tri_force(x, v, b, tv.area[tid], tv.mu[tid], tv.lam[tid], tv.damp[tid], f);
+#pragma unroll
+                for (int k = 0; k < 3; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
+            } else {
+                const float4 c0 = tv.c0[tid];
+                const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
+                vec3 f[4];
+                hinge_force(x, c0.x, c0.y, c0.z, f);
+#pragma unroll
+                for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
+            }
+        },
+        [&](const TileView<TYPE, false> &tv, int id, int env, int beg, int end, const float4 *sf) {
+            float ax = 0.f, ay = 0.f, az = 0.f;
+            for (int q = beg; q < end; q++) {
+                const float4 c = sf[tv.slots[q]];
+                ax += c.x; ay += c.y; az += c.z;
+            }
+            red_add_v4(f4 + (size_t)env * N + id, ax, ay, az);
+        });
+}
+
+// all element types of one substep in ONE persistent launch: a CTA walks its tets, then its triangles, then its
+// hinges (forces only meet in the global accumulator, so no grid-wide ordering is needed between the types)
 __global__ void __launch_bounds__(kTileElems) k_elements_fwd(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
-                                                             float4 *__restrict__ f4, int pmax) {
-    extern __shared__ float4 smem4[];
-    float4 *sx = smem4, *sv = smem4 + pmax;
-    float *sf = reinterpret_cast<float *>(smem4 + 2 * pmax);  // [3][4 * kTileElems]
-    constexpr int PL = 4 * kTileElems;
-    const int tid = threadIdx.x, env = blockIdx.y;
-    const int type = tile_type(md, blockIdx.x);
-    const ElemDev &es = md.es[type];
-    const int j = blockIdx.x - md.tile_begin[type];
-    const int p0 = es.tile_part_ptr[j], np = es.tile_part_ptr[j + 1] - p0;
-    const size_t eoff = (size_t)env * md.N;
-    for (int p = tid; p < np; p += kTileElems) {
-        const int id = es.tile_parts[p0 + p];
-        sx[p] = x4[eoff + id];
-        if (type != T_HINGE) sv[p] = v4[eoff + id];
-    }
-    __syncthreads();
-    const int e = j * kTileElems + tid;
-    if (e < es.count) {
-        const ushort4 li = es.lidx[e];
-        if (type == T_TET) {
-            const float4 c0 = es.c0[e], c1 = es.c1[e];
-            const float2 c2 = es.c2[e];
-            const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
-            const size_t pe = (size_t)env * es.count + e;
-            const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
-            const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
-            vec3 f[4];
-            tet_force(x, v, b, c2.y, es.mu[pe], es.lam[pe], es.damp[pe], f);
-#pragma unroll
-            for (int k = 0; k < 4; k++) { sf[k * kTileElems + tid] = f[k].x; sf[PL + k * kTileElems + tid] = f[k].y; sf[2 * PL + k * kTileElems + tid] = f[k].z; }
-        } else if (type == T_TRI) {
-            const float4 c0 = es.c0[e];
-            const float A = es.c1[e].x;
-            const float b[4] = {c0.x, c0.y, c0.z, c0.w};
-            const size_t pe = (size_t)env * es.count + e;
-            const vec3 x[3] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z])};
-            const vec3 v[3] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z])};
-            vec3 f[3];
-            tri_force(x, v, b, A, es.mu[pe], es.lam[pe], es.damp[pe], f);
-#pragma unroll
-            for (int k = 0; k < 3; k++) { sf[k * kTileElems + tid] = f[k].x; sf[PL + k * kTileElems + tid] = f[k].y; sf[2 * PL + k * kTileElems + tid] = f[k].z; }
-        } else {
-            const float4 c0 = es.c0[e];
-            const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
-            vec3 f[4];
-            hinge_force(x, c0.x, c0.y, c0.z, f);
-#pragma unroll
-            for (int k = 0; k < 4; k++) { sf[k * kTileElems + tid] = f[k].x; sf[PL + k * kTileElems + tid] = f[k].y; sf[2 * PL + k * kTileElems + tid] = f[k].z; }
-        }
-    }
-    __syncthreads();
-    const int arity = type == T_TRI ? 3 : 4;
-    const uint16_t *slots = es.csr_slots + (size_t)j * arity * kTileElems;
-    for (int p = tid; p < np; p += kTileElems) {
-        const int beg = p ? es.csr_end[p0 + p - 1] : 0, end = es.csr_end[p0 + p];
-        float ax = 0.f, ay = 0.f, az = 0.f;
-        for (int q = beg; q < end; q++) {
-            const int s = slots[q];
-            ax += sf[s]; ay += sf[PL + s]; az += sf[2 * PL + s];
-        }
-        red_add_v4(f4 + eoff + es.tile_parts[p0 + p], ax, ay, az);
-    }
+                                                             float4 *__restrict__ f4) {
+    extern __shared__ __align__(16) char smem[];
+    uint64_t *bars = (uint64_t *)smem;
+    init_barriers(bars);
+    int rot = 0;
+    if (md.es[T_TET].count) { tiles_fwd<T_TET>(md, smem + kBarBytes, bars, rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_fwd<T_TRI>(md, smem + kBarBytes, bars + 5, rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE>(md, smem + kBarBytes, bars + 10, rot, x4, v4, f4);
 }
 
 // ------------------------------------------------------------------------------------------ forward particles
@@ -167,96 +356,88 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
 }
 
 // ------------------------------------------------------------------------------------------ adjoint elements
+template <int TYPE>
+__device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64_t *bars, int rot, const float4 *__restrict__ x4,
+                                          const float4 *__restrict__ v4, const float4 *__restrict__ adjf, float4 *__restrict__ adjx,
+                                          float4 *__restrict__ adjv) {
+    TilePipe<TYPE, true> pipe(md, smem, bars, x4, v4, adjf);
+    const int N = md.N;
+    constexpr int PL = RecLayout<TYPE>::kArityT * kTileElems;  // second output plane: adj_v contributions
+    const ElemDev &es = md.es[TYPE];
+    const size_t gstride = (size_t)md.E * es.cpad;
+    pipe.run(
+        rot,
+        [&](const TileView<TYPE, true> &tv, int tile, int env, float4 *so) {
+            const int tid = threadIdx.x;
+            const ushort4 li = tv.lidx[tid];
+            if (TYPE == T_TET) {
+                const float4 c0 = tv.c0[tid], c1 = tv.c1[tid];
+                const float2 c2 = tv.c2[tid];
+                const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
+                const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
+                const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
+                const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
+                vec3 ax[4], av[4];
+                float gmu, glam, gk;
+                tet_adjoint(x, v, a, b, c2.y, tv.mu[tid], tv.lam[tid], tv.damp[tid], ax, av, gmu, glam, gk);
+                float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
+                red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
+#pragma unroll
+                for (int k = 0; k < 4; k++) {
+                    so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
+                    so[PL + k * kTileElems + tid] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
+                }
+            } else if (TYPE == T_TRI) {
+                const float4 c0 = tv.c0[tid];
+                const float b[4] = {c0.x, c0.y, c0.z, c0.w};
+                const vec3 x[3] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z])};
+                const vec3 v[3] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z])};
+                const vec3 a[3] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z])};
+                vec3 ax[3], av[3];
+                float gmu, glam, gk;
+                tri_adjoint(x, v, a, b, tv.area[tid], tv.mu[tid], tv.lam[tid], tv.damp[tid], ax, av, gmu, glam, gk);
+                float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
+                red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
+#pragma unroll
+                for (int k = 0; k < 3; k++) {
+                    so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
+                    so[PL + k * kTileElems + tid] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
+                }
+            } else {
+                const float4 c0 = tv.c0[tid];
+                const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
+                const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
+                vec3 ax[4];
+                hinge_adjoint(x, a, c0.x, c0.y, c0.z, ax);
+#pragma unroll
+                for (int k = 0; k < 4; k++) so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
+            }
+        },
+        [&](const TileView<TYPE, true> &tv, int id, int env, int beg, int end, const float4 *so) {
+            float ax = 0.f, ay = 0.f, az = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
+            for (int q = beg; q < end; q++) {
+                const int sl = tv.slots[q];
+                const float4 c = so[sl];
+                ax += c.x; ay += c.y; az += c.z;
+                if (TYPE != T_HINGE) {
+                    const float4 d = so[PL + sl];
+                    bx += d.x; by += d.y; bz += d.z;
+                }
+            }
+            red_add_v4(adjx + (size_t)env * N + id, ax, ay, az);
+            if (TYPE != T_HINGE) red_add_v4(adjv + (size_t)env * N + id, bx, by, bz);
+        });
+}
+
 __global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
-                                                             const float4 *__restrict__ adjf, float4 *__restrict__ adjx, float4 *__restrict__ adjv, int pmax) {
-    extern __shared__ float4 smem4[];
-    float4 *sx = smem4, *sv = smem4 + pmax, *sa = smem4 + 2 * pmax;
-    float *sf = reinterpret_cast<float *>(smem4 + 3 * pmax);  // [6][4 * kTileElems]: ax xyz, av xyz
-    constexpr int PL = 4 * kTileElems;
-    const int tid = threadIdx.x, env = blockIdx.y;
-    const int type = tile_type(md, blockIdx.x);
-    const ElemDev &es = md.es[type];
-    const int j = blockIdx.x - md.tile_begin[type];
-    const int p0 = es.tile_part_ptr[j], np = es.tile_part_ptr[j + 1] - p0;
-    const size_t eoff = (size_t)env * md.N;
-    for (int p = tid; p < np; p += kTileElems) {
-        const int id = es.tile_parts[p0 + p];
-        sx[p] = x4[eoff + id];
-        sa[p] = adjf[eoff + id];
-        if (type != T_HINGE) sv[p] = v4[eoff + id];
-    }
-    __syncthreads();
-    const int e = j * kTileElems + tid;
-    if (e < es.count) {
-        const ushort4 li = es.lidx[e];
-        if (type == T_TET) {
-            const float4 c0 = es.c0[e], c1 = es.c1[e];
-            const float2 c2 = es.c2[e];
-            const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
-            const size_t pe = (size_t)env * es.count + e;
-            const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
-            const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
-            const vec3 a[4] = {vec3(sa[li.x]), vec3(sa[li.y]), vec3(sa[li.z]), vec3(sa[li.w])};
-            vec3 ax[4], av[4];
-            float gmu, glam, gk;
-            tet_adjoint(x, v, a, b, c2.y, es.mu[pe], es.lam[pe], es.damp[pe], ax, av, gmu, glam, gk);
-            const size_t gs_ = (size_t)md.E * es.count;
-            es.g32[pe] += gmu; es.g32[gs_ + pe] += glam; es.g32[2 * gs_ + pe] += gk;
-#pragma unroll
-            for (int k = 0; k < 4; k++) {
-                sf[k * kTileElems + tid] = ax[k].x; sf[PL + k * kTileElems + tid] = ax[k].y; sf[2 * PL + k * kTileElems + tid] = ax[k].z;
-                sf[3 * PL + k * kTileElems + tid] = av[k].x; sf[4 * PL + k * kTileElems + tid] = av[k].y; sf[5 * PL + k * kTileElems + tid] = av[k].z;
-            }
-        } else if (type == T_TRI) {
-            const float4 c0 = es.c0[e];
-            const float A = es.c1[e].x;
-            const float b[4] = {c0.x, c0.y, c0.z, c0.w};
-            const size_t pe = (size_t)env * es.count + e;
-            const vec3 x[3] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z])};
-            const vec3 v[3] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z])};
-            const vec3 a[3] = {vec3(sa[li.x]), vec3(sa[li.y]), vec3(sa[li.z])};
-            vec3 ax[3], av[3];
-            float gmu, glam, gk;
-            tri_adjoint(x, v, a, b, A, es.mu[pe], es.lam[pe], es.damp[pe], ax, av, gmu, glam, gk);
-            const size_t gs_ = (size_t)md.E * es.count;
-            es.g32[pe] += gmu; es.g32[gs_ + pe] += glam; es.g32[2 * gs_ + pe] += gk;
-#pragma unroll
-            for (int k = 0; k < 3; k++) {
-                sf[k * kTileElems + tid] = ax[k].x; sf[PL + k * kTileElems + tid] = ax[k].y; sf[2 * PL + k * kTileElems + tid] = ax[k].z;
-                sf[3 * PL + k * kTileElems + tid] = av[k].x; sf[4 * PL + k * kTileElems + tid] = av[k].y; sf[5 * PL + k * kTileElems + tid] = av[k].z;
-            }
-        } else {
-            const float4 c0 = es.c0[e];
-            const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
-            const vec3 a[4] = {vec3(sa[li.x]), vec3(sa[li.y]), vec3(sa[li.z]), vec3(sa[li.w])};
-            vec3 ax[4];
-            hinge_adjoint(x, a, c0.x, c0.y, c0.z, ax);
-#pragma unroll
-            for (int k = 0; k < 4; k++) { sf[k * kTileElems + tid] = ax[k].x; sf[PL + k * kTileElems + tid] = ax[k].y; sf[2 * PL + k * kTileElems + tid] = ax[k].z; }
-        }
-    }
-    __syncthreads();
-    const int arity = type == T_TRI ? 3 : 4;
-    const uint16_t *slots = es.csr_slots + (size_t)j * arity * kTileElems;
-    for (int p = tid; p < np; p += kTileElems) {
-        const int beg = p ? es.csr_end[p0 + p - 1] : 0, end = es.csr_end[p0 + p];
-        float ax = 0.f, ay = 0.f, az = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-        if (type != T_HINGE) {
-            for (int q = beg; q < end; q++) {
-                const int s = slots[q];
-                ax += sf[s]; ay += sf[PL + s]; az += sf[2 * PL + s];
-                bx += sf[3 * PL + s]; by += sf[4 * PL + s]; bz += sf[5 * PL + s];
-            }
-        } else {
-            for (int q = beg; q < end; q++) {
-                const int s = slots[q];
-                ax += sf[s]; ay += sf[PL + s]; az += sf[2 * PL + s];
-            }
-        }
-        const int id = es.tile_parts[p0 + p];
-        red_add_v4(adjx + eoff + id, ax, ay, az);
-        if (type != T_HINGE) red_add_v4(adjv + eoff + id, bx, by, bz);
-    }
+                                                             const float4 *__restrict__ adjf, float4 *__restrict__ adjx, float4 *__restrict__ adjv) {
+    extern __shared__ __align__(16) char smem[];
+    uint64_t *bars = (uint64_t *)smem;
+    init_barriers(bars);
+    int rot = 0;
+    if (md.es[T_TET].count) { tiles_adj<T_TET>(md, smem + kBarBytes, bars, rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_adj<T_TRI>(md, smem + kBarBytes, bars + 5, rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_adj<T_HINGE>(md, smem + kBarBytes, bars + 10, rot, x4, v4, adjf, adjx, adjv);
 }
 
 // ------------------------------------------------------------------------------------------ layout conversion
@@ -290,21 +471,22 @@ __global__ void k_flush(float *__restrict__ g32, double *__restrict__ g64, size_
 __global__ void k_zero(float *__restrict__ g32, double *__restrict__ g64, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) { g64[i] = 0.0; g32[i] = 0.f; }
 }
-// out[env][perm[e]] = g64[env][e]
-__global__ void k_get_grads(const double *__restrict__ g64, const int *__restrict__ perm, float *__restrict__ out, int E, int count) {
+// out[env][perm[e]] = g64[env][e]; internal arrays have row stride `stride` (>= count)
+__global__ void k_get_grads(const double *__restrict__ g64, const int *__restrict__ perm, float *__restrict__ out, int E, int count, int stride) {
     const size_t total = (size_t)E * count;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / count), e = (int)(i - (size_t)env * count);
-        out[(size_t)env * count + perm[e]] = (float)g64[i];
+        out[(size_t)env * count + perm[e]] = (float)g64[(size_t)env * stride + e];
     }
 }
-__global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ perm, const float *__restrict__ src, int E, int count, int as_inv_mass) {
+// q < 0: dst is the [E][count] inverse-mass array; else dst is ElemDev::par and q the parameter (0 mu, 1 lambda, 2 damp)
+__global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ perm, const float *__restrict__ src, int E, int count, int n_tiles, int q) {
     const size_t total = (size_t)E * count;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / count), e = (int)(i - (size_t)env * count);
         const float val = src[(size_t)env * count + perm[e]];
-        if (as_inv_mass) { if (dst[i] != 0.f) dst[i] = 1.0f / val; }  // pinned particles stay pinned
-        else dst[i] = val;
+        if (q < 0) { if (dst[i] != 0.f) dst[i] = 1.0f / val; }  // pinned particles stay pinned
+        else dst[par_index(n_tiles, env, e, q)] = val;
     }
 }
 
@@ -315,28 +497,50 @@ static inline int grid_for(size_t n, int block = 256) {
     return (int)(g < 1 ? 1 : (g > cap ? cap : g));
 }
 
-int configure_stream_kernels(gs_model *m) {
-    int pmax = 1;
-    for (int t = 0; t < N_TYPES; t++) pmax = pmax > m->hes[t].max_tile_parts ? pmax : m->hes[t].max_tile_parts;
-    m->fwd_smem = 2 * pmax * (int)sizeof(float4) + 3 * 4 * kTileElems * (int)sizeof(float);
-    m->adj_smem = 3 * pmax * (int)sizeof(float4) + 6 * 4 * kTileElems * (int)sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(k_elements_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, m->fwd_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_elements_adj, cudaFuncAttributeMaxDynamicSharedMemorySize, m->adj_smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+template <class K>
+static int tile_kernel_setup(K kern, int smem, int *ctas_per_sm) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, kTileElems, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "tile kernel setup");
+    if (*ctas_per_sm < 1) { set_error("tile kernel does not fit an SM (%d bytes of shared memory)", smem); return GS_EINVAL; }
     return GS_OK;
 }
 
-static inline int pmax_of(const gs_model *m) {
-    int pmax = 1;
-    for (int t = 0; t < N_TYPES; t++) pmax = pmax > m->hes[t].max_tile_parts ? pmax : m->hes[t].max_tile_parts;
-    return pmax;
+int configure_stream_kernels(gs_model *m) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    m->n_sms = sms;
+    const ElemDev *es = m->dev.es;
+    int fwd = 0, adj = 0;
+    long long items = 0;
+    for (int t = 0; t < N_TYPES; t++) {
+        if (m->counts[t] == 0) continue;
+        const int pm = es[t].pmax, cm = es[t].cmax;
+        const int f = t == T_TET ? TileSmem<T_TET, false>::total_bytes(pm, cm) : t == T_TRI ? TileSmem<T_TRI, false>::total_bytes(pm, cm) : TileSmem<T_HINGE, false>::total_bytes(pm, cm);
+        const int a = t == T_TET ? TileSmem<T_TET, true>::total_bytes(pm, cm) : t == T_TRI ? TileSmem<T_TRI, true>::total_bytes(pm, cm) : TileSmem<T_HINGE, true>::total_bytes(pm, cm);
+        fwd = fwd > f ? fwd : f;
+        adj = adj > a ? adj : a;
+        items = std::max(items, (long long)es[t].n_tiles * m->E);
+    }
+    m->elem_items = items;
+    if (items == 0) return GS_OK;
+    m->smem_fwd = fwd + kBarBytes;
+    m->smem_adj = adj + kBarBytes;
+    int rc = tile_kernel_setup(k_elements_fwd, m->smem_fwd, &m->occ_fwd);
+    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj, m->smem_adj, &m->occ_adj);
+    return rc;
+}
+
+// persistent grid: every SM gets its full set of co-resident CTAs, never more CTAs than the largest type has work items
+static inline int tile_grid(const gs_model *m, int occ) {
+    const long long cap = (long long)m->n_sms * occ;
+    return (int)(m->elem_items < cap ? m->elem_items : cap);
 }
 
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
-    const int tiles = m->dev.tile_begin[N_TYPES];
-    if (tiles > 0) {
-        GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", k_elements_fwd<<<dim3(tiles, m->E), kTileElems, m->fwd_smem, st>>>(m->dev, x, v, m->d_f, pmax_of(m)));
-    }
+    if (m->elem_items > 0)
+        GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
+                 k_elements_fwd<<<tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st>>>(m->dev, x, v, m->d_f));
     GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", k_particles_fwd<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, m->d_f, xo, vo, substep));
     return GS_OK;
 }
@@ -346,11 +550,9 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
 int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st) {
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
              k_particles_adj<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
-    const int tiles = m->dev.tile_begin[N_TYPES];
-    if (tiles > 0) {
+    if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                 k_elements_adj<<<dim3(tiles, m->E), kTileElems, m->adj_smem, st>>>(m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv, pmax_of(m)));
-    }
+                 k_elements_adj<<<tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st>>>(m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
     return GS_OK;
 }
@@ -368,7 +570,7 @@ int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, flo
 int launch_flush_grads(gs_model *m, cudaStream_t st) {
     m->steps_since_flush = 0;
     for (int t = 0; t < 2; t++) {
-        const size_t n = 3 * (size_t)m->E * m->counts[t];
+        const size_t n = 3 * (size_t)m->E * m->hes[t].cpad;
         if (!n) continue;
         GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
@@ -378,7 +580,7 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
     m->steps_since_flush = 0;
     for (int t = 0; t < 2; t++) {
-        const size_t n = 3 * (size_t)m->E * m->counts[t];
+        const size_t n = 3 * (size_t)m->E * m->hes[t].cpad;
         if (!n) continue;
         GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
@@ -389,22 +591,22 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     int rc = launch_flush_grads(m, st);
     if (rc != GS_OK) return rc;
     if (group == GS_MASS) {
-        k_get_grads<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass64, m->dev.perm_p, d_out, m->E, m->N);
+        k_get_grads<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass64, m->dev.perm_p, d_out, m->E, m->N, m->N);
     } else {
         const int t = group / 3, q = group % 3, c = m->counts[t];
         if (c == 0) return GS_OK;
-        k_get_grads<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].g64 + (size_t)q * m->E * c, m->dev.es[t].perm, d_out, m->E, c);
+        k_get_grads<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].g64 + (size_t)q * m->E * m->hes[t].cpad, m->dev.es[t].perm, d_out, m->E, c, m->hes[t].cpad);
     }
     GS_LAUNCH_CHECK("k_get_grads");
     return GS_OK;
 }
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st) {
     if (group == GS_MASS) {
-        k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 1);
+        k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 0, -1);
     } else {
         const int t = group / 3, c = m->counts[t];
         if (c == 0) return GS_OK;
-        k_set_params<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->d_param[group], m->dev.es[t].perm, d_values, m->E, c, 0);
+        k_set_params<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].par, m->dev.es[t].perm, d_values, m->E, c, m->dev.es[t].n_tiles, group % 3);
     }
     GS_LAUNCH_CHECK("k_set_params");
     return GS_OK;
