@@ -30,8 +30,9 @@ constexpr int kResMaxTets = 2048;
 constexpr int kResMaxThreads = 1024;
 
 struct ResDev {
-    int M, N, nthreads;
+    int M, N, nthreads, kpp;   // kpp: lanes per particle in the particle phase (1, 2 or 4)
     const ushort4 *idx;        // [M] internal particle ids of each tet (internal element order)
+    const uint16_t *owner;     // [N] particle served by particle slot q, most incident tets first
     const uint16_t *csr_ptr;   // [N + 1]
     const uint16_t *csr_slots; // [4 M] slot = k * M + e
 };
@@ -44,9 +45,10 @@ struct ResHost {
 
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
-// shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float, csr_ptr, csr_slots
+// shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
 static size_t res_smem(int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * N * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float) + al16((size_t)(N + 1) * 2) + al16((size_t)4 * M * 2);
+    return (size_t)(adj ? 3 : 2) * N * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) +
+           al16((size_t)4 * M * 2);
 }
 
 static bool resident_fits(const gs_model_desc *d) {
@@ -54,12 +56,12 @@ static bool resident_fits(const gs_model_desc *d) {
     const int ept = d->n_tets > kResMaxThreads ? 2 : 1;
     const int nthreads = ((d->n_tets + ept - 1) / ept + 31) / 32 * 32;
     if (d->n_particles > nthreads) return false;
-    return res_smem(d->n_particles, d->n_tets, 6, true) <= 200 * 1024;
+    return res_smem(d->n_particles, d->n_tets, 2, true) <= 200 * 1024;
 }
 
 size_t resident_blob_bytes(const gs_model_desc *d) {
     if (!resident_fits(d)) return 0;
-    return 256 * 4 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
+    return 256 * 5 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(2 * d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
 }
 
 // ------------------------------------------------------------------------------------------ kernels
@@ -92,35 +94,61 @@ __device__ __forceinline__ void load_tets(const ModelDev &md, const ResDev &rd, 
     }
 }
 
-__device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint16_t *s_slots) {
+__device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint16_t *s_owner, uint16_t *s_slots) {
     for (int i = threadIdx.x; i <= rd.N; i += blockDim.x) s_ptr[i] = rd.csr_ptr[i];
+    for (int i = threadIdx.x; i < rd.N; i += blockDim.x) s_owner[i] = rd.owner[i];
     for (int i = threadIdx.x; i < 4 * rd.M; i += blockDim.x) s_slots[i] = rd.csr_slots[i];
+}
+
+// Particle ownership: particle slot q = tid / kpp is served by kpp adjacent lanes (kpp = 1, 2 or 4, the largest that
+// fits the CTA); slot q owns particle owner[q] (particles sorted by valence, so the lanes of a warp have near-equal
+// trip counts).  Lane j of the group sums the j-th part of the particle's slot run; the parts meet by shuffle and
+// lane 0 (the "lead") holds the particle's state in registers for the whole rollout.
+struct PartOwn {
+    bool is_p, lead;
+    int p, beg, end;
+};
+__device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_ptr, const uint16_t *s_owner) {
+    PartOwn o;
+    const int q = threadIdx.x / rd.kpp, j = threadIdx.x % rd.kpp;
+    o.is_p = q < rd.N;
+    o.lead = o.is_p && j == 0;
+    o.p = o.is_p ? s_owner[q] : 0;
+    const int b = s_ptr[o.p], len = o.is_p ? s_ptr[o.p + 1] - b : 0;
+    o.beg = b + (len * j) / rd.kpp;
+    o.end = b + (len * (j + 1)) / rd.kpp;
+    return o;
+}
+__device__ __forceinline__ float group_sum(float v, int kpp) {
+    if (kpp >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
+    if (kpp >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
+    return v;
 }
 
 // forward: substeps [0, T), tape slot s = (x4, v4) at base + 2 s S (+ S for v), S = E N
 template <int EPT, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, const ResDev rd, float4 *__restrict__ tape, size_t S, int T) {
     extern __shared__ float4 smem4[];
-    const int N = rd.N, M = rd.M, PL = 4 * M;
+    const int N = rd.N, M = rd.M;
     float4 *sx = smem4, *sv = smem4 + N;
-    float *sf = reinterpret_cast<float *>(smem4 + 2 * N);  // [3][4 M]
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 3 * PL);
-    uint16_t *s_slots = s_ptr + (((N + 1) + 7) & ~7);
+    float4 *sf = smem4 + 2 * N;  // [4 M] per element-vertex force
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 4 * M);
+    uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
+    uint16_t *s_slots = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
-    const size_t poff = (size_t)env * N + tid;
     TetReg tr[EPT];
     load_tets<EPT>(md, rd, env, tr);
-    load_csr(rd, s_ptr, s_slots);
-    const bool is_p = tid < N;
+    load_csr(rd, s_ptr, s_owner, s_slots);
+    __syncthreads();
+    const PartOwn po = part_own(rd, s_ptr, s_owner);
+    const size_t poff = (size_t)env * N + po.p;
     float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq;
-    if (is_p) { xq = tape[poff]; vq = tape[S + poff]; sx[tid] = xq; sv[tid] = vq; }
+    if (po.lead) { xq = tape[poff]; vq = tape[S + poff]; sx[po.p] = xq; sv[po.p] = vq; }
     ContactParams cp;
     cp.n = vec3(md.nx, md.ny, md.nz); cp.d = md.pd; cp.r = md.pr;
     cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
     const vec3 g(md.gx, md.gy, md.gz);
     __syncthreads();
-    int beg = 0, end = 0;
-    if (is_p) { beg = s_ptr[tid]; end = s_ptr[tid + 1]; }
     int bad = INT_MAX;
     for (int s = 0; s < T; s++) {
 #pragma unroll
@@ -133,23 +161,24 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
                 tet_force(x, v, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, f);
                 const int e = tid + j * blockDim.x;
 #pragma unroll
-                for (int k = 0; k < 4; k++) { sf[k * M + e] = f[k].x; sf[PL + k * M + e] = f[k].y; sf[2 * PL + k * M + e] = f[k].z; }
+                for (int k = 0; k < 4; k++) sf[k * M + e] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             }
         }
         __syncthreads();
-        if (is_p) {
-            float ax = 0.f, ay = 0.f, az = 0.f;
-            for (int q = beg; q < end; q++) {
-                const int sl = s_slots[q];
-                ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
-            }
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        for (int q = po.beg; q < po.end; q++) {
+            const float4 c = sf[s_slots[q]];
+            ax += c.x; ay += c.y; az += c.z;
+        }
+        ax = group_sum(ax, rd.kpp); ay = group_sum(ay, rd.kpp); az = group_sum(az, rd.kpp);
+        if (po.lead) {
             const vec3 x(xq), v(vq);
             const vec3 f = vec3(ax, ay, az) + contact_force(cp, x, v);
             vec3 x1, v1;
             integrate(x, v, f, xq.w, g, md.dt, x1, v1);
             xq = make_float4(x1.x, x1.y, x1.z, xq.w);
             vq = make_float4(v1.x, v1.y, v1.z, 0.f);
-            sx[tid] = xq; sv[tid] = vq;
+            sx[po.p] = xq; sv[po.p] = vq;
             float4 *slot = tape + (size_t)(2 * (s + 1)) * S;
             slot[poff] = xq; slot[S + poff] = vq;
             const float chk = x1.x + x1.y + x1.z + v1.x + v1.y + v1.z;
@@ -169,28 +198,30 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     extern __shared__ float4 smem4[];
     const int N = rd.N, M = rd.M, PL = 4 * M;
     float4 *sx = smem4, *sv = smem4 + N, *sa = smem4 + 2 * N;
-    float *sf = reinterpret_cast<float *>(smem4 + 3 * N);  // [6][4 M]
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 6 * PL);
-    uint16_t *s_slots = s_ptr + (((N + 1) + 7) & ~7);
+    float4 *sf = smem4 + 3 * N;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 2 * PL);
+    uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
+    uint16_t *s_slots = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
-    const size_t poff = (size_t)env * N + tid;
     TetReg tr[EPT];
     load_tets<EPT>(md, rd, env, tr);
-    load_csr(rd, s_ptr, s_slots);
-    const bool is_p = tid < N;
+    load_csr(rd, s_ptr, s_owner, s_slots);
+    __syncthreads();
+    const PartOwn po = part_own(rd, s_ptr, s_owner);
+    const size_t poff = (size_t)env * N + po.p;
     ContactParams cp;
     cp.n = vec3(md.nx, md.ny, md.nz); cp.d = md.pd; cp.r = md.pr;
     cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
     const vec3 g(md.gx, md.gy, md.gz);
     const float dt = md.dt;
-    vec3 bx = zero3(), bv = zero3();       // running cotangents of this thread's particle
+    vec3 bx = zero3(), bv = zero3();       // running cotangents of the lead thread's particle
     float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq, vnext = xq;
     const float *cot = nullptr;
-    if (is_p) {
+    if (po.lead) {
         bx = vec3(adjx[poff]); bv = vec3(adjv[poff]);
         vnext = tape[(size_t)(2 * T + 1) * S + poff];
         xq = tape[(size_t)(2 * (T - 1)) * S + poff]; vq = tape[(size_t)(2 * (T - 1) + 1) * S + poff];
-        if (frames) cot = frames + ((size_t)env * N + md.perm_p[tid]) * 3;
+        if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
     const size_t frame_elems = (size_t)md.E * N * 3;
     float gm32 = 0.f;
@@ -201,23 +232,28 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     for (int j = 0; j < EPT; j++)
 #pragma unroll
         for (int q = 0; q < 3; q++) { g32[j][q] = 0.f; g64[j][q] = 0.0; }
-    __syncthreads();
-    int beg = 0, end = 0;
-    if (is_p) { beg = s_ptr[tid]; end = s_ptr[tid + 1]; }
+    // the summed element contributions of the previous element phase, for this thread's particle (lead lane holds them)
+    auto gather = [&](vec3 &dx, vec3 &dv) {
+        float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
+        for (int q = po.beg; q < po.end; q++) {
+            const int sl = s_slots[q];
+            const float4 c = sf[sl], d = sf[PL + sl];
+            ax += c.x; ay += c.y; az += c.z;
+            cx += d.x; cy += d.y; cz += d.z;
+        }
+        dx = vec3(group_sum(ax, rd.kpp), group_sum(ay, rd.kpp), group_sum(az, rd.kpp));
+        dv = vec3(group_sum(cx, rd.kpp), group_sum(cy, rd.kpp), group_sum(cz, rd.kpp));
+    };
     for (int s = T - 1; s >= 0; s--) {
-        if (is_p) {
-            // prefetch the start state of the previous substep while this one is processed
-            float4 xp = xq, vp = vq;
-            if (s > 0) { xp = tape[(size_t)(2 * (s - 1)) * S + poff]; vp = tape[(size_t)(2 * (s - 1) + 1) * S + poff]; }
-            if (s != T - 1) {  // contributions of the element phase of substep s + 1
-                float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
-                for (int q = beg; q < end; q++) {
-                    const int sl = s_slots[q];
-                    ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
-                    cx += sf[3 * PL + sl]; cy += sf[4 * PL + sl]; cz += sf[5 * PL + sl];
-                }
-                bx += vec3(ax, ay, az); bv += vec3(cx, cy, cz);
-            }
+        // prefetch the start state of the previous substep while this one is processed
+        float4 xp = xq, vp = vq;
+        if (po.lead && s > 0) { xp = tape[(size_t)(2 * (s - 1)) * S + poff]; vp = tape[(size_t)(2 * (s - 1) + 1) * S + poff]; }
+        if (s != T - 1) {  // contributions of the element phase of substep s + 1 (all lanes: the sums meet by shuffle)
+            vec3 dx, dv;
+            gather(dx, dv);
+            bx += dx; bv += dv;
+        }
+        if (po.lead) {
             if (cot && (s + 1) % stride == 0 && (s + 1) / stride <= n_frames) {
                 const float *c = cot + (size_t)((s + 1) / stride - 1) * frame_elems;
                 bx += vec3(c[0], c[1], c[2]);
@@ -233,7 +269,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             }
             contact_adjoint(cp, x, v, af, ax, av);
             bx = ax; bv = av;
-            sx[tid] = xq; sv[tid] = vq; sa[tid] = make_float4(af.x, af.y, af.z, 0.f);
+            sx[po.p] = xq; sv[po.p] = vq; sa[po.p] = make_float4(af.x, af.y, af.z, 0.f);
             vnext = vq; xq = xp; vq = vp;
         }
         __syncthreads();
@@ -251,8 +287,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 const int e = tid + j * blockDim.x;
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
-                    sf[k * M + e] = ax[k].x; sf[PL + k * M + e] = ax[k].y; sf[2 * PL + k * M + e] = ax[k].z;
-                    sf[3 * PL + k * M + e] = av[k].x; sf[4 * PL + k * M + e] = av[k].y; sf[5 * PL + k * M + e] = av[k].z;
+                    sf[k * M + e] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
+                    sf[PL + k * M + e] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
                 }
             }
         }
@@ -265,14 +301,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         }
         __syncthreads();
     }
-    if (is_p) {
-        float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
-        for (int q = beg; q < end; q++) {
-            const int sl = s_slots[q];
-            ax += sf[sl]; ay += sf[PL + sl]; az += sf[2 * PL + sl];
-            cx += sf[3 * PL + sl]; cy += sf[4 * PL + sl]; cz += sf[5 * PL + sl];
-        }
-        bx += vec3(ax, ay, az); bv += vec3(cx, cy, cz);
+    {
+        vec3 dx, dv;
+        gather(dx, dv);
+        bx += dx; bv += dv;
+    }
+    if (po.lead) {
         adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
         adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
         md.gmass64[poff] += gm64;
@@ -339,7 +373,13 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     ushort4 *d_idx = (ushort4 *)take(idx.size() * sizeof(ushort4));
     uint16_t *d_ptr = (uint16_t *)take(ptr.size() * 2);
     uint16_t *d_slots = (uint16_t *)take(slots.size() * 2);
-    cudaError_t ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
+    // particle slots: most incident tets first (stable), so the lanes of a warp run near-equal gather loops
+    std::vector<uint16_t> owner(N);
+    for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
+    std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
+    uint16_t *d_owner = (uint16_t *)take(owner.size() * 2);
+    cudaError_t ce = cudaMemcpyAsync(d_owner, owner.data(), owner.size() * 2, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_slots, slots.data(), slots.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
@@ -348,9 +388,10 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     rh->ept = M > kResMaxThreads ? 2 : 1;
     rh->rd.M = M; rh->rd.N = N;
     rh->rd.nthreads = ((M + rh->ept - 1) / rh->ept + 31) / 32 * 32;
-    rh->rd.idx = d_idx; rh->rd.csr_ptr = d_ptr; rh->rd.csr_slots = d_slots;
-    rh->smem_fwd = res_smem(N, M, 3, false);
-    rh->smem_adj = res_smem(N, M, 6, true);
+    rh->rd.kpp = rh->rd.nthreads >= 4 * N ? 4 : (rh->rd.nthreads >= 2 * N ? 2 : 1);
+    rh->rd.idx = d_idx; rh->rd.owner = d_owner; rh->rd.csr_ptr = d_ptr; rh->rd.csr_slots = d_slots;
+    rh->smem_fwd = res_smem(N, M, 1, false);
+    rh->smem_adj = res_smem(N, M, 2, true);
     m->res_host = rh;
     int rc = GS_OK;
     if (rh->ept == 1 && rh->rd.nthreads <= 320) {
