@@ -69,51 +69,52 @@ __device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], cons
 
 // VJP: a[k] = dL/df_k.  Outputs ax[k] = dL/dx_k, av[k] = dL/dv_k contributions (overwritten) and the
 // parameter gradients of this element for this substep.
+// Everything downstream of A = adj_P = -V G B is linear in A, so the kernel works with A' = G B and folds -V into the
+// scalar coefficients; F:A = tr(F^T A) and (F S):A = S:sym(F^T A) reuse the entries of N = sym(F^T A').
 __device__ __forceinline__ void tet_adjoint(const vec3 x[4], const vec3 v[4], const vec3 a[4], const float *b, float V, float mu, float lam, float kd,
                                             vec3 ax[4], vec3 av[4], float &gmu, float &glam, float &gk) {
     TetKin k;
     tet_kin(x[0], x[1], x[2], x[3], b, k);
     vec3 g1, g2, g3;
     mat_cols_times_B(v[1] - v[0], v[2] - v[0], v[3] - v[0], b, g1, g2, g3);
-    // A = adj_P = -V G B, G = [a1-a0, a2-a0, a3-a0]
-    vec3 A1, A2, A3;
+    vec3 A1, A2, A3;  // A' = G B, G = [a1-a0, a2-a0, a3-a0]
     mat_cols_times_B(a[1] - a[0], a[2] - a[0], a[3] - a[0], b, A1, A2, A3);
-    A1 = -V * A1; A2 = -V * A2; A3 = -V * A3;
     const float ip1 = 1.0f / (k.Ic + 1.0f);
     const float s1 = k.Ic * ip1;
-    const float FA = dot(k.f1, A1) + dot(k.f2, A2) + dot(k.f3, A3);
-    const float CA = dot(k.c1, A1) + dot(k.c2, A2) + dot(k.c3, A3);
+    // S = sym(F^T Fdot), N = sym(F^T A')
     const float s11 = dot(k.f1, g1), s22 = dot(k.f2, g2), s33 = dot(k.f3, g3);
     const float s12 = 0.5f * (dot(k.f1, g2) + dot(k.f2, g1));
     const float s13 = 0.5f * (dot(k.f1, g3) + dot(k.f3, g1));
     const float s23 = 0.5f * (dot(k.f2, g3) + dot(k.f3, g2));
-    // parameter gradients: P is linear in mu, lambda, k
-    gmu = s1 * FA - 0.75f * CA;
-    glam = (k.J - 1.0f) * CA;
-    {
-        const vec3 q1 = madd(madd(s11 * k.f1, s12, k.f2), s13, k.f3);
-        const vec3 q2 = madd(madd(s12 * k.f1, s22, k.f2), s23, k.f3);
-        const vec3 q3 = madd(madd(s13 * k.f1, s23, k.f2), s33, k.f3);
-        gk = dot(q1, A1) + dot(q2, A2) + dot(q3, A3);
-    }
-    // adj_F = mu s1 A + 2 mu (F:A)/(Ic+1)^2 F + lambda (cof:A) cof + lambda (J - alpha) Dcof[A] + k (A S + Fdot N)
-    const float ms = mu * s1, q = 2.0f * mu * FA * ip1 * ip1, lc = lam * CA, ce = lam * (k.J - 1.0f) - 0.75f * mu;
     const float n11 = dot(k.f1, A1), n22 = dot(k.f2, A2), n33 = dot(k.f3, A3);
     const float n12 = 0.5f * (dot(k.f1, A2) + dot(k.f2, A1));
     const float n13 = 0.5f * (dot(k.f1, A3) + dot(k.f3, A1));
     const float n23 = 0.5f * (dot(k.f2, A3) + dot(k.f3, A2));
-    vec3 D1 = cross(A2, k.f3) + cross(k.f2, A3);
-    vec3 D2 = cross(A3, k.f1) + cross(k.f3, A1);
-    vec3 D3 = cross(A1, k.f2) + cross(k.f1, A2);
+    const float FA = n11 + n22 + n33;
+    const float CA = dot(k.c1, A1) + dot(k.c2, A2) + dot(k.c3, A3);
+    const float SN = fmaf(s11, n11, fmaf(s22, n22, s33 * n33)) + 2.0f * fmaf(s12, n12, fmaf(s13, n13, s23 * n23));
+    // parameter gradients: P is linear in mu, lambda, k
+    const float mV = -V;
+    gmu = mV * (s1 * FA - 0.75f * CA);
+    glam = mV * ((k.J - 1.0f) * CA);
+    gk = mV * SN;
+    // adj_F = mu s1 A + 2 mu (F:A)/(Ic+1)^2 F + lambda (cof:A) cof + lambda (J - alpha) Dcof[A] + k (A S + Fdot N),  A = -V A'
+    const float ms = mV * mu * s1, q = mV * 2.0f * mu * FA * ip1 * ip1, lc = mV * lam * CA, ce = mV * (lam * (k.J - 1.0f) - 0.75f * mu);
+    const float kv = mV * kd;
+    const float t11 = kv * s11, t22 = kv * s22, t33 = kv * s33, t12 = kv * s12, t13 = kv * s13, t23 = kv * s23;  // kv S
+    const float m11 = kv * n11, m22 = kv * n22, m33 = kv * n33, m12 = kv * n12, m13 = kv * n13, m23 = kv * n23;  // kv N
+    const vec3 D1 = cross(A2, k.f3) + cross(k.f2, A3);
+    const vec3 D2 = cross(A3, k.f1) + cross(k.f3, A1);
+    const vec3 D3 = cross(A1, k.f2) + cross(k.f1, A2);
     vec3 aF1 = madd(madd(madd(ms * A1, q, k.f1), lc, k.c1), ce, D1);
     vec3 aF2 = madd(madd(madd(ms * A2, q, k.f2), lc, k.c2), ce, D2);
     vec3 aF3 = madd(madd(madd(ms * A3, q, k.f3), lc, k.c3), ce, D3);
-    aF1 += kd * (madd(madd(s11 * A1, s12, A2), s13, A3) + madd(madd(n11 * g1, n12, g2), n13, g3));
-    aF2 += kd * (madd(madd(s12 * A1, s22, A2), s23, A3) + madd(madd(n12 * g1, n22, g2), n23, g3));
-    aF3 += kd * (madd(madd(s13 * A1, s23, A2), s33, A3) + madd(madd(n13 * g1, n23, g2), n33, g3));
-    const vec3 aG1 = kd * madd(madd(n11 * k.f1, n12, k.f2), n13, k.f3);
-    const vec3 aG2 = kd * madd(madd(n12 * k.f1, n22, k.f2), n23, k.f3);
-    const vec3 aG3 = kd * madd(madd(n13 * k.f1, n23, k.f2), n33, k.f3);
+    aF1 = madd(madd(madd(madd(madd(madd(aF1, t11, A1), t12, A2), t13, A3), m11, g1), m12, g2), m13, g3);
+    aF2 = madd(madd(madd(madd(madd(madd(aF2, t12, A1), t22, A2), t23, A3), m12, g1), m22, g2), m23, g3);
+    aF3 = madd(madd(madd(madd(madd(madd(aF3, t13, A1), t23, A2), t33, A3), m13, g1), m23, g2), m33, g3);
+    const vec3 aG1 = madd(madd(m11 * k.f1, m12, k.f2), m13, k.f3);
+    const vec3 aG2 = madd(madd(m12 * k.f1, m22, k.f2), m23, k.f3);
+    const vec3 aG3 = madd(madd(m13 * k.f1, m23, k.f2), m33, k.f3);
     // adj_Ds = adj_F B^T
     mat_cols_times_Bt(aF1, aF2, aF3, b, ax[1], ax[2], ax[3]);
     ax[0] = -(ax[1] + ax[2] + ax[3]);
@@ -132,13 +133,15 @@ __device__ __forceinline__ void tri_force(const vec3 x[3], const vec3 v[3], cons
     const float J = sqrtf(dot(c, c));
     const vec3 n = (1.0f / fmaxf(J, 1e-12f)) * c;
     const vec3 j1 = cross(f2, n), j2 = cross(n, f1);  // dJ/dF
-    const float ms = mu * Ic / (Ic + 1.0f);
-    const float ce = lam * (J - 1.0f) - (2.0f / 3.0f) * mu;  // lambda (J - alpha2), alpha2 = 1 + 2mu/(3 lambda)  (A4)
-    const float s11 = dot(f1, g1), s22 = dot(f2, g2), s12 = 0.5f * (dot(f1, g2) + dot(f2, g1));
-    const vec3 p1 = madd(ms * f1, ce, j1) + kd * madd(s11 * f1, s12, f2);
-    const vec3 p2 = madd(ms * f2, ce, j2) + kd * madd(s12 * f1, s22, f2);
-    f[1] = -A * madd(b[0] * p1, b[1], p2);
-    f[2] = -A * madd(b[2] * p1, b[3], p2);
+    // -A (rest area) is folded into the scalar coefficients: p1, p2 are the columns of -A P
+    const float ms = -A * mu * Ic / (Ic + 1.0f);
+    const float ce = -A * (lam * (J - 1.0f) - (2.0f / 3.0f) * mu);  // lambda (J - alpha2), alpha2 = 1 + 2mu/(3 lambda)  (A4)
+    const float kv = -A * kd;
+    const float s11 = kv * dot(f1, g1), s22 = kv * dot(f2, g2), s12 = 0.5f * kv * (dot(f1, g2) + dot(f2, g1));
+    const vec3 p1 = madd(madd(madd(ms * f1, ce, j1), s11, f1), s12, f2);
+    const vec3 p2 = madd(madd(madd(ms * f2, ce, j2), s12, f1), s22, f2);
+    f[1] = madd(b[0] * p1, b[1], p2);
+    f[2] = madd(b[2] * p1, b[3], p2);
     f[0] = -(f[1] + f[2]);
 }
 
@@ -148,7 +151,8 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
     const vec3 f1 = madd(b[0] * e1, b[2], e2), f2 = madd(b[1] * e1, b[3], e2);
     const vec3 g1 = madd(b[0] * w1, b[2], w2), g2 = madd(b[1] * w1, b[3], w2);
     const vec3 G1 = a[1] - a[0], G2 = a[2] - a[0];
-    const vec3 A1 = -A * madd(b[0] * G1, b[2], G2), A2 = -A * madd(b[1] * G1, b[3], G2);
+    // A' = G B; the rest area is folded into the scalar coefficients (everything below is linear in adj_P = -A A')
+    const vec3 A1 = madd(b[0] * G1, b[2], G2), A2 = madd(b[1] * G1, b[3], G2);
     const float Ic = dot(f1, f1) + dot(f2, f2);
     const vec3 c = cross(f1, f2);
     const float J = sqrtf(dot(c, c));
@@ -156,22 +160,25 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
     const vec3 n = iJ * c;
     const vec3 j1 = cross(f2, n), j2 = cross(n, f1);
     const float ip1 = 1.0f / (Ic + 1.0f), s1 = Ic * ip1;
-    const float FA = dot(f1, A1) + dot(f2, A2), JA = dot(j1, A1) + dot(j2, A2);
     const float s11 = dot(f1, g1), s22 = dot(f2, g2), s12 = 0.5f * (dot(f1, g2) + dot(f2, g1));
     const float n11 = dot(f1, A1), n22 = dot(f2, A2), n12 = 0.5f * (dot(f1, A2) + dot(f2, A1));
-    gmu = s1 * FA - (2.0f / 3.0f) * JA;
-    glam = (J - 1.0f) * JA;
-    gk = dot(madd(s11 * f1, s12, f2), A1) + dot(madd(s12 * f1, s22, f2), A2);
+    const float FA = n11 + n22, JA = dot(j1, A1) + dot(j2, A2);
+    const float mA = -A;
+    gmu = mA * (s1 * FA - (2.0f / 3.0f) * JA);
+    glam = mA * ((J - 1.0f) * JA);
+    gk = mA * (fmaf(s11, n11, s22 * n22) + 2.0f * s12 * n12);
     // D(dJ/dF)[A] = [A2 x n + f2 x dn, dn x f1 + n x A1], dc = A1 x f2 + f1 x A2, dn = (dc - n (n.dc))/J
     const vec3 dc = cross(A1, f2) + cross(f1, A2);
     const vec3 dn = iJ * (dc - dot(n, dc) * n);
     const vec3 D1 = cross(A2, n) + cross(f2, dn), D2 = cross(dn, f1) + cross(n, A1);
-    const float ms = mu * s1, q = 2.0f * mu * FA * ip1 * ip1, lj = lam * JA, ce = lam * (J - 1.0f) - (2.0f / 3.0f) * mu;
+    const float ms = mA * mu * s1, q = mA * 2.0f * mu * FA * ip1 * ip1, lj = mA * lam * JA, ce = mA * (lam * (J - 1.0f) - (2.0f / 3.0f) * mu);
+    const float kv = mA * kd;
+    const float t11 = kv * s11, t22 = kv * s22, t12 = kv * s12, m11 = kv * n11, m22 = kv * n22, m12 = kv * n12;
     vec3 aF1 = madd(madd(madd(ms * A1, q, f1), lj, j1), ce, D1);
     vec3 aF2 = madd(madd(madd(ms * A2, q, f2), lj, j2), ce, D2);
-    aF1 += kd * (madd(s11 * A1, s12, A2) + madd(n11 * g1, n12, g2));
-    aF2 += kd * (madd(s12 * A1, s22, A2) + madd(n12 * g1, n22, g2));
-    const vec3 aG1 = kd * madd(n11 * f1, n12, f2), aG2 = kd * madd(n12 * f1, n22, f2);
+    aF1 = madd(madd(madd(madd(aF1, t11, A1), t12, A2), m11, g1), m12, g2);
+    aF2 = madd(madd(madd(madd(aF2, t12, A1), t22, A2), m12, g1), m22, g2);
+    const vec3 aG1 = madd(m11 * f1, m12, f2), aG2 = madd(m12 * f1, m22, f2);
     ax[1] = madd(b[0] * aF1, b[1], aF2); ax[2] = madd(b[2] * aF1, b[3], aF2); ax[0] = -(ax[1] + ax[2]);
     av[1] = madd(b[0] * aG1, b[1], aG2); av[2] = madd(b[2] * aG1, b[3], aG2); av[0] = -(av[1] + av[2]);
 }
