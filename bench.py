@@ -63,6 +63,17 @@ def element_stream_bytes(sc, table):
     return E * (sc.tets.shape[0] * table["tet"] + sc.tris.shape[0] * table["tri"] + sc.hinges.shape[0] * table["hinge"])
 
 
+def ncu_traffic(workload, kernel, T):
+    """DRAM bytes per launch of `kernel` from the committed ncu capture of this workload (profiles/traffic.json), or None."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[workload][kernel]
+    except Exception:
+        return None
+    if "bytes_per_launch" in t:
+        return t["bytes_per_launch"]
+    return t["bytes_per_substep"] * T
+
+
 def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -313,6 +324,7 @@ def main():
         alg["k_resident_fwd"] = substep_bytes(sc, BYTES_FWD) * T
         alg["k_resident_adj"] = substep_bytes(sc, BYTES_ADJ) * T
         flops = {"k_resident_fwd": substep_flops(sc, FLOPS_FWD) * T, "k_resident_adj": substep_flops(sc, FLOPS_ADJ) * T}
+        elem_flops = {"k_elements_fwd": element_stream_bytes(sc, FLOPS_FWD), "k_elements_adj": element_stream_bytes(sc, FLOPS_ADJ)}
         dom = max(alg, key=lambda k: kernels[k]["ms_total"])
         for k in alg:
             if kernels[k]["us_avg"]:
@@ -326,13 +338,17 @@ def main():
             # the streaming-model HBM fraction is reported beside it
             ach = kernels[dom]["alg_tflops"]
             roofline = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS,
-                        "traffic": None, "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1965 MHz (DESIGN.md section 6)",
+                        "traffic": None if args.substeps or args.small else ncu_traffic(sc.name, dom, T), "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1965 MHz (DESIGN.md section 6)",
                         "alg_flops_per_launch": flops[dom], "us_per_launch": kernels[dom]["us_avg"],
                         "hbm_streaming_model": {"achieved": kernels[dom]["alg_gbs"], "peak": peak, "unit": "GB/s", "frac": kernels[dom]["alg_gbs"] / peak,
                                                 "alg_bytes_per_launch": alg[dom]}}
         elif kernels[dom]["us_avg"]:
             ach = kernels[dom]["alg_gbs"]
-            roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+            roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                        "traffic": None if args.small else ncu_traffic(sc.name, dom, T),
+                        # the element kernels execute more instructions than their bytes need time: fp32 ALU view
+                        "alu": ({"achieved": elem_flops[dom] / (kernels[dom]["us_avg"] * 1e-6) / 1e12, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                                 "frac": elem_flops[dom] / (kernels[dom]["us_avg"] * 1e-6) / 1e12 / ALU_PEAK_TFLOPS} if dom in elem_flops else None),
                         "peak_source": peak_src, "alg_bytes_per_launch": alg[dom], "us_per_launch": kernels[dom]["us_avg"]}
 
     if rank != 0:

@@ -5,10 +5,13 @@
 // 320 tets) two grid-wide launches per substep are pure launch latency, and streaming the state through HBM
 // every substep is wasted traffic.  Here
 //   - each thread owns EPT tets for the whole rollout: connectivity, B, V, mu, lambda, k_damp stay in registers;
-//   - each of the first N threads owns one particle: x, v (forward) or adj_x, adj_v (adjoint) stay in
-//     registers across substeps and are mirrored to shared memory for the element phase;
-//   - scatter is a shared-memory gather list: element threads write per-vertex
-//     contributions to conflict-free slots, the particle thread sums its slots -- no atomics, deterministic;
+//   - each particle is served by a group of 1, 2 or 4 adjacent lanes (the largest that fits the CTA); the group's lead
+//     lane keeps x, v (forward) or adj_x, adj_v (adjoint) in registers across substeps and mirrors them to shared
+//     memory for the element phase;
+//   - scatter is a shared-memory gather list: element threads write per-vertex contributions to
+//     conflict-free float4 slots, the lanes of a particle's group sum disjoint parts of its slot run and combine
+//     them by shuffle -- no atomics, deterministic; particles are assigned to groups in order of valence, so the
+//     lanes of a warp run near-equal loops;
 //   - the only HBM traffic is the tape: one coalesced float4 store of (x, v) per particle per substep in the
 //     forward pass, one prefetched load per substep in the adjoint;
 //   - parameter gradients (a10) accumulate in registers over the whole rollout (fp32 chunks of 32 substeps
