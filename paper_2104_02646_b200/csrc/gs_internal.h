@@ -66,7 +66,6 @@ __host__ __device__ inline size_t par_index(int n_tiles, int env, int e, int q) 
 struct ModelDev {
     int N, E;
     ElemDev es[N_TYPES];
-    int tile_begin[N_TYPES + 1];  // blockIdx.x ranges of the fused element kernels
     float gx, gy, gz, dt;
     float nx, ny, nz, pd, pr;
     const float *ke, *kd, *kf, *muc;  // [E]

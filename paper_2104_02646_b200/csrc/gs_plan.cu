@@ -189,7 +189,6 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     // ---- elements: rest quantities, Morton order, tiles
     ModelDev &dev = m->dev;
     memset(&dev, 0, sizeof dev);
-    int tile_cursor = 0;
     for (int t = 0; t < N_TYPES; t++) {
         const int c = counts[t], a = kArity[t];
         const int nt = (c + kTileElems - 1) / kTileElems;
@@ -352,11 +351,8 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         ed.rec = L.rec[t]; ed.tile_parts = L.tile_parts[t]; ed.par = L.par[t];
         ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
         ed.perm = L.perm[t];
-        dev.tile_begin[t] = tile_cursor;
-        tile_cursor += nt;
         m->counts[t] = c;
     }
-    dev.tile_begin[N_TYPES] = tile_cursor;
     dev.N = N; dev.E = E;
     dev.gx = d->gravity[0]; dev.gy = d->gravity[1]; dev.gz = d->gravity[2]; dev.dt = d->dt;
     {

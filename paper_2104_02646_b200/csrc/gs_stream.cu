@@ -1,20 +1,23 @@
-// gs_stream.cu -- the STREAMING plan: per substep, one persistent element kernel per element type plus one
-// particle kernel, forward and adjoint.
+// gs_stream.cu -- the STREAMING plan: per substep one persistent element kernel and one particle kernel, forward
+// and adjoint.
 //
-//   k_tiles_fwd<TYPE>  persistent CTAs (a multiple of the SM count) walk the Morton-ordered tiles of kTileElems
-//                      elements of one type.  A tile's streams -- its particle list, the gathered particle states
-//                      (x, v as float4), tile-local 16-bit connectivity, rest constants, parameters and the
-//                      per-tile gather lists -- are prefetched into shared memory with cp.async, double-buffered:
-//                      the particle ids two tiles ahead, everything else one tile ahead, so no thread ever waits on
-//                      a dependent global load.  One thread evaluates one element from shared memory, writes its
-//                      per-vertex forces to conflict-free float4 slots, and each tile-particle sums its slots
-//                      (no shared-memory atomics: fp32 smem atomics are CAS loops on sm_100a) and issues ONE
-//                      red.global.add.v4.f32 to the global force array.
-//   k_particles_fwd    per particle: contact + friction from (x-, v-), semi-implicit Euler, writes the next tape
-//                      slot, re-zeroes the force accumulator, flags non-finite states.
-//   k_particles_adj    adjoint of integrate + contact; mass gradient; produces adj_f.
-//   k_tiles_adj<TYPE>  gather-form VJP of the element forces with the same tiles and pipeline; parameter gradients
-//                      leave as fire-and-forget red.global.add.f32.
+//   k_elements_fwd   persistent CTAs (SM count x co-resident CTAs) walk the Morton-ordered tiles of kTileElems
+//                    elements: first their tets, then their triangles, then their hinges (all CTAs are in the same
+//                    type's code at the same time, which keeps the instruction cache warm).  A tile's streams arrive
+//                    in shared memory through a double-buffered asynchronous pipeline: the tile's particle ids two
+//                    tiles ahead and its packed static record (tile-local 16-bit connectivity, rest constants, gather
+//                    list) plus parameter block one tile ahead by cp.async.bulk (TMA 1-D) signalling an mbarrier,
+//                    issued by one thread; the particle states (x, v as float4) of the next tile by cp.async 16 B per
+//                    tile-particle from the ids already on chip.  No thread waits on a dependent global load.  One
+//                    thread evaluates one element from shared memory, writes its per-vertex forces to conflict-free
+//                    float4 slots; after one barrier every thread sums one chunk (<= kChunk slots) of one tile-particle
+//                    (no shared-memory atomics: fp32 smem atomics are CAS loops on sm_100a) and issues ONE
+//                    red.global.add.v4.f32 to the global force array.
+//   k_particles_fwd  per particle: contact + friction from (x-, v-), semi-implicit Euler, writes the next tape
+//                    slot, re-zeroes the force accumulator, flags non-finite states.
+//   k_particles_adj  adjoint of integrate + contact; mass gradient; produces adj_f.
+//   k_elements_adj   gather-form VJP of the element forces with the same tiles and pipeline (adj_f gathered too);
+//                    parameter gradients leave as fire-and-forget red.global.add.f32.
 //
 // a1-a10 of SURVEY.md 8(a); citations of the formulas are in gs_elements.cuh.
 #include <algorithm>
