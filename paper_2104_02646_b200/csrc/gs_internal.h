@@ -23,11 +23,12 @@ constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-
 //   c1     float4[256]   tets: B[4..7]
 //   c2     float2[256]   tets: (B[8], V)
 //   area   float[256]    tris: rest area
-//   slots  u16[arity*256] gather list: slot = k * 256 + local element, grouped by CHUNK: the element-vertices of one
-//                        tile-particle, cut into runs of at most kChunk so that the summation is spread over all
-//                        threads of the CTA with near-uniform trip counts (longest runs first)
-//   chunk_end  u16[cmax] end of each chunk's run in `slots`
-//   chunk_part u16[cmax] tile-local particle index of each chunk (0xFFFF = padding)
+//   slots     u16[4*128]  gather list: slot = k * 128 + local element of every element-vertex of the tile, sorted by
+//                         tile-particle (padded to 4 per element for every type)
+//   slot_desc u16[128]    thread t of the CTA sums entries 4t .. 4t+3 and issues one reduction per run of equal
+//                         particles (perfectly balanced, no loop); its descriptor packs: bits 0-9 the tile-local
+//                         particle of entry 4t, bits 10-12 "entry 4t+k (k = 1..3) starts the next particle" (entries
+//                         are sorted, so the next particle is the previous + 1), bits 13-15 the number of valid entries
 template <int TYPE>
 struct RecLayout {
     static constexpr int kArityT = TYPE == 1 ? 3 : 4;
@@ -37,22 +38,18 @@ struct RecLayout {
     static constexpr int oC2 = oC1 + (TYPE == 0 ? kTileElems * 16 : 0);
     static constexpr int oArea = oC2 + (TYPE == 0 ? kTileElems * 8 : 0);
     static constexpr int oSlots = oArea + (TYPE == 1 ? kTileElems * 4 : 0);
-    static constexpr int oChunkEnd = oSlots + kArityT * kTileElems * 2;
-    __host__ __device__ static constexpr int bytes(int cmax) { return oChunkEnd + cmax * 4; }
+    static constexpr int oSlotDesc = oSlots + 4 * kTileElems * 2;
+    static constexpr int kBytes = oSlotDesc + kTileElems * 2;
 };
-inline int rec_bytes_of(int type, int cmax) {
-    return type == 0 ? RecLayout<0>::bytes(cmax) : (type == 1 ? RecLayout<1>::bytes(cmax) : RecLayout<2>::bytes(cmax));
-}
-constexpr int kChunk = 8;  // longest run of slots one thread sums
+inline int rec_bytes_of(int type) { return type == 0 ? RecLayout<0>::kBytes : (type == 1 ? RecLayout<1>::kBytes : RecLayout<2>::kBytes); }
 constexpr int kParBytes = 3 * kTileElems * 4;  // one tile's (mu | lambda | k_damp) block of one environment
 
 // Device view of one element set (tets, triangles or hinges) in INTERNAL (Morton, tiled) order.
 struct ElemDev {
     int count, cpad, n_tiles, pmax;  // cpad = n_tiles * kTileElems; pmax: particle slots per tile (multiple of 8)
-    int cmax;                   // chunks per tile (multiple of 8, >= the tile with most chunks)
-    int rec_bytes;              // RecLayout<type>::bytes(cmax)
+    int rec_bytes;              // RecLayout<type>::kBytes
     const char *rec;            // [n_tiles][rec_bytes]
-    const int *tile_parts;      // [n_tiles][pmax] internal particle ids, most-referenced first, -1 padded
+    const int *tile_parts;      // [n_tiles][pmax] internal particle ids, ascending, -1 padded
     float *par;                 // [E][n_tiles][3][kTileElems]  mu, lambda, k_damp (tets, tris)
     float *g32;                 // [3][E][cpad] per-substep fp32 accumulators (mu, lambda, damp)
     double *g64;                // [3][E][cpad] fp64 masters
@@ -77,7 +74,7 @@ struct ModelDev {
 };
 
 struct HostElemSet {
-    int count = 0, cpad = 0, n_tiles = 0, max_tile_parts = 0, pmax = 0, cmax = 0;
+    int count = 0, cpad = 0, n_tiles = 0, max_tile_parts = 0, pmax = 0;
     std::vector<int> perm;  // internal -> caller
 };
 

@@ -66,7 +66,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     for (int t = 0; t < N_TYPES; t++) {
         const size_t c = counts[t], a = kArity[t], nt = (c + kTileElems - 1) / kTileElems, cp = nt * kTileElems;
         // upper bounds (pmax <= arity * kTileElems is only known after the mesh has been tiled)
-        L.rec[t] = b.take<char>(nt * (size_t)rec_bytes_of(t, (int)a * kTileElems));
+        L.rec[t] = b.take<char>(nt * (size_t)rec_bytes_of(t));
         L.tile_parts[t] = b.take<int>(a * cp);
         if (t != T_HINGE) {
             L.par[t] = b.take<float>(3 * E * cp);
@@ -236,8 +236,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         std::stable_sort(hs.perm.begin(), hs.perm.end(), [&](int x, int y) { return ekey[x] < ekey[y]; });
         const int cp = nt * kTileElems;
         hs.cpad = cp;
-        // tiles, pass 1: the particles of each tile, most-referenced first (near-uniform trip counts per warp in the
-        // kernels' gather loops), and the fullest tile
+        // tiles, pass 1: the particles of each tile and the fullest tile
         std::vector<std::vector<int>> tids(nt);
         std::vector<std::vector<int>> tcnt(nt);
         std::vector<int> ids, cnt, order;
@@ -256,26 +255,19 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
             }
             order.resize(uniq.size());
             std::iota(order.begin(), order.end(), 0);
-            std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return ucnt[x] > ucnt[y]; });
+            // ascending internal (Morton) id: the lanes of a warp gather neighbouring particles, i.e. few distinct 128-byte
+            // lines per cp.async instruction (measured: 18 L1 wavefronts per gather instruction with a valence-sorted list)
             tids[j].resize(uniq.size()); tcnt[j].resize(uniq.size());
             for (size_t q = 0; q < uniq.size(); q++) { tids[j][q] = uniq[order[q]]; tcnt[j][q] = ucnt[order[q]]; }
             hs.max_tile_parts = std::max(hs.max_tile_parts, (int)uniq.size());
         }
         const int pmax = std::max(8, (hs.max_tile_parts + 7) / 8 * 8);
         hs.pmax = pmax;
-        int max_chunks = 0;
-        for (int j = 0; j < nt; j++) {
-            int nc = 0;
-            for (int v : tcnt[j]) nc += (v + kChunk - 1) / kChunk;
-            max_chunks = std::max(max_chunks, nc);
-        }
-        const int cmax = std::max(8, (max_chunks + 7) / 8 * 8);
-        hs.cmax = cmax;
         // pass 2: one packed record per tile (RecLayout), fixed-stride particle lists
-        const int rb = rec_bytes_of(t, cmax);
+        const int rb = rec_bytes_of(t);
         const int oC0 = kTileElems * 8, oC1 = oC0 + kTileElems * 16, oC2 = oC1 + (t == T_TET ? kTileElems * 16 : 0);
         const int oArea = oC2 + (t == T_TET ? kTileElems * 8 : 0), oSlots = oArea + (t == T_TRI ? kTileElems * 4 : 0);
-        const int oChunkEnd = oSlots + a * kTileElems * 2;
+        const int oSlotDesc = oSlots + 4 * kTileElems * 2;
         std::vector<char> rec((size_t)nt * rb, 0);
         std::vector<int> tparts((size_t)nt * pmax, -1);
         std::vector<int> pos;
@@ -287,28 +279,31 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
             float4 *q0 = (float4 *)(R + oC0), *q1 = (float4 *)(R + oC1);
             float2 *q2 = (float2 *)(R + oC2);
             float *qa = (float *)(R + oArea);
-            uint16_t *slots = (uint16_t *)(R + oSlots), *chunk_end = (uint16_t *)(R + oChunkEnd), *chunk_part = chunk_end + cmax;
+            uint16_t *slots = (uint16_t *)(R + oSlots), *slot_desc = (uint16_t *)(R + oSlotDesc);
             // local index of a global id: sorted (id, local) pairs
             std::vector<std::pair<int, int>> look(P_);
             for (int q = 0; q < P_; q++) look[q] = {tids[j][q], q};
             std::sort(look.begin(), look.end());
-            // chunks: full runs of kChunk first, then the remainders, longest first; pos[q] = next free slot of particle q
-            std::vector<std::pair<int, int>> chunks;  // (particle, length)
-            for (int q = 0; q < P_; q++)
-                for (int r = tcnt[j][q]; r > 0; r -= kChunk) chunks.push_back({q, std::min(r, kChunk)});
-            std::stable_sort(chunks.begin(), chunks.end(), [](const std::pair<int, int> &x, const std::pair<int, int> &y) { return x.second > y.second; });
-            // slot ranges of the chunks, in chunk order; a particle's chunks take consecutive pieces of its incidences
-            std::vector<int> cbeg(chunks.size());
-            int run = 0;
-            for (size_t k = 0; k < chunks.size(); k++) { cbeg[k] = run; run += chunks[k].second; }
-            for (int k = 0; k < cmax; k++) {
-                chunk_end[k] = (uint16_t)(k < (int)chunks.size() ? cbeg[k] + chunks[k].second : run);
-                chunk_part[k] = (uint16_t)(k < (int)chunks.size() ? chunks[k].first : 0xFFFF);
+            // entries sorted by tile-particle: particle q owns entries [start[q], start[q] + count[q])
+            std::vector<int> start(P_ + 1, 0);
+            for (int q = 0; q < P_; q++) start[q + 1] = start[q] + tcnt[j][q];
+            for (int k = 0; k < 4 * kTileElems; k++) slots[k] = 0;
+            {
+                std::vector<int> part_of(start[P_]);
+                for (int q = 0; q < P_; q++)
+                    for (int r = 0; r < tcnt[j][q]; r++) part_of[start[q] + r] = q;
+                const int n_entries = start[P_];
+                for (int th = 0; th < kTileElems; th++) {
+                    const int b0 = 4 * th, nv = std::max(0, std::min(4, n_entries - b0));
+                    unsigned dsc = (unsigned)nv << 13;
+                    if (nv > 0) {
+                        dsc |= (unsigned)part_of[b0];
+                        for (int k = 1; k < nv; k++)
+                            if (part_of[b0 + k] != part_of[b0 + k - 1]) dsc |= 1u << (9 + k);
+                    }
+                    slot_desc[th] = (uint16_t)dsc;
+                }
             }
-            // per particle: queue of (next slot position, remaining in chunk) over its chunks
-            std::vector<std::vector<int>> pslots(P_);
-            for (size_t k = 0; k < chunks.size(); k++)
-                for (int r = 0; r < chunks[k].second; r++) pslots[chunks[k].first].push_back(cbeg[k] + r);
             pos.assign(P_ + 1, 0);  // pos[q]: how many incidences of particle q have been placed
             for (int q = 0; q < P_; q++) tparts[(size_t)j * pmax + q] = tids[j][q];
             for (int e = e0; e < e1; e++) {
@@ -317,7 +312,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                     const int gi = inv_p[conn[t][(size_t)hs.perm[e] * a + k]];
                     const int lp = std::lower_bound(look.begin(), look.end(), std::make_pair(gi, -1))->second;
                     li[k] = (unsigned short)lp;
-                    slots[pslots[lp][pos[lp]++]] = (uint16_t)(k * kTileElems + (e - e0));
+                    slots[start[lp] + pos[lp]++] = (uint16_t)(k * kTileElems + (e - e0));
                 }
                 lidx[e - e0] = make_ushort4(li[0], li[1], li[2], li[3]);
                 q0[e - e0] = r0[hs.perm[e]];
@@ -347,7 +342,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
             }
         }
         ElemDev &ed = dev.es[t];
-        ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.cmax = cmax; ed.rec_bytes = rb;
+        ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.rec_bytes = rb;
         ed.rec = L.rec[t]; ed.tile_parts = L.tile_parts[t]; ed.par = L.par[t];
         ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
         ed.perm = L.perm[t];

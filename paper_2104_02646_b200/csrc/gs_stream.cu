@@ -10,7 +10,7 @@
 //                    issued by one thread; the particle states (x, v as float4) of the next tile by cp.async 16 B per
 //                    tile-particle from the ids already on chip.  No thread waits on a dependent global load.  One
 //                    thread evaluates one element from shared memory, writes its per-vertex forces to conflict-free
-//                    float4 slots; after one barrier every thread sums one chunk (<= kChunk slots) of one tile-particle
+//                    float4 slots; after one barrier every thread sums four consecutive entries of the tile's gather list
 //                    (no shared-memory atomics: fp32 smem atomics are CAS loops on sm_100a) and issues ONE
 //                    red.global.add.v4.f32 to the global force array.
 //   k_particles_fwd  per particle: contact + friction from (x-, v-), semi-implicit Euler, writes the next tape
@@ -95,9 +95,9 @@ struct TileSmem {
     static constexpr bool kHasV = TYPE != T_HINGE;
     static constexpr int kGather = 1 + (kHasV ? 1 : 0) + (ADJ ? 1 : 0);
     static constexpr int kPar = TYPE != T_HINGE ? kParBytes : 0;
-    __host__ __device__ static int buf_bytes(int pmax, int cmax) { return pmax * 16 * kGather + R::bytes(cmax) + kPar; }
+    __host__ __device__ static int buf_bytes(int pmax) { return pmax * 16 * kGather + R::kBytes + kPar; }
     __host__ __device__ static int out_bytes() { return R::kArityT * kTileElems * 16 * ((ADJ && kHasV) ? 2 : 1); }
-    __host__ __device__ static int total_bytes(int pmax, int cmax) { return 3 * pmax * 4 + 2 * buf_bytes(pmax, cmax) + out_bytes(); }
+    __host__ __device__ static int total_bytes(int pmax) { return 3 * pmax * 4 + 2 * buf_bytes(pmax) + out_bytes(); }
 };
 
 template <int TYPE, bool ADJ>
@@ -110,8 +110,8 @@ struct TileView {
     const float4 *c0, *c1;
     const float2 *c2;
     const float *area, *mu, *lam, *damp;
-    const uint16_t *slots, *chunk_end, *chunk_part;
-    __device__ __forceinline__ TileView(char *base, int pmax, int cmax) {
+    const uint16_t *slots, *slot_desc;
+    __device__ __forceinline__ TileView(char *base, int pmax) {
         char *p = base;
         x = (float4 *)p; p += pmax * 16;
         v = (float4 *)p; if (S::kHasV) p += pmax * 16;
@@ -123,9 +123,8 @@ struct TileView {
         c2 = (const float2 *)(p + R::oC2);
         area = (const float *)(p + R::oArea);
         slots = (const uint16_t *)(p + R::oSlots);
-        chunk_end = (const uint16_t *)(p + R::oChunkEnd);
-        chunk_part = chunk_end + cmax;
-        p += R::bytes(cmax);
+        slot_desc = (const uint16_t *)(p + R::oSlotDesc);
+        p += R::kBytes;
         mu = (const float *)p; lam = mu + kTileElems; damp = lam + kTileElems;
     }
 };
@@ -136,14 +135,14 @@ template <int TYPE, bool ADJ>
 struct TilePipe {
     using S = TileSmem<TYPE, ADJ>;
     const ElemDev &es;
-    const int N, E, pmax, cmax, bb;
+    const int N, E, pmax, bb;
     int *idbuf;
     char *bufs;
     float4 *out;
     uint64_t *bars;  // full[0..1], idfull[0..2]
     const float4 *x4, *v4, *a4;
     __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_)
-        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), cmax(md.es[TYPE].cmax), bb(S::buf_bytes(md.es[TYPE].pmax, md.es[TYPE].cmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
+        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), bb(S::buf_bytes(md.es[TYPE].pmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
         idbuf = (int *)smem;
         bufs = smem + 3 * pmax * 4;
         out = (float4 *)(bufs + 2 * bb);
@@ -162,7 +161,7 @@ struct TilePipe {
     __device__ __forceinline__ void load_static(int item, int b) {  // one thread
         unsigned tile, env;
         split(item, tile, env);
-        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax, cmax);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax);
         mbar_expect_tx(bars + b, es.rec_bytes + S::kPar);
         bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b);
         if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b);
@@ -170,7 +169,7 @@ struct TilePipe {
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
         split(item, tile, env);
-        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax, cmax);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax);
         const int *ids = idbuf + slot * pmax;
         const size_t eoff = (size_t)env * N;
         for (int p = threadIdx.x; p < pmax; p += kTileElems) {
@@ -213,15 +212,11 @@ struct TilePipe {
             if (i + 1 < cnt) gather(item + G, s3n, (i + 1) & 1);
             unsigned tile, env;
             split(item, tile, env);
-            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, pmax, cmax);
+            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, pmax);
             if ((int)(tile * kTileElems + tid) < es.count) compute(tv, (int)tile, (int)env, out);
             __syncthreads();
             const int *ids = idbuf + s3 * pmax;
-            for (int c = tid; c < cmax; c += kTileElems) {
-                const int part = tv.chunk_part[c];
-                if (part == 0xFFFF) continue;
-                emit(tv, ids[part], (int)env, c ? tv.chunk_end[c - 1] : 0, tv.chunk_end[c], out);
-            }
+            emit(tv, ids, (int)env, out);
             if (s3n == 0) q3++;
             s3 = s3n;
         }
@@ -277,13 +272,28 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
                 for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             }
         },
-        [&](const TileView<TYPE, false> &tv, int id, int env, int beg, int end, const float4 *sf) {
-            float ax = 0.f, ay = 0.f, az = 0.f;
-            for (int q = beg; q < end; q++) {
-                const float4 c = sf[tv.slots[q]];
-                ax += c.x; ay += c.y; az += c.z;
+        [&](const TileView<TYPE, false> &tv, const int *ids, int env, const float4 *sf) {
+            // thread t sums gather-list entries 4t .. 4t+3 (sorted by tile-particle) and issues one vector reduction per
+            // run of equal particles: balanced over all lanes, no loop, no shared-memory atomics
+            const uint2 sl = reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x];
+            const unsigned dsc = tv.slot_desc[threadIdx.x], nv = dsc >> 13;
+            const unsigned s_[4] = {sl.x & 0xFFFFu, sl.x >> 16, sl.y & 0xFFFFu, sl.y >> 16};
+            float4 *dst = f4 + (size_t)env * N;
+            if (nv == 0) return;
+            unsigned cur = dsc & 1023u;
+            float4 c = sf[s_[0]];
+            float ax = c.x, ay = c.y, az = c.z;
+#pragma unroll
+            for (int k = 1; k < 4; k++) {
+                if ((unsigned)k < nv) {
+                    c = sf[s_[k]];
+                    if ((dsc >> (9 + k)) & 1u) {
+                        red_add_v4(dst + ids[cur], ax, ay, az);
+                        cur++; ax = c.x; ay = c.y; az = c.z;
+                    } else { ax += c.x; ay += c.y; az += c.z; }
+                }
             }
-            red_add_v4(f4 + (size_t)env * N + id, ax, ay, az);
+            red_add_v4(dst + ids[cur], ax, ay, az);
         });
 }
 
@@ -416,19 +426,29 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                 for (int k = 0; k < 4; k++) so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
             }
         },
-        [&](const TileView<TYPE, true> &tv, int id, int env, int beg, int end, const float4 *so) {
-            float ax = 0.f, ay = 0.f, az = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-            for (int q = beg; q < end; q++) {
-                const int sl = tv.slots[q];
-                const float4 c = so[sl];
-                ax += c.x; ay += c.y; az += c.z;
-                if (TYPE != T_HINGE) {
-                    const float4 d = so[PL + sl];
-                    bx += d.x; by += d.y; bz += d.z;
+        [&](const TileView<TYPE, true> &tv, const int *ids, int env, const float4 *so) {
+            const uint2 sl = reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x];
+            const unsigned dsc = tv.slot_desc[threadIdx.x], nv = dsc >> 13;
+            const unsigned s_[4] = {sl.x & 0xFFFFu, sl.x >> 16, sl.y & 0xFFFFu, sl.y >> 16};
+            float4 *dx = adjx + (size_t)env * N, *dv = adjv + (size_t)env * N;
+            if (nv == 0) return;
+            unsigned cur = dsc & 1023u;
+            float4 c = so[s_[0]], d = TYPE != T_HINGE ? so[PL + s_[0]] : make_float4(0.f, 0.f, 0.f, 0.f);
+            float ax = c.x, ay = c.y, az = c.z, bx = d.x, by = d.y, bz = d.z;
+#pragma unroll
+            for (int k = 1; k < 4; k++) {
+                if ((unsigned)k < nv) {
+                    c = so[s_[k]];
+                    if (TYPE != T_HINGE) d = so[PL + s_[k]];
+                    if ((dsc >> (9 + k)) & 1u) {
+                        red_add_v4(dx + ids[cur], ax, ay, az);
+                        if (TYPE != T_HINGE) red_add_v4(dv + ids[cur], bx, by, bz);
+                        cur++; ax = c.x; ay = c.y; az = c.z; bx = d.x; by = d.y; bz = d.z;
+                    } else { ax += c.x; ay += c.y; az += c.z; bx += d.x; by += d.y; bz += d.z; }
                 }
             }
-            red_add_v4(adjx + (size_t)env * N + id, ax, ay, az);
-            if (TYPE != T_HINGE) red_add_v4(adjv + (size_t)env * N + id, bx, by, bz);
+            red_add_v4(dx + ids[cur], ax, ay, az);
+            if (TYPE != T_HINGE) red_add_v4(dv + ids[cur], bx, by, bz);
         });
 }
 
@@ -518,9 +538,9 @@ int configure_stream_kernels(gs_model *m) {
     long long items = 0;
     for (int t = 0; t < N_TYPES; t++) {
         if (m->counts[t] == 0) continue;
-        const int pm = es[t].pmax, cm = es[t].cmax;
-        const int f = t == T_TET ? TileSmem<T_TET, false>::total_bytes(pm, cm) : t == T_TRI ? TileSmem<T_TRI, false>::total_bytes(pm, cm) : TileSmem<T_HINGE, false>::total_bytes(pm, cm);
-        const int a = t == T_TET ? TileSmem<T_TET, true>::total_bytes(pm, cm) : t == T_TRI ? TileSmem<T_TRI, true>::total_bytes(pm, cm) : TileSmem<T_HINGE, true>::total_bytes(pm, cm);
+        const int pm = es[t].pmax;
+        const int f = t == T_TET ? TileSmem<T_TET, false>::total_bytes(pm) : t == T_TRI ? TileSmem<T_TRI, false>::total_bytes(pm) : TileSmem<T_HINGE, false>::total_bytes(pm);
+        const int a = t == T_TET ? TileSmem<T_TET, true>::total_bytes(pm) : t == T_TRI ? TileSmem<T_TRI, true>::total_bytes(pm) : TileSmem<T_HINGE, true>::total_bytes(pm);
         fwd = fwd > f ? fwd : f;
         adj = adj > a ? adj : a;
         items = std::max(items, (long long)es[t].n_tiles * m->E);
