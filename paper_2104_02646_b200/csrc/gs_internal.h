@@ -46,10 +46,14 @@ constexpr int kParBytes = 3 * kTileElems * 4;  // one tile's (mu | lambda | k_da
 
 // Device view of one element set (tets, triangles or hinges) in INTERNAL (Morton, tiled) order.
 struct ElemDev {
-    int count, cpad, n_tiles, pmax;  // cpad = n_tiles * kTileElems; pmax: particle slots per tile (multiple of 8)
+    int count, cpad, n_tiles, pmax;  // cpad = n_tiles * kTileElems; pmax: particle list entries per tile (multiple of 8)
+    int lmax;                   // tile-local particle index space (multiple of 8, >= pmax): see tile_parts
     int rec_bytes;              // RecLayout<type>::kBytes
     const char *rec;            // [n_tiles][rec_bytes]
-    const int *tile_parts;      // [n_tiles][pmax] internal particle ids, ascending, -1 padded
+    const int *tile_parts;      // [n_tiles] blocks of { int id[pmax]; uint16_t loc[pmax]; }: the tile's particles, ascending
+                                // internal id (-1 padded), and the tile-local index each is staged at.  Local indices are
+                                // assigned by colouring: particles read by the same quarter-warp for the same vertex get
+                                // different residues mod 8, i.e. different 16-byte bank groups (conflict-free LDS.128)
     float *par;                 // [E][n_tiles][3][kTileElems]  mu, lambda, k_damp (tets, tris)
     float *g32;                 // [3][E][cpad] per-substep fp32 accumulators (mu, lambda, damp)
     double *g64;                // [3][E][cpad] fp64 masters
@@ -74,7 +78,7 @@ struct ModelDev {
 };
 
 struct HostElemSet {
-    int count = 0, cpad = 0, n_tiles = 0, max_tile_parts = 0, pmax = 0;
+    int count = 0, cpad = 0, n_tiles = 0, max_tile_parts = 0, pmax = 0, lmax = 0;
     std::vector<int> perm;  // internal -> caller
 };
 

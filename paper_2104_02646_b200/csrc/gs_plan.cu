@@ -67,7 +67,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
         const size_t c = counts[t], a = kArity[t], nt = (c + kTileElems - 1) / kTileElems, cp = nt * kTileElems;
         // upper bounds (pmax <= arity * kTileElems is only known after the mesh has been tiled)
         L.rec[t] = b.take<char>(nt * (size_t)rec_bytes_of(t));
-        L.tile_parts[t] = b.take<int>(a * cp);
+        L.tile_parts[t] = b.take<int>(2 * a * cp);  // 6 bytes per entry (id + local index), upper bound
         if (t != T_HINGE) {
             L.par[t] = b.take<float>(3 * E * cp);
             L.g32[t] = b.take<float>(3 * E * cp);
@@ -263,13 +263,60 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         }
         const int pmax = std::max(8, (hs.max_tile_parts + 7) / 8 * 8);
         hs.pmax = pmax;
+        // pass 1b: tile-local indices by greedy 8-colouring.  An LDS.128 is served a quarter-warp (8 lanes) at a time and is
+        // conflict-free when the 8 lanes hit 8 different 16-byte bank groups, i.e. local indices with different
+        // residues mod 8 (or the same index: broadcast).  Particles that one quarter-warp reads for the same vertex
+        // position therefore get different colours; colour c owns the local indices c, c + 8, c + 16, ...
+        std::vector<std::vector<int>> tloc(nt);
+        int lmax = 8;
+        {
+            std::vector<int> colour, seen_mask, csize(8);
+            for (int j = 0; j < nt; j++) {
+                const int e0 = j * kTileElems, e1 = std::min(c, e0 + kTileElems), P_ = (int)tids[j].size();
+                auto local_of = [&](int gi) { return (int)(std::lower_bound(tids[j].begin(), tids[j].end(), gi) - tids[j].begin()); };
+                // groups[(quarter, k)] = distinct list positions
+                const int nq = (e1 - e0 + 7) / 8;
+                std::vector<std::vector<int>> groups((size_t)nq * a), of_part(P_);
+                for (int e = e0; e < e1; e++)
+                    for (int k = 0; k < a; k++) {
+                        const int q = local_of(inv_p[conn[t][(size_t)hs.perm[e] * a + k]]), g = ((e - e0) / 8) * a + k;
+                        if (std::find(groups[g].begin(), groups[g].end(), q) == groups[g].end()) { groups[g].push_back(q); of_part[q].push_back(g); }
+                    }
+                colour.assign(P_, -1);
+                std::fill(csize.begin(), csize.end(), 0);
+                const int cap = (P_ + 7) / 8 + 1;  // bound the imbalance: lmax <= pmax + 16
+                for (int e = e0; e < e1; e++)
+                    for (int k = 0; k < a; k++) {
+                        const int q = local_of(inv_p[conn[t][(size_t)hs.perm[e] * a + k]]);
+                        if (colour[q] >= 0) continue;
+                        unsigned forbid = 0;
+                        for (int g : of_part[q])
+                            for (int r : groups[g])
+                                if (colour[r] >= 0) forbid |= 1u << colour[r];
+                        int best = -1;
+                        for (int cc = 0; cc < 8; cc++)
+                            if (!(forbid >> cc & 1u) && csize[cc] < cap && (best < 0 || csize[cc] < csize[best])) best = cc;
+                        if (best < 0)
+                            for (int cc = 0; cc < 8; cc++)
+                                if (csize[cc] < cap && (best < 0 || csize[cc] < csize[best])) best = cc;
+                        colour[q] = best;
+                        csize[best]++;
+                    }
+                tloc[j].resize(P_);
+                std::fill(csize.begin(), csize.end(), 0);
+                for (int q = 0; q < P_; q++) { tloc[j][q] = colour[q] + 8 * csize[colour[q]]; csize[colour[q]]++; }
+                for (int cc = 0; cc < 8; cc++) lmax = std::max(lmax, 8 * csize[cc]);
+            }
+        }
+        hs.lmax = lmax;
         // pass 2: one packed record per tile (RecLayout), fixed-stride particle lists
         const int rb = rec_bytes_of(t);
         const int oC0 = kTileElems * 8, oC1 = oC0 + kTileElems * 16, oC2 = oC1 + (t == T_TET ? kTileElems * 16 : 0);
         const int oArea = oC2 + (t == T_TET ? kTileElems * 8 : 0), oSlots = oArea + (t == T_TRI ? kTileElems * 4 : 0);
         const int oSlotDesc = oSlots + 4 * kTileElems * 2;
         std::vector<char> rec((size_t)nt * rb, 0);
-        std::vector<int> tparts((size_t)nt * pmax, -1);
+        const size_t tp_ints = (size_t)pmax * 6 / 4;  // ints per tile block: id[pmax] then loc[pmax] (u16)
+        std::vector<int> tparts((size_t)nt * tp_ints, -1);
         std::vector<int> pos;
         for (int j = 0; j < nt; j++) {
             const int e0 = j * kTileElems, e1 = std::min(c, e0 + kTileElems);
@@ -305,13 +352,16 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                 }
             }
             pos.assign(P_ + 1, 0);  // pos[q]: how many incidences of particle q have been placed
-            for (int q = 0; q < P_; q++) tparts[(size_t)j * pmax + q] = tids[j][q];
+            for (int q = 0; q < P_; q++) {
+                tparts[(size_t)j * tp_ints + q] = tids[j][q];
+                ((uint16_t *)(tparts.data() + (size_t)j * tp_ints + pmax))[q] = (uint16_t)tloc[j][q];
+            }
             for (int e = e0; e < e1; e++) {
                 unsigned short li[4] = {0, 0, 0, 0};
                 for (int k = 0; k < a; k++) {
                     const int gi = inv_p[conn[t][(size_t)hs.perm[e] * a + k]];
                     const int lp = std::lower_bound(look.begin(), look.end(), std::make_pair(gi, -1))->second;
-                    li[k] = (unsigned short)lp;
+                    li[k] = (unsigned short)tloc[j][lp];
                     slots[start[lp] + pos[lp]++] = (uint16_t)(k * kTileElems + (e - e0));
                 }
                 lidx[e - e0] = make_ushort4(li[0], li[1], li[2], li[3]);
@@ -342,7 +392,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
             }
         }
         ElemDev &ed = dev.es[t];
-        ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.rec_bytes = rb;
+        ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.lmax = lmax; ed.rec_bytes = rb;
         ed.rec = L.rec[t]; ed.tile_parts = L.tile_parts[t]; ed.par = L.par[t];
         ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
         ed.perm = L.perm[t];

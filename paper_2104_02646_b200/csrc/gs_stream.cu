@@ -22,6 +22,8 @@
 // a1-a10 of SURVEY.md 8(a); citations of the formulas are in gs_elements.cuh.
 #include <algorithm>
 #include <climits>
+#include <cstdio>
+#include <cstdlib>
 
 #include "gs_elements.cuh"
 #include "gs_internal.h"
@@ -95,9 +97,9 @@ struct TileSmem {
     static constexpr bool kHasV = TYPE != T_HINGE;
     static constexpr int kGather = 1 + (kHasV ? 1 : 0) + (ADJ ? 1 : 0);
     static constexpr int kPar = TYPE != T_HINGE ? kParBytes : 0;
-    __host__ __device__ static int buf_bytes(int pmax) { return pmax * 16 * kGather + R::kBytes + kPar; }
+    __host__ __device__ static int buf_bytes(int lmax) { return lmax * 16 * kGather + R::kBytes + kPar; }
     __host__ __device__ static int out_bytes() { return R::kArityT * kTileElems * 16 * ((ADJ && kHasV) ? 2 : 1); }
-    __host__ __device__ static int total_bytes(int pmax) { return 3 * pmax * 4 + 2 * buf_bytes(pmax) + out_bytes(); }
+    __host__ __device__ static int total_bytes(int pmax, int lmax) { return 3 * pmax * 4 + 2 * pmax * 2 + 2 * buf_bytes(lmax) + out_bytes(); }
 };
 
 template <int TYPE, bool ADJ>
@@ -111,11 +113,11 @@ struct TileView {
     const float2 *c2;
     const float *area, *mu, *lam, *damp;
     const uint16_t *slots, *slot_desc;
-    __device__ __forceinline__ TileView(char *base, int pmax) {
+    __device__ __forceinline__ TileView(char *base, int lmax) {
         char *p = base;
-        x = (float4 *)p; p += pmax * 16;
-        v = (float4 *)p; if (S::kHasV) p += pmax * 16;
-        a = (float4 *)p; if (ADJ) p += pmax * 16;
+        x = (float4 *)p; p += lmax * 16;
+        v = (float4 *)p; if (S::kHasV) p += lmax * 16;
+        a = (float4 *)p; if (ADJ) p += lmax * 16;
         rec = p;
         lidx = (const ushort4 *)(p + R::oLidx);
         c0 = (const float4 *)(p + R::oC0);
@@ -135,16 +137,18 @@ template <int TYPE, bool ADJ>
 struct TilePipe {
     using S = TileSmem<TYPE, ADJ>;
     const ElemDev &es;
-    const int N, E, pmax, bb;
-    int *idbuf;
+    const int N, E, pmax, lmax, bb;
+    int *idbuf;         // [3][pmax] particle ids of tiles i, i+1, i+2
+    uint16_t *locbuf;   // [2][pmax] tile-local staging index of each list entry (only live between load and gather)
     char *bufs;
     float4 *out;
     uint64_t *bars;  // full[0..1], idfull[0..2]
     const float4 *x4, *v4, *a4;
     __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_)
-        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), bb(S::buf_bytes(md.es[TYPE].pmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
+        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
         idbuf = (int *)smem;
-        bufs = smem + 3 * pmax * 4;
+        locbuf = (uint16_t *)(smem + 3 * pmax * 4);
+        bufs = smem + 3 * pmax * 4 + 2 * pmax * 2;
         out = (float4 *)(bufs + 2 * bb);
     }
     // work item -> (tile, env); single-environment models (the large meshes) skip the division
@@ -152,16 +156,19 @@ struct TilePipe {
         if (E == 1) { tile = (unsigned)item; env = 0u; }
         else { env = (unsigned)item / (unsigned)es.n_tiles; tile = (unsigned)item - env * (unsigned)es.n_tiles; }
     }
-    __device__ __forceinline__ void load_ids(int item, int slot) {  // one thread
+    // ids of the CTA's j-th item go to id buffer `slot` = j % 3, its staging indices to loc buffer `par` = j % 2
+    __device__ __forceinline__ void load_ids(int item, int slot, int par) {  // one thread
         unsigned tile, env;
         split(item, tile, env);
-        mbar_expect_tx(bars + 2 + slot, pmax * 4);
-        bulk_g2s(idbuf + slot * pmax, es.tile_parts + (size_t)tile * pmax, pmax * 4, bars + 2 + slot);
+        const char *blk = (const char *)es.tile_parts + (size_t)tile * pmax * 6;
+        mbar_expect_tx(bars + 2 + slot, pmax * 6);
+        bulk_g2s(idbuf + slot * pmax, blk, pmax * 4, bars + 2 + slot);
+        bulk_g2s(locbuf + par * pmax, blk + pmax * 4, pmax * 2, bars + 2 + slot);
     }
     __device__ __forceinline__ void load_static(int item, int b) {  // one thread
         unsigned tile, env;
         split(item, tile, env);
-        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, lmax);
         mbar_expect_tx(bars + b, es.rec_bytes + S::kPar);
         bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b);
         if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b);
@@ -169,15 +176,17 @@ struct TilePipe {
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
         split(item, tile, env);
-        TileView<TYPE, ADJ> tv(bufs + b * bb, pmax);
+        TileView<TYPE, ADJ> tv(bufs + b * bb, lmax);
         const int *ids = idbuf + slot * pmax;
+        const uint16_t *loc = locbuf + (b & 1) * pmax;  // the tile staged into buffer b is the CTA's item with parity b
         const size_t eoff = (size_t)env * N;
         for (int p = threadIdx.x; p < pmax; p += kTileElems) {
             const int id = ids[p];
             if (id >= 0) {
-                cp_async16(tv.x + p, x4 + eoff + id);
-                if (S::kHasV) cp_async16(tv.v + p, v4 + eoff + id);
-                if (ADJ) cp_async16(tv.a + p, a4 + eoff + id);
+                const int l = loc[p];
+                cp_async16(tv.x + l, x4 + eoff + id);
+                if (S::kHasV) cp_async16(tv.v + l, v4 + eoff + id);
+                if (ADJ) cp_async16(tv.a + l, a4 + eoff + id);
             }
         }
         cp_async_commit();
@@ -191,8 +200,8 @@ struct TilePipe {
         if (first >= n_items) return;
         const int cnt = (n_items - first + G - 1) / G;
         if (tid == 0) {
-            load_ids(first, 0);
-            if (cnt > 1) load_ids(first + G, 1);
+            load_ids(first, 0, 0);
+            if (cnt > 1) load_ids(first + G, 1, 1);
             load_static(first, 0);
         }
         mbar_wait(bars + 2, 0);
@@ -206,13 +215,13 @@ struct TilePipe {
             if (i + 1 < cnt) mbar_wait(bars + 2 + s3n, (q3 + (s3n == 0 ? 1 : 0)) & 1);
             __syncthreads();
             if (tid == 0) {
-                if (i + 2 < cnt) load_ids(item + 2 * G, s3nn);
+                if (i + 2 < cnt) load_ids(item + 2 * G, s3nn, i & 1);
                 if (i + 1 < cnt) load_static(item + G, (i + 1) & 1);
             }
             if (i + 1 < cnt) gather(item + G, s3n, (i + 1) & 1);
             unsigned tile, env;
             split(item, tile, env);
-            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, pmax);
+            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, lmax);
             if ((int)(tile * kTileElems + tid) < es.count) compute(tv, (int)tile, (int)env, out);
             __syncthreads();
             const int *ids = idbuf + s3 * pmax;
@@ -538,9 +547,9 @@ int configure_stream_kernels(gs_model *m) {
     long long items = 0;
     for (int t = 0; t < N_TYPES; t++) {
         if (m->counts[t] == 0) continue;
-        const int pm = es[t].pmax;
-        const int f = t == T_TET ? TileSmem<T_TET, false>::total_bytes(pm) : t == T_TRI ? TileSmem<T_TRI, false>::total_bytes(pm) : TileSmem<T_HINGE, false>::total_bytes(pm);
-        const int a = t == T_TET ? TileSmem<T_TET, true>::total_bytes(pm) : t == T_TRI ? TileSmem<T_TRI, true>::total_bytes(pm) : TileSmem<T_HINGE, true>::total_bytes(pm);
+        const int pm = es[t].pmax, lm = es[t].lmax;
+        const int f = t == T_TET ? TileSmem<T_TET, false>::total_bytes(pm, lm) : t == T_TRI ? TileSmem<T_TRI, false>::total_bytes(pm, lm) : TileSmem<T_HINGE, false>::total_bytes(pm, lm);
+        const int a = t == T_TET ? TileSmem<T_TET, true>::total_bytes(pm, lm) : t == T_TRI ? TileSmem<T_TRI, true>::total_bytes(pm, lm) : TileSmem<T_HINGE, true>::total_bytes(pm, lm);
         fwd = fwd > f ? fwd : f;
         adj = adj > a ? adj : a;
         items = std::max(items, (long long)es[t].n_tiles * m->E);
@@ -551,6 +560,9 @@ int configure_stream_kernels(gs_model *m) {
     m->smem_adj = adj + kBarBytes;
     int rc = tile_kernel_setup(k_elements_fwd, m->smem_fwd, &m->occ_fwd);
     if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj, m->smem_adj, &m->occ_adj);
+    if (getenv("GS_DEBUG"))
+        fprintf(stderr, "gradsim: element kernels smem fwd %d adj %d bytes, CTAs/SM fwd %d adj %d, pmax %d/%d/%d lmax %d/%d/%d\n", m->smem_fwd, m->smem_adj,
+                m->occ_fwd, m->occ_adj, es[0].pmax, es[1].pmax, es[2].pmax, es[0].lmax, es[1].lmax, es[2].lmax);
     return rc;
 }
 
