@@ -64,10 +64,26 @@ __device__ __forceinline__ void mbar_init(uint64_t *b, int count) { asm volatile
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *b, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *b) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)), "l"(gmem_src),
-                 "r"(bytes), "r"(smem_u32(b))
+// L2 policies: the static tile streams (records, parameters, particle lists: ~125 MB per pass on the 1M-tet scene, about
+// the size of L2) are read once per launch -> evict_first, so that they do not push out the particle arrays (state, force
+// and adjoint accumulators, ~8 MB each), which every tile re-reads and the next kernel needs -> evict_last.
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, uint64_t *b, uint64_t policy) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(b)), "l"(policy)
                  : "memory");
+}
+__device__ __forceinline__ void cp_async16_hint(void *smem_dst, const void *gmem_src, uint64_t policy) {
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "l"(policy) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
     asm volatile(
@@ -144,12 +160,15 @@ struct TilePipe {
     float4 *out;
     uint64_t *bars;  // full[0..1], idfull[0..2]
     const float4 *x4, *v4, *a4;
+    uint64_t pol_stream, pol_keep;
     __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_)
         : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
         idbuf = (int *)smem;
         locbuf = (uint16_t *)(smem + 3 * pmax * 4);
         bufs = smem + 3 * pmax * 4 + 2 * pmax * 2;
         out = (float4 *)(bufs + 2 * bb);
+        pol_stream = l2_policy_evict_first();
+        pol_keep = l2_policy_evict_last();
     }
     // work item -> (tile, env); single-environment models (the large meshes) skip the division
     __device__ __forceinline__ void split(int item, unsigned &tile, unsigned &env) const {
@@ -162,16 +181,16 @@ struct TilePipe {
         split(item, tile, env);
         const char *blk = (const char *)es.tile_parts + (size_t)tile * pmax * 6;
         mbar_expect_tx(bars + 2 + slot, pmax * 6);
-        bulk_g2s(idbuf + slot * pmax, blk, pmax * 4, bars + 2 + slot);
-        bulk_g2s(locbuf + par * pmax, blk + pmax * 4, pmax * 2, bars + 2 + slot);
+        bulk_g2s(idbuf + slot * pmax, blk, pmax * 4, bars + 2 + slot, pol_stream);
+        bulk_g2s(locbuf + par * pmax, blk + pmax * 4, pmax * 2, bars + 2 + slot, pol_stream);
     }
     __device__ __forceinline__ void load_static(int item, int b) {  // one thread
         unsigned tile, env;
         split(item, tile, env);
         TileView<TYPE, ADJ> tv(bufs + b * bb, lmax);
         mbar_expect_tx(bars + b, es.rec_bytes + S::kPar);
-        bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b);
-        if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b);
+        bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b, pol_stream);
+        if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b, pol_stream);
     }
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
@@ -184,9 +203,9 @@ struct TilePipe {
             const int id = ids[p];
             if (id >= 0) {
                 const int l = loc[p];
-                cp_async16(tv.x + l, x4 + eoff + id);
-                if (S::kHasV) cp_async16(tv.v + l, v4 + eoff + id);
-                if (ADJ) cp_async16(tv.a + l, a4 + eoff + id);
+                cp_async16_hint(tv.x + l, x4 + eoff + id, pol_keep);
+                if (S::kHasV) cp_async16_hint(tv.v + l, v4 + eoff + id, pol_keep);
+                if (ADJ) cp_async16_hint(tv.a + l, a4 + eoff + id, pol_keep);
             }
         }
         cp_async_commit();
