@@ -34,7 +34,11 @@ constexpr int kResMaxThreads = 1024;
 
 struct ResDev {
     int M, N, nthreads, kpp;   // kpp: lanes per particle in the particle phase (1, 2 or 4)
-    const ushort4 *idx;        // [M] internal particle ids of each tet (internal element order)
+    int L;                     // size of the shared-memory staging index space (multiple of 8, >= N)
+    const ushort4 *idx;        // [M] STAGING indices of each tet's particles (internal element order)
+    const uint16_t *rloc;      // [N] staging index of internal particle p: assigned by greedy 8-colouring so that the
+                               // particles one quarter-warp reads for the same vertex fall into different 16-byte bank
+                               // groups (conflict-free LDS.128), as in the streaming plan
     const uint16_t *owner;     // [N] particle served by particle slot q, most incident tets first
     const uint16_t *csr_ptr;   // [N + 1]
     const uint16_t *csr_slots; // [4 M] slot = k * M + e
@@ -49,8 +53,8 @@ struct ResHost {
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
 // shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
-static size_t res_smem(int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * N * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) +
+static size_t res_smem(int L, int N, int M, int planes, bool adj) {
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) +
            al16((size_t)4 * M * 2);
 }
 
@@ -59,12 +63,12 @@ static bool resident_fits(const gs_model_desc *d) {
     const int ept = d->n_tets > kResMaxThreads ? 2 : 1;
     const int nthreads = ((d->n_tets + ept - 1) / ept + 31) / 32 * 32;
     if (d->n_particles > nthreads) return false;
-    return res_smem(d->n_particles, d->n_tets, 2, true) <= 200 * 1024;
+    return res_smem(d->n_particles + 24, d->n_particles, d->n_tets, 2, true) <= 200 * 1024;
 }
 
 size_t resident_blob_bytes(const gs_model_desc *d) {
     if (!resident_fits(d)) return 0;
-    return 256 * 5 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(2 * d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
+    return 256 * 6 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(3 * d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
 }
 
 // ------------------------------------------------------------------------------------------ kernels
@@ -109,7 +113,7 @@ __device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint
 // lane 0 (the "lead") holds the particle's state in registers for the whole rollout.
 struct PartOwn {
     bool is_p, lead;
-    int p, beg, end;
+    int p, lp, beg, end;  // particle, its staging index, this lane's part of its slot run
 };
 __device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_ptr, const uint16_t *s_owner) {
     PartOwn o;
@@ -117,6 +121,7 @@ __device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_
     o.is_p = q < rd.N;
     o.lead = o.is_p && j == 0;
     o.p = o.is_p ? s_owner[q] : 0;
+    o.lp = rd.rloc[o.p];
     const int b = s_ptr[o.p], len = o.is_p ? s_ptr[o.p + 1] - b : 0;
     o.beg = b + (len * j) / rd.kpp;
     o.end = b + (len * (j + 1)) / rd.kpp;
@@ -132,9 +137,9 @@ __device__ __forceinline__ float group_sum(float v, int kpp) {
 template <int EPT, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, const ResDev rd, float4 *__restrict__ tape, size_t S, int T) {
     extern __shared__ float4 smem4[];
-    const int N = rd.N, M = rd.M;
-    float4 *sx = smem4, *sv = smem4 + N;
-    float4 *sf = smem4 + 2 * N;  // [4 M] per element-vertex force
+    const int N = rd.N, M = rd.M, L = rd.L;
+    float4 *sx = smem4, *sv = smem4 + L;
+    float4 *sf = smem4 + 2 * L;  // [4 M] per element-vertex force
     uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 4 * M);
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
     uint16_t *s_slots = s_owner + ((N + 7) & ~7);
@@ -146,7 +151,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
     const PartOwn po = part_own(rd, s_ptr, s_owner);
     const size_t poff = (size_t)env * N + po.p;
     float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq;
-    if (po.lead) { xq = tape[poff]; vq = tape[S + poff]; sx[po.p] = xq; sv[po.p] = vq; }
+    if (po.lead) { xq = tape[poff]; vq = tape[S + poff]; sx[po.lp] = xq; sv[po.lp] = vq; }
     ContactParams cp;
     cp.n = vec3(md.nx, md.ny, md.nz); cp.d = md.pd; cp.r = md.pr;
     cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
@@ -181,7 +186,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
             integrate(x, v, f, xq.w, g, md.dt, x1, v1);
             xq = make_float4(x1.x, x1.y, x1.z, xq.w);
             vq = make_float4(v1.x, v1.y, v1.z, 0.f);
-            sx[po.p] = xq; sv[po.p] = vq;
+            sx[po.lp] = xq; sv[po.lp] = vq;
             float4 *slot = tape + (size_t)(2 * (s + 1)) * S;
             slot[poff] = xq; slot[S + poff] = vq;
             const float chk = x1.x + x1.y + x1.z + v1.x + v1.y + v1.z;
@@ -199,9 +204,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                                                               float4 *__restrict__ adjx, float4 *__restrict__ adjv, const float *__restrict__ frames,
                                                               int n_frames, int stride) {
     extern __shared__ float4 smem4[];
-    const int N = rd.N, M = rd.M, PL = 4 * M;
-    float4 *sx = smem4, *sv = smem4 + N, *sa = smem4 + 2 * N;
-    float4 *sf = smem4 + 3 * N;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
+    const int N = rd.N, M = rd.M, PL = 4 * M, L = rd.L;
+    float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
+    float4 *sf = smem4 + 3 * L;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
     uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 2 * PL);
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
     uint16_t *s_slots = s_owner + ((N + 7) & ~7);
@@ -272,7 +277,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             }
             contact_adjoint(cp, x, v, af, ax, av);
             bx = ax; bv = av;
-            sx[po.p] = xq; sv[po.p] = vq; sa[po.p] = make_float4(af.x, af.y, af.z, 0.f);
+            sx[po.lp] = xq; sv[po.lp] = vq; sa[po.lp] = make_float4(af.x, af.y, af.z, 0.f);
             vnext = vq; xq = xp; vq = vp;
         }
         __syncthreads();
@@ -371,6 +376,43 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
         const unsigned short li[4] = {idx[e].x, idx[e].y, idx[e].z, idx[e].w};
         for (int k = 0; k < 4; k++) slots[pos[li[k]]++] = (uint16_t)(k * M + e);
     }
+    // staging indices by greedy 8-colouring of the (quarter-warp, vertex) read groups
+    std::vector<uint16_t> rloc(N);
+    int Lsp = 8;
+    {
+        const int nq = (M + 7) / 8;
+        std::vector<std::vector<int>> groups((size_t)nq * 4), of_part(N);
+        for (int e = 0; e < M; e++) {
+            const int li[4] = {idx[e].x, idx[e].y, idx[e].z, idx[e].w};
+            for (int k = 0; k < 4; k++) {
+                const int g = (e / 8) * 4 + k;
+                if (std::find(groups[g].begin(), groups[g].end(), li[k]) == groups[g].end()) { groups[g].push_back(li[k]); of_part[li[k]].push_back(g); }
+            }
+        }
+        std::vector<int> colour(N, -1), csize(8, 0);
+        const int cap = (N + 7) / 8 + 1;
+        auto assign = [&](int q) {
+            if (colour[q] >= 0) return;
+            unsigned forbid = 0;
+            for (int g : of_part[q])
+                for (int r : groups[g])
+                    if (colour[r] >= 0) forbid |= 1u << colour[r];
+            int best = -1;
+            for (int cc = 0; cc < 8; cc++)
+                if (!(forbid >> cc & 1u) && csize[cc] < cap && (best < 0 || csize[cc] < csize[best])) best = cc;
+            if (best < 0)
+                for (int cc = 0; cc < 8; cc++)
+                    if (csize[cc] < cap && (best < 0 || csize[cc] < csize[best])) best = cc;
+            colour[q] = best;
+            csize[best]++;
+        };
+        for (int e = 0; e < M; e++) { assign(idx[e].x); assign(idx[e].y); assign(idx[e].z); assign(idx[e].w); }
+        for (int q = 0; q < N; q++) assign(q);  // particles no tet touches
+        std::fill(csize.begin(), csize.end(), 0);
+        for (int q = 0; q < N; q++) { rloc[q] = (uint16_t)(colour[q] + 8 * csize[colour[q]]); csize[colour[q]]++; }
+        for (int cc = 0; cc < 8; cc++) Lsp = std::max(Lsp, 8 * csize[cc]);
+        for (int e = 0; e < M; e++) idx[e] = make_ushort4(rloc[idx[e].x], rloc[idx[e].y], rloc[idx[e].z], rloc[idx[e].w]);
+    }
     char *p = (char *)d_workspace + off;
     auto take = [&](size_t n) { char *q = p; p += (n + 255) & ~(size_t)255; return q; };
     ushort4 *d_idx = (ushort4 *)take(idx.size() * sizeof(ushort4));
@@ -381,7 +423,9 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
     std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
     uint16_t *d_owner = (uint16_t *)take(owner.size() * 2);
+    uint16_t *d_rloc = (uint16_t *)take(rloc.size() * 2);
     cudaError_t ce = cudaMemcpyAsync(d_owner, owner.data(), owner.size() * 2, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_rloc, rloc.data(), rloc.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_slots, slots.data(), slots.size() * 2, cudaMemcpyHostToDevice, st);
@@ -392,9 +436,10 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     rh->rd.M = M; rh->rd.N = N;
     rh->rd.nthreads = ((M + rh->ept - 1) / rh->ept + 31) / 32 * 32;
     rh->rd.kpp = rh->rd.nthreads >= 4 * N ? 4 : (rh->rd.nthreads >= 2 * N ? 2 : 1);
+    rh->rd.L = Lsp; rh->rd.rloc = d_rloc;
     rh->rd.idx = d_idx; rh->rd.owner = d_owner; rh->rd.csr_ptr = d_ptr; rh->rd.csr_slots = d_slots;
-    rh->smem_fwd = res_smem(N, M, 1, false);
-    rh->smem_adj = res_smem(N, M, 2, true);
+    rh->smem_fwd = res_smem(Lsp, N, M, 1, false);
+    rh->smem_adj = res_smem(Lsp, N, M, 2, true);
     m->res_host = rh;
     int rc = GS_OK;
     if (rh->ept == 1 && rh->rd.nthreads <= 320) {
