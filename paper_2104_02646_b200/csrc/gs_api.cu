@@ -148,6 +148,40 @@ extern "C" int gs_tape_create(gs_model *m, int n_substeps, int checkpoint_every,
 }
 extern "C" void gs_tape_destroy(gs_tape *t) { delete t; }
 
+// Runs `body(stream)` (a fixed sequence of kernel launches) through a CUDA graph: captured once on the tape's private
+// stream, then replayed on the caller's stream -- for small meshes the rollout is bound by per-launch latency
+// (SURVEY.md 8(a) a7 / north_star (6)).  Falls back to direct launches while per-kernel timing is on or if capture fails.
+template <class F>
+static int graph_run(gs_model *m, gs_tape *t, cudaGraphExec_t *exec, uint64_t *n_launch, cudaStream_t st, F body) {
+    if (m->timing || t->no_graph) return body(st);
+    if (!*exec) {
+        const uint64_t n0 = g_launches;
+        cudaGraph_t g = nullptr;
+        bool ok = t->cap_stream || cudaStreamCreateWithFlags(&t->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaStreamBeginCapture(t->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        int rc = GS_OK;
+        if (ok) {
+            rc = body(t->cap_stream);
+            ok = cudaStreamEndCapture(t->cap_stream, &g) == cudaSuccess && g != nullptr && rc == GS_OK;
+        }
+        if (ok) {
+            *n_launch = g_launches - n0;
+            ok = cudaGraphInstantiate(exec, g, 0) == cudaSuccess;
+        }
+        if (g) cudaGraphDestroy(g);
+        g_launches = n0;
+        if (!ok) {
+            cudaGetLastError();
+            *exec = nullptr;
+            t->no_graph = true;
+            return rc != GS_OK ? rc : body(st);
+        }
+    }
+    GS_CUDA(cudaGraphLaunch(*exec, st), "cudaGraphLaunch");
+    g_launches += *n_launch;
+    return GS_OK;
+}
+
 extern "C" int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const float *d_v0, float *d_x_T, float *d_v_T, gs_stream stream) {
     GS_REQUIRE(m && t && d_x0 && d_v0, GS_EINVAL, "null argument");
     GS_REQUIRE(t->m == m, GS_EINVAL, "tape belongs to another model");
@@ -157,10 +191,13 @@ extern "C" int gs_rollout(gs_model *m, gs_tape *t, const float *d_x0, const floa
     if (m->plan == GS_PLAN_RESIDENT && t->K == 1) {  // a checkpointed tape of a resident model runs the streaming loop
         GS_TRY(resident_rollout(m, t, st));
     } else {
-        for (int s = 0; s < t->T; s++) {
-            const int a = t->slot_fwd(s), b = t->slot_fwd(s + 1);
-            GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, st));
-        }
+        GS_TRY(graph_run(m, t, &t->g_fwd, &t->g_fwd_launches, st, [&](cudaStream_t q) {
+            for (int s = 0; s < t->T; s++) {
+                const int a = t->slot_fwd(s), b = t->slot_fwd(s + 1);
+                GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, q));
+            }
+            return (int)GS_OK;
+        }));
     }
     t->has_rollout = true;
     return launch_unpack(m, t->slot_x(t->slot_final()), t->slot_v(t->slot_final()), d_x_T, d_v_T, st);
@@ -187,20 +224,29 @@ extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int fr
     if (m->plan == GS_PLAN_RESIDENT && t->K == 1) {
         GS_TRY(resident_rollout_backward(m, t, n_frames, frame_stride, d_adj_x_frames, st));
     } else {
-        for (int c = t->n_ck - 1; c >= 0; c--) {
-            const int t0 = c * t->K, t1 = t0 + t->K < t->T ? t0 + t->K : t->T;
-            for (int s = t0; s + 1 < t1; s++) {  // regenerate the segment's states from its checkpoint
-                const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
-                GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, st));
-            }
-            for (int s = t1 - 1; s >= t0; s--) {
-                const float *cot = nullptr;
-                if (n_frames > 0 && (s + 1) % frame_stride == 0 && (s + 1) / frame_stride <= n_frames)
-                    cot = d_adj_x_frames + (size_t)((s + 1) / frame_stride - 1) * frame_elems;
-                const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
-                GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, st));
-            }
+        if (t->g_bwd && (t->g_bwd_frames != d_adj_x_frames || t->g_bwd_n_frames != n_frames || t->g_bwd_stride != frame_stride)) {
+            cudaGraphExecDestroy(t->g_bwd);  // other frame arguments: capture again
+            t->g_bwd = nullptr;
         }
+        t->g_bwd_frames = d_adj_x_frames; t->g_bwd_n_frames = n_frames; t->g_bwd_stride = frame_stride;
+        GS_TRY(graph_run(m, t, &t->g_bwd, &t->g_bwd_launches, st, [&](cudaStream_t q) {
+            GS_TRY(launch_flush_grads(m, q));  // fixed flush positions whatever ran before (resets the 32-substep counter)
+            for (int c = t->n_ck - 1; c >= 0; c--) {
+                const int t0 = c * t->K, t1 = t0 + t->K < t->T ? t0 + t->K : t->T;
+                for (int s = t0; s + 1 < t1; s++) {  // regenerate the segment's states from its checkpoint
+                    const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
+                    GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, q));
+                }
+                for (int s = t1 - 1; s >= t0; s--) {
+                    const float *cot = nullptr;
+                    if (n_frames > 0 && (s + 1) % frame_stride == 0 && (s + 1) / frame_stride <= n_frames)
+                        cot = d_adj_x_frames + (size_t)((s + 1) / frame_stride - 1) * frame_elems;
+                    const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
+                    GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, q));
+                }
+            }
+            return (int)GS_OK;
+        }));
     }
     GS_TRY(launch_flush_grads(m, st));
     return launch_unpack(m, m->d_adjx, m->d_adjv, d_adj_x0, d_adj_v0, st);

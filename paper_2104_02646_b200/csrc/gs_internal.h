@@ -120,6 +120,19 @@ struct gs_tape {
     size_t S = 0;  // float4 elements per array per slot = E * N
     float4 *base = nullptr;
     bool has_rollout = false;
+    // CUDA graphs of the streaming plan's launch sequences (the tape slots, and hence every kernel argument, are fixed
+    // per tape): captured on a private stream at the first rollout / backward, replayed on the caller's stream
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t g_fwd = nullptr, g_bwd = nullptr;
+    uint64_t g_fwd_launches = 0, g_bwd_launches = 0;
+    const float *g_bwd_frames = nullptr;  // the backward graph is specific to these frame arguments
+    int g_bwd_n_frames = -1, g_bwd_stride = 0;
+    bool no_graph = false;                // capture failed once: launch directly from then on
+    ~gs_tape() {
+        if (g_fwd) cudaGraphExecDestroy(g_fwd);
+        if (g_bwd) cudaGraphExecDestroy(g_bwd);
+        if (cap_stream) cudaStreamDestroy(cap_stream);
+    }
     // slot index helpers (each slot = x4[S] then v4[S])
     float4 *slot_x(int s) const { return base + (size_t)(2 * s) * S; }
     float4 *slot_v(int s) const { return base + (size_t)(2 * s + 1) * S; }
