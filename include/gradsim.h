@@ -18,7 +18,9 @@
  *    256-byte aligned.
  *  - All device work is enqueued on the caller's stream (a cudaStream_t passed as void*) and is
  *    asynchronous; only gs_model_create, gs_tape_create, gs_check_finite and the *_host entry
- *    points synchronise.  One model is used from one stream at a time.
+ *    points synchronise.  One model is used from one stream at a time.  On the streaming plan gs_rollout and
+ *    gs_rollout_backward replay a CUDA graph of their launch sequence (captured on a private stream the first time a
+ *    tape is used, or again when the frame arguments change); per-kernel timing switches the graphs off.
  *  - State arrays crossing the ABI are fp32, CALLER'S particle order, [E][N][3] (env-major).
  *    Per-element / per-particle parameter and gradient arrays are [E][count], caller's element order.
  *    Internally particles and elements are reordered (Morton) and tiled; the permutation is applied

@@ -275,9 +275,9 @@ extern "C" int gs_check_finite(gs_model *m, gs_stream stream, int *first_bad_sub
 
 // ------------------------------------------------------------------------------------------ losses
 // one CTA per environment
-__global__ void __launch_bounds__(256) k_loss_centroid(int N, const float *__restrict__ x, const float *__restrict__ target, float scale, int accumulate,
+__global__ void __launch_bounds__(1024) k_loss_centroid(int N, const float *__restrict__ x, const float *__restrict__ target, float scale, int accumulate,
                                                        float *__restrict__ loss, float *__restrict__ adj) {
-    __shared__ float red[3][8];
+    __shared__ float red[3][32];
     __shared__ float cen[3];
     const int env = blockIdx.x, tid = threadIdx.x;
     const float *xe = x + (size_t)env * N * 3;
@@ -302,9 +302,9 @@ __global__ void __launch_bounds__(256) k_loss_centroid(int N, const float *__res
         for (int i = tid; i < 3 * N; i += blockDim.x) ae[i] = k * cen[i % 3];
     }
 }
-__global__ void __launch_bounds__(256) k_loss_pos(int N, const float *__restrict__ x, const float *__restrict__ ref, float scale, int accumulate,
+__global__ void __launch_bounds__(1024) k_loss_pos(int N, const float *__restrict__ x, const float *__restrict__ ref, float scale, int accumulate,
                                                   float *__restrict__ loss, float *__restrict__ adj) {
-    __shared__ float red[8];
+    __shared__ float red[32];
     const int env = blockIdx.x, tid = threadIdx.x;
     const size_t o = (size_t)env * N * 3;
     float s = 0.f;
@@ -327,7 +327,7 @@ __global__ void __launch_bounds__(256) k_loss_pos(int N, const float *__restrict
 extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, const float *d_target, float scale, int accumulate, float *d_loss,
                                 float *d_adj_x, gs_stream stream) {
     GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_target && d_loss, GS_EINVAL, "bad argument");
-    k_loss_centroid<<<n_envs, 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_target, scale, accumulate, d_loss, d_adj_x);
+    k_loss_centroid<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_target, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_centroid");
     g_launches++;
     return GS_OK;
@@ -335,7 +335,7 @@ extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, c
 extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate, float *d_loss, float *d_adj_x,
                            gs_stream stream) {
     GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_ref && d_loss, GS_EINVAL, "bad argument");
-    k_loss_pos<<<n_envs, 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_ref, scale, accumulate, d_loss, d_adj_x);
+    k_loss_pos<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_ref, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_pos");
     g_launches++;
     return GS_OK;
