@@ -52,6 +52,13 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
 __device__ __forceinline__ void red_add_f32(float *addr, float a) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
 }
+// Programmatic dependent launch: the hot-path kernels are launched with programmatic stream serialization, so a kernel
+// may start (and run its prologue: barrier init, bulk copies of STATIC tile data) while its predecessor drains.
+// grid_dep_wait() blocks until the predecessor grid has completed and its writes are visible; nothing the predecessor
+// produces may be touched before it.  Both are no-ops in a kernel launched without the attribute.
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
@@ -224,6 +231,7 @@ struct TilePipe {
             load_static(first, 0);
         }
         mbar_wait(bars + 2, 0);
+        grid_dep_wait();  // the particle arrays gathered from here on are the predecessor kernel's output
         gather(first, 0, 0);
         int s3 = 0, q3 = 0;  // i % 3, i / 3: ids of the CTA's j-th item use id buffer j % 3 for the (j / 3)-th time
         for (int i = 0; i < cnt; i++) {
@@ -349,6 +357,8 @@ __device__ __forceinline__ ContactParams contact_params(const ModelDev &md, int 
 __global__ void __launch_bounds__(256) k_particles_fwd(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
                                                        float4 *__restrict__ f4, float4 *__restrict__ xo, float4 *__restrict__ vo, int substep) {
     const size_t total = (size_t)md.E * md.N;
+    grid_dep_launch();
+    grid_dep_wait();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / md.N);
         const float4 xq = x4[i], vq = v4[i], fq = f4[i];
@@ -371,6 +381,8 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
                                                        const float4 *__restrict__ v4n, const float *__restrict__ frame_cot,
                                                        float4 *__restrict__ adjx, float4 *__restrict__ adjv, float4 *__restrict__ adjf) {
     const size_t total = (size_t)md.E * md.N;
+    grid_dep_launch();
+    grid_dep_wait();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / md.N), id = (int)(i - (size_t)env * md.N);
         const float4 xq = x4[i], vq = v4[i], vn = v4n[i];
@@ -548,6 +560,18 @@ static inline int grid_for(size_t n, int block = 256) {
     return (int)(g < 1 ? 1 : (g > cap ? cap : g));
 }
 
+// launch with programmatic stream serialization (see grid_dep_wait)
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 template <class K>
 static int tile_kernel_setup(K kern, int smem, int *ctas_per_sm) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -594,8 +618,8 @@ static inline int tile_grid(const gs_model *m, int occ) {
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
     if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
-                 k_elements_fwd<<<tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st>>>(m->dev, x, v, m->d_f));
-    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", k_particles_fwd<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, m->d_f, xo, vo, substep));
+                 launch_pdl(k_elements_fwd, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, x, v, m->d_f));
+    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, substep));
     return GS_OK;
 }
 
@@ -603,10 +627,10 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
 // m->d_adjx / m->d_adjv (updated in place); frame_cot (caller order, may be null) is added to adj_x first.
 int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st) {
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
-             k_particles_adj<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
+             launch_pdl(k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                 k_elements_adj<<<tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st>>>(m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+                 launch_pdl(k_elements_adj, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
     return GS_OK;
 }
