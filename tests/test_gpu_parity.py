@@ -149,6 +149,45 @@ def test_checkpointed_backward_matches_full_tape():
             assert rel_inf(ck[k], ref[k]) <= TOL_GRAD, (K, k)
 
 
+def test_graph_replay_direct_launch_and_recapture_agree():
+    """gs_rollout / gs_rollout_backward replay a CUDA graph captured at first use (streaming plan).  The replay, the
+    direct-launch path (per-kernel timing on) and a re-captured backward (other frame-cotangent buffer) must agree up
+    to the summation order of the atomics, and the launch counter must advance the same in both modes."""
+    sc = scenes.make_scene(2, small=True)  # frame losses + checkpointed tape: forward replays inside the backward graph
+    ref = orc.run_scene(sc)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    L = gs.lib()
+    n0 = L.gs_launch_count()
+    a = gpu_run_scene(sc, ref["target"], model=m)      # captures
+    n1 = L.gs_launch_count()
+    b = gpu_run_scene(sc, ref["target"], model=m)      # new tape + new cotangent buffer: captures again
+    n2 = L.gs_launch_count()
+    gs._check(L.gs_kernel_timing(m.h, 1))              # direct launches
+    c = gpu_run_scene(sc, ref["target"], model=m)
+    n3 = L.gs_launch_count()
+    gs._check(L.gs_kernel_timing(m.h, 0))
+    assert n1 - n0 == n2 - n1 == n3 - n2 > 4 * sc.n_substeps
+    for k in ("xT", "adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_tet_damp", "g_mass"):
+        assert rel_inf(b[k], a[k]) <= 1e-4 and rel_inf(c[k], a[k]) <= 1e-4, k
+        assert rel_inf(a[k], ref[k]) <= (TOL_ROLLOUT if k == "xT" else TOL_GRAD), k
+    # one tape, several rollouts and backward passes with different cotangents: replay, then re-capture on a new pointer
+    tape = m.tape(sc.n_substeps, sc.checkpoint_every)
+    x0, v0 = dev(sc.x0), dev(sc.v0)
+    r = scenes.rng_for(2, "misc", 21)
+    c1 = dev(r.normal(size=sc.x0.shape).astype(np.float32))
+    outs = []
+    for rep in range(3):
+        m.zero_grads()
+        xT, _ = tape.rollout(x0, v0)
+        cot = c1 if rep < 2 else (2.0 * c1).contiguous()
+        ax0, _ = tape.backward(adj_x_T=cot)
+        outs.append((host(xT), host(ax0), host(m.param_grads("tet_mu"))))
+    assert np.abs(outs[0][0] - outs[1][0]).max() <= 1e-6 * sc.extent() and np.abs(outs[0][0] - outs[2][0]).max() <= 1e-6 * sc.extent()
+    assert rel_inf(outs[1][1], outs[0][1]) <= 1e-4 and rel_inf(outs[1][2], outs[0][2]) <= 1e-4
+    assert rel_inf(outs[2][1], 2.0 * outs[0][1]) <= 1e-4 and rel_inf(outs[2][2], 2.0 * outs[0][2]) <= 1e-4
+    assert m.check_finite() == -1
+
+
 def test_tape_read_and_intermediate_states():
     sc = scenes.make_scene(0, small=True)
     o = orc.Oracle(sc)
