@@ -260,6 +260,40 @@ def test_single_element_meshes_and_ragged_tiles():
         assert rel_inf(host(vg), vo) <= 2e-5
 
 
+def test_scattered_connectivity_large_tile_particle_lists():
+    """Elements that share almost no particles: every 128-element tile touches ~350 distinct particles (3-4x the
+    structured meshes), which exercises the largest per-tile particle lists, the staging-index colouring with many
+    classes and gather-list runs of length one.  One substep forward + adjoint against the oracle."""
+    r = np.random.default_rng(11)
+    N, Mt = 3000, 700
+    x = np.stack([r.uniform(0, 3, N), r.uniform(0.0, 0.02, N), r.uniform(0, 3, N)], 1)
+    tris = []
+    while len(tris) < Mt:
+        i = r.choice(N, 3, replace=False)
+        a = np.linalg.norm(np.cross(x[i[1]] - x[i[0]], x[i[2]] - x[i[0]]))
+        if a > 0.05:  # well away from degenerate
+            tris.append(i)
+    sc = scenes.custom_scene(x, tris=np.array(tris), hinges=np.zeros((0, 4), np.int32), tri_mu=50.0, tri_lam=50.0, tri_damp=0.1, mass=0.1)
+    xs = (sc.x0 + 0.01 * r.uniform(-1, 1, sc.x0.shape)).astype(np.float32)
+    xs[..., 1] -= 0.01  # part of the cloud below the ground plane
+    vs = r.uniform(-0.3, 0.3, sc.x0.shape).astype(np.float32)
+    o = orc.Oracle(sc)
+    xo, vo = o.step(xs, vs)
+    m = gs.Model(sc)
+    xg, vg = m.step_forward(dev(xs), dev(vs))
+    assert m.check_finite() == -1
+    assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
+    assert rel_inf(host(vg), vo) <= 2e-5
+    bx, bv = r.normal(size=xs.shape).astype(np.float32), r.normal(size=xs.shape).astype(np.float32)
+    o.zero_grads()
+    ax, av = o.step_adjoint(xs, vs, bx, bv)
+    m.zero_grads()
+    axg, avg = m.step_backward(dev(xs), dev(vs), dev(bx), dev(bv))
+    assert rel_inf(host(axg), ax) <= 1e-4 and rel_inf(host(avg), av) <= 1e-4
+    for g in ("tri_mu", "tri_lambda", "tri_damp", "mass"):
+        assert rel_inf(host(m.param_grads(g)), o.grads(g)) <= TOL_GRAD, g
+
+
 def test_pinned_particles_do_not_move_and_have_zero_mass_gradient():
     sc = scenes.make_scene(1, small=True)
     ref = orc.run_scene(sc)
