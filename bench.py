@@ -63,15 +63,24 @@ def element_stream_bytes(sc, table):
     return E * (sc.tets.shape[0] * table["tet"] + sc.tris.shape[0] * table["tri"] + sc.hinges.shape[0] * table["hinge"])
 
 
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the hot kernels, from the ncu --set full
+# captures summarised under profiles/ (r1c_ncu_config4_streaming.md, r1c_ncu_config3_resident.md).  The resident kernels
+# were captured at 64 substeps: bytes per substep of the launch, scaled by the rollout length.
+NCU_TRAFFIC = {
+    "config4-large-1000000tets-522242tris": {
+        "k_elements_fwd": ("per_launch", 162274048), "k_particles_fwd": ("per_launch", 22873856),
+        "k_elements_adj": ("per_launch", 200240383), "k_particles_adj": ("per_launch", 40039936),
+    },
+    "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3555996), "k_resident_adj": ("per_substep", 4708488)},
+}
+
+
 def ncu_traffic(workload, kernel, T):
-    """DRAM bytes per launch of `kernel` from the committed ncu capture of this workload (profiles/traffic.json), or None."""
-    try:
-        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[workload][kernel]
-    except Exception:
+    """DRAM bytes per launch of `kernel` from the committed ncu capture of this workload, or None."""
+    kind, val = NCU_TRAFFIC.get(workload, {}).get(kernel, (None, None))
+    if kind is None:
         return None
-    if "bytes_per_launch" in t:
-        return t["bytes_per_launch"]
-    return t["bytes_per_substep"] * T
+    return val if kind == "per_launch" else val * T
 
 
 def hbm_peak():
