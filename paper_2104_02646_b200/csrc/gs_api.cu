@@ -324,9 +324,100 @@ __global__ void __launch_bounds__(1024) k_loss_pos(int N, const float *__restric
     }
 }
 
+// ---- large meshes: the same losses over many CTAs per environment (one CTA per environment leaves 147 SMs idle on a
+// 476 k-particle scene).  No scratch memory exists (the library allocates nothing), so the centroid's partial sums
+// travel through the TAIL of the adj_x output itself: pass A writes kLossParts partial sums there, pass B (all CTAs) reads
+// them, finishes loss and cotangent everywhere except that tail, pass C (one CTA per environment) reads the partials
+// into registers, synchronises, and only then overwrites the tail with the cotangent.
+constexpr int kLossParts = 128;     // CTAs per environment
+constexpr int kLossMinN = 32768;    // below this one CTA per environment is faster than three launches
+
+__device__ __forceinline__ void block_sum3(float &sx, float &sy, float &sz, float (*red)[32]) {
+    const int tid = threadIdx.x;
+    for (int o = 16; o > 0; o >>= 1) { sx += __shfl_xor_sync(0xffffffffu, sx, o); sy += __shfl_xor_sync(0xffffffffu, sy, o); sz += __shfl_xor_sync(0xffffffffu, sz, o); }
+    if ((tid & 31) == 0) { red[0][tid >> 5] = sx; red[1][tid >> 5] = sy; red[2][tid >> 5] = sz; }
+    __syncthreads();
+    if (tid < 3) {
+        float s = 0.f;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) s += red[tid][w];
+        red[tid][0] = s;
+    }
+    __syncthreads();
+    sx = red[0][0]; sy = red[1][0]; sz = red[2][0];
+}
+// particles [lo, hi) of part b
+__device__ __forceinline__ void part_range(int N, int b, int &lo, int &hi) {
+    const int per = (N + kLossParts - 1) / kLossParts;
+    lo = b * per < N ? b * per : N;
+    hi = lo + per < N ? lo + per : N;
+}
+__global__ void __launch_bounds__(256) k_centroid_partial(int N, const float *__restrict__ x, float *__restrict__ adj) {
+    __shared__ float red[3][32];
+    const int env = blockIdx.y, b = blockIdx.x;
+    int lo, hi;
+    part_range(N, b, lo, hi);
+    const float *xe = x + (size_t)env * N * 3;
+    float sx = 0.f, sy = 0.f, sz = 0.f;
+    for (int i = lo + threadIdx.x; i < hi; i += blockDim.x) { sx += xe[3 * i]; sy += xe[3 * i + 1]; sz += xe[3 * i + 2]; }
+    block_sum3(sx, sy, sz, red);
+    if (threadIdx.x < 3) adj[(size_t)env * N * 3 + (size_t)3 * N - 3 * kLossParts + 3 * b + threadIdx.x] = threadIdx.x == 0 ? sx : (threadIdx.x == 1 ? sy : sz);
+}
+// tail_only = 0: every CTA finishes the centroid from the partials and writes its particles' cotangent except the tail;
+// tail_only = 1 (grid.x = 1): reads the partials, then overwrites the tail
+__global__ void __launch_bounds__(256) k_centroid_finish(int N, const float *__restrict__ target, float scale, int accumulate, float *__restrict__ loss,
+                                                         float *__restrict__ adj, int tail_only) {
+    __shared__ float cen[3];
+    const int env = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
+    float *ae = adj + (size_t)env * N * 3;
+    const size_t tail = (size_t)3 * N - 3 * kLossParts;
+    if (tid < 3) {
+        float s = 0.f;
+        for (int q = 0; q < kLossParts; q++) s += ae[tail + 3 * q + tid];
+        cen[tid] = s / (float)N - target[env * 3 + tid];
+    }
+    __syncthreads();
+    const float k = 2.0f * scale / (float)N;
+    if (tail_only) {
+        for (size_t i = tail + tid; i < (size_t)3 * N; i += blockDim.x) ae[i] = k * cen[i % 3];
+        return;
+    }
+    if (b == 0 && tid == 0) {
+        const float L = scale * (cen[0] * cen[0] + cen[1] * cen[1] + cen[2] * cen[2]);
+        loss[env] = accumulate ? loss[env] + L : L;
+    }
+    int lo, hi;
+    part_range(N, b, lo, hi);
+    for (size_t i = (size_t)3 * lo + tid; i < (size_t)3 * hi && i < tail; i += blockDim.x) ae[i] = k * cen[i % 3];
+}
+__global__ void __launch_bounds__(256) k_loss_pos_parts(int N, const float *__restrict__ x, const float *__restrict__ ref, float scale,
+                                                        float *__restrict__ loss, float *__restrict__ adj) {
+    __shared__ float red[3][32];
+    const int env = blockIdx.y, b = blockIdx.x;
+    int lo, hi;
+    part_range(N, b, lo, hi);
+    const size_t o = (size_t)env * N * 3;
+    float s = 0.f, u = 0.f, w = 0.f;
+    for (size_t i = (size_t)3 * lo + threadIdx.x; i < (size_t)3 * hi; i += blockDim.x) {
+        const float dlt = x[o + i] - ref[o + i];
+        s = fmaf(dlt, dlt, s);
+        if (adj) adj[o + i] = 2.0f * scale * dlt;
+    }
+    block_sum3(s, u, w, red);
+    if (threadIdx.x == 0) atomicAdd(loss + env, scale * s);
+}
+
 extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, const float *d_target, float scale, int accumulate, float *d_loss,
                                 float *d_adj_x, gs_stream stream) {
     GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_target && d_loss, GS_EINVAL, "bad argument");
+    if (n_particles >= kLossMinN && d_adj_x && n_envs <= 65535) {
+        cudaStream_t st = (cudaStream_t)stream;
+        k_centroid_partial<<<dim3(kLossParts, n_envs), 256, 0, st>>>(n_particles, d_x, d_adj_x);
+        k_centroid_finish<<<dim3(kLossParts, n_envs), 256, 0, st>>>(n_particles, d_target, scale, accumulate, d_loss, d_adj_x, 0);
+        k_centroid_finish<<<dim3(1, n_envs), 256, 0, st>>>(n_particles, d_target, scale, accumulate, d_loss, d_adj_x, 1);
+        GS_CUDA(cudaGetLastError(), "k_centroid_partial / k_centroid_finish");
+        g_launches += 3;
+        return GS_OK;
+    }
     k_loss_centroid<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_target, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_centroid");
     g_launches++;
@@ -335,6 +426,14 @@ extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, c
 extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate, float *d_loss, float *d_adj_x,
                            gs_stream stream) {
     GS_REQUIRE(n_envs > 0 && n_particles > 0 && d_x && d_ref && d_loss, GS_EINVAL, "bad argument");
+    if (n_particles >= kLossMinN && n_envs <= 65535) {
+        cudaStream_t st = (cudaStream_t)stream;
+        if (!accumulate) GS_CUDA(cudaMemsetAsync(d_loss, 0, sizeof(float) * (size_t)n_envs, st), "zero loss");
+        k_loss_pos_parts<<<dim3(kLossParts, n_envs), 256, 0, st>>>(n_particles, d_x, d_ref, scale, d_loss, d_adj_x);
+        GS_CUDA(cudaGetLastError(), "k_loss_pos_parts");
+        g_launches++;
+        return GS_OK;
+    }
     k_loss_pos<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_ref, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_pos");
     g_launches++;

@@ -304,6 +304,33 @@ def test_pinned_particles_do_not_move_and_have_zero_mass_gradient():
     assert (got["g_mass"][:, pin] == 0).all()
 
 
+@pytest.mark.parametrize("N", [1000, 40000])
+def test_loss_helpers_match_numpy(N):
+    """gs_loss_centroid / gs_loss_pos against their definitions, on both sides of the particle
+    count where they switch from one CTA per environment to 128 CTAs per environment; accumulate and no-adjoint variants."""
+    r = np.random.default_rng(5)
+    E = 2
+    x = r.normal(size=(E, N, 3)).astype(np.float32)
+    ref = (x + 0.1 * r.normal(size=x.shape)).astype(np.float32)
+    tgt = r.normal(size=(E, 3)).astype(np.float32)
+    xd = x.astype(np.float64)
+    c = xd.mean(1) - tgt
+    loss, adj = gs.loss_centroid(dev(x), dev(tgt), scale=0.7)
+    assert rel_inf(host(loss), 0.7 * (c * c).sum(1)) <= 1e-4
+    want = np.broadcast_to((2 * 0.7 / N) * c[:, None, :], x.shape)
+    assert np.abs(host(adj) - want).max() <= 1e-5 * np.abs(want).max()
+    loss2, _ = gs.loss_centroid(dev(x), dev(tgt), scale=0.3, loss=loss, accumulate=True)
+    assert rel_inf(host(loss2), 1.0 * (c * c).sum(1)) <= 1e-4
+    loss3, none = gs.loss_centroid(dev(x), dev(tgt), want_adj=False)
+    assert none is None and rel_inf(host(loss3), (c * c).sum(1)) <= 1e-4
+    d = xd - ref
+    lp, ap = gs.loss_pos(dev(x), dev(ref), scale=0.25)
+    assert rel_inf(host(lp), 0.25 * (d * d).sum((1, 2))) <= 1e-4
+    assert np.abs(host(ap) - 0.5 * d).max() <= 1e-6
+    lp2, _ = gs.loss_pos(dev(x), dev(ref), scale=0.75, loss=lp, accumulate=True)
+    assert rel_inf(host(lp2), 1.0 * (d * d).sum((1, 2))) <= 1e-4
+
+
 def test_error_paths():
     x = np.array([[0, 0.01, 0], [0.1, 0.01, 0], [0, 0.11, 0], [0, 0.01, 0.1]], float)
     with pytest.raises(gs.GradSimError) as e:  # inverted tet
