@@ -286,19 +286,26 @@ class Model:
         return Tape(self, n_substeps, checkpoint_every)
 
     def rollout_loss_backward_host(self, tape, h_x0, h_v0, h_target, groups=()):
-        """bench.py's e2e leg: HOST (numpy / pinned torch CPU) in, HOST out, one C call."""
+        """bench.py's e2e leg: HOST (numpy / pinned torch CPU) in, HOST out, one C call.  The returned pinned tensors
+        are owned by the model and overwritten by the next call."""
         torch = _torch()
         L = lib()
         if self._scratch is None:
             self._scratch = _aligned_bytes(L.gs_host_scratch_bytes(self.h), self.device)
         E, N = self.E, self.N
-        out = dict(
-            loss=torch.empty(E, dtype=torch.float32).pin_memory(),
-            adj_x0=torch.empty((E, N, 3), dtype=torch.float32).pin_memory(),
-            adj_v0=torch.empty((E, N, 3), dtype=torch.float32).pin_memory(),
-        )
         gl = [GROUPS[g] for g in groups]
-        gbuf = [torch.empty((E, self.group_count(g)), dtype=torch.float32).pin_memory() for g in groups]
+        key = tuple(gl)
+        if getattr(self, "_host_out", None) is None or self._host_out[0] != key:
+            # pinned result buffers are allocated once and reused (page-locking 20+ MB per call costs milliseconds)
+            bufs = dict(
+                loss=torch.empty(E, dtype=torch.float32).pin_memory(),
+                adj_x0=torch.empty((E, N, 3), dtype=torch.float32).pin_memory(),
+                adj_v0=torch.empty((E, N, 3), dtype=torch.float32).pin_memory(),
+            )
+            gb = [torch.empty((E, self.group_count(g)), dtype=torch.float32).pin_memory() for g in groups]
+            self._host_out = (key, bufs, gb)
+        out = dict(self._host_out[1])
+        gbuf = self._host_out[2]
         garr = (C.c_int * max(len(gl), 1))(*gl)
         gptr = (C.c_void_p * max(len(gl), 1))(*[b.data_ptr() for b in gbuf])
         _check(L.gs_rollout_loss_backward_host(
