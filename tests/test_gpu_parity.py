@@ -129,6 +129,10 @@ def test_resident_plan_edge_cases():
     assert np.abs(a["xT"] - b["xT"]).max() <= 1e-4 * sc0.extent()
     for k in ("adj_x0", "g_tet_mu", "g_mass"):
         assert rel_inf(b[k], ref0[k]) <= TOL_GRAD, k
+    # the resident plan has no atomics: two runs are bitwise identical (hazard H6 does not apply to it)
+    a2 = gpu_run_scene(sc0, ref0["target"], K=1, plan=gs.GS_PLAN_RESIDENT)
+    for k in ("xT", "vT", "adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_tet_damp", "g_mass"):
+        assert np.array_equal(a[k], a2[k]), k
     # non-finite states are reported with their substep by the resident kernel too
     m = a["model"]
     tape = m.tape(8)
