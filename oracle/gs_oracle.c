@@ -58,6 +58,7 @@ typedef struct {
     double *g_tet_mu, *g_tet_lambda, *g_tet_damp; /* [E][M] */
     double *g_tri_mu, *g_tri_lambda, *g_tri_damp; /* [E][Mt] */
     double *g_mass;                               /* [E][N] */
+    double *g_hinge_kb;                           /* [E][Mh]  dL/dk_b per hinge (Table 5: bending stiffness is optimisable) */
 } orc_model;
 
 static char g_err[256] = "";
@@ -130,7 +131,7 @@ void orc_destroy(orc_model *m) {
     free(m->ke); free(m->kd); free(m->kf); free(m->mu_c);
     free(m->inc_ptr); free(m->inc_slot);
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
-    free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass);
+    free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb);
     free(m);
 }
 
@@ -189,6 +190,7 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_tet_mu = zeros_d((size_t)E * M); m->g_tet_lambda = zeros_d((size_t)E * M); m->g_tet_damp = zeros_d((size_t)E * M);
     m->g_tri_mu = zeros_d((size_t)E * Mt); m->g_tri_lambda = zeros_d((size_t)E * Mt); m->g_tri_damp = zeros_d((size_t)E * Mt);
     m->g_mass = zeros_d((size_t)E * N);
+    m->g_hinge_kb = zeros_d((size_t)E * Mh);
 
     /* tets: D_m = [X1-X0, X2-X0, X3-X0] (columns), B = D_m^-1, V = det(D_m)/6  (V_e) */
     for (int e = 0; e < M; e++) {
@@ -253,18 +255,20 @@ void orc_get_rest(const orc_model *m, double *tet_B, double *tet_V, double *tri_
     if (l0) memcpy(l0, m->hinge_l0, sizeof(double) * m->Mh);
 }
 
-/* set one parameter group for all envs; group: 0 tet_mu 1 tet_lambda 2 tet_damp 3 tri_mu 4 tri_lambda 5 tri_damp 6 mass */
+/* set one parameter group for all envs; group: 0 tet_mu 1 tet_lambda 2 tet_damp 3 tri_mu 4 tri_lambda 5 tri_damp 6 mass
+   7 hinge_kb (shared by all environments: row 0 of v is taken) */
 int orc_set_params(orc_model *m, int group, const double *v) {
     double *dst[7] = {m->tet_mu, m->tet_lambda, m->tet_damp, m->tri_mu, m->tri_lambda, m->tri_damp, m->mass};
     size_t n[7] = {(size_t)m->M, (size_t)m->M, (size_t)m->M, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->N};
+    if (group == 7) { memcpy(m->hinge_kb, v, sizeof(double) * m->Mh); return 0; }
     if (group < 0 || group > 6) return -1;
     memcpy(dst[group], v, sizeof(double) * n[group] * m->E);
     return 0;
 }
 int orc_get_grads(const orc_model *m, int group, double *out) {
-    const double *src[7] = {m->g_tet_mu, m->g_tet_lambda, m->g_tet_damp, m->g_tri_mu, m->g_tri_lambda, m->g_tri_damp, m->g_mass};
-    size_t n[7] = {(size_t)m->M, (size_t)m->M, (size_t)m->M, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->N};
-    if (group < 0 || group > 6) return -1;
+    const double *src[8] = {m->g_tet_mu, m->g_tet_lambda, m->g_tet_damp, m->g_tri_mu, m->g_tri_lambda, m->g_tri_damp, m->g_mass, m->g_hinge_kb};
+    size_t n[8] = {(size_t)m->M, (size_t)m->M, (size_t)m->M, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->N, (size_t)m->Mh};
+    if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
     return 0;
 }
@@ -273,6 +277,7 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_tet_mu, 0, sizeof(double) * E * m->M); memset(m->g_tet_lambda, 0, sizeof(double) * E * m->M); memset(m->g_tet_damp, 0, sizeof(double) * E * m->M);
     memset(m->g_tri_mu, 0, sizeof(double) * E * m->Mt); memset(m->g_tri_lambda, 0, sizeof(double) * E * m->Mt); memset(m->g_tri_damp, 0, sizeof(double) * E * m->Mt);
     memset(m->g_mass, 0, sizeof(double) * E * m->N);
+    memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
 }
 
 /* ---------------------------------------------------------------- tets */
@@ -455,7 +460,8 @@ static void hinge_force(const double *x[4], double theta0, double l0, double kb,
     for (int k = 0; k < 4; k++) v_scale(s, d[k], f[k]);
 }
 /* VJP = JVP (conservative force, symmetric Jacobian): adj_x_j += -E'' s d_j + E' Dd_j[a], s = sum d_i.a_i */
-static void hinge_adjoint(const double *x[4], const double *a[4], double theta0, double l0, double kb, double ax[4][3]) {
+/* f_i = k_b l0 sin(ph) d_i is linear in k_b: dL/dk_b += l0 sin(ph) sum_i d_i . a_i */
+static void hinge_adjoint(const double *x[4], const double *a[4], double theta0, double l0, double kb, double ax[4][3], double *g_kb) {
     const double *x1 = x[0], *x2 = x[1], *x3 = x[2], *x4 = x[3];
     double p13[3], p14[3], p23[3], p24[3], n1[3], n2[3], e[3], eh[3];
     v_sub(x1, x3, p13); v_sub(x1, x4, p14); v_sub(x2, x3, p23); v_sub(x2, x4, p24);
@@ -494,6 +500,7 @@ static void hinge_adjoint(const double *x[4], const double *a[4], double theta0,
     double ph = 0.5 * (th - theta0);
     double E1 = kb * l0 * sin(ph), E2 = 0.5 * kb * l0 * cos(ph);
     for (int k = 0; k < 4; k++) for (int r = 0; r < 3; r++) ax[k][r] += -E2 * s * d[k][r] + E1 * dd[k][r];
+    if (g_kb) *g_kb += l0 * sin(ph) * s;
 }
 
 /* ---------------------------------------------------------------- contact (A7, A8) */
@@ -705,7 +712,7 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         const double *xe[4], *ae[4];
         for (int k = 0; k < 4; k++) { xe[k] = x + 3 * h[k]; ae[k] = af + 3 * h[k]; }
         double cx[4][3] = {{0}};
-        hinge_adjoint(xe, ae, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], cx);
+        hinge_adjoint(xe, ae, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], cx, &m->g_hinge_kb[(size_t)env * Mh + e]);
         memcpy(slots + 3 * (4 * (size_t)M + 3 * (size_t)Mt + 4 * (size_t)e), cx, sizeof cx);
     }
 #pragma omp parallel for if (par) schedule(static)

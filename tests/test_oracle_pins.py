@@ -320,8 +320,9 @@ def test_p7_step_param_gradients_vs_fd(group):
     o.step_adjoint(x, v, bx, bv)
     g = o.grads(group)[0]
     attr = {"tet_mu": "tet_mu", "tet_lambda": "tet_lambda", "tet_damp": "tet_damp", "tri_mu": "tri_mu",
-            "tri_lambda": "tri_lambda", "tri_damp": "tri_damp", "mass": "mass"}[group]
-    base = getattr(sc, attr).astype(np.float64)[0]
+            "tri_lambda": "tri_lambda", "tri_damp": "tri_damp", "mass": "mass", "hinge_kb": "hinge_kb"}[group]
+    base = getattr(sc, attr).astype(np.float64)
+    base = base if group == "hinge_kb" else base[0]  # k_b is one array shared by all environments
     fd = np.zeros_like(base)
     for e in range(base.size):
         h = 1e-6 * base[e]
@@ -373,7 +374,7 @@ def test_p8_rollout_adjoint_vs_central_fd(which):
     else:  # config-1-shaped cloth with pins, bending, contact
         sc = scenes.cloth_scene(n=5, n_substeps=200, y0=0.003)
         sc.tri_mu[:] = rng.uniform(5e2, 2e3, sc.tri_mu.shape)
-        groups = ["tri_mu", "tri_lambda", "tri_damp", "mass"]
+        groups = ["tri_mu", "tri_lambda", "tri_damp", "mass", "hinge_kb"]
     T, lt = sc.n_substeps, sc.loss_times()
     o = orc.Oracle(sc)
     x0, v0 = sc.x0.astype(np.float64), sc.v0.astype(np.float64)
@@ -399,7 +400,8 @@ def test_p8_rollout_adjoint_vs_central_fd(which):
         return False
 
     for g in groups:
-        base = getattr(sc, {"mass": "mass"}.get(g, g)).astype(np.float64)[0]
+        base = getattr(sc, {"mass": "mass"}.get(g, g)).astype(np.float64)
+        base = base if g == "hinge_kb" else base[0]
         scale = np.abs(grads[g]).max()
         assert scale > 0
         idx = rng.choice(base.size, size=min(6, base.size), replace=False)
@@ -458,8 +460,9 @@ def test_p8_smooth_regime_strict():
     ax0, av0 = o.rollout_backward(ro, [T], cot)
     for g in orc.GROUPS:
         an = o.grads(g)[0].copy()
-        base = getattr(sc, g).astype(np.float64)[0]
-        for e in rng.choice(base.size, size=4, replace=False):
+        base = getattr(sc, g).astype(np.float64)
+        base = base if g == "hinge_kb" else base[0]  # k_b is one array shared by all environments
+        for e in rng.choice(base.size, size=min(4, base.size), replace=False):
             if g == "mass" and sc.pinned[e]:
                 assert an[e] == 0
                 continue
