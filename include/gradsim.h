@@ -57,7 +57,9 @@ enum gs_param_group {
     GS_TET_MU = 0, GS_TET_LAMBDA = 1, GS_TET_DAMP = 2,
     GS_TRI_MU = 3, GS_TRI_LAMBDA = 4, GS_TRI_DAMP = 5,
     GS_MASS = 6,
-    GS_NUM_GROUPS = 7
+    GS_HINGE_KB = 7, /* bending stiffness per hinge: one array [Mh] shared by all environments --
+                        gs_set_params takes row 0 of its [E][Mh] argument; gs_param_grads returns dL/dk_b per environment */
+    GS_NUM_GROUPS = 8
 };
 
 /* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */
@@ -121,7 +123,7 @@ void gs_model_destroy(gs_model *m);
 int gs_model_plan(const gs_model *m);
 int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, int32_t *n_envs);
 
-/* Replace one parameter group from DEVICE values [E][count] in caller order (count = M, Mt or N). */
+/* Replace one parameter group from DEVICE values [E][count] in caller order (count = M, Mt, N or Mh). */
 int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream stream);
 
 /*

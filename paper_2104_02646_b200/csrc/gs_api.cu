@@ -447,7 +447,7 @@ extern "C" size_t gs_host_scratch_bytes(const gs_model *m) {
     if (!m) return 0;
     const size_t st = al256((size_t)m->E * m->N * 3 * sizeof(float));
     int cmax = m->N;
-    for (int t = 0; t < 2; t++) cmax = cmax > m->counts[t] ? cmax : m->counts[t];
+    for (int t = 0; t < N_TYPES; t++) cmax = cmax > m->counts[t] ? cmax : m->counts[t];
     return 6 * st + al256((size_t)m->E * 3 * sizeof(float)) + al256((size_t)m->E * sizeof(float)) + al256((size_t)m->E * cmax * sizeof(float)) + 256;
 }
 
@@ -478,7 +478,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
     for (int k = 0; k < n_groups; k++) {
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
-        const int c = g == GS_MASS ? m->N : m->counts[g / 3];
+        const int c = g == GS_MASS ? m->N : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3]);
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
         // the staging buffer is reused: order the copy before the next group's kernel on the same stream

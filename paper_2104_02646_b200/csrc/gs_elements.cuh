@@ -239,7 +239,8 @@ __device__ __forceinline__ void hinge_force(const vec3 x[4], float s0h, float c0
     f[0] = s * d[0]; f[1] = s * d[1]; f[2] = s * d[2]; f[3] = s * d[3];
 }
 // VJP = JVP (the force is conservative): ax_j = -E'' s d_j + E' Dd_j[a], s = sum_i d_i . a_i
-__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float s0h, float c0h, float kl, vec3 ax[4]) {
+// gkb = dL/dk_b of this substep: the force is linear in k_b, dL/dk_b = l0 sin((theta - theta0)/2) sum_i d_i . a_i
+__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float s0h, float c0h, float kl, float l0, vec3 ax[4], float &gkb) {
     HingeGeo h;
     hinge_geo(x, s0h, c0h, h);
     vec3 d[4];
@@ -258,6 +259,7 @@ __device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], 
     // so the plain sum cancels to ~1e-4 of its terms and would lose that many digits in fp32
     const float s = dot(h.m1, h.c13 * q14 - h.c14 * q13) + dot(h.m2, h.c23 * q24 - h.c24 * q23);
     const float E1 = kl * h.sh, E2s = 0.5f * kl * h.ch * s;
+    gkb = l0 * h.sh * s;
     ax[0] = madd(-E2s * d[0], E1, madd(dL * h.m1, h.L, dm1));
     ax[1] = madd(-E2s * d[1], E1, madd(dL * h.m2, h.L, dm2));
     ax[2] = madd(-E2s * d[2], E1, madd(madd(madd(dc14 * h.m1, h.c14, dm1), dc24, h.m2), h.c24, dm2));

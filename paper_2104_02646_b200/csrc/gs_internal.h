@@ -12,6 +12,7 @@ namespace gs {
 
 enum { T_TET = 0, T_TRI = 1, T_HINGE = 2, N_TYPES = 3 };
 static const int kArity[N_TYPES] = {4, 3, 4};
+static const int kNumGrads[N_TYPES] = {3, 3, 1};  // accumulated parameter gradients per element: (mu, lambda, k_damp) x2, k_b
 
 constexpr int kTileElems = 128;      // elements per tile = threads per CTA of the streaming element kernels
 constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
@@ -19,7 +20,7 @@ constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-
 // Byte layout of one tile's RECORD: everything static a tile of kTileElems elements needs, packed contiguously so
 // that ONE bulk copy (cp.async.bulk, TMA) brings it into shared memory:
 //   lidx   ushort4[256]  tile-local particle indices (w unused for triangles)
-//   c0     float4[256]   tets: B[0..3]; tris: 2x2 B; hinges: (sin(theta0/2), cos(theta0/2), kb * l0, -)
+//   c0     float4[256]   tets: B[0..3]; tris: 2x2 B; hinges: (sin(theta0/2), cos(theta0/2), kb * l0, l0)
 //   c1     float4[256]   tets: B[4..7]
 //   c2     float2[256]   tets: (B[8], V)
 //   area   float[256]    tris: rest area
@@ -55,8 +56,8 @@ struct ElemDev {
                                 // assigned by colouring: particles read by the same quarter-warp for the same vertex get
                                 // different residues mod 8, i.e. different 16-byte bank groups (conflict-free LDS.128)
     float *par;                 // [E][n_tiles][3][kTileElems]  mu, lambda, k_damp (tets, tris)
-    float *g32;                 // [3][E][cpad] per-substep fp32 accumulators (mu, lambda, damp)
-    double *g64;                // [3][E][cpad] fp64 masters
+    float *g32;                 // [kNumGrads][E][cpad] per-substep fp32 accumulators (mu, lambda, damp; hinges: k_b)
+    double *g64;                // [kNumGrads][E][cpad] fp64 masters
     const int *perm;            // [count] internal -> caller element index
 };
 // index of parameter q (0 mu, 1 lambda, 2 damp) of internal element e of environment env inside ElemDev::par

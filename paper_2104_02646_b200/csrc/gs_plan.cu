@@ -73,8 +73,9 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
             L.g32[t] = b.take<float>(3 * E * cp);
             L.g64[t] = b.take<double>(3 * E * cp);
         } else {
-            L.par[t] = L.g32[t] = nullptr;
-            L.g64[t] = nullptr;
+            L.par[t] = nullptr;
+            L.g32[t] = b.take<float>(E * cp);
+            L.g64[t] = b.take<double>(E * cp);
         }
         L.perm[t] = b.take<int>(c);
     }
@@ -229,7 +230,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                 if (!(l0 > 0) || !(a1 > 1e-12) || !(a2 > 1e-12)) { set_error("hinge %d: degenerate rest shape", e); return GS_EMESH; }
                 d3 eh = scl(1.0 / l0, ed);
                 double th = std::atan2(dt3(crs(scl(1 / a1, n1), scl(1 / a2, n2)), eh), dt3(n1, n2) / (a1 * a2));
-                r0[e] = make_float4((float)std::sin(0.5 * th), (float)std::cos(0.5 * th), (float)((double)d->hinge_kb[e] * l0), 0.f);
+                r0[e] = make_float4((float)std::sin(0.5 * th), (float)std::cos(0.5 * th), (float)((double)d->hinge_kb[e] * l0), (float)l0);
             }
         }
         std::iota(hs.perm.begin(), hs.perm.end(), 0);
@@ -390,6 +391,11 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                 if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * cp, stream);
                 if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
             }
+        }
+        if (t == T_HINGE && c > 0) {
+            cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * (size_t)E * cp, stream);
+            if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * (size_t)E * cp, stream);
+            if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
         }
         ElemDev &ed = dev.es[t];
         ed.count = c; ed.cpad = cp; ed.n_tiles = nt; ed.pmax = pmax; ed.lmax = lmax; ed.rec_bytes = rb;

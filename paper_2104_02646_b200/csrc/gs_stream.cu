@@ -461,7 +461,9 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4];
-                hinge_adjoint(x, a, c0.x, c0.y, c0.z, ax);
+                float gkb;
+                hinge_adjoint(x, a, c0.x, c0.y, c0.z, c0.w, ax, gkb);
+                red_add_f32(es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid, gkb);
 #pragma unroll
                 for (int k = 0; k < 4; k++) so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
             }
@@ -550,6 +552,14 @@ __global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ pe
         const float val = src[(size_t)env * count + perm[e]];
         if (q < 0) { if (dst[i] != 0.f) dst[i] = 1.0f / val; }  // pinned particles stay pinned
         else dst[par_index(n_tiles, env, e, q)] = val;
+    }
+}
+
+// k_b is shared by all environments and lives in the hinge records as kl = k_b * l0 (c0.z; l0 in c0.w): row 0 of src
+__global__ void k_set_hinge_kb(char *__restrict__ rec, int rec_bytes, const int *__restrict__ perm, const float *__restrict__ src, int count) {
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+        float4 *c0 = reinterpret_cast<float4 *>(rec + (size_t)(e / kTileElems) * rec_bytes + RecLayout<T_HINGE>::oC0) + (e % kTileElems);
+        c0->z = src[perm[e]] * c0->w;
     }
 }
 
@@ -647,8 +657,8 @@ int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, flo
 
 int launch_flush_grads(gs_model *m, cudaStream_t st) {
     m->steps_since_flush = 0;
-    for (int t = 0; t < 2; t++) {
-        const size_t n = 3 * (size_t)m->E * m->hes[t].cpad;
+    for (int t = 0; t < N_TYPES; t++) {
+        const size_t n = m->counts[t] ? kNumGrads[t] * (size_t)m->E * m->hes[t].cpad : 0;
         if (!n) continue;
         GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
@@ -657,8 +667,8 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
 }
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
     m->steps_since_flush = 0;
-    for (int t = 0; t < 2; t++) {
-        const size_t n = 3 * (size_t)m->E * m->hes[t].cpad;
+    for (int t = 0; t < N_TYPES; t++) {
+        const size_t n = m->counts[t] ? kNumGrads[t] * (size_t)m->E * m->hes[t].cpad : 0;
         if (!n) continue;
         GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
@@ -671,7 +681,7 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     if (group == GS_MASS) {
         k_get_grads<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass64, m->dev.perm_p, d_out, m->E, m->N, m->N);
     } else {
-        const int t = group / 3, q = group % 3, c = m->counts[t];
+        const int t = group == GS_HINGE_KB ? T_HINGE : group / 3, q = group == GS_HINGE_KB ? 0 : group % 3, c = m->counts[t];
         if (c == 0) return GS_OK;
         k_get_grads<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].g64 + (size_t)q * m->E * m->hes[t].cpad, m->dev.es[t].perm, d_out, m->E, c, m->hes[t].cpad);
     }
@@ -681,6 +691,10 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st) {
     if (group == GS_MASS) {
         k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 0, -1);
+    } else if (group == GS_HINGE_KB) {
+        const int c = m->counts[T_HINGE];
+        if (c == 0) return GS_OK;
+        k_set_hinge_kb<<<grid_for((size_t)c), 256, 0, st>>>(const_cast<char *>(m->dev.es[T_HINGE].rec), m->dev.es[T_HINGE].rec_bytes, m->dev.es[T_HINGE].perm, d_values, c);
     } else {
         const int t = group / 3, c = m->counts[t];
         if (c == 0) return GS_OK;

@@ -33,6 +33,8 @@ def _groups(sc):
         g += ["tet_mu", "tet_lambda", "tet_damp"]
     if sc.tris.shape[0]:
         g += ["tri_mu", "tri_lambda", "tri_damp"]
+    if sc.hinges.shape[0]:
+        g += ["hinge_kb"]
     return g
 
 

@@ -30,6 +30,8 @@ def _grad_groups(sc):
         g += ["tet_mu", "tet_lambda", "tet_damp"]
     if sc.tris.shape[0]:
         g += ["tri_mu", "tri_lambda", "tri_damp"]
+    if sc.hinges.shape[0]:
+        g += ["hinge_kb"]
     return g
 
 
@@ -221,6 +223,32 @@ def test_set_params_changes_the_result_like_the_oracle():
     xg, vg = m.step_forward(dev(x), dev(v))
     assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
     assert rel_inf(host(vg), vo) <= 2e-5
+
+
+def test_set_hinge_kb_changes_forces_and_gradients_like_the_oracle():
+    """Bending stiffness is a settable parameter with a gradient: after gs_set_params the
+    substep and dL/dk_b follow the oracle with the same values."""
+    sc = scenes.make_scene(1, small=True)
+    x, v = scenes.perturbed_state(sc)
+    r = scenes.rng_for(1, "misc", 8)
+    x = (x + 0.002 * r.normal(size=x.shape)).astype(np.float32)  # fold the sheet a little: non-zero dihedral angles
+    new_kb = r.uniform(2.0, 30.0, sc.hinge_kb.shape).astype(np.float32)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    m.set_params("hinge_kb", dev(new_kb[None]))
+    sc.hinge_kb = new_kb
+    o = orc.Oracle(sc)
+    xo, vo = o.step(x, v)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
+    assert rel_inf(host(vg), vo) <= 2e-5
+    bx, bv = r.normal(size=x.shape).astype(np.float32), r.normal(size=x.shape).astype(np.float32)
+    o.zero_grads()
+    o.step_adjoint(x, v, bx, bv)
+    m.zero_grads()
+    m.step_backward(dev(x), dev(v), dev(bx), dev(bv))
+    g = o.grads("hinge_kb")
+    assert np.abs(g).max() > 0
+    assert rel_inf(host(m.param_grads("hinge_kb")), g) <= TOL_GRAD
 
 
 # ------------------------------------------------------------------------------------------ edge cases
