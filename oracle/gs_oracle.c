@@ -58,6 +58,7 @@ typedef struct {
     double *g_tet_mu, *g_tet_lambda, *g_tet_damp; /* [E][M] */
     double *g_tri_mu, *g_tri_lambda, *g_tri_damp; /* [E][Mt] */
     double *g_mass;                               /* [E][N] */
+    double *g_ke, *g_kd, *g_kf, *g_muc;           /* [E]  dL/d(contact parameters) per environment (Table 5: contact parameters are optimisable) */
     double *g_hinge_kb;                           /* [E][Mh]  dL/dk_b per hinge (Table 5: bending stiffness is optimisable) */
 } orc_model;
 
@@ -131,7 +132,7 @@ void orc_destroy(orc_model *m) {
     free(m->ke); free(m->kd); free(m->kf); free(m->mu_c);
     free(m->inc_ptr); free(m->inc_slot);
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
-    free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb);
+    free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb); free(m->g_ke); free(m->g_kd); free(m->g_kf); free(m->g_muc);
     free(m);
 }
 
@@ -191,6 +192,7 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_tri_mu = zeros_d((size_t)E * Mt); m->g_tri_lambda = zeros_d((size_t)E * Mt); m->g_tri_damp = zeros_d((size_t)E * Mt);
     m->g_mass = zeros_d((size_t)E * N);
     m->g_hinge_kb = zeros_d((size_t)E * Mh);
+    m->g_ke = zeros_d((size_t)E); m->g_kd = zeros_d((size_t)E); m->g_kf = zeros_d((size_t)E); m->g_muc = zeros_d((size_t)E);
 
     /* tets: D_m = [X1-X0, X2-X0, X3-X0] (columns), B = D_m^-1, V = det(D_m)/6  (V_e) */
     for (int e = 0; e < M; e++) {
@@ -261,6 +263,11 @@ int orc_set_params(orc_model *m, int group, const double *v) {
     double *dst[7] = {m->tet_mu, m->tet_lambda, m->tet_damp, m->tri_mu, m->tri_lambda, m->tri_damp, m->mass};
     size_t n[7] = {(size_t)m->M, (size_t)m->M, (size_t)m->M, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->N};
     if (group == 7) { memcpy(m->hinge_kb, v, sizeof(double) * m->Mh); return 0; }
+    if (group >= 8 && group <= 11) { /* 8 ke 9 kd 10 kf 11 mu_c: one value per environment */
+        double *cd[4] = {m->ke, m->kd, m->kf, m->mu_c};
+        memcpy(cd[group - 8], v, sizeof(double) * m->E);
+        return 0;
+    }
     if (group < 0 || group > 6) return -1;
     memcpy(dst[group], v, sizeof(double) * n[group] * m->E);
     return 0;
@@ -268,6 +275,11 @@ int orc_set_params(orc_model *m, int group, const double *v) {
 int orc_get_grads(const orc_model *m, int group, double *out) {
     const double *src[8] = {m->g_tet_mu, m->g_tet_lambda, m->g_tet_damp, m->g_tri_mu, m->g_tri_lambda, m->g_tri_damp, m->g_mass, m->g_hinge_kb};
     size_t n[8] = {(size_t)m->M, (size_t)m->M, (size_t)m->M, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->Mt, (size_t)m->N, (size_t)m->Mh};
+    if (group >= 8 && group <= 11) {
+        const double *cs[4] = {m->g_ke, m->g_kd, m->g_kf, m->g_muc};
+        memcpy(out, cs[group - 8], sizeof(double) * m->E);
+        return 0;
+    }
     if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
     return 0;
@@ -278,6 +290,7 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_tri_mu, 0, sizeof(double) * E * m->Mt); memset(m->g_tri_lambda, 0, sizeof(double) * E * m->Mt); memset(m->g_tri_damp, 0, sizeof(double) * E * m->Mt);
     memset(m->g_mass, 0, sizeof(double) * E * m->N);
     memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
+    memset(m->g_ke, 0, sizeof(double) * E); memset(m->g_kd, 0, sizeof(double) * E); memset(m->g_kf, 0, sizeof(double) * E); memset(m->g_muc, 0, sizeof(double) * E);
 }
 
 /* ---------------------------------------------------------------- tets */
@@ -515,7 +528,10 @@ static void contact_force(const orc_model *m, int env, const double *x, const do
     double coef = fmin(m->kf[env], m->mu_c[env] * fn / fmax(s, 1e-12));
     for (int r = 0; r < 3; r++) f[r] = m->n[r] * fn - coef * vt[r];
 }
-static void contact_adjoint(const orc_model *m, int env, const double *x, const double *v, const double *a, double ax[3], double av[3]) {
+/* gp[4] (may be NULL): this particle's contributions to dL/dk_e, dL/dk_d, dL/dk_f, dL/dmu_c.  With a.f = f_n afn (afn as
+   below): d/dk_e = -c afn, d/dk_d = -min(v_n, 0) afn; stick: d/dk_f = -(v_t.a_t); slip: d/dmu_c = -f_n (v_t.a_t)/s */
+static void contact_adjoint(const orc_model *m, int env, const double *x, const double *v, const double *a, double ax[3], double av[3], double *gp) {
+    if (gp) gp[0] = gp[1] = gp[2] = gp[3] = 0.0;
     double c = v_dot(m->n, x) - m->d - m->r;
     if (!(c < 0)) return;
     const double *n = m->n;
@@ -530,11 +546,14 @@ static void contact_adjoint(const orc_model *m, int env, const double *x, const 
     if (muc * fn / sg >= kf) { /* stick: f_f = -k_f v_t */
         afn = na;
         v_scale(-kf, at, avt);
+        if (gp) gp[2] = -v_dot(vt, at);
     } else { /* slip: f_f = -mu_c f_n v_t / s */
         double vta = v_dot(vt, at);
         afn = na - muc * vta / sg;
+        if (gp) gp[3] = -fn * vta / sg;
         for (int r = 0; r < 3; r++) avt[r] = -muc * fn * (at[r] / sg - vt[r] * vta / (sg * sg * sg));
     }
+    if (gp) { gp[0] = -c * afn; gp[1] = -fmin(vn, 0.0) * afn; }
     v_axpy(1.0, avt, av);
     v_axpy(-m->ke[env] * afn, n, ax);
     if (vn < 0) v_axpy(-m->kd[env] * afn, n, av);
@@ -663,6 +682,7 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
     const int N = m->N, M = m->M, Mt = m->Mt, Mh = m->Mh;
     const double dt = m->dt;
     env_forces(m, env, x, v, f, slots, ORC_ALL, par); /* total force of the forward step */
+    double *gp = (double *)malloc(sizeof(double) * 4 * (size_t)(N ? N : 1)); /* per-particle contact-parameter contributions */
     /* 1. integrate: v+ = v + (f w + g [w>0]) dt, x+ = x + v+ dt */
 #pragma omp parallel for if (par) schedule(static)
     for (int i = 0; i < N; i++) {
@@ -677,8 +697,12 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         }
         if (w > 0) m->g_mass[(size_t)env * N + i] += -w * w * aw; /* w = 1/m (A11) */
         /* 2. contact */
-        contact_adjoint(m, env, x + 3 * i, v + 3 * i, af + 3 * i, ax + 3 * i, av + 3 * i);
+        contact_adjoint(m, env, x + 3 * i, v + 3 * i, af + 3 * i, ax + 3 * i, av + 3 * i, gp + 4 * (size_t)i);
     }
+    for (int i = 0; i < N; i++) { /* serial, particle order: independent of the thread count */
+        m->g_ke[env] += gp[4 * (size_t)i]; m->g_kd[env] += gp[4 * (size_t)i + 1]; m->g_kf[env] += gp[4 * (size_t)i + 2]; m->g_muc[env] += gp[4 * (size_t)i + 3];
+    }
+    free(gp);
     /* 3-5. elements: per-element-vertex contributions into private slots, then gather per particle */
     memset(slots, 0, sizeof(double) * 3 * (m->n_slots ? m->n_slots : 1));
     memset(slots_v, 0, sizeof(double) * 3 * (m->n_slots ? m->n_slots : 1));
