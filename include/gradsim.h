@@ -59,7 +59,9 @@ enum gs_param_group {
     GS_MASS = 6,
     GS_HINGE_KB = 7, /* bending stiffness per hinge: one array [Mh] shared by all environments --
                         gs_set_params takes row 0 of its [E][Mh] argument; gs_param_grads returns dL/dk_b per environment */
-    GS_NUM_GROUPS = 8
+    GS_CONTACT_KE = 8, GS_CONTACT_KD = 9, GS_CONTACT_KF = 10, GS_CONTACT_MUC = 11, /* contact parameters (NEXT-2): one value
+                        per environment, arrays [E] (count = 1) */
+    GS_NUM_GROUPS = 12
 };
 
 /* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */

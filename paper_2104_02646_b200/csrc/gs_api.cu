@@ -478,7 +478,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
     for (int k = 0; k < n_groups; k++) {
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
-        const int c = g == GS_MASS ? m->N : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3]);
+        const int c = g == GS_MASS ? m->N : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3]));
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
         // the staging buffer is reused: order the copy before the next group's kernel on the same stream

@@ -282,8 +282,11 @@ __device__ __forceinline__ vec3 contact_force(const ContactParams &cp, const vec
     const float coef = fminf(cp.kf, __fdiv_rn(cp.mu * fn, fmaxf(s, 1e-12f)));
     return fn * cp.n - coef * vt;
 }
-// a = dL/df; adds the contact VJP to ax, av
-__device__ __forceinline__ void contact_adjoint(const ContactParams &cp, const vec3 &x, const vec3 &v, const vec3 &a, vec3 &ax, vec3 &av) {
+// a = dL/df; adds the contact VJP to ax, av.  gp[4] = this particle's contributions to dL/dk_e, dL/dk_d, dL/dk_f,
+// dL/dmu_c (zero when not in contact): with a.f = f_n afn, d/dk_e = -c afn, d/dk_d = -min(v_n, 0) afn;
+// stick: d/dk_f = -(v_t.a_t); slip: d/dmu_c = -f_n (v_t.a_t)/s
+__device__ __forceinline__ void contact_adjoint(const ContactParams &cp, const vec3 &x, const vec3 &v, const vec3 &a, vec3 &ax, vec3 &av, float gp[4]) {
+    gp[0] = gp[1] = gp[2] = gp[3] = 0.0f;
     const float c = dot(cp.n, x) - cp.d - cp.r;
     if (!(c < 0.0f)) return;
     const float vn = dot(cp.n, v);
@@ -292,16 +295,21 @@ __device__ __forceinline__ void contact_adjoint(const ContactParams &cp, const v
     const float s = sqrtf(dot(vt, vt)), sg = fmaxf(s, 1e-12f);
     const float na = dot(cp.n, a);
     const vec3 at = a - na * cp.n;
+    const float vta = dot(vt, at);
     float afn;
     vec3 avt;
     if (__fdiv_rn(cp.mu * fn, sg) >= cp.kf) {  // stick
         afn = na;
         avt = -cp.kf * at;
+        gp[2] = -vta;
     } else {  // slip
-        const float vta = dot(vt, at), is = __fdiv_rn(1.0f, sg);
+        const float is = __fdiv_rn(1.0f, sg);
         afn = na - cp.mu * vta * is;
         avt = (-cp.mu * fn * is) * (at - (vta * is * is) * vt);
+        gp[3] = -fn * vta * is;
     }
+    gp[0] = -c * afn;
+    gp[1] = -fminf(vn, 0.0f) * afn;
     av += avt;
     ax += (-cp.ke * afn) * cp.n;
     if (vn < 0.0f) av += (-cp.kd * afn) * cp.n;

@@ -15,6 +15,7 @@ static const int kArity[N_TYPES] = {4, 3, 4};
 static const int kNumGrads[N_TYPES] = {3, 3, 1};  // accumulated parameter gradients per element: (mu, lambda, k_damp) x2, k_b
 
 constexpr int kTileElems = 128;      // elements per tile = threads per CTA of the streaming element kernels
+constexpr int kConSlots = 64;        // accumulator slots per environment for the contact-parameter gradients
 constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
 
 // Byte layout of one tile's RECORD: everything static a tile of kTileElems elements needs, packed contiguously so
@@ -75,6 +76,9 @@ struct ModelDev {
     const float *inv_mass;            // [E][N] internal order (0 = pinned)
     float *gmass32;                   // [E][N]
     double *gmass64;                  // [E][N]
+    float *gcon32;                    // [E][kConSlots][4] dL/d(k_e, k_d, k_f, mu_c): fp32 partial sums, spread over slots so
+                                      // that the warps of a launch do not all reduce into one L2 sector
+    double *gcon64;                   // [E][4] fp64 masters
     int *bad;                         // first non-finite substep (INT_MAX = none)
 };
 

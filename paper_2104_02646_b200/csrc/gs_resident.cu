@@ -53,9 +53,10 @@ struct ResHost {
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
 // shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
+// adjoint only: per-particle accumulators of the contact-parameter gradients, double[4][N] then float[4][N]
 static size_t res_smem(int L, int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) +
-           al16((size_t)4 * M * 2);
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)4 * N * 12) : 0) +
+           al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)4 * M * 2);
 }
 
 static bool resident_fits(const gs_model_desc *d) {
@@ -207,7 +208,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     const int N = rd.N, M = rd.M, PL = 4 * M, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
     float4 *sf = smem4 + 3 * L;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 2 * PL);
+    // dL/d(k_e, k_d, k_f, mu_c): per-particle partial sums (only the particle's lead lane touches its entries), fp32 chunks
+    // of kFlushEvery substeps folded into fp64 (hazard H4), summed in particle order at the end: deterministic
+    double *dgc = reinterpret_cast<double *>(sf + 2 * PL);  // [4][N]
+    float *sgc = reinterpret_cast<float *>(dgc + 4 * N);     // [4][N]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((4 * N * 12 + 15) & ~15));
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
     uint16_t *s_slots = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
@@ -231,6 +236,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         xq = tape[(size_t)(2 * (T - 1)) * S + poff]; vq = tape[(size_t)(2 * (T - 1) + 1) * S + poff];
         if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
+    if (po.lead)
+        for (int q = 0; q < 4; q++) { dgc[q * N + po.p] = 0.0; sgc[q * N + po.p] = 0.f; }
     const size_t frame_elems = (size_t)md.E * N * 3;
     float gm32 = 0.f;
     double gm64 = 0.0;
@@ -275,7 +282,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 const vec3 dvf = (vec3(vnext) - v) - dt * g;
                 gm32 += -w * dot(dvf, lv);
             }
-            contact_adjoint(cp, x, v, af, ax, av);
+            float gp[4];
+            contact_adjoint(cp, x, v, af, ax, av, gp);
+            if (gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f) {
+#pragma unroll
+                for (int q = 0; q < 4; q++) sgc[q * N + po.p] += gp[q];
+            }
             bx = ax; bv = av;
             sx[po.lp] = xq; sv[po.lp] = vq; sa[po.lp] = make_float4(af.x, af.y, af.z, 0.f);
             vnext = vq; xq = xp; vq = vp;
@@ -301,6 +313,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             }
         }
         if ((s & (kFlushEvery - 1)) == 0) {  // fold the fp32 chunk into fp64 (hazard H4)
+            if (po.lead) {
+#pragma unroll
+                for (int q = 0; q < 4; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
+            }
             gm64 += (double)gm32; gm32 = 0.f;
 #pragma unroll
             for (int j = 0; j < EPT; j++)
@@ -318,6 +334,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
         adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
         md.gmass64[poff] += gm64;
+    }
+    __syncthreads();
+    if (tid < 4) {
+        double t = 0.0;
+        for (int p = 0; p < N; p++) t += dgc[tid * N + p];
+        md.gcon64[(size_t)env * 4 + tid] += t;
     }
     const ElemDev &es = md.es[T_TET];
     const size_t gstride = (size_t)md.E * es.cpad;

@@ -383,28 +383,56 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
     const size_t total = (size_t)md.E * md.N;
     grid_dep_launch();
     grid_dep_wait();
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int env = (int)(i / md.N), id = (int)(i - (size_t)env * md.N);
-        const float4 xq = x4[i], vq = v4[i], vn = v4n[i];
-        vec3 bx(adjx[i]), bv(adjv[i]);
-        if (frame_cot) {
-            const float *c = frame_cot + ((size_t)env * md.N + md.perm_p[id]) * 3;
-            bx += vec3(c[0], c[1], c[2]);
+    const int lane = threadIdx.x & 31;
+    // block-uniform trip count: the contact-parameter gradients are reduced with full-warp shuffles
+    for (size_t base = (size_t)blockIdx.x * blockDim.x; base < total; base += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = base + threadIdx.x;
+        float gp[4] = {0.f, 0.f, 0.f, 0.f};
+        int env = -1;
+        if (i < total) {
+            env = (int)(i / md.N);
+            const int id = (int)(i - (size_t)env * md.N);
+            const float4 xq = x4[i], vq = v4[i], vn = v4n[i];
+            vec3 bx(adjx[i]), bv(adjv[i]);
+            if (frame_cot) {
+                const float *c = frame_cot + ((size_t)env * md.N + md.perm_p[id]) * 3;
+                bx += vec3(c[0], c[1], c[2]);
+            }
+            const float w = xq.w, dt = md.dt;
+            const vec3 x(xq), v(vq);
+            const vec3 lv = madd(bv, dt, bx);  // cotangent of v+
+            const vec3 af = (dt * w) * lv;
+            vec3 ax = bx, av = lv;
+            if (w > 0.0f) {
+                // f w dt = v+ - v- - g dt  =>  dL/dm = -w^2 dt f.lv = -w (v+ - v- - g dt).lv   (A11)
+                const vec3 dvf = (vec3(vn) - v) - dt * vec3(md.gx, md.gy, md.gz);
+                md.gmass32[i] += -w * dot(dvf, lv);
+            }
+            contact_adjoint(contact_params(md, env), x, v, af, ax, av, gp);
+            adjx[i] = make_float4(ax.x, ax.y, ax.z, 0.f);
+            adjv[i] = make_float4(av.x, av.y, av.z, 0.f);
+            adjf[i] = make_float4(af.x, af.y, af.z, 0.f);
         }
-        const float w = xq.w, dt = md.dt;
-        const vec3 x(xq), v(vq);
-        const vec3 lv = madd(bv, dt, bx);  // cotangent of v+
-        const vec3 af = (dt * w) * lv;
-        vec3 ax = bx, av = lv;
-        if (w > 0.0f) {
-            // f w dt = v+ - v- - g dt  =>  dL/dm = -w^2 dt f.lv = -w (v+ - v- - g dt).lv   (A11)
-            const vec3 dvf = (vec3(vn) - v) - dt * vec3(md.gx, md.gy, md.gz);
-            md.gmass32[i] += -w * dot(dvf, lv);
+        // dL/d(k_e, k_d, k_f, mu_c) of this warp's particles in contact: shuffle-reduce, one reduction per parameter
+        const bool mine = gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f;
+        const unsigned act = __ballot_sync(0xffffffffu, mine);
+        if (act) {
+            const int env0 = __shfl_sync(0xffffffffu, env, __ffs(act) - 1);
+            float *slot = md.gcon32 + ((size_t)env0 * kConSlots + (blockIdx.x & (kConSlots - 1))) * 4;
+            if (__all_sync(0xffffffffu, !mine || env == env0)) {
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    float t = gp[q];
+                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                    if (lane == 0 && t != 0.f) red_add_f32(slot + q, t);
+                }
+            } else if (mine) {  // a warp that straddles two environments (N not a multiple of 32)
+                float *sl = md.gcon32 + ((size_t)env * kConSlots + (blockIdx.x & (kConSlots - 1))) * 4;
+#pragma unroll
+                for (int q = 0; q < 4; q++)
+                    if (gp[q] != 0.f) red_add_f32(sl + q, gp[q]);
+            }
         }
-        contact_adjoint(contact_params(md, env), x, v, af, ax, av);
-        adjx[i] = make_float4(ax.x, ax.y, ax.z, 0.f);
-        adjv[i] = make_float4(av.x, av.y, av.z, 0.f);
-        adjf[i] = make_float4(af.x, af.y, af.z, 0.f);
     }
 }
 
@@ -555,6 +583,26 @@ __global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ pe
     }
 }
 
+// contact-parameter gradients: fold the fp32 slots of (env, q) into the fp64 master and clear them
+__global__ void k_flush_contact(float *__restrict__ g32, double *__restrict__ g64, int n, int zero_master) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int env = i >> 2, q = i & 3;
+        double s = 0.0;
+        for (int k = 0; k < kConSlots; k++) {
+            float *p = g32 + ((size_t)env * kConSlots + k) * 4 + q;
+            s += (double)*p;
+            *p = 0.f;
+        }
+        g64[i] = zero_master ? 0.0 : g64[i] + s;
+    }
+}
+__global__ void k_get_contact(const double *__restrict__ g64, float *__restrict__ out, int E, int q) {
+    for (int env = blockIdx.x * blockDim.x + threadIdx.x; env < E; env += gridDim.x * blockDim.x) out[env] = (float)g64[env * 4 + q];
+}
+__global__ void k_set_scalar(float *__restrict__ dst, const float *__restrict__ src, int E) {
+    for (int env = blockIdx.x * blockDim.x + threadIdx.x; env < E; env += gridDim.x * blockDim.x) dst[env] = src[env];
+}
+
 // k_b is shared by all environments and lives in the hinge records as kl = k_b * l0 (c0.z; l0 in c0.w): row 0 of src
 __global__ void k_set_hinge_kb(char *__restrict__ rec, int rec_bytes, const int *__restrict__ perm, const float *__restrict__ src, int count) {
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
@@ -663,6 +711,7 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
         GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
     GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
+    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * 4), 256, 0, st>>>(m->dev.gcon32, m->dev.gcon64, m->E * 4, 0));
     return GS_OK;
 }
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
@@ -673,6 +722,7 @@ int launch_zero_grads(gs_model *m, cudaStream_t st) {
         GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
     GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
+    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * 4), 256, 0, st>>>(m->dev.gcon32, m->dev.gcon64, m->E * 4, 1));
     return GS_OK;
 }
 int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
@@ -680,6 +730,8 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     if (rc != GS_OK) return rc;
     if (group == GS_MASS) {
         k_get_grads<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass64, m->dev.perm_p, d_out, m->E, m->N, m->N);
+    } else if (group >= GS_CONTACT_KE && group <= GS_CONTACT_MUC) {
+        k_get_contact<<<grid_for((size_t)m->E), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, group - GS_CONTACT_KE);
     } else {
         const int t = group == GS_HINGE_KB ? T_HINGE : group / 3, q = group == GS_HINGE_KB ? 0 : group % 3, c = m->counts[t];
         if (c == 0) return GS_OK;
@@ -691,6 +743,9 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st) {
     if (group == GS_MASS) {
         k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 0, -1);
+    } else if (group >= GS_CONTACT_KE && group <= GS_CONTACT_MUC) {
+        const float *dst[4] = {m->dev.ke, m->dev.kd, m->dev.kf, m->dev.muc};
+        k_set_scalar<<<grid_for((size_t)m->E), 256, 0, st>>>(const_cast<float *>(dst[group - GS_CONTACT_KE]), d_values, m->E);
     } else if (group == GS_HINGE_KB) {
         const int c = m->counts[T_HINGE];
         if (c == 0) return GS_OK;

@@ -8,6 +8,8 @@ seeded inputs (north_star tolerances; "relative" as in DESIGN.md reading A18):
 Small variants of the five configs (several tiles + a ragged tail, seconds in the oracle) run
 element-by-element; the full-size configs are compared in test_gpu_full_size.py.
 """
+import copy
+
 import numpy as np
 import pytest
 import torch
@@ -64,6 +66,20 @@ def test_one_substep_forward_and_adjoint(config, plan):
     assert rel_inf(host(axg), ax) <= 1e-4 and rel_inf(host(avg), av) <= 1e-4
 
 
+TOL_CONTACT = 1e-2
+
+
+def _check_contact_grads(got, ref, tag):
+    """dL/d(k_e, k_d, k_f, mu_c): ONE number per environment, the sum over all particles in
+    contact and all substeps of mixed-sign terms, so cancellation amplifies the fp32 rounding of the terms (seen: a total
+    of 9e-9 off by 4e-3).  Tolerance 1e-2 of the largest environment's value; a regime no particle visited (all-zero
+    oracle gradient, e.g. k_f without a sticking particle) is not compared."""
+    for k in ("ke", "kd", "kf", "mu_c"):
+        b = ref["g_" + k]
+        if np.abs(b).max() > 0:
+            assert rel_inf(got["g_" + k], b) <= TOL_CONTACT, (tag, k)
+
+
 @pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("plan", PLANS)
 def test_small_rollout_and_gradients(config, plan):
@@ -82,6 +98,8 @@ def test_small_rollout_and_gradients(config, plan):
             a, b = got["g_" + g].sum(1), ref["g_" + g].sum(1)
             assert np.abs(a - b).max() <= TOL_GRAD * np.abs(b).max(), g
         assert rel_inf(got["g_" + g], ref["g_" + g]) <= TOL_GRAD, g
+    _check_contact_grads(got, ref, config)
+    assert np.abs(ref["g_ke"]).max() > 0  # every small config reaches the ground
 
 
 @pytest.mark.parametrize("config", [0, 3])
@@ -223,6 +241,25 @@ def test_set_params_changes_the_result_like_the_oracle():
     xg, vg = m.step_forward(dev(x), dev(v))
     assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
     assert rel_inf(host(vg), vo) <= 2e-5
+
+
+def test_set_contact_params_and_their_gradients():
+    """k_e, k_d, k_f, mu_c are settable per environment and have gradients, on both plans."""
+    sc = scenes.make_scene(3, small=True)  # 5 environments
+    E = sc.n_envs
+    r = scenes.rng_for(3, "misc", 31)
+    new = dict(ke=r.uniform(5e3, 2e4, E), kd=r.uniform(2.0, 20.0, E), kf=r.uniform(5.0, 40.0, E), mu_c=r.uniform(0.2, 0.9, E))
+    for plan in (gs.GS_PLAN_STREAMING, gs.GS_PLAN_RESIDENT):
+        m = gs.Model(sc, plan=plan)
+        s2 = copy.copy(sc)
+        for k, val in new.items():
+            m.set_params(k, dev(val.astype(np.float32)[:, None]))
+            setattr(s2, k, val.astype(np.float32))
+        ref = orc.run_scene(s2)
+        got = gpu_run_scene(s2, ref["target"], model=m)
+        assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * sc.extent()
+        _check_contact_grads(got, ref, plan)
+        assert np.abs(ref["g_ke"]).max() > 0 and np.abs(ref["g_mu_c"]).max() > 0
 
 
 def test_set_hinge_kb_changes_forces_and_gradients_like_the_oracle():
