@@ -52,7 +52,8 @@ enum gs_status {
 };
 
 /* parameter groups of gs_set_params / gs_param_grads (Table 5: the optimisable
-   parameters this path carries: Lame parameters and damping per element, mass per particle) */
+   parameters this path carries: Lame parameters and damping per element, mass per particle; from the "next"
+   list bending stiffness per hinge and the contact parameters per environment) */
 enum gs_param_group {
     GS_TET_MU = 0, GS_TET_LAMBDA = 1, GS_TET_DAMP = 2,
     GS_TRI_MU = 3, GS_TRI_LAMBDA = 4, GS_TRI_DAMP = 5,
