@@ -62,6 +62,11 @@ def test_one_substep_forward_and_adjoint(config, plan):
     assert rel_inf(host(avg), av) <= TOL_GRAD
     for g in _grad_groups(sc):
         assert rel_inf(host(m.param_grads(g)), o.grads(g)) <= TOL_GRAD, g
+    for g in ("ke", "kd", "kf", "mu_c"):  # contact parameters (one substep: no cancellation over time, 2e-3 holds)
+        b = o.grads(g)
+        assert g not in ("ke", "kf") or np.abs(b).max() > 0, g  # particles below the plane, sticking ones among them
+        if np.abs(b).max() > 0:  # a friction regime no particle is in has an all-zero gradient
+            assert rel_inf(host(m.param_grads(g)), b) <= TOL_GRAD, g
     # the fp32 path is far inside the budget on a single substep: keep it that way
     assert rel_inf(host(axg), ax) <= 1e-4 and rel_inf(host(avg), av) <= 1e-4
 
