@@ -14,8 +14,8 @@
 //     lanes of a warp run near-equal loops;
 //   - the only HBM traffic is the tape: one coalesced float4 store of (x, v) per particle per substep in the
 //     forward pass, one prefetched load per substep in the adjoint;
-//   - parameter gradients (a10) accumulate in registers over the whole rollout (fp32 chunks of 32 substeps
-//     folded into fp64, hazard H4) and are written once.
+//   - parameter gradients (a10) accumulate in fp32 registers; every 32 substeps the chunk is folded into the fp64
+//     masters in global memory (hazard H4; each thread owns its entries, so no atomics).
 // Two __syncthreads per substep.  Bound: plain fp32 ALU + barrier latency, not HBM.
 //
 // Tets only (the element functions are those of gs_elements.cuh, shared with the streaming plan); meshes with
@@ -239,14 +239,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     if (po.lead)
         for (int q = 0; q < 4; q++) { dgc[q * N + po.p] = 0.0; sgc[q * N + po.p] = 0.f; }
     const size_t frame_elems = (size_t)md.E * N * 3;
+    const size_t gstride = (size_t)md.E * md.es[T_TET].cpad;
     float gm32 = 0.f;
-    double gm64 = 0.0;
     float g32[EPT][3];
-    double g64[EPT][3];
 #pragma unroll
     for (int j = 0; j < EPT; j++)
 #pragma unroll
-        for (int q = 0; q < 3; q++) { g32[j][q] = 0.f; g64[j][q] = 0.0; }
+        for (int q = 0; q < 3; q++) g32[j][q] = 0.f;
     // the summed element contributions of the previous element phase, for this thread's particle (lead lane holds them)
     auto gather = [&](vec3 &dx, vec3 &dv) {
         float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
@@ -317,11 +316,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
 #pragma unroll
                 for (int q = 0; q < 4; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
             }
-            gm64 += (double)gm32; gm32 = 0.f;
+            // the fp64 masters live in global memory (each thread owns its entries; one update per kFlushEvery substeps),
+            // which keeps 8 registers free for the element VJP
+            if (po.lead) md.gmass64[poff] += (double)gm32;
+            gm32 = 0.f;
 #pragma unroll
             for (int j = 0; j < EPT; j++)
 #pragma unroll
-                for (int q = 0; q < 3; q++) { g64[j][q] += (double)g32[j][q]; g32[j][q] = 0.f; }
+                for (int q = 0; q < 3; q++) {
+                    if (tr[j].on) md.es[T_TET].g64[q * gstride + (size_t)env * md.es[T_TET].cpad + tid + j * blockDim.x] += (double)g32[j][q];
+                    g32[j][q] = 0.f;
+                }
         }
         __syncthreads();
     }
@@ -333,23 +338,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     if (po.lead) {
         adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
         adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
-        md.gmass64[poff] += gm64;
     }
     __syncthreads();
     if (tid < 4) {
         double t = 0.0;
         for (int p = 0; p < N; p++) t += dgc[tid * N + p];
         md.gcon64[(size_t)env * 4 + tid] += t;
-    }
-    const ElemDev &es = md.es[T_TET];
-    const size_t gstride = (size_t)md.E * es.cpad;
-#pragma unroll
-    for (int j = 0; j < EPT; j++) {
-        if (tr[j].on) {
-            const size_t pe = (size_t)env * es.cpad + tid + j * blockDim.x;
-#pragma unroll
-            for (int q = 0; q < 3; q++) es.g64[q * gstride + pe] += g64[j][q];
-        }
     }
 }
 
