@@ -68,10 +68,10 @@ def element_stream_bytes(sc, table):
 # were captured at 64 substeps: bytes per substep of the launch, scaled by the rollout length.
 NCU_TRAFFIC = {
     "config4-large-1000000tets-522242tris": {
-        "k_elements_fwd": ("per_launch", 162274048), "k_particles_fwd": ("per_launch", 22873856),
-        "k_elements_adj": ("per_launch", 200240383), "k_particles_adj": ("per_launch", 40039936),
+        "k_elements_fwd": ("per_launch", 162763776), "k_particles_fwd": ("per_launch", 22875136),
+        "k_elements_adj": ("per_launch", 201722624), "k_particles_adj": ("per_launch", 40084480),
     },
-    "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3555996), "k_resident_adj": ("per_substep", 4708488)},
+    "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3554932), "k_resident_adj": ("per_substep", 4639652)},
 }
 
 
