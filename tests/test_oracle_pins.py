@@ -340,6 +340,39 @@ def test_p7_step_param_gradients_vs_fd(group):
     assert np.abs(g - fd).max() <= 1e-6 * np.abs(fd).max()
 
 
+def test_contact_parameter_gradients_closed_form():
+    """Two free particles below the plane, no elements, one substep, L = bx.x+ + bv.v+ (A7, A8).
+    Particle 0 slides fast and approaches (slip + normal damping), particle 1 creeps (stick).  With lam = bv + dt bx
+    (cotangent of v+), w = 1/m:  dL/dk_e = sum w dt lam.(d f/d k_e) etc., written out by hand:
+      slip : f = (-mu fn, fn, 0) for v_t along +x, fn = -k_e c - k_d v_n   ->  d/dk_e = -c (-mu, 1, 0), d/dk_d = -v_n (-mu, 1, 0),
+             d/dmu = (-fn, 0, 0), d/dk_f = 0
+      stick: f = (-k_f v_x, fn, -k_f v_z)                                  ->  d/dk_f = (-v_x, 0, -v_z), d/dk_e = -c (0, 1, 0), d/dmu = 0."""
+    dt, m, ke, kd, kf, mu = 1.0 / 1920.0, 0.1, 1e4, 10.0, 50.0, 0.5
+    x = np.array([[0.0, -0.010, 0.0], [1.0, -0.002, 0.0]])
+    v = np.array([[3.0, -0.2, 0.0], [1e-3, 0.0, -2e-3]])
+    sc = scenes.custom_scene(x, v0=v, dt=dt, mass=m, ke=ke, kd=kd, kf=kf, mu_c=mu)
+    o = orc.Oracle(sc)
+    x, v, m = sc.x0[0].astype(np.float64), sc.v0[0].astype(np.float64), float(sc.mass[0, 0])  # the fp32-rounded inputs (A19)
+    bx = np.array([[0.3, -0.7, 0.2], [0.5, 0.4, -0.6]]); bv = np.array([[-0.2, 0.9, 0.1], [0.8, -0.3, 0.25]])
+    o.zero_grads()
+    o.step_adjoint(x, v, bx, bv)
+    lam = bv + dt * bx
+    w = 1.0 / m
+    c0, vn0, c1 = x[0, 1], v[0, 1], x[1, 1]
+    fn0 = -ke * c0 - kd * vn0
+    assert mu * fn0 / 3.0 < kf            # particle 0 slips
+    assert mu * (-ke * c1) / np.hypot(v[1, 0], v[1, 2]) >= kf   # particle 1 sticks
+    want = dict(
+        ke=w * dt * (lam[0] @ (-c0 * np.array([-mu, 1.0, 0.0])) + lam[1] @ (-c1 * np.array([0.0, 1.0, 0.0]))),
+        kd=w * dt * (lam[0] @ (-vn0 * np.array([-mu, 1.0, 0.0]))),
+        mu_c=w * dt * (lam[0] @ np.array([-fn0, 0.0, 0.0])),
+        kf=w * dt * (lam[1] @ np.array([-v[1, 0], 0.0, -v[1, 2]])),
+    )
+    for k, val in want.items():
+        got = o.grads(k)[0, 0]
+        assert abs(got - val) <= 1e-12 * max(abs(val), 1e-30), (k, got, val)
+
+
 def test_p7_conservative_forces_have_symmetric_jacobian():
     """Position-VJP of an elastic force equals its directional derivative (f(x+ea)-f(x-ea))/2e."""
     rng = np.random.default_rng(12)
