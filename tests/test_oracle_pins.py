@@ -340,6 +340,40 @@ def test_p7_step_param_gradients_vs_fd(group):
     assert np.abs(g - fd).max() <= 1e-6 * np.abs(fd).max()
 
 
+@pytest.mark.parametrize("fold", [0.0, 0.3, -0.8, 2.0])
+def test_hinge_force_closed_form_symmetric_fold(fold):
+    """Worked example of PAPER.md:585-586 with readings A5, A6: a hinge whose edge (length L) lies on the z axis, both wings
+    at distance h from it at mid-edge, rest shape flat, folded by the angle `fold`.  Then d_wing = n_hat / h (|n| = L h), so
+    the wing forces have magnitude k_b L |sin(fold/2)| / h along their face normals, the edge vertices share the opposite
+    force equally, and dL/dk_b of a substep is sum_i a_i.f_i / k_b (the force is linear in k_b)."""
+    L, h, kb, dt, m = 0.5, 0.25, 7.0, 1.0 / 1920.0, 0.1  # L, h, k_b exact in fp32 (inputs are rounded once, A19)
+    rest = np.array([[h, 0.0, L / 2], [-h, 0.0, L / 2], [0.0, 0.0, 0.0], [0.0, 0.0, L]])  # wing1, wing2, edge a, edge b
+    sc = scenes.custom_scene(rest, tris=[[2, 3, 0], [3, 2, 1]], hinges=[[0, 1, 2, 3]], kb=kb, dt=dt, mass=m, gravity=(0.0, 0.0, 0.0), plane_d=-1e6)
+    o = orc.Oracle(sc)
+    x = rest.copy()
+    x[1] = [-h * np.cos(fold), h * np.sin(fold), L / 2]  # rotate wing 2 about the edge
+    f = o.forces(x, mask=orc.HINGES)[0]
+    mag = kb * L * abs(np.sin(fold / 2)) / h
+    assert abs(np.linalg.norm(f[0]) - mag) <= 1e-12 * max(mag, 1.0) and abs(np.linalg.norm(f[1]) - mag) <= 1e-12 * max(mag, 1.0)
+    assert np.abs(f.sum(0)).max() <= 1e-12 * max(mag, 1.0)
+    assert np.abs(f[2] - f[3]).max() <= 1e-12 * max(mag, 1.0)            # mid-edge wings: the edge vertices share equally
+    if fold != 0.0:
+        n1 = np.cross(x[0] - x[2], x[0] - x[3]); n1 /= np.linalg.norm(n1)
+        assert abs(abs(f[0] @ n1) - mag) <= 1e-12 * mag                    # along the face normal
+        # unfolding: the work of the wing forces along an opening motion of wing 2 is positive
+        open_dir = np.array([h * np.sin(fold), h * np.cos(fold), 0.0]) * (-np.sign(fold))
+        assert f[1] @ open_dir > 0
+    # dL/dk_b of one substep by linearity of the force in k_b
+    rng = np.random.default_rng(3)
+    bx, bv = rng.normal(size=(4, 3)), rng.normal(size=(4, 3))
+    v = np.zeros_like(x)
+    o.zero_grads()
+    o.step_adjoint(x, v, bx, bv)
+    a = dt * (1.0 / float(sc.mass[0, 0])) * (bv + dt * bx)               # cotangent of the force
+    want = (a * f).sum() / float(sc.hinge_kb[0])
+    assert abs(o.grads("hinge_kb")[0, 0] - want) <= 1e-12 * max(abs(want), 1e-30)
+
+
 def test_contact_parameter_gradients_closed_form():
     """Two free particles below the plane, no elements, one substep, L = bx.x+ + bv.v+ (A7, A8).
     Particle 0 slides fast and approaches (slip + normal damping), particle 1 creeps (stick).  With lam = bv + dt bx
