@@ -340,6 +340,29 @@ def test_p7_step_param_gradients_vs_fd(group):
     assert np.abs(g - fd).max() <= 1e-6 * np.abs(fd).max()
 
 
+@pytest.mark.parametrize("s", [0.8, 1.0, 1.25])
+def test_uniform_stretch_closed_forms(s):
+    """Closed forms of the elastic nodal forces under a uniform stretch x = s X (readings A1, A4).
+    Corner tet with legs a: F = s I, I_C = 3 s^2, J = s^3, cof F = s^2 I, so P = p I with
+    p = mu (1 - 1/(3 s^2 + 1)) s + (lambda (s^3 - 1) - 3 mu / 4) s^2 and H = -V P B^T = -(a^2 p / 6) I.
+    Right triangle with legs a: F = s Q (Q the 3x2 rest frame), I_C = 2 s^2, J = s^2, dJ/dF = s Q, so P = p2 Q with
+    p2 = s [mu (1 - 1/(2 s^2 + 1)) + lambda (s^2 - 1) - 2 mu / 3] and H = -A P B^T = -(a p2 / 2) Q.  Both vanish at s = 1."""
+    a, mu, lam = 0.25, 1.25e4, 2.0e4  # exact in fp32 (inputs are rounded once, A19)
+    X = np.array([[0, 0, 0], [a, 0, 0], [0, a, 0], [0, 0, a]], dtype=np.float64)
+    sc = _free(scenes.custom_scene(X, tets=[[0, 1, 2, 3]], mu=mu, lam=lam, damp=0.0))
+    f = orc.Oracle(sc).forces(s * X, mask=orc.TETS)[0]
+    p = mu * (1 - 1 / (3 * s * s + 1)) * s + (lam * (s ** 3 - 1) - 0.75 * mu) * s * s
+    want = np.vstack([np.full(3, a * a * p / 6), -a * a * p / 6 * np.eye(3)])
+    assert np.abs(f - want).max() <= 1e-12 * max(abs(a * a * p / 6), 1.0)
+    Xt = np.array([[0, 0, 0], [a, 0, 0], [0, 0, -a]], dtype=np.float64)  # legs along +x and -z: normal +y
+    sc = _free(scenes.custom_scene(Xt, tris=[[0, 1, 2]], hinges=np.zeros((0, 4), np.int32), tri_mu=mu, tri_lam=lam, tri_damp=0.0))
+    f = orc.Oracle(sc).forces(s * Xt, mask=orc.TRIS)[0]
+    p2 = s * (mu * (1 - 1 / (2 * s * s + 1)) + lam * (s * s - 1) - 2 * mu / 3)
+    f1, f2 = -(a * p2 / 2) * np.array([1.0, 0, 0]), -(a * p2 / 2) * np.array([0, 0, -1.0])
+    want = np.vstack([-(f1 + f2), f1, f2])
+    assert np.abs(f - want).max() <= 1e-12 * max(abs(a * p2 / 2), 1.0)
+
+
 @pytest.mark.parametrize("fold", [0.0, 0.3, -0.8, 2.0])
 def test_hinge_force_closed_form_symmetric_fold(fold):
     """Worked example of PAPER.md:585-586 with readings A5, A6: a hinge whose edge (length L) lies on the z axis, both wings
