@@ -363,6 +363,24 @@ def test_uniform_stretch_closed_forms(s):
     assert np.abs(f - want).max() <= 1e-12 * max(abs(a * p2 / 2), 1.0)
 
 
+def test_uniform_expansion_rate_damping_closed_forms():
+    """Damping force (reading A3: P_damp = k F sym(F^T Fdot)) for x = s X, v = r X: F = s I (or s Q), Fdot = r I (r Q),
+    sym(F^T Fdot) = s r I, so P_damp = k s^2 r I: H = -(a^2 k s^2 r / 6) I for the corner tet, -(a k s^2 r / 2) Q for the
+    right triangle; elastic part removed by differencing against v = 0."""
+    a, mu, lam, k, s_, r = 0.25, 1.25e4, 2.0e4, 3.0, 1.125, 0.75
+    X = np.array([[0, 0, 0], [a, 0, 0], [0, a, 0], [0, 0, a]], dtype=np.float64)
+    o = orc.Oracle(_free(scenes.custom_scene(X, tets=[[0, 1, 2, 3]], mu=mu, lam=lam, damp=k)))
+    fd = o.forces(s_ * X, v=r * X, mask=orc.TETS)[0] - o.forces(s_ * X, mask=orc.TETS)[0]
+    c = a * a * k * s_ * s_ * r / 6
+    assert np.abs(fd - np.vstack([np.full(3, c), -c * np.eye(3)])).max() <= 1e-10 * c  # difference of two O(1e3) forces
+    Xt = np.array([[0, 0, 0], [a, 0, 0], [0, 0, -a]], dtype=np.float64)
+    o = orc.Oracle(_free(scenes.custom_scene(Xt, tris=[[0, 1, 2]], hinges=np.zeros((0, 4), np.int32), tri_mu=mu, tri_lam=lam, tri_damp=k)))
+    fd = o.forces(s_ * Xt, v=r * Xt, mask=orc.TRIS)[0] - o.forces(s_ * Xt, mask=orc.TRIS)[0]
+    c = a * k * s_ * s_ * r / 2
+    f1, f2 = -c * np.array([1.0, 0, 0]), -c * np.array([0, 0, -1.0])
+    assert np.abs(fd - np.vstack([-(f1 + f2), f1, f2])).max() <= 1e-10 * c
+
+
 @pytest.mark.parametrize("fold", [0.0, 0.3, -0.8, 2.0])
 def test_hinge_force_closed_form_symmetric_fold(fold):
     """Worked example of PAPER.md:585-586 with readings A5, A6: a hinge whose edge (length L) lies on the z axis, both wings
