@@ -26,3 +26,13 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """The tests exercise the in-tree libgradsim.so: build it (nvcc, sm_100a; a no-op when up to date) before the first
+    test instead of failing on a fresh checkout.  The product path itself never builds or falls back: gradsim.lib()
+    raises when the library is missing."""
+    from paper_2104_02646_b200 import build as gs_build
+
+    gs_build.build()
