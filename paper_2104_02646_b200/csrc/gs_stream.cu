@@ -49,6 +49,42 @@ __device__ __forceinline__ void red_add_v4(float4 *addr, float a, float b, float
     // one vector reduction per particle instead of three scalar ones (REDG.E.ADD.F32x4)
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(0.0f) : "memory");
 }
+// the same, predicated: no branch, so the emit phase stays convergent
+__device__ __forceinline__ void red_add_v4_if(unsigned pred, float4 *addr, float a, float b, float c) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n\t}" ::"l"(addr), "f"(a), "f"(b), "f"(c),
+                 "f"(0.0f), "r"(pred)
+                 : "memory");
+}
+// Segmented sum over a thread's 4 consecutive gather-list entries (sorted by tile-particle), branch-free.  Descriptor:
+// bits 0-9 index of the first entry's particle in the tile's id list, bits 10-12 "entry k starts a new run" (k = 1..3),
+// bits 13-15 number of valid entries.  Invalid entries point at slot 0 and are never flushed.
+struct EmitPlan {
+    unsigned s[4];       // slot of each entry
+    unsigned fl;         // bit k: a run ends at entry k -> one reduction
+    unsigned r[4];       // run number of entry k
+    float keep[3];       // 0 if entry k+1 starts a new run, else 1
+    const int *idp;
+    __device__ __forceinline__ EmitPlan(uint2 sl, unsigned dsc, const int *ids) {
+        const unsigned nv = dsc >> 13, bb = (dsc >> 10) & 7u;
+        s[0] = sl.x & 0xFFFFu; s[1] = sl.x >> 16; s[2] = sl.y & 0xFFFFu; s[3] = sl.y >> 16;
+        fl = bb | (1u << (nv - 1u));
+        r[0] = 0u; r[1] = bb & 1u; r[2] = r[1] + ((bb >> 1) & 1u); r[3] = r[2] + (bb >> 2);
+        keep[0] = (bb & 1u) ? 0.f : 1.f; keep[1] = (bb & 2u) ? 0.f : 1.f; keep[2] = (bb & 4u) ? 0.f : 1.f;
+        idp = ids + (dsc & 1023u);
+    }
+    // running sums a[k] of the runs; a[k] is final where bit k of fl is set
+    __device__ __forceinline__ void sums(const float4 *src, float3 a[4]) const {
+        const float4 c0 = src[s[0]], c1 = src[s[1]], c2 = src[s[2]], c3 = src[s[3]];
+        a[0] = make_float3(c0.x, c0.y, c0.z);
+        a[1] = make_float3(fmaf(a[0].x, keep[0], c1.x), fmaf(a[0].y, keep[0], c1.y), fmaf(a[0].z, keep[0], c1.z));
+        a[2] = make_float3(fmaf(a[1].x, keep[1], c2.x), fmaf(a[1].y, keep[1], c2.y), fmaf(a[1].z, keep[1], c2.z));
+        a[3] = make_float3(fmaf(a[2].x, keep[2], c3.x), fmaf(a[2].y, keep[2], c3.y), fmaf(a[2].z, keep[2], c3.z));
+    }
+    __device__ __forceinline__ void flush(float4 *dst, const float3 a[4]) const {
+#pragma unroll
+        for (int k = 0; k < 4; k++) red_add_v4_if(fl & (1u << k), dst + idp[r[k]], a[k].x, a[k].y, a[k].z);
+    }
+};
 __device__ __forceinline__ void red_add_f32(float *addr, float a) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
 }
@@ -310,26 +346,13 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
         },
         [&](const TileView<TYPE, false> &tv, const int *ids, int env, const float4 *sf) {
             // thread t sums gather-list entries 4t .. 4t+3 (sorted by tile-particle) and issues one vector reduction per
-            // run of equal particles: balanced over all lanes, no loop, no shared-memory atomics
-            const uint2 sl = reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x];
-            const unsigned dsc = tv.slot_desc[threadIdx.x], nv = dsc >> 13;
-            const unsigned s_[4] = {sl.x & 0xFFFFu, sl.x >> 16, sl.y & 0xFFFFu, sl.y >> 16};
-            float4 *dst = f4 + (size_t)env * N;
-            if (nv == 0) return;
-            unsigned cur = dsc & 1023u;
-            float4 c = sf[s_[0]];
-            float ax = c.x, ay = c.y, az = c.z;
-#pragma unroll
-            for (int k = 1; k < 4; k++) {
-                if ((unsigned)k < nv) {
-                    c = sf[s_[k]];
-                    if ((dsc >> (9 + k)) & 1u) {
-                        red_add_v4(dst + ids[cur], ax, ay, az);
-                        cur++; ax = c.x; ay = c.y; az = c.z;
-                    } else { ax += c.x; ay += c.y; az += c.z; }
-                }
-            }
-            red_add_v4(dst + ids[cur], ax, ay, az);
+            // run of equal particles: balanced over all lanes, no loop, no branch, no shared-memory atomics
+            const unsigned dsc = tv.slot_desc[threadIdx.x];
+            if ((dsc >> 13) == 0u) return;
+            const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
+            float3 a[4];
+            ep.sums(sf, a);
+            ep.flush(f4 + (size_t)env * N, a);
         });
 }
 
@@ -497,28 +520,16 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
             }
         },
         [&](const TileView<TYPE, true> &tv, const int *ids, int env, const float4 *so) {
-            const uint2 sl = reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x];
-            const unsigned dsc = tv.slot_desc[threadIdx.x], nv = dsc >> 13;
-            const unsigned s_[4] = {sl.x & 0xFFFFu, sl.x >> 16, sl.y & 0xFFFFu, sl.y >> 16};
-            float4 *dx = adjx + (size_t)env * N, *dv = adjv + (size_t)env * N;
-            if (nv == 0) return;
-            unsigned cur = dsc & 1023u;
-            float4 c = so[s_[0]], d = TYPE != T_HINGE ? so[PL + s_[0]] : make_float4(0.f, 0.f, 0.f, 0.f);
-            float ax = c.x, ay = c.y, az = c.z, bx = d.x, by = d.y, bz = d.z;
-#pragma unroll
-            for (int k = 1; k < 4; k++) {
-                if ((unsigned)k < nv) {
-                    c = so[s_[k]];
-                    if (TYPE != T_HINGE) d = so[PL + s_[k]];
-                    if ((dsc >> (9 + k)) & 1u) {
-                        red_add_v4(dx + ids[cur], ax, ay, az);
-                        if (TYPE != T_HINGE) red_add_v4(dv + ids[cur], bx, by, bz);
-                        cur++; ax = c.x; ay = c.y; az = c.z; bx = d.x; by = d.y; bz = d.z;
-                    } else { ax += c.x; ay += c.y; az += c.z; bx += d.x; by += d.y; bz += d.z; }
-                }
+            const unsigned dsc = tv.slot_desc[threadIdx.x];
+            if ((dsc >> 13) == 0u) return;
+            const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
+            float3 a[4];
+            ep.sums(so, a);
+            ep.flush(adjx + (size_t)env * N, a);
+            if (TYPE != T_HINGE) {
+                ep.sums(so + PL, a);
+                ep.flush(adjv + (size_t)env * N, a);
             }
-            red_add_v4(dx + ids[cur], ax, ay, az);
-            if (TYPE != T_HINGE) red_add_v4(dv + ids[cur], bx, by, bz);
         });
 }
 
