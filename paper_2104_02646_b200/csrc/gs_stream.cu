@@ -125,6 +125,9 @@ __device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, u
                  "l"(gmem_src), "r"(bytes), "r"(smem_u32(b)), "l"(policy)
                  : "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gmem_src, unsigned bytes, uint64_t policy) {
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(gmem_src), "r"(bytes), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void cp_async16_hint(void *smem_dst, const void *gmem_src, uint64_t policy) {
     asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "l"(policy) : "memory");
 }
@@ -156,7 +159,8 @@ struct TileSmem {
     static constexpr bool kHasV = TYPE != T_HINGE;
     static constexpr int kGather = 1 + (kHasV ? 1 : 0) + (ADJ ? 1 : 0);
     static constexpr int kPar = TYPE != T_HINGE ? kParBytes : 0;
-    __host__ __device__ static int buf_bytes(int lmax) { return lmax * 16 * kGather + R::kBytes + kPar; }
+    static constexpr int kEmitBytes = R::kBytes - R::oSlots;  // gather-list slots + run descriptors: the only record fields other threads read
+    __host__ __device__ static int buf_bytes(int lmax) { return lmax * 16 * kGather + kEmitBytes; }
     __host__ __device__ static int out_bytes() { return R::kArityT * kTileElems * 16 * ((ADJ && kHasV) ? 2 : 1); }
     __host__ __device__ static int total_bytes(int pmax, int lmax) { return 3 * pmax * 4 + 2 * pmax * 2 + 2 * buf_bytes(lmax) + out_bytes(); }
 };
@@ -166,28 +170,27 @@ struct TileView {
     using R = RecLayout<TYPE>;
     using S = TileSmem<TYPE, ADJ>;
     float4 *x, *v, *a;
-    char *rec;
-    const ushort4 *lidx;
-    const float4 *c0, *c1;
-    const float2 *c2;
-    const float *area, *mu, *lam, *damp;
+    char *emit;
     const uint16_t *slots, *slot_desc;
     __device__ __forceinline__ TileView(char *base, int lmax) {
         char *p = base;
         x = (float4 *)p; p += lmax * 16;
         v = (float4 *)p; if (S::kHasV) p += lmax * 16;
         a = (float4 *)p; if (ADJ) p += lmax * 16;
-        rec = p;
-        lidx = (const ushort4 *)(p + R::oLidx);
-        c0 = (const float4 *)(p + R::oC0);
-        c1 = (const float4 *)(p + R::oC1);
-        c2 = (const float2 *)(p + R::oC2);
-        area = (const float *)(p + R::oArea);
-        slots = (const uint16_t *)(p + R::oSlots);
-        slot_desc = (const uint16_t *)(p + R::oSlotDesc);
-        p += R::kBytes;
-        mu = (const float *)p; lam = mu + kTileElems; damp = lam + kTileElems;
+        emit = p;
+        slots = (const uint16_t *)p;
+        slot_desc = (const uint16_t *)(p + (R::oSlotDesc - R::oSlots));
     }
+};
+
+// The record fields only the owning thread reads (connectivity as staging indices, rest constants, material
+// parameters) never pass through shared memory: each thread loads its own, coalesced, one tile ahead, into registers.
+template <int TYPE>
+struct ElemRegs {
+    ushort4 li;
+    float4 c0, c1;
+    float2 c2;
+    float area, mu, lam, damp;
 };
 
 // The persistent tile loop shared by the forward and adjoint kernels.  `compute(tv, tile, env, e_local)` evaluates one
@@ -231,9 +234,29 @@ struct TilePipe {
         unsigned tile, env;
         split(item, tile, env);
         TileView<TYPE, ADJ> tv(bufs + b * bb, lmax);
-        mbar_expect_tx(bars + b, es.rec_bytes + S::kPar);
-        bulk_g2s(tv.rec, es.rec + (size_t)tile * es.rec_bytes, es.rec_bytes, bars + b, pol_stream);
-        if (S::kPar) bulk_g2s((void *)tv.mu, es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, bars + b, pol_stream);
+        const char *rec = es.rec + (size_t)tile * es.rec_bytes;
+        mbar_expect_tx(bars + b, S::kEmitBytes);
+        bulk_g2s(tv.emit, rec + S::R::oSlots, S::kEmitBytes, bars + b, pol_stream);
+        // the thread-private part of the record goes to L2 now and to registers (load_regs) one tile later
+        bulk_prefetch_l2(rec, S::R::oSlots, pol_stream);
+        if (S::kPar) bulk_prefetch_l2(es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, pol_stream);
+    }
+    __device__ __forceinline__ void load_regs(int item, ElemRegs<TYPE> &er) const {  // all threads
+        unsigned tile, env;
+        split(item, tile, env);
+        const char *rec = es.rec + (size_t)tile * es.rec_bytes;
+        const int tid = threadIdx.x;
+        er.li = __ldcs((const ushort4 *)(rec + S::R::oLidx) + tid);
+        er.c0 = __ldcs((const float4 *)(rec + S::R::oC0) + tid);
+        if (TYPE == T_TET) {
+            er.c1 = __ldcs((const float4 *)(rec + S::R::oC1) + tid);
+            er.c2 = __ldcs((const float2 *)(rec + S::R::oC2) + tid);
+        }
+        if (TYPE == T_TRI) er.area = __ldcs((const float *)(rec + S::R::oArea) + tid);
+        if (S::kPar) {
+            const float *q = es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems) + tid;
+            er.mu = __ldcs(q); er.lam = __ldcs(q + kTileElems); er.damp = __ldcs(q + 2 * kTileElems);
+        }
     }
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
@@ -266,6 +289,8 @@ struct TilePipe {
             if (cnt > 1) load_ids(first + G, 1, 1);
             load_static(first, 0);
         }
+        ElemRegs<TYPE> er;
+        load_regs(first, er);
         mbar_wait(bars + 2, 0);
         grid_dep_wait();  // the particle arrays gathered from here on are the predecessor kernel's output
         gather(first, 0, 0);
@@ -285,7 +310,8 @@ struct TilePipe {
             unsigned tile, env;
             split(item, tile, env);
             const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, lmax);
-            if ((int)(tile * kTileElems + tid) < es.count) compute(tv, (int)tile, (int)env, out);
+            if ((int)(tile * kTileElems + tid) < es.count) compute(tv, er, (int)tile, (int)env, out);
+            if (i + 1 < cnt) load_regs(item + G, er);  // in flight across the barrier, the emit phase and the next waits
             __syncthreads();
             const int *ids = idbuf + s3 * pmax;
             emit(tv, ids, (int)env, out);
@@ -313,30 +339,30 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
     const int N = md.N;
     pipe.run(
         rot,
-        [&](const TileView<TYPE, false> &tv, int, int, float4 *sf) {
+        [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int, float4 *sf) {
             const int tid = threadIdx.x;
-            const ushort4 li = tv.lidx[tid];
+            const ushort4 li = er.li;
             if (TYPE == T_TET) {
-                const float4 c0 = tv.c0[tid], c1 = tv.c1[tid];
-                const float2 c2 = tv.c2[tid];
+                const float4 c0 = er.c0, c1 = er.c1;
+                const float2 c2 = er.c2;
                 const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
                 vec3 f[4];
-                tet_force(x, v, b, c2.y, tv.mu[tid], tv.lam[tid], tv.damp[tid], f);
+                tet_force(x, v, b, c2.y, er.mu, er.lam, er.damp, f);
 #pragma unroll
                 for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             } else if (TYPE == T_TRI) {
-                const float4 c0 = tv.c0[tid];
+                const float4 c0 = er.c0;
                 const float b[4] = {c0.x, c0.y, c0.z, c0.w};
                 const vec3 x[3] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z])};
                 const vec3 v[3] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z])};
                 vec3 f[3];
-                tri_force(x, v, b, tv.area[tid], tv.mu[tid], tv.lam[tid], tv.damp[tid], f);
+                tri_force(x, v, b, er.area, er.mu, er.lam, er.damp, f);
 #pragma unroll
                 for (int k = 0; k < 3; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             } else {
-                const float4 c0 = tv.c0[tid];
+                const float4 c0 = er.c0;
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 vec3 f[4];
                 hinge_force(x, c0.x, c0.y, c0.z, f);
@@ -471,19 +497,19 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
     const size_t gstride = (size_t)md.E * es.cpad;
     pipe.run(
         rot,
-        [&](const TileView<TYPE, true> &tv, int tile, int env, float4 *so) {
+        [&](const TileView<TYPE, true> &tv, const ElemRegs<TYPE> &er, int tile, int env, float4 *so) {
             const int tid = threadIdx.x;
-            const ushort4 li = tv.lidx[tid];
+            const ushort4 li = er.li;
             if (TYPE == T_TET) {
-                const float4 c0 = tv.c0[tid], c1 = tv.c1[tid];
-                const float2 c2 = tv.c2[tid];
+                const float4 c0 = er.c0, c1 = er.c1;
+                const float2 c2 = er.c2;
                 const float b[9] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4], av[4];
                 float gmu, glam, gk;
-                tet_adjoint(x, v, a, b, c2.y, tv.mu[tid], tv.lam[tid], tv.damp[tid], ax, av, gmu, glam, gk);
+                tet_adjoint(x, v, a, b, c2.y, er.mu, er.lam, er.damp, ax, av, gmu, glam, gk);
                 float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
                 red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
 #pragma unroll
@@ -492,14 +518,14 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                     so[PL + k * kTileElems + tid] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
                 }
             } else if (TYPE == T_TRI) {
-                const float4 c0 = tv.c0[tid];
+                const float4 c0 = er.c0;
                 const float b[4] = {c0.x, c0.y, c0.z, c0.w};
                 const vec3 x[3] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z])};
                 const vec3 v[3] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z])};
                 const vec3 a[3] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z])};
                 vec3 ax[3], av[3];
                 float gmu, glam, gk;
-                tri_adjoint(x, v, a, b, tv.area[tid], tv.mu[tid], tv.lam[tid], tv.damp[tid], ax, av, gmu, glam, gk);
+                tri_adjoint(x, v, a, b, er.area, er.mu, er.lam, er.damp, ax, av, gmu, glam, gk);
                 float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
                 red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
 #pragma unroll
@@ -508,7 +534,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                     so[PL + k * kTileElems + tid] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
                 }
             } else {
-                const float4 c0 = tv.c0[tid];
+                const float4 c0 = er.c0;
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4];
