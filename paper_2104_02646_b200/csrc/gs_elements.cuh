@@ -13,6 +13,14 @@
 
 namespace gs {
 
+// MUFU.RCP, <= 1 ulp, no IEEE slow path: element geometry and invariants only (arguments >= 1 or clamped away from 0);
+// never contact (hazard H3)
+__device__ __forceinline__ float rcp_fast(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 // ------------------------------------------------------------------------------------------ tets
 // B = D_m^-1 row-major b[k*3+c], V = rest volume.  F = D_s B: column c of F = sum_k d_k b[k][c].
 struct TetKin {
@@ -51,7 +59,7 @@ __device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], cons
     vec3 g1, g2, g3;
     mat_cols_times_B(v[1] - v[0], v[2] - v[0], v[3] - v[0], b, g1, g2, g3);
     // -V is folded into the three scalar coefficients, so the columns below are those of -V P
-    const float s1 = k.Ic / (k.Ic + 1.0f);
+    const float s1 = k.Ic * rcp_fast(k.Ic + 1.0f);
     const float ce = -V * (lam * (k.J - 1.0f) - 0.75f * mu);  // lambda (J - alpha), alpha = 1 + 3mu/(4 lambda)  (A1)
     const float ms = -V * mu * s1;
     const float kv = -V * kd, kh = 0.5f * kv;
@@ -131,10 +139,10 @@ __device__ __forceinline__ void tri_force(const vec3 x[3], const vec3 v[3], cons
     const float Ic = dot(f1, f1) + dot(f2, f2);
     const vec3 c = cross(f1, f2);
     const float J = sqrtf(dot(c, c));
-    const vec3 n = (1.0f / fmaxf(J, 1e-12f)) * c;
+    const vec3 n = rcp_fast(fmaxf(J, 1e-12f)) * c;
     const vec3 j1 = cross(f2, n), j2 = cross(n, f1);  // dJ/dF
     // -A (rest area) is folded into the scalar coefficients: p1, p2 are the columns of -A P
-    const float ms = -A * mu * Ic / (Ic + 1.0f);
+    const float ms = -A * mu * Ic * rcp_fast(Ic + 1.0f);
     const float ce = -A * (lam * (J - 1.0f) - (2.0f / 3.0f) * mu);  // lambda (J - alpha2), alpha2 = 1 + 2mu/(3 lambda)  (A4)
     const float kv = -A * kd;
     const float s11 = kv * dot(f1, g1), s22 = kv * dot(f2, g2), s12 = 0.5f * kv * (dot(f1, g2) + dot(f2, g1));
@@ -156,10 +164,10 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
     const float Ic = dot(f1, f1) + dot(f2, f2);
     const vec3 c = cross(f1, f2);
     const float J = sqrtf(dot(c, c));
-    const float iJ = 1.0f / fmaxf(J, 1e-12f);
+    const float iJ = rcp_fast(fmaxf(J, 1e-12f));
     const vec3 n = iJ * c;
     const vec3 j1 = cross(f2, n), j2 = cross(n, f1);
-    const float ip1 = 1.0f / (Ic + 1.0f), s1 = Ic * ip1;
+    const float ip1 = rcp_fast(Ic + 1.0f), s1 = Ic * ip1;
     const float s11 = dot(f1, g1), s22 = dot(f2, g2), s12 = 0.5f * (dot(f1, g2) + dot(f2, g1));
     const float n11 = dot(f1, A1), n22 = dot(f2, A2), n12 = 0.5f * (dot(f1, A2) + dot(f2, A1));
     const float FA = n11 + n22, JA = dot(j1, A1) + dot(j2, A2);
@@ -187,11 +195,6 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
 // vertices: x[0], x[1] wings; x[2], x[3] the shared edge.  theta = signed dihedral (0 when flat);
 // f_i = k_b l0 sin((theta - theta0)/2) d_i, d_i = -d(theta)/dx_i (Bridson directions).
 // Rest constants per hinge: s0h = sin(theta0/2), c0h = cos(theta0/2), kl = k_b * l0 (fp64 on the host).
-__device__ __forceinline__ float rcp_fast(float x) {  // MUFU.RCP, <= 1 ulp: geometry of well-shaped hinges only (not contact, hazard H3)
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
 struct HingeGeo {
     vec3 p13, p14, p23, p24, n1, n2, eh, m1, m2;
     float L, iL, i1, i2, c13, c14, c23, c24, sh, ch;  // sh, ch = sin, cos of (theta - theta0)/2

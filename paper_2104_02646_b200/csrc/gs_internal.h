@@ -106,6 +106,7 @@ struct gs_model {
     int n_sms = 148;
     int smem_fwd = 0, smem_adj = 0;  // dynamic shared memory of the element kernels
     int occ_fwd = 1, occ_adj = 1;    // co-resident CTAs per SM
+    bool pdl = true;                 // programmatic dependent launch of the hot-path kernels (small meshes only: configure_stream_kernels)
     long long elem_items = 0;        // work items (tile x environment) of the largest element type
     int step_counter = 0;  // substep index written to dev.bad on a non-finite state
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan

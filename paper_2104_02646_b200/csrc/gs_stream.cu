@@ -187,7 +187,7 @@ struct TileView {
 // parameters) never pass through shared memory: each thread loads its own, coalesced, one tile ahead, into registers.
 template <int TYPE>
 struct ElemRegs {
-    ushort4 li;
+    uint2 li;  // four 16-bit staging indices, unpacked only when the element is evaluated (keeps the load in flight)
     float4 c0, c1;
     float2 c2;
     float area, mu, lam, damp;
@@ -246,7 +246,7 @@ struct TilePipe {
         split(item, tile, env);
         const char *rec = es.rec + (size_t)tile * es.rec_bytes;
         const int tid = threadIdx.x;
-        er.li = __ldcs((const ushort4 *)(rec + S::R::oLidx) + tid);
+        er.li = __ldcs((const uint2 *)(rec + S::R::oLidx) + tid);
         er.c0 = __ldcs((const float4 *)(rec + S::R::oC0) + tid);
         if (TYPE == T_TET) {
             er.c1 = __ldcs((const float4 *)(rec + S::R::oC1) + tid);
@@ -341,7 +341,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
         rot,
         [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int, float4 *sf) {
             const int tid = threadIdx.x;
-            const ushort4 li = er.li;
+            const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
             if (TYPE == T_TET) {
                 const float4 c0 = er.c0, c1 = er.c1;
                 const float2 c2 = er.c2;
@@ -499,7 +499,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
         rot,
         [&](const TileView<TYPE, true> &tv, const ElemRegs<TYPE> &er, int tile, int env, float4 *so) {
             const int tid = threadIdx.x;
-            const ushort4 li = er.li;
+            const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
             if (TYPE == T_TET) {
                 const float4 c0 = er.c0, c1 = er.c1;
                 const float2 c2 = er.c2;
@@ -657,13 +657,13 @@ static inline int grid_for(size_t n, int block = 256) {
 
 // launch with programmatic stream serialization (see grid_dep_wait)
 template <class... KArgs, class... Args>
-static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+static cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
@@ -698,6 +698,16 @@ int configure_stream_kernels(gs_model *m) {
     m->smem_adj = adj + kBarBytes;
     int rc = tile_kernel_setup(k_elements_fwd, m->smem_fwd, &m->occ_fwd);
     if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj, m->smem_adj, &m->occ_adj);
+    // Programmatic dependent launch pays where a kernel is a few microseconds long (configs 1, 2: -15 % per step): the
+    // next kernel's CTAs are resident and past their prologue when the predecessor drains.  Once the element grid fills
+    // the machine it costs instead (config 4: +3.5 % per step; +14 % with a grid of 6 CTAs per SM where 9 fit): CTAs that
+    // launch into whatever slots free up first are placed unevenly over the SMs.  Measured crossover unknown between
+    // 157 and 7813 tiles; the rule below keeps the launch attribute while a type has at most two tiles per SM.
+    m->pdl = items <= 2LL * sms;
+    // experiment overrides (not part of the interface)
+    if (const char *q = getenv("GS_PDL")) m->pdl = atoi(q) != 0;
+    if (const char *q = getenv("GS_OCC_FWD")) m->occ_fwd = std::min(m->occ_fwd, std::max(1, atoi(q)));
+    if (const char *q = getenv("GS_OCC_ADJ")) m->occ_adj = std::min(m->occ_adj, std::max(1, atoi(q)));
     if (getenv("GS_DEBUG"))
         fprintf(stderr, "gradsim: element kernels smem fwd %d adj %d bytes, CTAs/SM fwd %d adj %d, pmax %d/%d/%d lmax %d/%d/%d\n", m->smem_fwd, m->smem_adj,
                 m->occ_fwd, m->occ_adj, es[0].pmax, es[1].pmax, es[2].pmax, es[0].lmax, es[1].lmax, es[2].lmax);
@@ -713,8 +723,8 @@ static inline int tile_grid(const gs_model *m, int occ) {
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
     if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
-                 launch_pdl(k_elements_fwd, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, x, v, m->d_f));
-    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, substep));
+                 launch_pdl(m->pdl, k_elements_fwd, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, x, v, m->d_f));
+    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, substep));
     return GS_OK;
 }
 
@@ -722,10 +732,10 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
 // m->d_adjx / m->d_adjv (updated in place); frame_cot (caller order, may be null) is added to adj_x first.
 int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st) {
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
-             launch_pdl(k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
+             launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                 launch_pdl(k_elements_adj, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+                 launch_pdl(m->pdl, k_elements_adj, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
     return GS_OK;
 }
