@@ -79,6 +79,10 @@ struct ModelDev {
     float *gcon32;                    // [E][kConSlots][4] dL/d(k_e, k_d, k_f, mu_c): fp32 partial sums, spread over slots so
                                       // that the warps of a launch do not all reduce into one L2 sector
     double *gcon64;                   // [E][4] fp64 masters
+    int *tile_ctr;                    // [6] dynamic tile queues of the element kernels: forward tets/tris/hinges, adjoint
+                                      // tets/tris/hinges.  Zero between launches: k_particles_fwd re-zeroes the forward
+                                      // three after every k_elements_fwd, k_particles_adj the adjoint three before every
+                                      // k_elements_adj
     int *bad;                         // first non-finite substep (INT_MAX = none)
 };
 

@@ -55,6 +55,7 @@ struct Layout {
     int *perm_p, *bad;
     float *inv_mass, *gmass32, *ke, *kd, *kf, *muc, *gcon32;
     double *gmass64, *gcon64;
+    int *tile_ctr;
     float4 *f, *xs[2], *vs[2], *adjx, *adjv, *adjf;
     size_t bytes;
 };
@@ -85,6 +86,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     L.gmass64 = b.take<double>(EN);
     L.gcon32 = b.take<float>((size_t)E * kConSlots * 4);
     L.gcon64 = b.take<double>((size_t)E * 4);
+    L.tile_ctr = b.take<int>(8);
     L.ke = b.take<float>(E); L.kd = b.take<float>(E); L.kf = b.take<float>(E); L.muc = b.take<float>(E);
     L.bad = b.take<int>(1);
     L.f = b.take<float4>(EN);
@@ -415,7 +417,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     }
     dev.pd = d->plane_d; dev.pr = d->particle_radius;
     dev.ke = L.ke; dev.kd = L.kd; dev.kf = L.kf; dev.muc = L.muc;
-    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gcon32 = L.gcon32; dev.gcon64 = L.gcon64; dev.bad = L.bad;
+    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gcon32 = L.gcon32; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad;
     m->N = N; m->E = E;
     m->d_f = L.f; m->d_xs[0] = L.xs[0]; m->d_xs[1] = L.xs[1]; m->d_vs[0] = L.vs[0]; m->d_vs[1] = L.vs[1];
     m->d_adjx = L.adjx; m->d_adjv = L.adjv; m->d_adjf = L.adjf;
@@ -426,6 +428,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gmass64, 0, sizeof(double) * EN, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gcon32, 0, sizeof(float) * (size_t)E * kConSlots * 4, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gcon64, 0, sizeof(double) * (size_t)E * 4, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int) * 8, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.bad, 0x7f, sizeof(int), stream);
     if (ce != cudaSuccess) return cuda_fail(ce, "memset workspace");
     ce = cudaStreamSynchronize(stream);

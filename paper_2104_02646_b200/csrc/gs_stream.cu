@@ -279,7 +279,7 @@ struct TilePipe {
     // `rot` rotates which CTAs get the odd extra tile, so that the types of one launch do not pile their remainders
     // onto the same CTAs
     template <class Compute, class Emit>
-    __device__ __forceinline__ void run(int rot, Compute compute, Emit emit) {
+    __device__ __forceinline__ void run_static(int rot, Compute compute, Emit emit) {
         const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
         const int first = (int)((blockIdx.x + (unsigned)rot) % (unsigned)G);
         if (first >= n_items) return;
@@ -319,10 +319,68 @@ struct TilePipe {
             s3 = s3n;
         }
     }
+    // Work distribution.  Forward kernel (kQueue): the CTA's first two items are static, (blockIdx + rot) mod G and that
+    // + G (`rot` rotates the types of one launch against each other); every further item is claimed from the type's
+    // global queue (`ctr`, zero at launch) by thread 0, one iteration before its particle ids are requested, i.e. three
+    // tiles ahead of its evaluation, so the atomic's round trip is never waited on.  The queue evens out the tail of the
+    // persistent grid (config 4 forward: -6 %).  Adjoint kernel: static stride G throughout -- with the queue the
+    // compiler's register allocation tips from 80 to 96 registers (6 -> 5 CTAs per SM) and the kernel loses 5 %.
+    static constexpr bool kQueue = !ADJ;
+    template <class Compute, class Emit>
+    __device__ __forceinline__ void run(int rot, int *ctr, int *next_slot, Compute compute, Emit emit) {
+        if (!kQueue) { run_static(rot, compute, emit); return; }
+        const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
+        const int first = (int)((blockIdx.x + (unsigned)rot) % (unsigned)G);
+        if (first >= n_items) return;
+        const bool queue = kQueue && 2 * G < n_items;  // otherwise the static items cover everything
+        int item = first, item_n = first + G;  // items i, i+1 (all threads)
+        int claimed = n_items;                 // kQueue: item i+2, thread 0 only until published through next_slot
+        if (tid == 0) {
+            load_ids(first, 0, 0);
+            if (item_n < n_items) load_ids(item_n, 1, 1);
+            load_static(first, 0);
+        }
+        ElemRegs<TYPE> er;
+        load_regs(first, er);
+        mbar_wait(bars + 2, 0);
+        grid_dep_wait();  // the particle arrays gathered from here on are the predecessor kernel's output
+        if (kQueue && tid == 0 && queue) claimed = 2 * G + atomicAdd(ctr, 1);
+        gather(first, 0, 0);
+        int s3 = 0, q3 = 0;  // i % 3, i / 3: ids of the CTA's j-th item use id buffer j % 3 for the (j / 3)-th time
+        for (int i = 0;; i++) {
+            const int s3n = s3 == 2 ? 0 : s3 + 1, s3nn = s3n == 2 ? 0 : s3n + 1;
+            const bool has_n = item_n < n_items;
+            cp_async_wait_all();
+            mbar_wait(bars + (i & 1), (i >> 1) & 1);
+            if (has_n) mbar_wait(bars + 2 + s3n, (q3 + (s3n == 0 ? 1 : 0)) & 1);
+            __syncthreads();
+            if (tid == 0) {
+                const int item_nn = kQueue ? claimed : item_n + G;  // item i+2
+                if (kQueue) *next_slot = claimed;                   // read by everybody after the next barrier
+                if (has_n && item_nn < n_items) load_ids(item_nn, s3nn, i & 1);
+                if (has_n) load_static(item_n, (i + 1) & 1);
+                if (kQueue) claimed = (queue && claimed < n_items) ? 2 * G + atomicAdd(ctr, 1) : n_items;  // item i+3
+            }
+            if (has_n) gather(item_n, s3n, (i + 1) & 1);
+            unsigned tile, env;
+            split(item, tile, env);
+            const TileView<TYPE, ADJ> tv(bufs + (i & 1) * bb, lmax);
+            if ((int)(tile * kTileElems + tid) < es.count) compute(tv, er, (int)tile, (int)env, out);
+            if (has_n) load_regs(item_n, er);  // in flight across the barrier, the emit phase and the next waits
+            __syncthreads();
+            const int *ids = idbuf + s3 * pmax;
+            emit(tv, ids, (int)env, out);
+            if (!has_n) break;
+            item = item_n;
+            item_n = kQueue ? *next_slot : item_n + G;
+            if (s3n == 0) q3++;
+            s3 = s3n;
+        }
+    }
 };
 
 // ------------------------------------------------------------------------------------------ forward elements
-constexpr int kBarBytes = 128;  // 15 mbarriers at the start of shared memory: 5 per element type
+constexpr int kBarBytes = 128;  // 15 mbarriers at the start of shared memory (5 per element type) + the queue hand-over slot
 
 __device__ __forceinline__ void init_barriers(uint64_t *bars) {
     if (threadIdx.x == 0) {
@@ -333,12 +391,12 @@ __device__ __forceinline__ void init_barriers(uint64_t *bars) {
 }
 
 template <int TYPE>
-__device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64_t *bars, int rot, const float4 *__restrict__ x4,
+__device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, float4 *__restrict__ f4) {
     TilePipe<TYPE, false> pipe(md, smem, bars, x4, v4, nullptr);
     const int N = md.N;
     pipe.run(
-        rot,
+        rot, md.tile_ctr + TYPE, next_slot,
         [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int, float4 *sf) {
             const int tid = threadIdx.x;
             const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
@@ -390,9 +448,9 @@ __global__ void __launch_bounds__(kTileElems) k_elements_fwd(const ModelDev md, 
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_fwd<T_TET>(md, smem + kBarBytes, bars, rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_fwd<T_TRI>(md, smem + kBarBytes, bars + 5, rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE>(md, smem + kBarBytes, bars + 10, rot, x4, v4, f4);
+    if (md.es[T_TET].count) { tiles_fwd<T_TET>(md, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_fwd<T_TRI>(md, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE>(md, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
 }
 
 // ------------------------------------------------------------------------------------------ forward particles
@@ -408,6 +466,7 @@ __global__ void __launch_bounds__(256) k_particles_fwd(const ModelDev md, const 
     const size_t total = (size_t)md.E * md.N;
     grid_dep_launch();
     grid_dep_wait();
+    if (blockIdx.x == 0 && threadIdx.x < 3) md.tile_ctr[threadIdx.x] = 0;  // the forward element kernel's tile queues
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / md.N);
         const float4 xq = x4[i], vq = v4[i], fq = f4[i];
@@ -432,6 +491,7 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
     const size_t total = (size_t)md.E * md.N;
     grid_dep_launch();
     grid_dep_wait();
+    if (blockIdx.x == 0 && threadIdx.x < 3) md.tile_ctr[3 + threadIdx.x] = 0;  // the adjoint element kernel's tile queues
     const int lane = threadIdx.x & 31;
     // block-uniform trip count: the contact-parameter gradients are reduced with full-warp shuffles
     for (size_t base = (size_t)blockIdx.x * blockDim.x; base < total; base += (size_t)gridDim.x * blockDim.x) {
@@ -487,7 +547,7 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
 
 // ------------------------------------------------------------------------------------------ adjoint elements
 template <int TYPE>
-__device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64_t *bars, int rot, const float4 *__restrict__ x4,
+__device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, const float4 *__restrict__ adjf, float4 *__restrict__ adjx,
                                           float4 *__restrict__ adjv) {
     TilePipe<TYPE, true> pipe(md, smem, bars, x4, v4, adjf);
@@ -496,7 +556,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
     const ElemDev &es = md.es[TYPE];
     const size_t gstride = (size_t)md.E * es.cpad;
     pipe.run(
-        rot,
+        rot, md.tile_ctr + 3 + TYPE, next_slot,
         [&](const TileView<TYPE, true> &tv, const ElemRegs<TYPE> &er, int tile, int env, float4 *so) {
             const int tid = threadIdx.x;
             const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
@@ -565,9 +625,9 @@ __global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, 
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_adj<T_TET>(md, smem + kBarBytes, bars, rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_adj<T_TRI>(md, smem + kBarBytes, bars + 5, rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_adj<T_HINGE>(md, smem + kBarBytes, bars + 10, rot, x4, v4, adjf, adjx, adjv);
+    if (md.es[T_TET].count) { tiles_adj<T_TET>(md, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_adj<T_TRI>(md, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_adj<T_HINGE>(md, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
 }
 
 // ------------------------------------------------------------------------------------------ layout conversion
