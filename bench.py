@@ -68,8 +68,8 @@ def element_stream_bytes(sc, table):
 # were captured at 64 substeps: bytes per substep of the launch, scaled by the rollout length.
 NCU_TRAFFIC = {
     "config4-large-1000000tets-522242tris": {
-        "k_elements_fwd": ("per_launch", 162186240), "k_particles_fwd": ("per_launch", 22874880),
-        "k_elements_adj": ("per_launch", 204269824), "k_particles_adj": ("per_launch", 40077056),
+        "k_elements_fwd": ("per_launch", 161568256), "k_particles_fwd": ("per_launch", 22874368),
+        "k_elements_adj": ("per_launch", 204752896), "k_particles_adj": ("per_launch", 40113664),
     },
     "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3554932), "k_resident_adj": ("per_substep", 4639652)},
 }
