@@ -276,12 +276,12 @@ struct TilePipe {
         }
         cp_async_commit();
     }
-    // `rot` rotates which CTAs get the odd extra tile, so that the types of one launch do not pile their remainders
-    // onto the same CTAs
+    // `rot` = number of items of the types already walked: the round-robin deal of items to CTAs continues across the
+    // types of one launch, so their remainders do not pile onto the same CTAs
     template <class Compute, class Emit>
     __device__ __forceinline__ void run_static(int rot, Compute compute, Emit emit) {
         const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
-        const int first = (int)((blockIdx.x + (unsigned)rot) % (unsigned)G);
+        const int first = (int)((blockIdx.x + (unsigned)G - (unsigned)rot % (unsigned)G) % (unsigned)G);  // item j of this type -> CTA (j + rot) mod G
         if (first >= n_items) return;
         const int cnt = (n_items - first + G - 1) / G;
         if (tid == 0) {
@@ -330,7 +330,7 @@ struct TilePipe {
     __device__ __forceinline__ void run(int rot, int *ctr, int *next_slot, Compute compute, Emit emit) {
         if (!kQueue) { run_static(rot, compute, emit); return; }
         const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
-        const int first = (int)((blockIdx.x + (unsigned)rot) % (unsigned)G);
+        const int first = (int)((blockIdx.x + (unsigned)G - (unsigned)rot % (unsigned)G) % (unsigned)G);  // item j of this type -> CTA (j + rot) mod G
         if (first >= n_items) return;
         const bool queue = kQueue && 2 * G < n_items;  // otherwise the static items cover everything
         int item = first, item_n = first + G;  // items i, i+1 (all threads)
