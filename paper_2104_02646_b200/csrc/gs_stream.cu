@@ -758,11 +758,11 @@ int configure_stream_kernels(gs_model *m) {
     m->smem_adj = adj + kBarBytes;
     int rc = tile_kernel_setup(k_elements_fwd, m->smem_fwd, &m->occ_fwd);
     if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj, m->smem_adj, &m->occ_adj);
-    // Programmatic dependent launch pays where a kernel is a few microseconds long (configs 1, 2: -15 % per step): the
-    // next kernel's CTAs are resident and past their prologue when the predecessor drains.  Once the element grid fills
-    // the machine it costs instead (config 4: +3.5 % per step; +14 % with a grid of 6 CTAs per SM where 9 fit): CTAs that
-    // launch into whatever slots free up first are placed unevenly over the SMs.  Measured crossover unknown between
-    // 157 and 7813 tiles; the rule below keeps the launch attribute while a type has at most two tiles per SM.
+    // Programmatic dependent launch pays where a kernel is a few microseconds long (20k tets, 157 tiles: -9 % per substep
+    // pair): the next kernel's CTAs are resident and past their prologue when the predecessor drains.  It is neutral
+    // from 350 to 650 tiles and costs beyond (250k tets +2.5 %, 490k tets +5 %): CTAs that launch into whatever slots
+    // free up first are placed unevenly over the SMs.  The rule keeps the launch attribute while the largest type has
+    // at most two tiles per SM.
     m->pdl = items <= 2LL * sms;
     // experiment overrides (not part of the interface)
     if (const char *q = getenv("GS_PDL")) m->pdl = atoi(q) != 0;
