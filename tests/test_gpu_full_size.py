@@ -171,6 +171,14 @@ def test_config4_full_size_substep_and_short_rollout():
     assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
     for k in ["adj_x0", "adj_v0"] + ["g_" + g for g in _groups(sc)]:
         assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
+    # entry points interleaved on one model at full size (the forward kernel's tile queues are re-zeroed by the
+    # particle kernel of every substep, whichever call launched it): two single steps == a 2-substep rollout, up to
+    # the order of the atomic sums
+    x1, v1 = m.step_forward(dev(x), dev(v))
+    x2, v2 = m.step_forward(x1, v1)
+    xT, vT = m.tape(2).rollout(dev(x), dev(v))
+    assert np.abs(host(x2) - host(xT)).max() <= 1e-6 * ext
+    assert rel_inf(host(v2), host(vT)) <= 1e-5
 
 
 def test_config4_full_rollout_properties():
