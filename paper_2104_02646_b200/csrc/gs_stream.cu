@@ -4,11 +4,14 @@
 //   k_elements_fwd   persistent CTAs (SM count x co-resident CTAs) walk the Morton-ordered tiles of kTileElems
 //                    elements: first their tets, then their triangles, then their hinges (all CTAs are in the same
 //                    type's code at the same time, which keeps the instruction cache warm).  A tile's streams arrive
-//                    in shared memory through a double-buffered asynchronous pipeline: the tile's particle ids two
-//                    tiles ahead and its packed static record (tile-local 16-bit connectivity, rest constants, gather
-//                    list) plus parameter block one tile ahead by cp.async.bulk (TMA 1-D) signalling an mbarrier,
-//                    issued by one thread; the particle states (x, v as float4) of the next tile by cp.async 16 B per
-//                    tile-particle from the ids already on chip.  No thread waits on a dependent global load.  One
+//                    through a double-buffered asynchronous pipeline: the tile's particle ids two tiles ahead and the
+//                    gather list of its packed record one tile ahead by cp.async.bulk (TMA 1-D) signalling an
+//                    mbarrier, issued by one thread; the particle states (x, v as float4) of the next tile by cp.async
+//                    16 B per tile-particle from the ids already on chip; the thread-private record fields (16-bit
+//                    staging indices, rest constants, material parameters) by a bulk L2 prefetch two tiles ahead and
+//                    one coalesced register load per thread one tile ahead.  No thread waits on a dependent global
+//                    load.  Tiles are dealt round-robin; the forward kernel claims its third and later tiles from a
+//                    global queue.  One
 //                    thread evaluates one element from shared memory, writes its per-vertex forces to conflict-free
 //                    float4 slots; after one barrier every thread sums four consecutive entries of the tile's gather list
 //                    (no shared-memory atomics: fp32 smem atomics are CAS loops on sm_100a) and issues ONE
@@ -148,11 +151,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
 // ------------------------------------------------------------------------------------------ tile pipeline
 // Shared memory of one CTA of a tile kernel (ADJ adds the gathered adj_f and a second output plane):
 //   ids   int[3][pmax]                      particle ids of tiles i, i+1, i+2      (bulk copy, two tiles ahead)
-//   buf   [2] { x, (v), (a) float4[pmax];   gathered particle states               (cp.async 16 B, one tile ahead)
-//               rec  RecLayout<TYPE>;       the tile's packed static record         (bulk copy, one tile ahead)
-//               par  float[3][256] }        mu | lambda | k_damp of (env, tile)     (bulk copy, one tile ahead)
-//   out   float4[arity][256] (x2 for ADJ with velocities)   per element-vertex contributions
-//   bars  uint64[5]                         full[2], idfull[3]
+//   loc   uint16[2][pmax]                   staging index of each list entry       (same bulk copy; dead after the gather)
+//   buf   [2] { x, (v), (a) float4[lmax];   gathered particle states               (cp.async 16 B, one tile ahead)
+//               slots uint16[4][128], slot_desc uint16[128] }   the record's gather list (bulk copy, one tile ahead)
+//   out   float4[arity][128] (x2 for ADJ with velocities)   per element-vertex contributions
+//   bars  uint64[5] per element type: full[2], idfull[3]; one int for the tile-queue hand-over
+// The rest of the record (connectivity, rest constants) and the parameters never enter shared memory: ElemRegs.
 template <int TYPE, bool ADJ>
 struct TileSmem {
     using R = RecLayout<TYPE>;
