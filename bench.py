@@ -64,14 +64,14 @@ def element_stream_bytes(sc, table):
 
 
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the hot kernels, from the ncu --set full
-# captures summarised under profiles/ (r1d_ncu_config4_streaming.md, r1c_ncu_config3_resident.md).  The resident kernels
+# captures summarised under profiles/ (r1d_ncu_config4_streaming.md, r1d_ncu_config3_resident.md).  The resident kernels
 # were captured at 64 substeps: bytes per substep of the launch, scaled by the rollout length.
 NCU_TRAFFIC = {
     "config4-large-1000000tets-522242tris": {
         "k_elements_fwd": ("per_launch", 161568256), "k_particles_fwd": ("per_launch", 22874368),
         "k_elements_adj": ("per_launch", 204752896), "k_particles_adj": ("per_launch", 40113664),
     },
-    "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3554932), "k_resident_adj": ("per_substep", 4639652)},
+    "config3-sysid-E1024": {"k_resident_fwd": ("per_substep", 3468752), "k_resident_adj": ("per_substep", 4660056)},
 }
 
 
