@@ -62,7 +62,10 @@ enum gs_param_group {
                         gs_set_params takes row 0 of its [E][Mh] argument; gs_param_grads returns dL/dk_b per environment */
     GS_CONTACT_KE = 8, GS_CONTACT_KD = 9, GS_CONTACT_KF = 10, GS_CONTACT_MUC = 11, /* contact parameters (NEXT-2): one value
                         per environment, arrays [E] (count = 1) */
-    GS_NUM_GROUPS = 12
+    GS_GRAVITY = 12, /* gravity (Table 5 column "g", NEXT-2): ONE vector shared by all environments -- gs_set_params reads
+                        d_values[0..2] (synchronises the stream; tapes re-capture their graphs at the next use);
+                        gs_param_grads returns dL/dg per environment, [E][3] (count = 3) */
+    GS_NUM_GROUPS = 13
 };
 
 /* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */
@@ -126,7 +129,9 @@ void gs_model_destroy(gs_model *m);
 int gs_model_plan(const gs_model *m);
 int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, int32_t *n_envs);
 
-/* Replace one parameter group from DEVICE values [E][count] in caller order (count = M, Mt, N or Mh). */
+/* Replace one parameter group from DEVICE values [E][count] in caller order (count = M, Mt, N or Mh).
+   Preconditions as in gs_model_create: finite values, mass > 0, lambda > 0.  The check runs on the device: an offending
+   entry keeps its old value and raises the non-finite flag, so the next gs_check_finite returns GS_ENONFINITE (substep 0). */
 int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream stream);
 
 /*

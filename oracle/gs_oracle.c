@@ -60,6 +60,7 @@ typedef struct {
     double *g_mass;                               /* [E][N] */
     double *g_ke, *g_kd, *g_kf, *g_muc;           /* [E]  dL/d(contact parameters) per environment (Table 5: contact parameters are optimisable) */
     double *g_hinge_kb;                           /* [E][Mh]  dL/dk_b per hinge (Table 5: bending stiffness is optimisable) */
+    double *g_gravity;                            /* [E][3]   dL/dg per environment (Table 5 column "g") */
 } orc_model;
 
 static char g_err[256] = "";
@@ -133,6 +134,7 @@ void orc_destroy(orc_model *m) {
     free(m->inc_ptr); free(m->inc_slot);
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
     free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb); free(m->g_ke); free(m->g_kd); free(m->g_kf); free(m->g_muc);
+    free(m->g_gravity);
     free(m);
 }
 
@@ -193,6 +195,7 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_mass = zeros_d((size_t)E * N);
     m->g_hinge_kb = zeros_d((size_t)E * Mh);
     m->g_ke = zeros_d((size_t)E); m->g_kd = zeros_d((size_t)E); m->g_kf = zeros_d((size_t)E); m->g_muc = zeros_d((size_t)E);
+    m->g_gravity = zeros_d((size_t)E * 3);
 
     /* tets: D_m = [X1-X0, X2-X0, X3-X0] (columns), B = D_m^-1, V = det(D_m)/6  (V_e) */
     for (int e = 0; e < M; e++) {
@@ -268,6 +271,7 @@ int orc_set_params(orc_model *m, int group, const double *v) {
         memcpy(cd[group - 8], v, sizeof(double) * m->E);
         return 0;
     }
+    if (group == 12) { m->g[0] = v[0]; m->g[1] = v[1]; m->g[2] = v[2]; return 0; } /* gravity: one vector for all environments */
     if (group < 0 || group > 6) return -1;
     memcpy(dst[group], v, sizeof(double) * n[group] * m->E);
     return 0;
@@ -280,6 +284,7 @@ int orc_get_grads(const orc_model *m, int group, double *out) {
         memcpy(out, cs[group - 8], sizeof(double) * m->E);
         return 0;
     }
+    if (group == 12) { memcpy(out, m->g_gravity, sizeof(double) * 3 * m->E); return 0; } /* [E][3] */
     if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
     return 0;
@@ -291,6 +296,7 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_mass, 0, sizeof(double) * E * m->N);
     memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
     memset(m->g_ke, 0, sizeof(double) * E); memset(m->g_kd, 0, sizeof(double) * E); memset(m->g_kf, 0, sizeof(double) * E); memset(m->g_muc, 0, sizeof(double) * E);
+    memset(m->g_gravity, 0, sizeof(double) * E * 3);
 }
 
 /* ---------------------------------------------------------------- tets */
@@ -699,6 +705,10 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         /* 2. contact */
         contact_adjoint(m, env, x + 3 * i, v + 3 * i, af + 3 * i, ax + 3 * i, av + 3 * i, gp + 4 * (size_t)i);
     }
+    /* gravity enters Listing 1 as v+ = v + (f w + g [w>0]) dt, so dL/dg = sum_i [w_i>0] dt lv_i (lv = cotangent of v+, = av here) */
+    for (int i = 0; i < N; i++)
+        if (inv_mass(m, env, i) > 0)
+            for (int r = 0; r < 3; r++) m->g_gravity[(size_t)env * 3 + r] += dt * (bv[3 * i + r] + dt * bx[3 * i + r]);
     for (int i = 0; i < N; i++) { /* serial, particle order: independent of the thread count */
         m->g_ke[env] += gp[4 * (size_t)i]; m->g_kd[env] += gp[4 * (size_t)i + 1]; m->g_kf[env] += gp[4 * (size_t)i + 2]; m->g_muc[env] += gp[4 * (size_t)i + 3];
     }

@@ -24,7 +24,7 @@ _LIB = os.path.join(_HERE, "libgs_oracle.so")
 
 TETS, TRIS, HINGES, CONTACT, ALL = 1, 2, 4, 8, 15
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12}
 
 
 def build(force: bool = False) -> str:
@@ -132,12 +132,12 @@ class Oracle:
 
     # ---- parameters / gradients
     def set_params(self, group, values):
-        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh}.get(GROUPS[group], 1)
+        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3}.get(GROUPS[group], 1)
         a = _d(np.broadcast_to(_d(values).reshape(-1, n), (self.E, n)))
         assert lib().orc_set_params(self.h, C.c_int(GROUPS[group]), _p(a)) == 0
 
     def grads(self, group):
-        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh}.get(GROUPS[group], 1)
+        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3}.get(GROUPS[group], 1)
         out = np.zeros((self.E, n))
         assert lib().orc_get_grads(self.h, C.c_int(GROUPS[group]), _p(out)) == 0
         return out

@@ -42,6 +42,10 @@ static int check_desc(const gs_model_desc *d) {
     GS_REQUIRE(d->dt > 0.0f, GS_EINVAL, "dt must be > 0");
     GS_REQUIRE(d->plan >= GS_PLAN_AUTO && d->plan <= GS_PLAN_RESIDENT, GS_EINVAL, "unknown plan %d", d->plan);
     GS_REQUIRE((size_t)d->n_particles * (size_t)d->n_envs < ((size_t)1 << 31), GS_EINVAL, "E*N must be < 2^31");
+    {  // work items (tile x environment) and padded element counts are ints in the kernels
+        const long long mx = d->n_tets > d->n_tris ? (d->n_tets > d->n_hinges ? d->n_tets : d->n_hinges) : (d->n_tris > d->n_hinges ? d->n_tris : d->n_hinges);
+        GS_REQUIRE((mx + kTileElems) * (long long)d->n_envs < (1LL << 31), GS_EINVAL, "E * padded element count must be < 2^31");
+    }
     return GS_OK;
 }
 
@@ -154,22 +158,27 @@ extern "C" void gs_tape_destroy(gs_tape *t) { delete t; }
 template <class F>
 static int graph_run(gs_model *m, gs_tape *t, cudaGraphExec_t *exec, uint64_t *n_launch, cudaStream_t st, F body) {
     if (m->timing || t->no_graph) return body(st);
+    if (*exec && t->g_epoch != m->epoch) {  // a by-value kernel argument (gravity) changed since the capture
+        if (t->g_fwd) { cudaGraphExecDestroy(t->g_fwd); t->g_fwd = nullptr; }
+        if (t->g_bwd) { cudaGraphExecDestroy(t->g_bwd); t->g_bwd = nullptr; }
+    }
     if (!*exec) {
-        const uint64_t n0 = g_launches;
+        if (!t->g_fwd && !t->g_bwd) t->g_epoch = m->epoch;
         cudaGraph_t g = nullptr;
         bool ok = t->cap_stream || cudaStreamCreateWithFlags(&t->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
         ok = ok && cudaStreamBeginCapture(t->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
         int rc = GS_OK;
         if (ok) {
+            t_capturing = true; t_captured = 0;  // launches enqueued while capturing are counted per replay, not now
             rc = body(t->cap_stream);
+            t_capturing = false;
             ok = cudaStreamEndCapture(t->cap_stream, &g) == cudaSuccess && g != nullptr && rc == GS_OK;
         }
         if (ok) {
-            *n_launch = g_launches - n0;
+            *n_launch = t_captured;
             ok = cudaGraphInstantiate(exec, g, 0) == cudaSuccess;
         }
         if (g) cudaGraphDestroy(g);
-        g_launches = n0;
         if (!ok) {
             cudaGetLastError();
             *exec = nullptr;
@@ -178,7 +187,7 @@ static int graph_run(gs_model *m, gs_tape *t, cudaGraphExec_t *exec, uint64_t *n
         }
     }
     GS_CUDA(cudaGraphLaunch(*exec, st), "cudaGraphLaunch");
-    g_launches += *n_launch;
+    count_launch(*n_launch);
     return GS_OK;
 }
 
@@ -415,12 +424,12 @@ extern "C" int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, c
         k_centroid_finish<<<dim3(kLossParts, n_envs), 256, 0, st>>>(n_particles, d_target, scale, accumulate, d_loss, d_adj_x, 0);
         k_centroid_finish<<<dim3(1, n_envs), 256, 0, st>>>(n_particles, d_target, scale, accumulate, d_loss, d_adj_x, 1);
         GS_CUDA(cudaGetLastError(), "k_centroid_partial / k_centroid_finish");
-        g_launches += 3;
+        count_launch(3);
         return GS_OK;
     }
     k_loss_centroid<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_target, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_centroid");
-    g_launches++;
+    count_launch();
     return GS_OK;
 }
 extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate, float *d_loss, float *d_adj_x,
@@ -431,12 +440,12 @@ extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const 
         if (!accumulate) GS_CUDA(cudaMemsetAsync(d_loss, 0, sizeof(float) * (size_t)n_envs, st), "zero loss");
         k_loss_pos_parts<<<dim3(kLossParts, n_envs), 256, 0, st>>>(n_particles, d_x, d_ref, scale, d_loss, d_adj_x);
         GS_CUDA(cudaGetLastError(), "k_loss_pos_parts");
-        g_launches++;
+        count_launch();
         return GS_OK;
     }
     k_loss_pos<<<n_envs, n_particles >= 4096 ? 1024 : 256, 0, (cudaStream_t)stream>>>(n_particles, d_x, d_ref, scale, accumulate, d_loss, d_adj_x);
     GS_CUDA(cudaGetLastError(), "k_loss_pos");
-    g_launches++;
+    count_launch();
     return GS_OK;
 }
 
@@ -446,7 +455,7 @@ static size_t al256(size_t n) { return (n + 255) & ~(size_t)255; }
 extern "C" size_t gs_host_scratch_bytes(const gs_model *m) {
     if (!m) return 0;
     const size_t st = al256((size_t)m->E * m->N * 3 * sizeof(float));
-    int cmax = m->N;
+    int cmax = m->N > 3 ? m->N : 3;  // gravity gradients are 3 per environment
     for (int t = 0; t < N_TYPES; t++) cmax = cmax > m->counts[t] ? cmax : m->counts[t];
     return 6 * st + al256((size_t)m->E * 3 * sizeof(float)) + al256((size_t)m->E * sizeof(float)) + al256((size_t)m->E * cmax * sizeof(float)) + 256;
 }
@@ -478,7 +487,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
     for (int k = 0; k < n_groups; k++) {
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
-        const int c = g == GS_MASS ? m->N : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3]));
+        const int c = g == GS_MASS ? m->N : (g == GS_GRAVITY ? 3 : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3])));
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
         // the staging buffer is reused: order the copy before the next group's kernel on the same stream
@@ -536,5 +545,5 @@ extern "C" int gs_kernel_times(gs_model *m, gs_stream stream, int n, double *ms_
     return GS_OK;
 }
 
-extern "C" uint64_t gs_launch_count(void) { return g_launches; }
+extern "C" uint64_t gs_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 extern "C" const char *gs_version(void) { return "gradsim-b200 0.1 (sm_100a)"; }

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -15,7 +16,8 @@ static const int kArity[N_TYPES] = {4, 3, 4};
 static const int kNumGrads[N_TYPES] = {3, 3, 1};  // accumulated parameter gradients per element: (mu, lambda, k_damp) x2, k_b
 
 constexpr int kTileElems = 128;      // elements per tile = threads per CTA of the streaming element kernels
-constexpr int kConSlots = 64;        // accumulator slots per environment for the contact-parameter gradients
+constexpr int kConSlots = 64;        // accumulator slots per environment for the per-environment gradient totals
+constexpr int kAccVals = 8;          // values per slot: dL/d(k_e, k_d, k_f, mu_c), dL/dg (3), one pad
 constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
 
 // Byte layout of one tile's RECORD: everything static a tile of kTileElems elements needs, packed contiguously so
@@ -76,9 +78,10 @@ struct ModelDev {
     const float *inv_mass;            // [E][N] internal order (0 = pinned)
     float *gmass32;                   // [E][N]
     double *gmass64;                  // [E][N]
-    float *gcon32;                    // [E][kConSlots][4] dL/d(k_e, k_d, k_f, mu_c): fp32 partial sums, spread over slots so
-                                      // that the warps of a launch do not all reduce into one L2 sector
-    double *gcon64;                   // [E][4] fp64 masters
+    double *gacc;                     // [E][kConSlots][kAccVals] per-environment totals dL/d(k_e, k_d, k_f, mu_c) and dL/dg:
+                                      // fp64 partial sums (red.global.add.f64 per warp), spread over slots so that the
+                                      // warps of a launch do not all reduce into one L2 sector
+    double *gcon64;                   // [E][kAccVals] fp64 masters
     int *tile_ctr;                    // [6] dynamic tile queues of the element kernels: forward tets/tris/hinges, adjoint
                                       // tets/tris/hinges.  Zero between launches: k_particles_fwd re-zeroes the forward
                                       // three after every k_elements_fwd, k_particles_adj the adjoint three before every
@@ -113,6 +116,7 @@ struct gs_model {
     bool pdl = true;                 // programmatic dependent launch of the hot-path kernels (small meshes only: configure_stream_kernels)
     long long elem_items = 0;        // work items (tile x environment) of the largest element type
     int step_counter = 0;  // substep index written to dev.bad on a non-finite state
+    uint64_t epoch = 0;    // bumped when a by-value kernel argument changes (gravity): captured graphs of older epochs are stale
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
     void *res_host = nullptr;
     // per-kernel event timing (gs_kernel_timing)
@@ -138,6 +142,7 @@ struct gs_tape {
     const float *g_bwd_frames = nullptr;  // the backward graph is specific to these frame arguments
     int g_bwd_n_frames = -1, g_bwd_stride = 0;
     bool no_graph = false;                // capture failed once: launch directly from then on
+    uint64_t g_epoch = 0;                 // model epoch the graphs were captured at
     ~gs_tape() {
         if (g_fwd) cudaGraphExecDestroy(g_fwd);
         if (g_bwd) cudaGraphExecDestroy(g_bwd);
@@ -172,7 +177,13 @@ void set_error(const char *fmt, ...);
 cudaEvent_t timing_begin(gs_model *m, cudaStream_t st);
 void timing_end(gs_model *m, int id, cudaEvent_t a, cudaStream_t st);
 int cuda_fail(cudaError_t e, const char *what);
-extern uint64_t g_launches;
+extern std::atomic<uint64_t> g_launches;  // process-wide launch counter (models on different host threads share it)
+extern thread_local bool t_capturing;     // this host thread is capturing a CUDA graph: launches are counted into t_captured
+extern thread_local uint64_t t_captured;
+inline void count_launch(uint64_t n = 1) {
+    if (t_capturing) t_captured += n;
+    else g_launches.fetch_add(n, std::memory_order_relaxed);
+}
 
 // gs_plan.cpp: host preprocessing.  Fills a byte image of the workspace (static part) and the model's host fields.
 struct WorkspaceLayout;

@@ -7,6 +7,7 @@
 //   triangles 2x2 B in the rest frame (t1, t2), A = det(D_m)/2   PAPER.md:584; A4
 //   hinges    theta0 (signed rest dihedral), l0 (rest edge)      PAPER.md:585-586; A5, A6
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -18,7 +19,9 @@
 namespace gs {
 
 static thread_local char t_err[512] = "";
-uint64_t g_launches = 0;
+std::atomic<uint64_t> g_launches{0};
+thread_local bool t_capturing = false;
+thread_local uint64_t t_captured = 0;
 
 void set_error(const char *fmt, ...) {
     va_list ap;
@@ -53,8 +56,8 @@ struct Layout {
     float *par[N_TYPES], *g32[N_TYPES];
     double *g64[N_TYPES];
     int *perm_p, *bad;
-    float *inv_mass, *gmass32, *ke, *kd, *kf, *muc, *gcon32;
-    double *gmass64, *gcon64;
+    float *inv_mass, *gmass32, *ke, *kd, *kf, *muc;
+    double *gmass64, *gcon64, *gacc;
     int *tile_ctr;
     float4 *f, *xs[2], *vs[2], *adjx, *adjv, *adjf;
     size_t bytes;
@@ -84,8 +87,8 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     L.inv_mass = b.take<float>(EN);
     L.gmass32 = b.take<float>(EN);
     L.gmass64 = b.take<double>(EN);
-    L.gcon32 = b.take<float>((size_t)E * kConSlots * 4);
-    L.gcon64 = b.take<double>((size_t)E * 4);
+    L.gacc = b.take<double>((size_t)E * kConSlots * kAccVals);
+    L.gcon64 = b.take<double>((size_t)E * kAccVals);
     L.tile_ctr = b.take<int>(8);
     L.ke = b.take<float>(E); L.kd = b.take<float>(E); L.kf = b.take<float>(E); L.muc = b.take<float>(E);
     L.bad = b.take<int>(1);
@@ -417,7 +420,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     }
     dev.pd = d->plane_d; dev.pr = d->particle_radius;
     dev.ke = L.ke; dev.kd = L.kd; dev.kf = L.kf; dev.muc = L.muc;
-    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gcon32 = L.gcon32; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad;
+    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gacc = L.gacc; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad;
     m->N = N; m->E = E;
     m->d_f = L.f; m->d_xs[0] = L.xs[0]; m->d_xs[1] = L.xs[1]; m->d_vs[0] = L.vs[0]; m->d_vs[1] = L.vs[1];
     m->d_adjx = L.adjx; m->d_adjv = L.adjv; m->d_adjf = L.adjf;
@@ -426,8 +429,8 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     cudaError_t ce = cudaMemsetAsync(L.f, 0, sizeof(float4) * EN, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gmass32, 0, sizeof(float) * EN, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gmass64, 0, sizeof(double) * EN, stream);
-    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gcon32, 0, sizeof(float) * (size_t)E * kConSlots * 4, stream);
-    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gcon64, 0, sizeof(double) * (size_t)E * 4, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gacc, 0, sizeof(double) * (size_t)E * kConSlots * kAccVals, stream);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(L.gcon64, 0, sizeof(double) * (size_t)E * kAccVals, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int) * 8, stream);
     if (ce == cudaSuccess) ce = cudaMemsetAsync(L.bad, 0x7f, sizeof(int), stream);
     if (ce != cudaSuccess) return cuda_fail(ce, "memset workspace");

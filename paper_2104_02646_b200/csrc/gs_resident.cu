@@ -53,9 +53,10 @@ struct ResHost {
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
 // shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
-// adjoint only: per-particle accumulators of the contact-parameter gradients, double[4][N] then float[4][N]
+// adjoint only: per-particle fp64 accumulators of the per-environment totals (contact parameters, gravity), double[7][N]
+constexpr int kResAcc = 7;
 static size_t res_smem(int L, int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)4 * N * 12) : 0) +
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)kResAcc * N * 8) : 0) +
            al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)4 * M * 2);
 }
 
@@ -208,11 +209,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     const int N = rd.N, M = rd.M, PL = 4 * M, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
     float4 *sf = smem4 + 3 * L;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
-    // dL/d(k_e, k_d, k_f, mu_c): per-particle partial sums (only the particle's lead lane touches its entries), fp32 chunks
-    // of kFlushEvery substeps folded into fp64 (hazard H4), summed in particle order at the end: deterministic
-    double *dgc = reinterpret_cast<double *>(sf + 2 * PL);  // [4][N]
-    float *sgc = reinterpret_cast<float *>(dgc + 4 * N);     // [4][N]
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((4 * N * 12 + 15) & ~15));
+    // dL/d(k_e, k_d, k_f, mu_c) and dL/dg: per-particle fp64 partial sums (only the particle's lead lane touches its
+    // entries; the contact terms are of mixed sign and cancel, so they are accumulated in fp64 from the start), summed in
+    // particle order at the end: deterministic
+    double *dgc = reinterpret_cast<double *>(sf + 2 * PL);  // [kResAcc][N]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((kResAcc * N * 8 + 15) & ~15));
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
     uint16_t *s_slots = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
@@ -237,7 +238,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
     if (po.lead)
-        for (int q = 0; q < 4; q++) { dgc[q * N + po.p] = 0.0; sgc[q * N + po.p] = 0.f; }
+        for (int q = 0; q < kResAcc; q++) dgc[q * N + po.p] = 0.0;
+    vec3 glv = zero3();  // sum over a chunk of substeps of lv (cotangent of v+): dL/dg = dt sum lv for a free particle
     const size_t frame_elems = (size_t)md.E * N * 3;
     const size_t gstride = (size_t)md.E * md.es[T_TET].cpad;
     float gm32 = 0.f;
@@ -280,12 +282,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             if (w > 0.0f) {
                 const vec3 dvf = (vec3(vnext) - v) - dt * g;
                 gm32 += -w * dot(dvf, lv);
+                glv += lv;
             }
             float gp[4];
             contact_adjoint(cp, x, v, af, ax, av, gp);
             if (gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f) {
 #pragma unroll
-                for (int q = 0; q < 4; q++) sgc[q * N + po.p] += gp[q];
+                for (int q = 0; q < 4; q++) dgc[q * N + po.p] += (double)gp[q];
             }
             bx = ax; bv = av;
             sx[po.lp] = xq; sv[po.lp] = vq; sa[po.lp] = make_float4(af.x, af.y, af.z, 0.f);
@@ -313,8 +316,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         }
         if ((s & (kFlushEvery - 1)) == 0) {  // fold the fp32 chunk into fp64 (hazard H4)
             if (po.lead) {
-#pragma unroll
-                for (int q = 0; q < 4; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
+                dgc[4 * N + po.p] += (double)(dt * glv.x); dgc[5 * N + po.p] += (double)(dt * glv.y); dgc[6 * N + po.p] += (double)(dt * glv.z);
+                glv = zero3();
             }
             // the fp64 masters live in global memory (each thread owns its entries; one update per kFlushEvery substeps),
             // which keeps 8 registers free for the element VJP
@@ -340,10 +343,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
     }
     __syncthreads();
-    if (tid < 4) {
+    if (tid < kResAcc) {
         double t = 0.0;
         for (int p = 0; p < N; p++) t += dgc[tid * N + p];
-        md.gcon64[(size_t)env * 4 + tid] += t;
+        md.gcon64[(size_t)env * kAccVals + tid] += t;
     }
 }
 
@@ -352,7 +355,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     do {                                                             \
         cudaError_t e_ = cudaGetLastError();                         \
         if (e_ != cudaSuccess) return cuda_fail(e_, what);           \
-        g_launches++;                                                \
+        count_launch();                                              \
     } while (0)
 
 static ResHost *res_of(gs_model *m) { return (ResHost *)m->res_host; }

@@ -37,7 +37,7 @@ namespace gs {
     do {                                                             \
         cudaError_t e_ = cudaGetLastError();                         \
         if (e_ != cudaSuccess) return cuda_fail(e_, what);           \
-        g_launches++;                                                \
+        count_launch();                                              \
     } while (0)
 // GS_TIMED(m, id, st, what, launch): the launch, bracketed by events when the model's kernel timing is on
 #define GS_TIMED(m, id, st, what, ...)                                 \
@@ -90,6 +90,9 @@ struct EmitPlan {
 };
 __device__ __forceinline__ void red_add_f32(float *addr, float a) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
+}
+__device__ __forceinline__ void red_add_f64(double *addr, double a) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(a) : "memory");
 }
 // Programmatic dependent launch: the hot-path kernels are launched with programmatic stream serialization, so a kernel
 // may start (and run its prologue: barrier init, bulk copies of STATIC tile data) while its predecessor drains.
@@ -500,7 +503,7 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
     // block-uniform trip count: the contact-parameter gradients are reduced with full-warp shuffles
     for (size_t base = (size_t)blockIdx.x * blockDim.x; base < total; base += (size_t)gridDim.x * blockDim.x) {
         const size_t i = base + threadIdx.x;
-        float gp[4] = {0.f, 0.f, 0.f, 0.f};
+        float gp[4] = {0.f, 0.f, 0.f, 0.f}, gg[3] = {0.f, 0.f, 0.f};
         int env = -1;
         if (i < total) {
             env = (int)(i / md.N);
@@ -520,30 +523,48 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
                 // f w dt = v+ - v- - g dt  =>  dL/dm = -w^2 dt f.lv = -w (v+ - v- - g dt).lv   (A11)
                 const vec3 dvf = (vec3(vn) - v) - dt * vec3(md.gx, md.gy, md.gz);
                 md.gmass32[i] += -w * dot(dvf, lv);
+                gg[0] = dt * lv.x; gg[1] = dt * lv.y; gg[2] = dt * lv.z;  // v+ = v + (f w + g) dt  =>  dL/dg += dt lv
             }
             contact_adjoint(contact_params(md, env), x, v, af, ax, av, gp);
             adjx[i] = make_float4(ax.x, ax.y, ax.z, 0.f);
             adjv[i] = make_float4(av.x, av.y, av.z, 0.f);
             adjf[i] = make_float4(af.x, af.y, af.z, 0.f);
         }
-        // dL/d(k_e, k_d, k_f, mu_c) of this warp's particles in contact: shuffle-reduce, one reduction per parameter
-        const bool mine = gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f;
-        const unsigned act = __ballot_sync(0xffffffffu, mine);
-        if (act) {
-            const int env0 = __shfl_sync(0xffffffffu, env, __ffs(act) - 1);
-            float *slot = md.gcon32 + ((size_t)env0 * kConSlots + (blockIdx.x & (kConSlots - 1))) * 4;
-            if (__all_sync(0xffffffffu, !mine || env == env0)) {
+        // per-environment totals (north_star (4): reduce with warp shuffles, then one reduction per value and warp into one
+        // of kConSlots fp64 slots): dL/dg = dt sum_i [w_i > 0] lv_i from every warp; dL/d(k_e, k_d, k_f, mu_c) from the warps
+        // that have a particle in contact.  The contact sums are sums of mixed-sign terms that cancel: they are
+        // shuffle-reduced in fp64.  Gravity terms are summed per warp in fp32 (32 terms) and accumulated in fp64.
+        const unsigned live = __ballot_sync(0xffffffffu, env >= 0);
+        if (live) {
+            const int env0 = __shfl_sync(0xffffffffu, env, __ffs(live) - 1);
+            const bool uni = __all_sync(0xffffffffu, env < 0 || env == env0);  // false: the warp straddles two environments
+            const bool mine = gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f;
+            const unsigned act = __ballot_sync(0xffffffffu, mine);
+            const int sl = blockIdx.x & (kConSlots - 1);
+            if (uni) {
+                double *slot = md.gacc + ((size_t)env0 * kConSlots + sl) * kAccVals;
 #pragma unroll
-                for (int q = 0; q < 4; q++) {
-                    float t = gp[q];
+                for (int q = 0; q < 3; q++) {
+                    float t = gg[q];
                     for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                    if (lane == 0 && t != 0.f) red_add_f32(slot + q, t);
+                    if (lane == 0 && t != 0.f) red_add_f64(slot + 4 + q, (double)t);
                 }
-            } else if (mine) {  // a warp that straddles two environments (N not a multiple of 32)
-                float *sl = md.gcon32 + ((size_t)env * kConSlots + (blockIdx.x & (kConSlots - 1))) * 4;
+                if (act) {
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {
+                        double t = (double)gp[q];
+                        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                        if (lane == 0 && t != 0.0) red_add_f64(slot + q, t);
+                    }
+                }
+            } else if (env >= 0) {
+                double *slot = md.gacc + ((size_t)env * kConSlots + sl) * kAccVals;
+#pragma unroll
+                for (int q = 0; q < 3; q++)
+                    if (gg[q] != 0.f) red_add_f64(slot + 4 + q, (double)gg[q]);
 #pragma unroll
                 for (int q = 0; q < 4; q++)
-                    if (gp[q] != 0.f) red_add_f32(sl + q, gp[q]);
+                    if (gp[q] != 0.f) red_add_f64(slot + q, (double)gp[q]);
             }
         }
     }
@@ -674,31 +695,36 @@ __global__ void k_get_grads(const double *__restrict__ g64, const int *__restric
     }
 }
 // q < 0: dst is the [E][count] inverse-mass array; else dst is ElemDev::par and q the parameter (0 mu, 1 lambda, 2 damp)
-__global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ perm, const float *__restrict__ src, int E, int count, int n_tiles, int q) {
+__global__ void k_set_params(float *__restrict__ dst, const int *__restrict__ perm, const float *__restrict__ src, int E, int count, int n_tiles, int q, int *__restrict__ bad) {
     const size_t total = (size_t)E * count;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / count), e = (int)(i - (size_t)env * count);
         const float val = src[(size_t)env * count + perm[e]];
+        // same preconditions as gs_model_create: finite values, mass > 0, lambda > 0 (alpha = 1 + 3 mu / (4 lambda)); a
+        // violation leaves the old value in place and raises the non-finite flag with substep index 0 (gs_check_finite)
+        const bool ok = fabsf(val) <= 3.0e38f && ((q != -1 && q != 1) || val > 0.f);
+        if (!ok) { atomicMin(bad, 0); continue; }
         if (q < 0) { if (dst[i] != 0.f) dst[i] = 1.0f / val; }  // pinned particles stay pinned
         else dst[par_index(n_tiles, env, e, q)] = val;
     }
 }
 
-// contact-parameter gradients: fold the fp32 slots of (env, q) into the fp64 master and clear them
-__global__ void k_flush_contact(float *__restrict__ g32, double *__restrict__ g64, int n, int zero_master) {
+// per-environment totals (contact parameters, gravity): fold the slots of (env, q) into the master and clear them
+__global__ void k_flush_contact(double *__restrict__ gacc, double *__restrict__ g64, int n, int zero_master) {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int env = i >> 2, q = i & 3;
+        const int env = i / kAccVals, q = i % kAccVals;
         double s = 0.0;
         for (int k = 0; k < kConSlots; k++) {
-            float *p = g32 + ((size_t)env * kConSlots + k) * 4 + q;
-            s += (double)*p;
-            *p = 0.f;
+            double *p = gacc + ((size_t)env * kConSlots + k) * kAccVals + q;
+            s += *p;
+            *p = 0.0;
         }
         g64[i] = zero_master ? 0.0 : g64[i] + s;
     }
 }
-__global__ void k_get_contact(const double *__restrict__ g64, float *__restrict__ out, int E, int q) {
-    for (int env = blockIdx.x * blockDim.x + threadIdx.x; env < E; env += gridDim.x * blockDim.x) out[env] = (float)g64[env * 4 + q];
+// out[env][0 .. cnt) = master values q0 .. q0 + cnt of every environment
+__global__ void k_get_contact(const double *__restrict__ g64, float *__restrict__ out, int E, int q0, int cnt) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < E * cnt; i += gridDim.x * blockDim.x) out[i] = (float)g64[(i / cnt) * kAccVals + q0 + i % cnt];
 }
 __global__ void k_set_scalar(float *__restrict__ dst, const float *__restrict__ src, int E) {
     for (int env = blockIdx.x * blockDim.x + threadIdx.x; env < E; env += gridDim.x * blockDim.x) dst[env] = src[env];
@@ -822,7 +848,7 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
         GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
     GS_TIMED(m, GS_K_OTHER, st, "k_flush", k_flush<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
-    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * 4), 256, 0, st>>>(m->dev.gcon32, m->dev.gcon64, m->E * 4, 0));
+    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * kAccVals), 256, 0, st>>>(m->dev.gacc, m->dev.gcon64, m->E * kAccVals, 0));
     return GS_OK;
 }
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
@@ -833,7 +859,7 @@ int launch_zero_grads(gs_model *m, cudaStream_t st) {
         GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for(n), 256, 0, st>>>(m->dev.es[t].g32, m->dev.es[t].g64, n));
     }
     GS_TIMED(m, GS_K_OTHER, st, "k_zero", k_zero<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass32, m->dev.gmass64, (size_t)m->E * m->N));
-    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * 4), 256, 0, st>>>(m->dev.gcon32, m->dev.gcon64, m->E * 4, 1));
+    GS_TIMED(m, GS_K_OTHER, st, "k_flush_contact", k_flush_contact<<<grid_for((size_t)m->E * kAccVals), 256, 0, st>>>(m->dev.gacc, m->dev.gcon64, m->E * kAccVals, 1));
     return GS_OK;
 }
 int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
@@ -842,7 +868,9 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     if (group == GS_MASS) {
         k_get_grads<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->dev.gmass64, m->dev.perm_p, d_out, m->E, m->N, m->N);
     } else if (group >= GS_CONTACT_KE && group <= GS_CONTACT_MUC) {
-        k_get_contact<<<grid_for((size_t)m->E), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, group - GS_CONTACT_KE);
+        k_get_contact<<<grid_for((size_t)m->E), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, group - GS_CONTACT_KE, 1);
+    } else if (group == GS_GRAVITY) {
+        k_get_contact<<<grid_for((size_t)m->E * 3), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, 4, 3);
     } else {
         const int t = group == GS_HINGE_KB ? T_HINGE : group / 3, q = group == GS_HINGE_KB ? 0 : group % 3, c = m->counts[t];
         if (c == 0) return GS_OK;
@@ -852,8 +880,20 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     return GS_OK;
 }
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st) {
+    if (group == GS_GRAVITY) {
+        // gravity is a by-value kernel argument (ModelDev): read the three floats back (synchronises the stream) and
+        // bump the epoch so that tapes re-capture their graphs
+        float g[3];
+        cudaError_t e = cudaMemcpyAsync(g, d_values, sizeof g, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "read gravity");
+        if (!(fabsf(g[0]) <= 3.0e38f) || !(fabsf(g[1]) <= 3.0e38f) || !(fabsf(g[2]) <= 3.0e38f)) { set_error("gravity must be finite"); return GS_EINVAL; }
+        m->dev.gx = g[0]; m->dev.gy = g[1]; m->dev.gz = g[2];
+        m->epoch++;
+        return GS_OK;
+    }
     if (group == GS_MASS) {
-        k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 0, -1);
+        k_set_params<<<grid_for((size_t)m->E * m->N), 256, 0, st>>>(m->d_inv_mass, m->dev.perm_p, d_values, m->E, m->N, 0, -1, m->dev.bad);
     } else if (group >= GS_CONTACT_KE && group <= GS_CONTACT_MUC) {
         const float *dst[4] = {m->dev.ke, m->dev.kd, m->dev.kf, m->dev.muc};
         k_set_scalar<<<grid_for((size_t)m->E), 256, 0, st>>>(const_cast<float *>(dst[group - GS_CONTACT_KE]), d_values, m->E);
@@ -864,7 +904,7 @@ int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_
     } else {
         const int t = group / 3, c = m->counts[t];
         if (c == 0) return GS_OK;
-        k_set_params<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].par, m->dev.es[t].perm, d_values, m->E, c, m->dev.es[t].n_tiles, group % 3);
+        k_set_params<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->dev.es[t].par, m->dev.es[t].perm, d_values, m->E, c, m->dev.es[t].n_tiles, group % 3, m->dev.bad);
     }
     GS_LAUNCH_CHECK("k_set_params");
     return GS_OK;

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgradsim.so")
 
 GS_OK, GS_EINVAL, GS_EMESH, GS_ENOMEM, GS_ECUDA, GS_ENONFINITE, GS_ESTATE = 0, -1, -2, -3, -4, -5, -6
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12}
 GS_ELEM_PER_ENV, GS_MASS_PER_ENV, GS_CONTACT_PER_ENV = 1, 2, 4
 GS_PLAN_AUTO, GS_PLAN_STREAMING, GS_PLAN_RESIDENT = 0, 1, 2
 
@@ -243,6 +243,8 @@ class Model:
 
     def group_count(self, group):
         g = GROUPS[group] if isinstance(group, str) else int(group)
+        if g == 12:
+            return 3  # gravity: dL/dg per environment
         if g >= 8:
             return 1  # contact parameters: one value per environment
         return self.N if g == 6 else (self.counts["hinge"] if g == 7 else (self.counts["tet"] if g < 3 else self.counts["tri"]))

@@ -8,10 +8,20 @@ config 3          the full 1024-environment launch; the oracle recomputes a seed
                   outcomes.  Those are recognised with the oracle alone -- its own result moves by more than the
                   tolerance under perturbations of the initial state of the size of fp32 rounding -- and excluded;
                   every other sampled environment must agree, and the excluded fraction is bounded.
-config 4          one substep forward + adjoint at full size from a deformed state, then a short rollout
-                  (the oracle needs ~1.2 s per substep pair at this size) with loss and every gradient.
+config 4          one substep forward + adjoint at full size from a deformed state and a short airborne rollout, then
+                  the FULL 256-substep rollout with the scene's own loss and the whole backward pass against the oracle
+                  (~5 min of oracle on the box's host cores), every output element by element.
+
+Relaxed branch (A20).  Only dL/dx0 and dL/dv0 may exceed 2e-3, and only up to what the oracle's own answer
+moves under fp32-sized perturbations of x0; parameter gradients are held to 2e-3 flat.  Every use of the relaxed branch is
+recorded: it must be listed in tests/golden/parity_relaxed_allow.json (so the set cannot grow silently), it raises a
+warning that `pytest -q` prints in its summary, and the measured errors / spreads are appended to
+$GS_PARITY_REPORT (default gpurun_out/parity_report.jsonl).
 """
 import copy
+import json
+import os
+import warnings
 
 import numpy as np
 import pytest
@@ -25,6 +35,21 @@ from gpu_util import dev, gpu_run_scene, host, rel_inf
 pytestmark = pytest.mark.gpu
 
 TOL_STEP, TOL_ROLLOUT, TOL_GRAD = 1e-5, 1e-3, 2e-3
+STATE_GRADS = ("adj_x0", "adj_v0")  # the only arrays eligible for the relaxed branch
+_HERE = os.path.dirname(os.path.abspath(__file__))
+ALLOW = json.load(open(os.path.join(_HERE, "golden", "parity_relaxed_allow.json")))
+
+
+def _report(record):
+    """Append one JSON record to the parity report and surface it in the pytest summary."""
+    path = os.environ.get("GS_PARITY_REPORT", os.path.join(os.path.dirname(_HERE), "gpurun_out", "parity_report.jsonl"))
+    try:
+        os.makedirs(os.path.dirname(path), exist_ok=True)
+        with open(path, "a") as f:
+            f.write(json.dumps(record) + "\n")
+    except OSError:
+        pass
+    warnings.warn("parity report: " + json.dumps(record))
 
 
 def _groups(sc):
@@ -67,18 +92,25 @@ def test_full_rollout_and_gradients(config):
     assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
     assert np.abs(got["rec_x"] - ref["rec_x"]).max() <= TOL_ROLLOUT * ext
     assert rel_inf(got["loss"], ref["loss"]) <= TOL_GRAD
-    keys = ["adj_x0", "adj_v0"] + ["g_" + g for g in _groups(sc)]
+    _compare_gradients(f"config{config}", sc, ref, got)
+
+
+def _compare_gradients(tag, sc, ref, got):
+    """Parameter gradients: 2e-3 flat.  dL/dx0, dL/dv0: 2e-3, or the relaxed branch described in the module docstring."""
+    keys = list(STATE_GRADS) + ["g_" + g for g in _groups(sc)]
     errs = {k: rel_inf(got[k], ref[k]) for k in keys}
     for k in keys:
         assert np.abs(ref[k]).max() > 0, k
-    late = [k for k in keys if errs[k] > TOL_GRAD]
-    if late:
+        if k not in STATE_GRADS:
+            assert errs[k] <= TOL_GRAD, (tag, k, errs[k])
+    late = [k for k in STATE_GRADS if errs[k] > TOL_GRAD]
+    spread = _oracle_spread(sc, ref, late) if late else {}
+    _report({"test": tag, "errors": errs, "relaxed": {k: {"error": errs[k], "oracle_spread": spread[k]} for k in late}})
+    for k in late:
         # beyond the stated tolerance: only acceptable where the oracle itself is no better conditioned than that
-        # (measured with the oracle alone), and never beyond 10x the tolerance
-        spread = _oracle_spread(sc, ref, late)
-        print(f"config {config}: conditioning-limited arrays {[(k, errs[k], spread[k]) for k in late]}")
-        for k in late:
-            assert errs[k] <= min(4.0 * spread[k], 10.0 * TOL_GRAD), (k, errs[k], spread[k])
+        # (measured with the oracle alone), never beyond 10x the tolerance, and only where a previous round recorded it
+        assert k in ALLOW.get(tag, []), f"{tag}: {k} off by {errs[k]:.2e} and not in parity_relaxed_allow.json"
+        assert errs[k] <= min(4.0 * spread[k], 10.0 * TOL_GRAD), (tag, k, errs[k], spread[k])
 
 
 def _env_scene(sc, e):
@@ -91,13 +123,24 @@ def _env_scene(sc, e):
     return s1
 
 
+C3_KEYS = ("loss", "adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_tet_damp", "g_mass")
+
+
 def _env_metrics(a, ref, ext):
-    """(rollout error / extent, worst per-environment-total gradient error) of one environment"""
+    """(rollout error / extent, worst gradient error) of one environment: the loss, dL/dx0, dL/dv0 and the per-tet /
+    per-particle gradient ARRAYS (A18 norm per array), plus the per-environment totals BASELINE.json configs[3] asks for"""
     ex = np.abs(a["xT"] - ref["xT"]).max() / ext
-    eg = 0.0
-    for g in ("tet_mu", "tet_lambda", "mass"):  # per-environment totals (BASELINE.json configs[3])
+    eg = max(rel_inf(a[k], ref[k]) for k in C3_KEYS)
+    for g in ("tet_mu", "tet_lambda", "mass"):
         eg = max(eg, abs(a["g_" + g].sum() - ref["g_" + g].sum()) / abs(ref["g_" + g].sum()))
     return ex, eg
+
+
+# Measured in round 2 (gpurun_out/parity_report.jsonl, summarised in DESIGN.md A20): 16 of these 128 environments
+# (12.5 %) sit at a contact discontinuity -- their ORACLE gradients move by 2 .. 235 tolerances under 1e-6 m
+# perturbations of x0 -- now that every per-tet / per-particle array is compared, not only the totals.  The cap leaves
+# room for two more; the property is the workload's (a box bouncing on a penalty plane for 1300 substeps), not the GPU's.
+C3_SAMPLE, C3_MAX_AMBIGUOUS = 128, 18
 
 
 def test_config3_full_batch_sampled_environments():
@@ -109,12 +152,12 @@ def test_config3_full_batch_sampled_environments():
     assert got["bad"] == -1
     assert np.isfinite(got["loss"]).all() and np.isfinite(got["g_tet_mu"]).all()
     ext = sc.extent() / 1.0
-    sample = scenes.rng_for(3, "misc", 11).choice(sc.n_envs, size=48, replace=False)
-    n_ambiguous, worst = 0, (0.0, 0.0)
+    sample = scenes.rng_for(3, "misc", 11).choice(sc.n_envs, size=C3_SAMPLE, replace=False)
+    ambiguous, worst = [], (0.0, 0.0)
     for e in sample:
         s1 = _env_scene(sc, int(e))
         ref = orc.run_scene(s1, target=target[:, e:e + 1])
-        a = {k: got[k][e:e + 1] for k in ("xT", "g_tet_mu", "g_tet_lambda", "g_mass")}
+        a = {k: got[k][e:e + 1] for k in ("xT",) + C3_KEYS}
         ex, eg = _env_metrics(a, ref, ext)
         if ex <= TOL_ROLLOUT and eg <= TOL_GRAD:
             worst = (max(worst[0], ex), max(worst[1], eg))
@@ -130,10 +173,10 @@ def test_config3_full_batch_sampled_environments():
             px, pg = _env_metrics(p, ref, ext)
             spread = max(spread, px / TOL_ROLLOUT, pg / TOL_GRAD)
         assert spread > 0.5, f"env {e}: GPU off by ({ex:.1e}, {eg:.1e}) while the oracle is stable there (spread {spread:.2f})"
-        n_ambiguous += 1
-    print(f"config 3: {len(sample) - n_ambiguous}/{len(sample)} sampled environments compared, worst rollout {worst[0]:.1e} grad {worst[1]:.1e}; "
-          f"{n_ambiguous} at a contact discontinuity")
-    assert n_ambiguous <= len(sample) // 4
+        ambiguous.append({"env": int(e), "rollout_err": ex, "grad_err": eg, "oracle_spread_in_tolerances": spread})
+    _report({"test": "config3", "sampled": len(sample), "compared": len(sample) - len(ambiguous), "worst_rollout": worst[0], "worst_grad": worst[1],
+             "at_contact_discontinuity": ambiguous})
+    assert len(ambiguous) <= C3_MAX_AMBIGUOUS
 
 
 def test_config4_full_size_substep_and_short_rollout():
@@ -179,6 +222,26 @@ def test_config4_full_size_substep_and_short_rollout():
     xT, vT = m.tape(2).rollout(dev(x), dev(v))
     assert np.abs(host(x2) - host(xT)).max() <= 1e-6 * ext
     assert rel_inf(host(v2), host(vT)) <= 1e-5
+
+
+def test_config4_full_rollout_vs_oracle():
+    """The whole config-4 workload exactly as bench.py times it (1M tets + 522k triangles + 782k hinges, 256 substeps,
+    full tape, the scene's own final-position loss, backward pass) against the oracle, element by element:
+    xT <= 1e-3 extent, loss and every parameter gradient <= 2e-3 (north_star).  ~5 min of oracle on 16 host cores."""
+    sc = scenes.make_scene(4)
+    assert sc.n_substeps == 256 and sc.loss == "pos_mse_frames" and sc.loss_times() == [256]
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"])
+    assert got["bad"] == -1
+    ext = sc.extent()
+    # both bodies reached the ground inside the rollout (impact ~ substep 123; the sheet is in its first rebound at
+    # T): nearly every particle's final velocity is far from free fall, i.e. contact is exercised at full size
+    free_fall_vy = -9.8 * sc.n_substeps * sc.dt
+    assert (np.abs(ref["vT"][..., 1] - free_fall_vy) > 0.5).sum() > 300_000
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
+    assert rel_inf(got["vT"], ref["vT"]) <= 1e-2  # velocities are not part of the stated tolerances: sanity bound
+    assert rel_inf(got["loss"], ref["loss"]) <= TOL_GRAD
+    _compare_gradients("config4", sc, ref, got)
 
 
 def test_config4_full_rollout_properties():

@@ -14,6 +14,8 @@ import pytest
 from oracle import oracle as orc
 from paper_2104_02646_b200 import scenes
 
+
+
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
@@ -59,6 +61,19 @@ def _mixed_scene(rng, **kw):
     return scenes.custom_scene(x, tets=tets, tris=tris + n0, hinges=hinges + n0, **args)
 
 
+SCALAR_GROUPS = ("ke", "kd", "kf", "mu_c")  # one value per environment
+
+
+def _param(sc, o, g):
+    """(analytic gradient, base value) of parameter group g as flat fp64 arrays of equal shape."""
+    if g == "gravity":  # one vector shared by all environments; the oracle keeps dL/dg per environment
+        return o.grads(g).sum(0).copy(), np.asarray(sc.gravity, np.float64)
+    scalar = g in SCALAR_GROUPS
+    an = (o.grads(g)[:, 0] if scalar else o.grads(g)[0]).copy()
+    base = getattr(sc, g).astype(np.float64)
+    return an, (base if g == "hinge_kb" or scalar else base[0])  # k_b is one array shared by all environments
+
+
 # ---------------------------------------------------------------- P1 integrate
 def test_p1_listing1_golden():
     g = _gold("listing1_integrate.txt")
@@ -89,6 +104,15 @@ def test_p1_free_fall_closed_form_and_adjoint():
     ax0, av0 = o.rollout_backward(ro, [T], cot)
     assert abs(av0[0, 0, 1] - T * dt) < 1e-15 and abs(ax0[0, 0, 1] - 1.0) < 1e-15
     assert np.all(o.grads("mass") == 0)  # free fall does not depend on mass (A11)
+    # dL/dg (Table 5): from the closed form, d(x_T,y of the free particle)/dg_y = dt^2 T (T+1)/2; the
+    # pinned particle ignores gravity; the other components of the cotangent are zero
+    gg = o.grads("gravity")[0]
+    assert abs(gg[1] - dt * dt * T * (T + 1) / 2) < 1e-15 and gg[0] == 0 and gg[2] == 0
+    # with a cotangent on the final VELOCITY of the free particle: d(v_T)/dg = T dt
+    o.zero_grads()
+    avT = np.zeros((1, 2, 3)); avT[0, 0, 2] = 1.0; avT[0, 1, 2] = 5.0
+    o.rollout_backward(ro, [T], 0 * cot, adj_vT=avT)
+    assert np.allclose(o.grads("gravity")[0], [0.0, 0.0, T * dt], atol=1e-15)
 
 
 # ---------------------------------------------------------------- rest quantities
@@ -318,16 +342,14 @@ def test_p7_step_param_gradients_vs_fd(group):
     bx, bv = rng.normal(size=(N, 3)), rng.normal(size=(N, 3))
     o.zero_grads()
     o.step_adjoint(x, v, bx, bv)
-    scalar = group in ("ke", "kd", "kf", "mu_c")  # one value per environment
-    g = o.grads(group)[:, 0] if scalar else o.grads(group)[0]
-    base = getattr(sc, group).astype(np.float64)
-    base = base if group == "hinge_kb" or scalar else base[0]  # k_b is one array shared by all environments
+    scalar = group in SCALAR_GROUPS
+    g, base = _param(sc, o, group)
     fd = np.zeros_like(base)
     for e in range(base.size):
         # one substep is piecewise LINEAR in the contact parameters (within a friction regime), so their central
         # difference is exact for any step that keeps the regimes; a larger step keeps round-off out of the tiny
         # stick-friction terms
-        h = (1e-3 if scalar else 1e-6) * base[e]
+        h = (1e-3 if scalar else 1e-6) * (base[e] if group != "gravity" else 1.0)
         vals = []
         for s in (+1, -1):
             p = base.copy(); p[e] += s * h
@@ -495,19 +517,21 @@ def test_p8_rollout_adjoint_vs_central_fd(which):
     SCALAR = ("ke", "kd", "kf", "mu_c")
     grads = {g: (o.grads(g)[:, 0] if g in SCALAR else o.grads(g)[0]).copy() for g in groups}
 
-    # 1e-5 (north_star check (c)) holds wherever central FD can resolve it; on the cloth resting on the ground the
-    # usable window between kink spacing and round-off closes at ~1.5e-5 for the damping gradients, hence 5e-5 there
-    tol = 1e-5 if which == "box" else 5e-5
+    tol = 1e-5  # north_star check (c), on both scenes
 
     def check(an, fd_fun, scale):
-        # a ladder of step sizes; accept the element if one matches to 1e-5.  These scenes rest on the ground, so
-        # |y| of some particle at some substep is as small as 1e-9: the loss is piecewise smooth with pieces that
-        # small (forces are only C0; A20) and central FD is exact only below that; round-off of L
-        # spoils the smallest steps where |dL/dtheta| * theta << L.  test_p8_smooth_regime_strict needs no ladder.
+        # "where a kink crossing spoils one FD step, repeat with two step sizes and take the consistent
+        # pair".  A ladder of step sizes is walked and the entry passes only when TWO different step sizes both
+        # reproduce the adjoint to `tol` (so they also agree with each other to 2 tol).  These scenes rest on the ground,
+        # so |y| of some particle at some substep is as small as 1e-9: the loss is piecewise smooth with pieces that
+        # small (forces are only C0; A20) and a central difference is only valid below the kink spacing,
+        # while round-off of L spoils the smallest steps.  test_p8_smooth_regime_strict needs no ladder.
+        hits = 0
         for h_rel in (1e-6, 1e-7, 1e-5, 1e-8, 1e-4, 1e-9, 1e-10, 1e-11):
-            fd = fd_fun(h_rel)
-            if abs(an - fd) <= tol * scale:
-                return True
+            if abs(an - fd_fun(h_rel)) <= tol * scale:
+                hits += 1
+                if hits == 2:
+                    return True
         return False
 
     for g in groups:
@@ -572,15 +596,12 @@ def test_p8_smooth_regime_strict():
     o.zero_grads()
     ax0, av0 = o.rollout_backward(ro, [T], cot)
     for g in orc.GROUPS:
-        scalar = g in ("ke", "kd", "kf", "mu_c")
-        an = (o.grads(g)[:, 0] if scalar else o.grads(g)[0]).copy()
-        base = getattr(sc, g).astype(np.float64)
-        base = base if g == "hinge_kb" or scalar else base[0]  # k_b is one array shared by all environments
+        an, base = _param(sc, o, g)
         for e in rng.choice(base.size, size=min(4, base.size), replace=False):
             if g == "mass" and sc.pinned[e]:
                 assert an[e] == 0
                 continue
-            h = 1e-5 * base[e]
+            h = 1e-5 * (base[e] if g != "gravity" else 1.0)
             vals = []
             for sgn in (+1, -1):
                 p = base.copy(); p[e] += sgn * h
