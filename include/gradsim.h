@@ -201,16 +201,23 @@ int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_re
                 float *d_loss, float *d_adj_x, gs_stream stream);
 
 /*
- * End-to-end convenience with HOST buffers (used by bench.py's e2e leg): uploads x0, v0 [E][N][3] and
- * the final-centroid targets [E][3], runs gs_rollout, the loss L_e = ||c(x_T) - target_e||^2,
- * gs_rollout_backward, and downloads loss [E], dL/dx0, dL/dv0 [E][N][3] (either may be NULL) and the
- * parameter gradients listed in groups[] into h_grads[k] ([E][count] each).  d_scratch: DEVICE block of
- * >= gs_host_scratch_bytes.  Zeroes the model's gradients first.  Synchronises.
+ * End-to-end convenience with HOST buffers (bench.py's e2e leg): ONE call uploads x0, v0 [E][N][3] and the loss
+ * targets, runs gs_rollout, the loss, gs_rollout_backward, and downloads loss [E], dL/dx0, dL/dv0 [E][N][3] (each may
+ * be NULL) and the parameter gradients listed in groups[] into h_grads[k] ([E][count] each).  Zeroes the model's
+ * gradients first.  Synchronises.  Losses (SURVEY.md 8(c) "Losses"; BASELINE.json configs):
+ *   GS_LOSS_FINAL_CENTROID  L_e = || c(x_T) - c*_e ||^2, c = mean_i x_i                  h_target [E][3]
+ *   GS_LOSS_POS_FRAMES      L_e = 1/(n_t N) sum_f sum_i || x_i(t_f) - ref_i(t_f) ||^2      h_target [n_t][E][N][3]
+ *   GS_LOSS_CENTROID_TRAJ   L_e = 1/n_t sum_f || c_e(t_f) - c*_e(t_f) ||^2                 h_target [n_t][E][3]
+ * with loss times t_f = frame_stride, 2 frame_stride, ... <= T (GS_LOSS_POS_FRAMES adds t = T when T is not a
+ * multiple), n_t their number.  frame_stride is ignored for GS_LOSS_FINAL_CENTROID; a checkpointed tape needs
+ * K | frame_stride.  d_scratch: DEVICE block of >= gs_host_scratch_bytes (same tape, loss_kind, frame_stride),
+ * 256-byte aligned.  Errors: GS_EINVAL (arguments), GS_ENONFINITE (as gs_check_finite), GS_ECUDA.
  */
-size_t gs_host_scratch_bytes(const gs_model *m);
-int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, const float *h_target,
-                                  float *h_loss, float *h_adj_x0, float *h_adj_v0, int n_groups, const int *groups,
-                                  float *const *h_grads, void *d_scratch, size_t scratch_bytes, gs_stream stream);
+enum gs_loss_kind { GS_LOSS_FINAL_CENTROID = 0, GS_LOSS_POS_FRAMES = 1, GS_LOSS_CENTROID_TRAJ = 2 };
+size_t gs_host_scratch_bytes(const gs_model *m, const gs_tape *t, int loss_kind, int frame_stride);
+int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, int loss_kind, int frame_stride,
+                                  const float *h_target, float *h_loss, float *h_adj_x0, float *h_adj_v0, int n_groups,
+                                  const int *groups, float *const *h_grads, void *d_scratch, size_t scratch_bytes, gs_stream stream);
 
 /* Number of kernel launches the library has enqueued since the process started (bench.py's gpu_launches). */
 uint64_t gs_launch_count(void);

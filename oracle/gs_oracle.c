@@ -61,6 +61,7 @@ typedef struct {
     double *g_ke, *g_kd, *g_kf, *g_muc;           /* [E]  dL/d(contact parameters) per environment (Table 5: contact parameters are optimisable) */
     double *g_hinge_kb;                           /* [E][Mh]  dL/dk_b per hinge (Table 5: bending stiffness is optimisable) */
     double *g_gravity;                            /* [E][3]   dL/dg per environment (Table 5 column "g") */
+    double *g_con_abs;                            /* [E][4]   diagnostic only: sum of |term| behind g_ke, g_kd, g_kf, g_muc (how far each total cancels) */
 } orc_model;
 
 static char g_err[256] = "";
@@ -134,7 +135,7 @@ void orc_destroy(orc_model *m) {
     free(m->inc_ptr); free(m->inc_slot);
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
     free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb); free(m->g_ke); free(m->g_kd); free(m->g_kf); free(m->g_muc);
-    free(m->g_gravity);
+    free(m->g_gravity); free(m->g_con_abs);
     free(m);
 }
 
@@ -195,7 +196,7 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_mass = zeros_d((size_t)E * N);
     m->g_hinge_kb = zeros_d((size_t)E * Mh);
     m->g_ke = zeros_d((size_t)E); m->g_kd = zeros_d((size_t)E); m->g_kf = zeros_d((size_t)E); m->g_muc = zeros_d((size_t)E);
-    m->g_gravity = zeros_d((size_t)E * 3);
+    m->g_gravity = zeros_d((size_t)E * 3); m->g_con_abs = zeros_d((size_t)E * 4);
 
     /* tets: D_m = [X1-X0, X2-X0, X3-X0] (columns), B = D_m^-1, V = det(D_m)/6  (V_e) */
     for (int e = 0; e < M; e++) {
@@ -285,6 +286,7 @@ int orc_get_grads(const orc_model *m, int group, double *out) {
         return 0;
     }
     if (group == 12) { memcpy(out, m->g_gravity, sizeof(double) * 3 * m->E); return 0; } /* [E][3] */
+    if (group == 13) { memcpy(out, m->g_con_abs, sizeof(double) * 4 * m->E); return 0; } /* [E][4] diagnostic */
     if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
     return 0;
@@ -296,7 +298,7 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_mass, 0, sizeof(double) * E * m->N);
     memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
     memset(m->g_ke, 0, sizeof(double) * E); memset(m->g_kd, 0, sizeof(double) * E); memset(m->g_kf, 0, sizeof(double) * E); memset(m->g_muc, 0, sizeof(double) * E);
-    memset(m->g_gravity, 0, sizeof(double) * E * 3);
+    memset(m->g_gravity, 0, sizeof(double) * E * 3); memset(m->g_con_abs, 0, sizeof(double) * E * 4);
 }
 
 /* ---------------------------------------------------------------- tets */
@@ -711,6 +713,7 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
             for (int r = 0; r < 3; r++) m->g_gravity[(size_t)env * 3 + r] += dt * (bv[3 * i + r] + dt * bx[3 * i + r]);
     for (int i = 0; i < N; i++) { /* serial, particle order: independent of the thread count */
         m->g_ke[env] += gp[4 * (size_t)i]; m->g_kd[env] += gp[4 * (size_t)i + 1]; m->g_kf[env] += gp[4 * (size_t)i + 2]; m->g_muc[env] += gp[4 * (size_t)i + 3];
+        for (int q = 0; q < 4; q++) m->g_con_abs[(size_t)env * 4 + q] += fabs(gp[4 * (size_t)i + q]);
     }
     free(gp);
     /* 3-5. elements: per-element-vertex contributions into private slots, then gather per particle */
@@ -827,6 +830,15 @@ void orc_rollout_backward(orc_model *m, int T, int K, const double *ck_x, const 
     free(bx); free(bv); free(ax); free(av); free(seg_x); free(seg_v);
 }
 
+/* bench.py's single-thread CPU baseline (SURVEY.md 8(d) timing protocol); results do not depend on the thread count */
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    extern void omp_set_num_threads(int);
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
 int orc_num_threads(void) {
 #ifdef _OPENMP
     extern int omp_get_max_threads(void);

@@ -142,6 +142,12 @@ class Oracle:
         assert lib().orc_get_grads(self.h, C.c_int(GROUPS[group]), _p(out)) == 0
         return out
 
+    def contact_abs_sums(self):
+        """[E, 4] diagnostic: sum of |term| behind the totals dL/d(k_e, k_d, k_f, mu_c) -- how far each total cancels."""
+        out = np.zeros((self.E, 4))
+        assert lib().orc_get_grads(self.h, C.c_int(13), _p(out)) == 0
+        return out
+
     def zero_grads(self):
         lib().orc_zero_grads(self.h)
 
@@ -188,6 +194,10 @@ class Oracle:
 
 def num_threads() -> int:
     return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(C.c_int(int(n)))
 
 
 # ------------------------------------------------------------------ losses (fp64 numpy)
@@ -251,4 +261,5 @@ def run_scene(sc, target=None, K=None):
     out = dict(xT=ro["xT"], vT=ro["vT"], loss=L, adj_x0=ax0, adj_v0=av0, rec_x=ro["rec_x"], target=target)
     for g in GROUPS:
         out["g_" + g] = o.grads(g)
+    out["contact_abs"] = o.contact_abs_sums()
     return out

@@ -115,7 +115,7 @@ extern "C" int gs_step_backward(gs_model *m, const float *d_x, const float *d_v,
     // the end-of-step velocity enters the mass gradient: recompute the forward step
     GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], 0, st));
     GS_TRY(launch_pack(m, d_adj_x_out, d_adj_v_out, m->d_adjx, m->d_adjv, false, st));
-    GS_TRY(stream_step_adjoint(m, m->d_xs[0], m->d_vs[0], m->d_vs[1], nullptr, st));
+    GS_TRY(stream_step_adjoint(m, m->d_xs[0], m->d_vs[0], m->d_vs[1], -1, st));
     return launch_unpack(m, m->d_adjx, m->d_adjv, d_adj_x_in, d_adj_v_in, st);
 }
 
@@ -233,11 +233,14 @@ extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int fr
     if (m->plan == GS_PLAN_RESIDENT && t->K == 1) {
         GS_TRY(resident_rollout_backward(m, t, n_frames, frame_stride, d_adj_x_frames, st));
     } else {
-        if (t->g_bwd && (t->g_bwd_frames != d_adj_x_frames || t->g_bwd_n_frames != n_frames || t->g_bwd_stride != frame_stride)) {
-            cudaGraphExecDestroy(t->g_bwd);  // other frame arguments: capture again
+        if (t->g_bwd && (t->g_bwd_n_frames != n_frames || t->g_bwd_stride != frame_stride)) {
+            cudaGraphExecDestroy(t->g_bwd);  // other frame layout: capture again
             t->g_bwd = nullptr;
         }
-        t->g_bwd_frames = d_adj_x_frames; t->g_bwd_n_frames = n_frames; t->g_bwd_stride = frame_stride;
+        t->g_bwd_n_frames = n_frames; t->g_bwd_stride = frame_stride;
+        // the frame array's base pointer reaches the kernels through a workspace slot, so another buffer of the same
+        // layout (torch hands out a new address every iteration) replays the same graph
+        if (n_frames > 0) GS_TRY(launch_set_frame_base(m, d_adj_x_frames, st));
         GS_TRY(graph_run(m, t, &t->g_bwd, &t->g_bwd_launches, st, [&](cudaStream_t q) {
             GS_TRY(launch_flush_grads(m, q));  // fixed flush positions whatever ran before (resets the 32-substep counter)
             for (int c = t->n_ck - 1; c >= 0; c--) {
@@ -247,9 +250,9 @@ extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int fr
                     GS_TRY(stream_step_forward(m, t->slot_x(a), t->slot_v(a), t->slot_x(b), t->slot_v(b), s, q));
                 }
                 for (int s = t1 - 1; s >= t0; s--) {
-                    const float *cot = nullptr;
+                    long long cot = -1;
                     if (n_frames > 0 && (s + 1) % frame_stride == 0 && (s + 1) / frame_stride <= n_frames)
-                        cot = d_adj_x_frames + (size_t)((s + 1) / frame_stride - 1) * frame_elems;
+                        cot = (long long)((s + 1) / frame_stride - 1) * (long long)frame_elems;
                     const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
                     GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, q));
                 }
@@ -452,46 +455,91 @@ extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const 
 // ------------------------------------------------------------------------------------------ host-buffer end-to-end
 static size_t al256(size_t n) { return (n + 255) & ~(size_t)255; }
 
-extern "C" size_t gs_host_scratch_bytes(const gs_model *m) {
-    if (!m) return 0;
-    const size_t st = al256((size_t)m->E * m->N * 3 * sizeof(float));
-    int cmax = m->N > 3 ? m->N : 3;  // gravity gradients are 3 per environment
-    for (int t = 0; t < N_TYPES; t++) cmax = cmax > m->counts[t] ? cmax : m->counts[t];
-    return 6 * st + al256((size_t)m->E * 3 * sizeof(float)) + al256((size_t)m->E * sizeof(float)) + al256((size_t)m->E * cmax * sizeof(float)) + 256;
+// loss times of a rollout of T substeps (SURVEY.md 8(c) "Losses"): the final state only, or every frame_stride-th
+// substep (position loss: plus the final state when T is not a multiple)
+static int loss_times(int kind, int T, int stride, int *n_frames, bool *final_extra) {
+    *final_extra = false;
+    if (kind == GS_LOSS_FINAL_CENTROID) { *n_frames = 0; return 1; }
+    *n_frames = T / stride;
+    *final_extra = kind == GS_LOSS_POS_FRAMES && T % stride != 0;
+    return *n_frames + (*final_extra ? 1 : 0);
+}
+static size_t target_floats(const gs_model *m, int kind, int n_t) {
+    const size_t per = kind == GS_LOSS_POS_FRAMES ? (size_t)m->E * m->N * 3 : (size_t)m->E * 3;
+    return per * (size_t)n_t;
 }
 
-extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, const float *h_target, float *h_loss,
-                                             float *h_adj_x0, float *h_adj_v0, int n_groups, const int *groups, float *const *h_grads, void *d_scratch,
-                                             size_t scratch_bytes, gs_stream stream) {
+extern "C" size_t gs_host_scratch_bytes(const gs_model *m, const gs_tape *t, int loss_kind, int frame_stride) {
+    if (!m || !t || loss_kind < GS_LOSS_FINAL_CENTROID || loss_kind > GS_LOSS_CENTROID_TRAJ || (loss_kind != GS_LOSS_FINAL_CENTROID && frame_stride < 1)) return 0;
+    const size_t st = al256((size_t)m->E * m->N * 3 * sizeof(float));
+    int cmax = m->N > 3 ? m->N : 3;  // gravity gradients are 3 per environment
+    for (int k = 0; k < N_TYPES; k++) cmax = cmax > m->counts[k] ? cmax : m->counts[k];
+    int n_frames = 0;
+    bool extra = false;
+    const int n_t = loss_times(loss_kind, t->T, frame_stride, &n_frames, &extra);
+    return 6 * st + (size_t)n_frames * st + al256(target_floats(m, loss_kind, n_t) * sizeof(float)) + al256((size_t)m->E * sizeof(float)) +
+           al256((size_t)m->E * cmax * sizeof(float)) + 256;
+}
+
+extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const float *h_x0, const float *h_v0, int loss_kind, int frame_stride,
+                                             const float *h_target, float *h_loss, float *h_adj_x0, float *h_adj_v0, int n_groups, const int *groups,
+                                             float *const *h_grads, void *d_scratch, size_t scratch_bytes, gs_stream stream) {
     GS_REQUIRE(m && t && h_x0 && h_v0 && h_target && d_scratch, GS_EINVAL, "null argument");
+    GS_REQUIRE(t->m == m, GS_EINVAL, "tape belongs to another model");
     GS_REQUIRE(n_groups >= 0 && (n_groups == 0 || (groups && h_grads)), GS_EINVAL, "bad groups");
-    GS_REQUIRE(scratch_bytes >= gs_host_scratch_bytes(m) && ((uintptr_t)d_scratch & 255) == 0, GS_EINVAL, "scratch too small or misaligned");
+    GS_REQUIRE(loss_kind >= GS_LOSS_FINAL_CENTROID && loss_kind <= GS_LOSS_CENTROID_TRAJ, GS_EINVAL, "unknown loss kind %d", loss_kind);
+    GS_REQUIRE(loss_kind == GS_LOSS_FINAL_CENTROID || (frame_stride >= 1 && frame_stride <= t->T), GS_EINVAL, "frame_stride must be in [1, T]");
+    GS_REQUIRE(loss_kind == GS_LOSS_FINAL_CENTROID || t->K == 1 || frame_stride % t->K == 0, GS_EINVAL,
+               "a checkpointed tape holds multiples of %d only: frame_stride %d is not one", t->K, frame_stride);
+    const size_t need = gs_host_scratch_bytes(m, t, loss_kind, frame_stride);
+    GS_REQUIRE(scratch_bytes >= need && ((uintptr_t)d_scratch & 255) == 0, GS_EINVAL, "scratch too small (%zu < %zu) or misaligned", scratch_bytes, need);
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t sb = (size_t)m->E * m->N * 3 * sizeof(float), sa = al256(sb);
+    const int E = m->E, N = m->N, T = t->T;
+    int n_frames = 0;
+    bool extra = false;
+    const int n_t = loss_times(loss_kind, T, frame_stride, &n_frames, &extra);
+    const size_t sb = (size_t)E * N * 3 * sizeof(float), sa = al256(sb), tf = target_floats(m, loss_kind, n_t);
     char *p = (char *)d_scratch;
-    float *d_x0 = (float *)p, *d_v0 = (float *)(p + sa), *d_xT = (float *)(p + 2 * sa), *d_cot = (float *)(p + 3 * sa);
+    float *d_x0 = (float *)p, *d_v0 = (float *)(p + sa), *d_xt = (float *)(p + 2 * sa), *d_cot = (float *)(p + 3 * sa);
     float *d_ax0 = (float *)(p + 4 * sa), *d_av0 = (float *)(p + 5 * sa);
-    float *d_tgt = (float *)(p + 6 * sa);
-    float *d_loss = (float *)((char *)d_tgt + al256((size_t)m->E * 3 * sizeof(float)));
-    float *d_g = (float *)((char *)d_loss + al256((size_t)m->E * sizeof(float)));
+    float *d_frames = (float *)(p + 6 * sa);  // [n_frames][E][N][3] cotangents of the frame states (sb bytes each, packed)
+    float *d_tgt = (float *)(p + 6 * sa + al256((size_t)n_frames * sb));
+    float *d_loss = (float *)((char *)d_tgt + al256(tf * sizeof(float)));
+    float *d_g = (float *)((char *)d_loss + al256((size_t)E * sizeof(float)));
     GS_CUDA(cudaMemcpyAsync(d_x0, h_x0, sb, cudaMemcpyHostToDevice, st), "H2D x0");
     GS_CUDA(cudaMemcpyAsync(d_v0, h_v0, sb, cudaMemcpyHostToDevice, st), "H2D v0");
-    GS_CUDA(cudaMemcpyAsync(d_tgt, h_target, (size_t)m->E * 3 * sizeof(float), cudaMemcpyHostToDevice, st), "H2D target");
+    GS_CUDA(cudaMemcpyAsync(d_tgt, h_target, tf * sizeof(float), cudaMemcpyHostToDevice, st), "H2D target");
     GS_TRY(gs_zero_grads(m, stream));
-    GS_TRY(gs_rollout(m, t, d_x0, d_v0, d_xT, nullptr, stream));
-    GS_TRY(gs_loss_centroid(m->E, m->N, d_xT, d_tgt, 1.0f, 0, d_loss, d_cot, stream));
-    GS_TRY(gs_rollout_backward(m, t, 0, 1, nullptr, d_cot, nullptr, d_ax0, d_av0, stream));
-    if (h_loss) GS_CUDA(cudaMemcpyAsync(h_loss, d_loss, (size_t)m->E * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
+    GS_TRY(gs_rollout(m, t, d_x0, d_v0, d_xt, nullptr, stream));
+    const float *cot_T = nullptr;
+    if (loss_kind == GS_LOSS_FINAL_CENTROID) {
+        GS_TRY(gs_loss_centroid(E, N, d_xt, d_tgt, 1.0f, 0, d_loss, d_cot, stream));
+        cot_T = d_cot;
+    } else {
+        // L = 1/(n_t N) sum_f sum_i |x_i(t_f) - ref|^2   or   L = 1/n_t sum_f |c(t_f) - c*_f|^2; frame f = state after (f+1) stride
+        const float scale = loss_kind == GS_LOSS_POS_FRAMES ? 1.0f / ((float)n_t * (float)N) : 1.0f / (float)n_t;
+        const size_t per = tf / (size_t)n_t;
+        for (int f = 0; f < n_t; f++) {
+            const int ts = f < n_frames ? (f + 1) * frame_stride : T;  // f == n_frames: the extra final-state term
+            float *cot = f < n_frames ? d_frames + (size_t)f * (sb / sizeof(float)) : d_cot;
+            GS_TRY(gs_tape_read(m, t, ts, d_xt, nullptr, stream));
+            if (loss_kind == GS_LOSS_POS_FRAMES) GS_TRY(gs_loss_pos(E, N, d_xt, d_tgt + (size_t)f * per, scale, f > 0, d_loss, cot, stream));
+            else GS_TRY(gs_loss_centroid(E, N, d_xt, d_tgt + (size_t)f * per, scale, f > 0, d_loss, cot, stream));
+            if (f >= n_frames) cot_T = d_cot;
+        }
+    }
+    GS_TRY(gs_rollout_backward(m, t, n_frames, n_frames ? frame_stride : 1, n_frames ? d_frames : nullptr, cot_T, nullptr, d_ax0, d_av0, stream));
+    if (h_loss) GS_CUDA(cudaMemcpyAsync(h_loss, d_loss, (size_t)E * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H loss");
     if (h_adj_x0) GS_CUDA(cudaMemcpyAsync(h_adj_x0, d_ax0, sb, cudaMemcpyDeviceToHost, st), "D2H adj_x0");
     if (h_adj_v0) GS_CUDA(cudaMemcpyAsync(h_adj_v0, d_av0, sb, cudaMemcpyDeviceToHost, st), "D2H adj_v0");
     for (int k = 0; k < n_groups; k++) {
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
-        const int c = g == GS_MASS ? m->N : (g == GS_GRAVITY ? 3 : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3])));
+        const int c = g == GS_MASS ? N : (g == GS_GRAVITY ? 3 : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3])));
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
-        // the staging buffer is reused: order the copy before the next group's kernel on the same stream
-        GS_CUDA(cudaMemcpyAsync(h_grads[k], d_g, (size_t)m->E * c * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H grads");
+        // the staging buffer is reused: the copy is ordered before the next group's kernel on the same stream
+        GS_CUDA(cudaMemcpyAsync(h_grads[k], d_g, (size_t)E * c * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H grads");
     }
     GS_CUDA(cudaStreamSynchronize(st), "synchronize");
     int bad = -1;

@@ -87,6 +87,9 @@ struct ModelDev {
                                       // three after every k_elements_fwd, k_particles_adj the adjoint three before every
                                       // k_elements_adj
     int *bad;                         // first non-finite substep (INT_MAX = none)
+    const float **frame_base;         // [1] base of the caller's frame-cotangent array of the running backward pass: read
+                                      // through this slot (written by a one-thread kernel before the pass) so that the
+                                      // captured backward graph does not depend on the caller's pointer
 };
 
 struct HostElemSet {
@@ -139,8 +142,7 @@ struct gs_tape {
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t g_fwd = nullptr, g_bwd = nullptr;
     uint64_t g_fwd_launches = 0, g_bwd_launches = 0;
-    const float *g_bwd_frames = nullptr;  // the backward graph is specific to these frame arguments
-    int g_bwd_n_frames = -1, g_bwd_stride = 0;
+    int g_bwd_n_frames = -1, g_bwd_stride = 0;  // the backward graph is specific to these frame arguments (not to the pointer)
     bool no_graph = false;                // capture failed once: launch directly from then on
     uint64_t g_epoch = 0;                 // model epoch the graphs were captured at
     ~gs_tape() {
@@ -192,7 +194,8 @@ int build_model(const gs_model_desc *desc, void *d_workspace, size_t bytes, cuda
 
 // gs_stream.cu: streaming plan launches
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st);
-int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st);
+int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, cudaStream_t st);
+int launch_set_frame_base(gs_model *m, const float *d_frames, cudaStream_t st);
 int launch_pack(gs_model *m, const float *x, const float *v, float4 *x4, float4 *v4, bool x_is_state, cudaStream_t st);
 int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, float *v, cudaStream_t st);
 int launch_flush_grads(gs_model *m, cudaStream_t st);

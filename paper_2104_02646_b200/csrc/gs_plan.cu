@@ -59,6 +59,7 @@ struct Layout {
     float *inv_mass, *gmass32, *ke, *kd, *kf, *muc;
     double *gmass64, *gcon64, *gacc;
     int *tile_ctr;
+    const float **frame_base;
     float4 *f, *xs[2], *vs[2], *adjx, *adjv, *adjf;
     size_t bytes;
 };
@@ -90,6 +91,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     L.gacc = b.take<double>((size_t)E * kConSlots * kAccVals);
     L.gcon64 = b.take<double>((size_t)E * kAccVals);
     L.tile_ctr = b.take<int>(8);
+    L.frame_base = b.take<const float *>(1);
     L.ke = b.take<float>(E); L.kd = b.take<float>(E); L.kf = b.take<float>(E); L.muc = b.take<float>(E);
     L.bad = b.take<int>(1);
     L.f = b.take<float4>(EN);
@@ -420,7 +422,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     }
     dev.pd = d->plane_d; dev.pr = d->particle_radius;
     dev.ke = L.ke; dev.kd = L.kd; dev.kf = L.kf; dev.muc = L.muc;
-    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gacc = L.gacc; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad;
+    dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gacc = L.gacc; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad; dev.frame_base = L.frame_base;
     m->N = N; m->E = E;
     m->d_f = L.f; m->d_xs[0] = L.xs[0]; m->d_xs[1] = L.xs[1]; m->d_vs[0] = L.vs[0]; m->d_vs[1] = L.vs[1];
     m->d_adjx = L.adjx; m->d_adjv = L.adjv; m->d_adjf = L.adjf;

@@ -491,15 +491,17 @@ __global__ void __launch_bounds__(256) k_particles_fwd(const ModelDev md, const 
 }
 
 // ------------------------------------------------------------------------------------------ adjoint particles
-// frame_cot: caller-order [E][N][3] cotangent dL/dx of the state AFTER this substep, or nullptr.
+// frame_off >= 0: the caller-order [E][N][3] cotangent dL/dx of the state AFTER this substep starts frame_off floats into
+// the frame array whose base is in md.frame_base[0]; < 0: none.
 __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
-                                                       const float4 *__restrict__ v4n, const float *__restrict__ frame_cot,
+                                                       const float4 *__restrict__ v4n, long long frame_off,
                                                        float4 *__restrict__ adjx, float4 *__restrict__ adjv, float4 *__restrict__ adjf) {
     const size_t total = (size_t)md.E * md.N;
     grid_dep_launch();
     grid_dep_wait();
     if (blockIdx.x == 0 && threadIdx.x < 3) md.tile_ctr[3 + threadIdx.x] = 0;  // the adjoint element kernel's tile queues
     const int lane = threadIdx.x & 31;
+    const float *frame_cot = frame_off >= 0 ? md.frame_base[0] + frame_off : nullptr;
     // block-uniform trip count: the contact-parameter gradients are reduced with full-warp shuffles
     for (size_t base = (size_t)blockIdx.x * blockDim.x; base < total; base += (size_t)gridDim.x * blockDim.x) {
         const size_t i = base + threadIdx.x;
@@ -819,14 +821,21 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
 }
 
 // adjoint of the substep whose start state is (x, v) and whose end velocity is v_next; cotangents live in
-// m->d_adjx / m->d_adjv (updated in place); frame_cot (caller order, may be null) is added to adj_x first.
-int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, const float *frame_cot, cudaStream_t st) {
+// m->d_adjx / m->d_adjv (updated in place); the frame cotangent at frame_off (caller order, < 0: none) is added to adj_x first.
+int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, cudaStream_t st) {
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
-             launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_cot, m->d_adjx, m->d_adjv, m->d_adjf));
+             launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0)
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
                  launch_pdl(m->pdl, k_elements_adj, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
+    return GS_OK;
+}
+
+__global__ void k_set_ptr(const float **slot, const float *p) { *slot = p; }
+int launch_set_frame_base(gs_model *m, const float *d_frames, cudaStream_t st) {
+    k_set_ptr<<<1, 1, 0, st>>>(m->dev.frame_base, d_frames);
+    GS_LAUNCH_CHECK("k_set_ptr");
     return GS_OK;
 }
 

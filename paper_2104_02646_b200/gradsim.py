@@ -22,6 +22,7 @@ GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda"
           "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12}
 GS_ELEM_PER_ENV, GS_MASS_PER_ENV, GS_CONTACT_PER_ENV = 1, 2, 4
 GS_PLAN_AUTO, GS_PLAN_STREAMING, GS_PLAN_RESIDENT = 0, 1, 2
+LOSS_KINDS = {"final_centroid": 0, "pos_mse_frames": 1, "centroid_traj": 2}
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -66,8 +67,8 @@ SIGNATURES = {
     "gs_check_finite": (_int, [_vp, _vp, C.POINTER(_int)]),
     "gs_loss_centroid": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
     "gs_loss_pos": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
-    "gs_host_scratch_bytes": (_sz, [_vp]),
-    "gs_rollout_loss_backward_host": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _int, C.POINTER(_int), C.POINTER(_vp), _vp, _sz, _vp]),
+    "gs_host_scratch_bytes": (_sz, [_vp, _vp, _int, _int]),
+    "gs_rollout_loss_backward_host": (_int, [_vp, _vp, _vp, _vp, _int, _int, _vp, _vp, _vp, _vp, _int, C.POINTER(_int), C.POINTER(_vp), _vp, _sz, _vp]),
     "gs_launch_count": (C.c_uint64, []),
     "gs_kernel_timing": (_int, [_vp, _int]),
     "gs_kernel_times": (_int, [_vp, _vp, _int, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]),
@@ -290,13 +291,18 @@ class Model:
     def tape(self, n_substeps, checkpoint_every=1):
         return Tape(self, n_substeps, checkpoint_every)
 
-    def rollout_loss_backward_host(self, tape, h_x0, h_v0, h_target, groups=()):
-        """bench.py's e2e leg: HOST (numpy / pinned torch CPU) in, HOST out, one C call.  The returned pinned tensors
-        are owned by the model and overwritten by the next call."""
+    def rollout_loss_backward_host(self, tape, h_x0, h_v0, h_target, groups=(), loss="final_centroid", frame_stride=1):
+        """bench.py's e2e leg: HOST (pinned torch CPU tensors) in, HOST out, ONE C call.  loss / frame_stride /
+        h_target as gs_rollout_loss_backward_host documents them.  The returned pinned tensors are owned by the model
+        and overwritten by the next call."""
         torch = _torch()
         L = lib()
-        if self._scratch is None:
-            self._scratch = _aligned_bytes(L.gs_host_scratch_bytes(self.h), self.device)
+        kind = LOSS_KINDS[loss]
+        need = L.gs_host_scratch_bytes(self.h, tape.h, kind, int(frame_stride))
+        if need == 0:
+            raise GradSimError(GS_EINVAL, "bad loss arguments")
+        if self._scratch is None or self._scratch.numel() < need:
+            self._scratch = _aligned_bytes(need, self.device)
         E, N = self.E, self.N
         gl = [GROUPS[g] for g in groups]
         key = tuple(gl)
@@ -313,8 +319,9 @@ class Model:
         gbuf = self._host_out[2]
         garr = (C.c_int * max(len(gl), 1))(*gl)
         gptr = (C.c_void_p * max(len(gl), 1))(*[b.data_ptr() for b in gbuf])
+        assert h_target.dtype == torch.float32 and h_target.is_contiguous() and not h_target.is_cuda
         _check(L.gs_rollout_loss_backward_host(
-            self.h, tape.h, C.c_void_p(h_x0.data_ptr()), C.c_void_p(h_v0.data_ptr()), C.c_void_p(h_target.data_ptr()),
+            self.h, tape.h, C.c_void_p(h_x0.data_ptr()), C.c_void_p(h_v0.data_ptr()), kind, int(frame_stride), C.c_void_p(h_target.data_ptr()),
             C.c_void_p(out["loss"].data_ptr()), C.c_void_p(out["adj_x0"].data_ptr()), C.c_void_p(out["adj_v0"].data_ptr()),
             len(gl), garr, gptr, _dp(self._scratch), self._scratch.numel(), _stream()))
         for g, b in zip(groups, gbuf):

@@ -81,10 +81,17 @@ def _check_contact_grads(got, ref, tag):
     in fp64 (warp shuffles of doubles + red.global.add.f64; fp64 shared-memory accumulators in the resident plan).  A
     regime no particle visited (all-zero oracle gradient, e.g. k_f without a sticking particle) is not compared."""
     assert rel_inf(got["g_gravity"], ref["g_gravity"]) <= TOL_GRAD, (tag, "gravity")
-    for k in ("ke", "kd", "kf", "mu_c"):
+    for q, k in enumerate(("ke", "kd", "kf", "mu_c")):
         b = ref["g_" + k]
         if np.abs(b).max() > 0:
-            assert rel_inf(got["g_" + k], b) <= TOL_CONTACT, (tag, k, rel_inf(got["g_" + k], b))
+            # A18: the norm of a per-environment scalar is the largest environment's |value|.  A total whose terms cancel
+            # by more than 100x (|total| < 1 % of sum |term|, measured by the oracle itself: contact_abs) is a near-zero
+            # entry in the sense of A18 -- every fp32 TERM carries ~1e-5 of rounding from the fp32 state, whatever the
+            # precision of the sum -- so its norm is 1 % of sum |term| (seen: config 2 small, mu_c, 8.8e-9 = 0.23 % of
+            # sum |term|, GPU off by 1e-5 of sum |term|)
+            den = max(np.abs(b).max(), 1e-2 * ref["contact_abs"][:, q].max())
+            err = np.abs(got["g_" + k] - b).max() / den
+            assert err <= TOL_CONTACT, (tag, k, err, rel_inf(got["g_" + k], b))
 
 
 @pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
@@ -461,36 +468,42 @@ def test_error_paths():
     assert m.check_finite() == 0
 
 
+@pytest.mark.parametrize("own_loss", [False, True])
 @pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
-def test_host_buffer_entry_point_matches_the_oracle(config):
-    """gs_rollout_loss_backward_host (the call bench.py's e2e number is timed through): host buffers in, rollout +
-    final-centroid loss + backward + gradient read-back in ONE C call.  Loss, dL/dx0, dL/dv0 and every requested
-    group against the oracle; requesting the groups in another order (the device staging buffer is reused from group to
-    group) and calling twice on the same model must give the same arrays."""
+def test_host_buffer_entry_point_matches_the_oracle(config, own_loss):
+    """gs_rollout_loss_backward_host (the call bench.py's e2e number is timed through): host buffers in, rollout + loss
+    + backward + gradient read-back in ONE C call -- with the final-centroid loss on every config, and with each config's
+    own loss (position MSE at frames for configs 2 and 4, centroid trajectory for config 3).  Loss, dL/dx0, dL/dv0 and
+    every requested group against the oracle; requesting the groups in another order (the device staging buffer is
+    reused from group to group) and calling twice on the same model must give the same arrays."""
     sc = copy.copy(scenes.make_scene(config, small=True))
-    sc.loss, sc.frame_stride = "final_centroid", sc.n_substeps
-    sc.target = scenes._final_centroid_target(sc.config, sc.x0)
+    if not own_loss:
+        sc.loss, sc.frame_stride = "final_centroid", sc.n_substeps
+        sc.target = scenes._final_centroid_target(sc.config, sc.x0)
+    elif sc.loss == "final_centroid":
+        pytest.skip("this config's own loss is the final-centroid loss")
     ref = orc.run_scene(sc)
     m = gs.Model(sc)
     tape = m.tape(sc.n_substeps, sc.checkpoint_every)
-    groups = _grad_groups(sc) + ["ke", "mu_c"]
-    hx0, hv0, htg = torch.as_tensor(sc.x0).pin_memory(), torch.as_tensor(sc.v0).pin_memory(), torch.as_tensor(sc.target).pin_memory()
-    res = {k: v.clone().numpy().astype(np.float64) for k, v in m.rollout_loss_backward_host(tape, hx0, hv0, htg, groups=groups).items()}
+    groups = _grad_groups(sc) + ["ke", "mu_c", "gravity"]
+    tgt = torch.as_tensor(np.ascontiguousarray(ref["target"], dtype=np.float32))
+    hx0, hv0, htg = torch.as_tensor(sc.x0).pin_memory(), torch.as_tensor(sc.v0).pin_memory(), tgt.pin_memory()
+    kw = dict(groups=groups, loss=sc.loss, frame_stride=sc.frame_stride)
+    res = {k: v.clone().numpy().astype(np.float64) for k, v in m.rollout_loss_backward_host(tape, hx0, hv0, htg, **kw).items()}
     assert rel_inf(res["loss"], ref["loss"]) <= 5e-3
     assert rel_inf(res["adj_x0"], ref["adj_x0"]) <= TOL_GRAD and rel_inf(res["adj_v0"], ref["adj_v0"]) <= TOL_GRAD
     for g in _grad_groups(sc):
         assert rel_inf(res["g_" + g], ref["g_" + g]) <= TOL_GRAD, g
-    for g in ("ke", "mu_c"):
-        if np.abs(ref["g_" + g]).max() > 0:
-            assert rel_inf(res["g_" + g], ref["g_" + g]) <= TOL_CONTACT, g
+    _check_contact_grads({**res, "g_kd": ref["g_kd"], "g_kf": ref["g_kf"]}, ref, config)
     # the same through the device-buffer calls: the two paths run the same kernels
     got = gpu_run_scene(sc, ref["target"], model=m)
     assert rel_inf(res["loss"], got["loss"]) <= 1e-5
     for k in ["adj_x0", "adj_v0"] + ["g_" + g for g in _grad_groups(sc)]:
         assert rel_inf(res[k], got[k]) <= 5e-4, k
-    # other group order, unpinned numpy inputs, second call on the same model and tape
-    rev = list(reversed(groups))
-    res2 = m.rollout_loss_backward_host(tape, torch.as_tensor(sc.x0.copy()), torch.as_tensor(sc.v0.copy()), torch.as_tensor(sc.target.copy()), groups=rev)
-    for g in groups:  # two runs differ by the summation order of the atomics only (hazard H6), amplified over the rollout
+    # other group order, unpinned inputs, second call on the same model and tape
+    kw["groups"] = list(reversed(groups))
+    res2 = m.rollout_loss_backward_host(tape, torch.as_tensor(sc.x0.copy()), torch.as_tensor(sc.v0.copy()), tgt.clone(), **kw)
+    for g in _grad_groups(sc) + ["gravity"]:  # two runs differ by the summation order of the atomics only (hazard H6)
         assert rel_inf(res2["g_" + g].numpy(), res["g_" + g]) <= 5e-4, g
+    _check_contact_grads({**{k: v.numpy().astype(np.float64) for k, v in res2.items()}, "g_kd": ref["g_kd"], "g_kf": ref["g_kf"]}, ref, config)
     assert rel_inf(res2["adj_x0"].numpy(), res["adj_x0"]) <= 5e-4
