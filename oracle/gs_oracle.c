@@ -23,6 +23,8 @@
  *                               "triangular structure ... computed explicitly")
  *   rollout, rollout_backward   PAPER.md:613 (reverse mode stores the input state of every step);
  *                               checkpoint + replay per BASELINE.json configs[2]
+ *   actuation inputs            PAPER.md:579 (per-tet alpha of (J - alpha)^2), 585-586 (per-edge alpha of sin(phi/2 + alpha)),
+ *                               777 (App. E: activations produced in time by a controller); SURVEY.md 8(f) NEXT-1
  * Readings A1..A20 are listed in DESIGN.md ("Readings of the paper").
  *
  * Pins (tests/test_oracle_pins.py): P1..P10 of DESIGN.md.  Unpinned: the CHOICE among
@@ -61,6 +63,17 @@ typedef struct {
     double *g_ke, *g_kd, *g_kf, *g_muc;           /* [E]  dL/d(contact parameters) per environment (Table 5: contact parameters are optimisable) */
     double *g_hinge_kb;                           /* [E][Mh]  dL/dk_b per hinge (Table 5: bending stiffness is optimisable) */
     double *g_gravity;                            /* [E][3]   dL/dg per environment (Table 5 column "g") */
+    /* actuation ("alpha is a per-element actuation value that allows the element to expand and contract";
+       585-586 "alpha is a per-edge actuation value that allows the mesh to flex inwards or outwards"): CURRENT values used by
+       orc_step / orc_step_adjoint, and their per-substep gradients.  Rollouts copy one frame of the schedule in before every
+       substep (piecewise-constant control, one frame per act_stride substeps: App. E, a controller evaluated
+       in time) and add the substep's gradient to that frame's slot. */
+    double *tet_act, *hinge_act;                  /* [E][M], [E][Mh]; zero = passive */
+    double *g_tet_act, *g_hinge_act;              /* [E][M], [E][Mh] dL/d(act) of the substeps since they were last cleared */
+    int act_frames, act_stride;                   /* schedule: frame f holds for substeps [f stride, (f+1) stride); 0 frames = none */
+    double *sched_tet, *sched_hinge;              /* [F][E][M], [F][E][Mh] (NULL = that kind is not actuated) */
+    double *g_sched_tet, *g_sched_hinge;          /* gradients of the schedule, same shapes */
+    double *g_hinge_theta0;                       /* [E][Mh] dL/d(rest angle) (Table 5 column "rest": the rest configuration of the bending springs) */
     double *g_con_abs;                            /* [E][4]   diagnostic only: sum of |term| behind g_ke, g_kd, g_kf, g_muc (how far each total cancels) */
 } orc_model;
 
@@ -136,6 +149,8 @@ void orc_destroy(orc_model *m) {
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
     free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb); free(m->g_ke); free(m->g_kd); free(m->g_kf); free(m->g_muc);
     free(m->g_gravity); free(m->g_con_abs);
+    free(m->tet_act); free(m->hinge_act); free(m->g_tet_act); free(m->g_hinge_act); free(m->sched_tet); free(m->sched_hinge);
+    free(m->g_sched_tet); free(m->g_sched_hinge); free(m->g_hinge_theta0);
     free(m);
 }
 
@@ -197,6 +212,8 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_hinge_kb = zeros_d((size_t)E * Mh);
     m->g_ke = zeros_d((size_t)E); m->g_kd = zeros_d((size_t)E); m->g_kf = zeros_d((size_t)E); m->g_muc = zeros_d((size_t)E);
     m->g_gravity = zeros_d((size_t)E * 3); m->g_con_abs = zeros_d((size_t)E * 4);
+    m->tet_act = zeros_d((size_t)E * M); m->hinge_act = zeros_d((size_t)E * Mh);
+    m->g_tet_act = zeros_d((size_t)E * M); m->g_hinge_act = zeros_d((size_t)E * Mh); m->g_hinge_theta0 = zeros_d((size_t)E * Mh);
 
     /* tets: D_m = [X1-X0, X2-X0, X3-X0] (columns), B = D_m^-1, V = det(D_m)/6  (V_e) */
     for (int e = 0; e < M; e++) {
@@ -273,6 +290,7 @@ int orc_set_params(orc_model *m, int group, const double *v) {
         return 0;
     }
     if (group == 12) { m->g[0] = v[0]; m->g[1] = v[1]; m->g[2] = v[2]; return 0; } /* gravity: one vector for all environments */
+    if (group == 13) { memcpy(m->hinge_theta0, v, sizeof(double) * m->Mh); return 0; } /* rest angles: one array for all environments */
     if (group < 0 || group > 6) return -1;
     memcpy(dst[group], v, sizeof(double) * n[group] * m->E);
     return 0;
@@ -286,7 +304,8 @@ int orc_get_grads(const orc_model *m, int group, double *out) {
         return 0;
     }
     if (group == 12) { memcpy(out, m->g_gravity, sizeof(double) * 3 * m->E); return 0; } /* [E][3] */
-    if (group == 13) { memcpy(out, m->g_con_abs, sizeof(double) * 4 * m->E); return 0; } /* [E][4] diagnostic */
+    if (group == 13) { memcpy(out, m->g_hinge_theta0, sizeof(double) * m->Mh * m->E); return 0; } /* [E][Mh] */
+    if (group == 100) { memcpy(out, m->g_con_abs, sizeof(double) * 4 * m->E); return 0; } /* [E][4] diagnostic */
     if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
     return 0;
@@ -299,6 +318,10 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
     memset(m->g_ke, 0, sizeof(double) * E); memset(m->g_kd, 0, sizeof(double) * E); memset(m->g_kf, 0, sizeof(double) * E); memset(m->g_muc, 0, sizeof(double) * E);
     memset(m->g_gravity, 0, sizeof(double) * E * 3); memset(m->g_con_abs, 0, sizeof(double) * E * 4);
+    memset(m->g_tet_act, 0, sizeof(double) * E * m->M); memset(m->g_hinge_act, 0, sizeof(double) * E * m->Mh);
+    memset(m->g_hinge_theta0, 0, sizeof(double) * E * m->Mh);
+    if (m->g_sched_tet) memset(m->g_sched_tet, 0, sizeof(double) * m->act_frames * E * m->M);
+    if (m->g_sched_hinge) memset(m->g_sched_hinge, 0, sizeof(double) * m->act_frames * E * m->Mh);
 }
 
 /* ---------------------------------------------------------------- tets */
@@ -308,19 +331,19 @@ static void tet_kin(const double *x[4], const double *B, double *F) {
     for (int k = 0; k < 3; k++) { v_sub(x[k + 1], x[0], c); m_setcol(Ds, k, c); }
     m_mul(Ds, B, F);
 }
-static double tet_energy(const double *x[4], const double *B, double V, double mu, double lam) {
+static double tet_energy(const double *x[4], const double *B, double V, double mu, double lam, double act) {
     double F[9]; tet_kin(x, B, F);
-    double Ic = m_ddot(F, F), J = m_det(F), alpha = 1.0 + 0.75 * mu / lam;
+    double Ic = m_ddot(F, F), J = m_det(F), alpha = 1.0 + 0.75 * mu / lam + act; /* A1: passive alpha + actuation */
     return V * (0.5 * mu * (Ic - 3.0) + 0.5 * lam * (J - alpha) * (J - alpha) - 0.5 * mu * log(Ic + 1.0));
 }
 /* first Piola-Kirchhoff stress P = dPsi/dF + damping stress k F sym(F^T Fdot) (A3); also returns the
    three parameter directions Pmu, Plam, Pk with P = mu Pmu + lam Plam + k Pk */
-static void tet_stress(const double *F, const double *Fd, double mu, double lam, double kd, double *P, double *Pmu, double *Plam, double *Pk) {
+static void tet_stress(const double *F, const double *Fd, double mu, double lam, double kd, double act, double *P, double *Pmu, double *Plam, double *Pk) {
     double C[9], S[9], T[9], pm[9], pl[9], pk[9];
     double Ic = m_ddot(F, F), J = m_det(F);
     m_cof(F, C);
     double s1 = 1.0 - 1.0 / (Ic + 1.0);
-    for (int i = 0; i < 9; i++) { pm[i] = s1 * F[i] - 0.75 * C[i]; pl[i] = (J - 1.0) * C[i]; }
+    for (int i = 0; i < 9; i++) { pm[i] = s1 * F[i] - 0.75 * C[i]; pl[i] = (J - 1.0 - act) * C[i]; } /* lambda (J - alpha) cof F, alpha = 1 + 3mu/(4 lambda) + act */
     m_mul_tn(F, Fd, T); m_sym(T, S); m_mul(F, S, pk);
     for (int i = 0; i < 9; i++) P[i] = mu * pm[i] + lam * pl[i] + kd * pk[i];
     if (Pmu) memcpy(Pmu, pm, sizeof pm);
@@ -328,10 +351,10 @@ static void tet_stress(const double *F, const double *Fd, double mu, double lam,
     if (Pk) memcpy(Pk, pk, sizeof pk);
 }
 /* nodal forces: H = -V P B^T, f_{1..3} = columns of H, f_0 = -(sum) */
-static void tet_force(const double *x[4], const double *v[4], const double *B, double V, double mu, double lam, double kd, double f[4][3]) {
+static void tet_force(const double *x[4], const double *v[4], const double *B, double V, double mu, double lam, double kd, double act, double f[4][3]) {
     double F[9], Fd[9], P[9], H[9];
     tet_kin(x, B, F); tet_kin(v, B, Fd);
-    tet_stress(F, Fd, mu, lam, kd, P, NULL, NULL, NULL);
+    tet_stress(F, Fd, mu, lam, kd, act, P, NULL, NULL, NULL);
     m_mul_nt(P, B, H);
     f[0][0] = f[0][1] = f[0][2] = 0;
     for (int k = 0; k < 3; k++) {
@@ -341,20 +364,21 @@ static void tet_force(const double *x[4], const double *v[4], const double *B, d
     }
 }
 /* VJP: given a_k = dL/df_k, add to ax_k = dL/dx_k, av_k = dL/dv_k, and parameter gradients */
-static void tet_adjoint(const double *x[4], const double *v[4], const double *a[4], const double *B, double V, double mu, double lam, double kd,
-                        double ax[4][3], double av[4][3], double *gmu, double *glam, double *gk) {
+static void tet_adjoint(const double *x[4], const double *v[4], const double *a[4], const double *B, double V, double mu, double lam, double kd, double act,
+                        double ax[4][3], double av[4][3], double *gmu, double *glam, double *gk, double *gact) {
     double F[9], Fd[9], P[9], Pmu[9], Plam[9], Pk[9], G[9], A[9], c[3];
     tet_kin(x, B, F); tet_kin(v, B, Fd);
-    tet_stress(F, Fd, mu, lam, kd, P, Pmu, Plam, Pk);
+    tet_stress(F, Fd, mu, lam, kd, act, P, Pmu, Plam, Pk);
     for (int k = 0; k < 3; k++) { v_sub(a[k + 1], a[0], c); m_setcol(G, k, c); }
     m_mul(G, B, A);
     for (int i = 0; i < 9; i++) A[i] *= -V; /* A = adj_P = -V G B */
     *gmu += m_ddot(Pmu, A); *glam += m_ddot(Plam, A); *gk += m_ddot(Pk, A);
     /* adj_F = (dP/dF)^T[A]; the elastic Hessian is symmetric */
     double C[9], D[9], aF[9], aFd[9], S[9], Nn[9], T[9], T2[9];
-    double Ic = m_ddot(F, F), J = m_det(F), alpha = 1.0 + 0.75 * mu / lam;
+    double Ic = m_ddot(F, F), J = m_det(F), alpha = 1.0 + 0.75 * mu / lam + act;
     m_cof(F, C); m_dcof(F, A, D);
     double s1 = 1.0 - 1.0 / (Ic + 1.0), FA = m_ddot(F, A), CA = m_ddot(C, A);
+    *gact += -lam * CA; /* dP/d(act) = -lambda cof F */
     for (int i = 0; i < 9; i++)
         aF[i] = mu * s1 * A[i] + 2.0 * mu * FA / ((Ic + 1.0) * (Ic + 1.0)) * F[i] + lam * CA * C[i] + lam * (J - alpha) * D[i];
     /* damping P_d = k F S, S = sym(F^T Fd): adj_F += k (A S + Fd N), adj_Fd = k F N, N = sym(F^T A) */
@@ -470,19 +494,22 @@ static void tri_adjoint(const double *x[3], const double *v[3], const double *a[
 
 /* ---------------------------------------------------------------- hinges (A5, A6) */
 /* E_b = 2 k_b l0 (1 - cos((theta - theta0)/2)),  f_i = k_b l0 sin((theta - theta0)/2) d_i */
-static double hinge_energy(const double *x[4], double theta0, double l0, double kb) {
+static double hinge_energy(const double *x[4], double theta0, double l0, double kb, double act) {
     double th = hinge_angle(x[0], x[1], x[2], x[3], NULL);
-    return 2.0 * kb * l0 * (1.0 - cos(0.5 * (th - theta0)));
+    return 2.0 * kb * l0 * (1.0 - cos(0.5 * (th - theta0) + act));
 }
-static void hinge_force(const double *x[4], double theta0, double l0, double kb, double f[4][3]) {
+/* f_i = k_b l0 sin(phi/2 + alpha) d_i, phi = theta - theta0, alpha = the per-edge actuation */
+static void hinge_force(const double *x[4], double theta0, double l0, double kb, double act, double f[4][3]) {
     double d[4][3];
     double th = hinge_angle(x[0], x[1], x[2], x[3], d);
-    double s = kb * l0 * sin(0.5 * (th - theta0));
+    double s = kb * l0 * sin(0.5 * (th - theta0) + act);
     for (int k = 0; k < 4; k++) v_scale(s, d[k], f[k]);
 }
 /* VJP = JVP (conservative force, symmetric Jacobian): adj_x_j += -E'' s d_j + E' Dd_j[a], s = sum d_i.a_i */
 /* f_i = k_b l0 sin(ph) d_i is linear in k_b: dL/dk_b += l0 sin(ph) sum_i d_i . a_i */
-static void hinge_adjoint(const double *x[4], const double *a[4], double theta0, double l0, double kb, double ax[4][3], double *g_kb) {
+/* dL/d(alpha) += k_b l0 cos(ph) sum_i d_i . a_i; the rest angle enters as -theta0/2 in the same argument: dL/d(theta0) = -1/2 of that */
+static void hinge_adjoint(const double *x[4], const double *a[4], double theta0, double l0, double kb, double act, double ax[4][3], double *g_kb,
+                          double *g_act, double *g_theta0) {
     const double *x1 = x[0], *x2 = x[1], *x3 = x[2], *x4 = x[3];
     double p13[3], p14[3], p23[3], p24[3], n1[3], n2[3], e[3], eh[3];
     v_sub(x1, x3, p13); v_sub(x1, x4, p14); v_sub(x2, x3, p23); v_sub(x2, x4, p24);
@@ -518,10 +545,12 @@ static void hinge_adjoint(const double *x[4], const double *a[4], double theta0,
     }
     double s = 0;
     for (int k = 0; k < 4; k++) s += v_dot(d[k], a[k]);
-    double ph = 0.5 * (th - theta0);
+    double ph = 0.5 * (th - theta0) + act;
     double E1 = kb * l0 * sin(ph), E2 = 0.5 * kb * l0 * cos(ph);
     for (int k = 0; k < 4; k++) for (int r = 0; r < 3; r++) ax[k][r] += -E2 * s * d[k][r] + E1 * dd[k][r];
     if (g_kb) *g_kb += l0 * sin(ph) * s;
+    if (g_act) *g_act += 2.0 * E2 * s;
+    if (g_theta0) *g_theta0 += -E2 * s;
 }
 
 /* ---------------------------------------------------------------- contact (A7, A8) */
@@ -581,7 +610,7 @@ static void env_forces(const orc_model *m, int env, const double *x, const doubl
             const double *xe[4], *ve[4];
             for (int k = 0; k < 4; k++) { xe[k] = x + 3 * t[k]; ve[k] = v + 3 * t[k]; }
             double fe[4][3];
-            tet_force(xe, ve, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[(size_t)env * M + e], m->tet_lambda[(size_t)env * M + e], m->tet_damp[(size_t)env * M + e], fe);
+            tet_force(xe, ve, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[(size_t)env * M + e], m->tet_lambda[(size_t)env * M + e], m->tet_damp[(size_t)env * M + e], m->tet_act[(size_t)env * M + e], fe);
             memcpy(slots + 3 * (4 * (size_t)e), fe, sizeof fe);
         }
     }
@@ -603,7 +632,7 @@ static void env_forces(const orc_model *m, int env, const double *x, const doubl
             const double *xe[4];
             for (int k = 0; k < 4; k++) xe[k] = x + 3 * h[k];
             double fe[4][3];
-            hinge_force(xe, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], fe);
+            hinge_force(xe, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], m->hinge_act[(size_t)env * Mh + e], fe);
             memcpy(slots + 3 * (4 * (size_t)M + 3 * (size_t)Mt + 4 * (size_t)e), fe, sizeof fe);
         }
     }
@@ -640,7 +669,7 @@ void orc_energy(const orc_model *m, const double *x, int mask, double *U) {
         if (mask & ORC_TETS) for (int e = 0; e < m->M; e++) {
             const int *t = m->tets + 4 * e; const double *xe[4];
             for (int k = 0; k < 4; k++) xe[k] = xe_ + 3 * t[k];
-            u += tet_energy(xe, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[(size_t)env * m->M + e], m->tet_lambda[(size_t)env * m->M + e]);
+            u += tet_energy(xe, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[(size_t)env * m->M + e], m->tet_lambda[(size_t)env * m->M + e], m->tet_act[(size_t)env * m->M + e]);
         }
         if (mask & ORC_TRIS) for (int e = 0; e < m->Mt; e++) {
             const int *t = m->tris + 3 * e; const double *xe[3];
@@ -650,7 +679,7 @@ void orc_energy(const orc_model *m, const double *x, int mask, double *U) {
         if (mask & ORC_HINGES) for (int e = 0; e < m->Mh; e++) {
             const int *h = m->hinges + 4 * e; const double *xe[4];
             for (int k = 0; k < 4; k++) xe[k] = xe_ + 3 * h[k];
-            u += hinge_energy(xe, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e]);
+            u += hinge_energy(xe, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], m->hinge_act[(size_t)env * m->Mh + e]);
         }
         U[env] = u;
     }
@@ -726,8 +755,8 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         for (int k = 0; k < 4; k++) { xe[k] = x + 3 * t[k]; ve[k] = v + 3 * t[k]; ae[k] = af + 3 * t[k]; }
         double cx[4][3] = {{0}}, cv[4][3] = {{0}};
         size_t pe = (size_t)env * M + e;
-        tet_adjoint(xe, ve, ae, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[pe], m->tet_lambda[pe], m->tet_damp[pe], cx, cv,
-                    &m->g_tet_mu[pe], &m->g_tet_lambda[pe], &m->g_tet_damp[pe]);
+        tet_adjoint(xe, ve, ae, m->tet_B + 9 * e, m->tet_V[e], m->tet_mu[pe], m->tet_lambda[pe], m->tet_damp[pe], m->tet_act[pe], cx, cv,
+                    &m->g_tet_mu[pe], &m->g_tet_lambda[pe], &m->g_tet_damp[pe], &m->g_tet_act[pe]);
         memcpy(slots + 3 * (4 * (size_t)e), cx, sizeof cx);
         memcpy(slots_v + 3 * (4 * (size_t)e), cv, sizeof cv);
     }
@@ -749,7 +778,8 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         const double *xe[4], *ae[4];
         for (int k = 0; k < 4; k++) { xe[k] = x + 3 * h[k]; ae[k] = af + 3 * h[k]; }
         double cx[4][3] = {{0}};
-        hinge_adjoint(xe, ae, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], cx, &m->g_hinge_kb[(size_t)env * Mh + e]);
+        size_t pe = (size_t)env * Mh + e;
+        hinge_adjoint(xe, ae, m->hinge_theta0[e], m->hinge_l0[e], m->hinge_kb[e], m->hinge_act[pe], cx, &m->g_hinge_kb[pe], &m->g_hinge_act[pe], &m->g_hinge_theta0[pe]);
         memcpy(slots + 3 * (4 * (size_t)M + 3 * (size_t)Mt + 4 * (size_t)e), cx, sizeof cx);
     }
 #pragma omp parallel for if (par) schedule(static)
@@ -771,12 +801,55 @@ void orc_step_adjoint(orc_model *m, const double *x, const double *v, const doub
     }
 }
 
+/* ---------------------------------------------------------------- actuation inputs */
+/* CURRENT activation of every tet / hinge, [E][M] / [E][Mh]; NULL leaves that kind as it is.  Used by orc_step,
+   orc_step_adjoint, orc_forces, orc_energy. */
+void orc_set_act_current(orc_model *m, const double *tet_act, const double *hinge_act) {
+    if (tet_act) memcpy(m->tet_act, tet_act, sizeof(double) * m->E * m->M);
+    if (hinge_act) memcpy(m->hinge_act, hinge_act, sizeof(double) * m->E * m->Mh);
+}
+/* dL/d(current activation) accumulated by the adjoint substeps since the last orc_zero_grads */
+void orc_get_act_grads_current(const orc_model *m, double *g_tet, double *g_hinge) {
+    if (g_tet) memcpy(g_tet, m->g_tet_act, sizeof(double) * m->E * m->M);
+    if (g_hinge) memcpy(g_hinge, m->g_hinge_act, sizeof(double) * m->E * m->Mh);
+}
+/* Activation SCHEDULE of rollouts: n_frames frames, frame f holds during substeps [f stride, (f+1) stride) (the last
+   frame holds to the end).  tet [F][E][M], hinge [F][E][Mh], either may be NULL; n_frames = 0 removes the schedule. */
+void orc_set_act_schedule(orc_model *m, int n_frames, int stride, const double *tet, const double *hinge) {
+    free(m->sched_tet); free(m->sched_hinge); free(m->g_sched_tet); free(m->g_sched_hinge);
+    m->sched_tet = m->sched_hinge = m->g_sched_tet = m->g_sched_hinge = NULL;
+    m->act_frames = n_frames; m->act_stride = stride > 0 ? stride : 1;
+    if (n_frames <= 0) { m->act_frames = 0; return; }
+    if (tet) { m->sched_tet = dup_d(tet, (size_t)n_frames * m->E * m->M); m->g_sched_tet = zeros_d((size_t)n_frames * m->E * m->M); }
+    if (hinge) { m->sched_hinge = dup_d(hinge, (size_t)n_frames * m->E * m->Mh); m->g_sched_hinge = zeros_d((size_t)n_frames * m->E * m->Mh); }
+}
+void orc_get_act_schedule_grads(const orc_model *m, double *g_tet, double *g_hinge) {
+    if (g_tet && m->g_sched_tet) memcpy(g_tet, m->g_sched_tet, sizeof(double) * m->act_frames * m->E * m->M);
+    if (g_hinge && m->g_sched_hinge) memcpy(g_hinge, m->g_sched_hinge, sizeof(double) * m->act_frames * m->E * m->Mh);
+}
+static int act_frame_of(const orc_model *m, int t) { int f = t / m->act_stride; return f < m->act_frames ? f : m->act_frames - 1; }
+/* the activation of substep t becomes current */
+static void act_load(orc_model *m, int t) {
+    if (m->act_frames <= 0) return;
+    int f = act_frame_of(m, t);
+    if (m->sched_tet) memcpy(m->tet_act, m->sched_tet + (size_t)f * m->E * m->M, sizeof(double) * m->E * m->M);
+    if (m->sched_hinge) memcpy(m->hinge_act, m->sched_hinge + (size_t)f * m->E * m->Mh, sizeof(double) * m->E * m->Mh);
+}
+/* the gradient the adjoint of substep t just added to the current accumulators moves to the schedule's frame */
+static void act_collect(orc_model *m, int t) {
+    if (m->act_frames <= 0) return;
+    int f = act_frame_of(m, t);
+    size_t nt = (size_t)m->E * m->M, nh = (size_t)m->E * m->Mh;
+    if (m->g_sched_tet) for (size_t i = 0; i < nt; i++) { m->g_sched_tet[f * nt + i] += m->g_tet_act[i]; m->g_tet_act[i] = 0; }
+    if (m->g_sched_hinge) for (size_t i = 0; i < nh; i++) { m->g_sched_hinge[f * nh + i] += m->g_hinge_act[i]; m->g_hinge_act[i] = 0; }
+}
+
 /* ---------------------------------------------------------------- rollout + tape */
 /* Forward T substeps from (x0, v0) [E][N][3].  Checkpoints: state after t substeps for t = 0, K, 2K, ... < T
    go to ck_x, ck_v [n_ck][E][N][3], n_ck = ceil(T/K)  (K = 1: the full tape).  States after rec_t[j]
    substeps (sorted ascending, 0 <= rec_t <= T) are copied to rec_x, rec_v [n_rec][E][N][3] (either may
    be NULL).  Final state to xT, vT (may be NULL). */
-void orc_rollout(const orc_model *m, int T, int K, const double *x0, const double *v0, double *ck_x, double *ck_v,
+void orc_rollout(orc_model *m, int T, int K, const double *x0, const double *v0, double *ck_x, double *ck_v,
                  int n_rec, const int *rec_t, double *rec_x, double *rec_v, double *xT, double *vT) {
     const size_t S = (size_t)m->N * 3, ES = S * m->E;
     double *xa = dup_d(x0, ES), *va = dup_d(v0, ES), *xb = zeros_d(ES), *vb = zeros_d(ES);
@@ -789,6 +862,7 @@ void orc_rollout(const orc_model *m, int T, int K, const double *x0, const doubl
             jr++;
         }
         if (t == T) break;
+        act_load(m, t);
         orc_step(m, xa, va, xb, vb);
         double *tmp = xa; xa = xb; xb = tmp; tmp = va; va = vb; vb = tmp;
     }
@@ -813,15 +887,19 @@ void orc_rollout_backward(orc_model *m, int T, int K, const double *ck_x, const 
         int t0 = c * K, t1 = t0 + K < T ? t0 + K : T;
         memcpy(seg_x, ck_x + (size_t)c * ES, sizeof(double) * ES);
         memcpy(seg_v, ck_v + (size_t)c * ES, sizeof(double) * ES);
-        for (int t = t0; t + 1 < t1; t++) /* replay: state t+1 from state t */
+        for (int t = t0; t + 1 < t1; t++) { /* replay: state t+1 from state t */
+            act_load(m, t);
             orc_step(m, seg_x + (size_t)(t - t0) * ES, seg_v + (size_t)(t - t0) * ES, seg_x + (size_t)(t + 1 - t0) * ES, seg_v + (size_t)(t + 1 - t0) * ES);
+        }
         for (int t = t1 - 1; t >= t0; t--) {
             while (jl >= 0 && loss_t[jl] == t + 1) { /* inject dL/dx_{t+1} */
                 const double *la = loss_ax + (size_t)jl * ES;
                 for (size_t i = 0; i < ES; i++) bx[i] += la[i];
                 jl--;
             }
+            act_load(m, t);
             orc_step_adjoint(m, seg_x + (size_t)(t - t0) * ES, seg_v + (size_t)(t - t0) * ES, bx, bv, ax, av);
+            act_collect(m, t);
             double *tmp = bx; bx = ax; ax = tmp; tmp = bv; bv = av; av = tmp;
         }
     }

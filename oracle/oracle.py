@@ -24,7 +24,7 @@ _LIB = os.path.join(_HERE, "libgs_oracle.so")
 
 TETS, TRIS, HINGES, CONTACT, ALL = 1, 2, 4, 8, 15
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13}
 
 
 def build(force: bool = False) -> str:
@@ -132,12 +132,12 @@ class Oracle:
 
     # ---- parameters / gradients
     def set_params(self, group, values):
-        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3}.get(GROUPS[group], 1)
+        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3, 13: self.Mh}.get(GROUPS[group], 1)
         a = _d(np.broadcast_to(_d(values).reshape(-1, n), (self.E, n)))
         assert lib().orc_set_params(self.h, C.c_int(GROUPS[group]), _p(a)) == 0
 
     def grads(self, group):
-        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3}.get(GROUPS[group], 1)
+        n = {0: self.M, 1: self.M, 2: self.M, 3: self.Mt, 4: self.Mt, 5: self.Mt, 6: self.N, 7: self.Mh, 12: 3, 13: self.Mh}.get(GROUPS[group], 1)
         out = np.zeros((self.E, n))
         assert lib().orc_get_grads(self.h, C.c_int(GROUPS[group]), _p(out)) == 0
         return out
@@ -145,8 +145,37 @@ class Oracle:
     def contact_abs_sums(self):
         """[E, 4] diagnostic: sum of |term| behind the totals dL/d(k_e, k_d, k_f, mu_c) -- how far each total cancels."""
         out = np.zeros((self.E, 4))
-        assert lib().orc_get_grads(self.h, C.c_int(13), _p(out)) == 0
+        assert lib().orc_get_grads(self.h, C.c_int(100), _p(out)) == 0
         return out
+
+    # ---- actuation (PAPER.md:579, 585-586): current values for single substeps, schedules for rollouts
+    def set_act_current(self, tet_act=None, hinge_act=None):
+        t = None if tet_act is None else _d(np.broadcast_to(_d(tet_act).reshape(-1, self.M), (self.E, self.M)))
+        h = None if hinge_act is None else _d(np.broadcast_to(_d(hinge_act).reshape(-1, self.Mh), (self.E, self.Mh)))
+        lib().orc_set_act_current(self.h, _p(t), _p(h))
+
+    def act_grads_current(self):
+        gt, gh = np.zeros((self.E, self.M)), np.zeros((self.E, self.Mh))
+        lib().orc_get_act_grads_current(self.h, _p(gt), _p(gh))
+        return gt, gh
+
+    def set_act_schedule(self, stride, tet=None, hinge=None):
+        """tet [F, E, M], hinge [F, E, Mh] (either None): frame f holds during substeps [f stride, (f+1) stride)."""
+        F = 0
+        t = h = None
+        if tet is not None:
+            t = _d(tet); F = t.shape[0]; assert t.shape == (F, self.E, self.M)
+        if hinge is not None:
+            h = _d(hinge); assert F in (0, h.shape[0]); F = h.shape[0]; assert h.shape == (F, self.E, self.Mh)
+        self._sched = (F, t is not None, h is not None)
+        lib().orc_set_act_schedule(self.h, C.c_int(F), C.c_int(int(stride)), _p(t), _p(h))
+
+    def act_schedule_grads(self):
+        F, ht, hh = getattr(self, "_sched", (0, False, False))
+        gt = np.zeros((F, self.E, self.M)) if ht else None
+        gh = np.zeros((F, self.E, self.Mh)) if hh else None
+        lib().orc_get_act_schedule_grads(self.h, _p(gt), _p(gh))
+        return gt, gh
 
     def zero_grads(self):
         lib().orc_zero_grads(self.h)
@@ -253,6 +282,9 @@ def run_scene(sc, target=None, K=None):
     o = Oracle(sc)
     if target is None:
         target = truth_targets(sc)
+    act = getattr(sc, "act", None)  # optional actuation schedule: dict(stride=, tet=[F,E,M] or None, hinge=[F,E,Mh] or None)
+    if act:
+        o.set_act_schedule(act["stride"], act.get("tet"), act.get("hinge"))
     K = sc.checkpoint_every if K is None else K
     lt = sc.loss_times()
     ro = o.rollout(sc.x0, sc.v0, sc.n_substeps, K=K, rec_times=lt)
@@ -262,4 +294,6 @@ def run_scene(sc, target=None, K=None):
     for g in GROUPS:
         out["g_" + g] = o.grads(g)
     out["contact_abs"] = o.contact_abs_sums()
+    if act:
+        out["g_act_tet"], out["g_act_hinge"] = o.act_schedule_grads()
     return out

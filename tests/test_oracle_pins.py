@@ -62,12 +62,15 @@ def _mixed_scene(rng, **kw):
 
 
 SCALAR_GROUPS = ("ke", "kd", "kf", "mu_c")  # one value per environment
+ABS_STEP = ("gravity", "hinge_theta0")       # parameters whose value may be 0: absolute FD steps
 
 
 def _param(sc, o, g):
     """(analytic gradient, base value) of parameter group g as flat fp64 arrays of equal shape."""
     if g == "gravity":  # one vector shared by all environments; the oracle keeps dL/dg per environment
         return o.grads(g).sum(0).copy(), np.asarray(sc.gravity, np.float64)
+    if g == "hinge_theta0":  # rest angles (derived from x_rest; one array shared by all environments)
+        return o.grads(g).sum(0).copy(), o.rest()["theta0"].copy()
     scalar = g in SCALAR_GROUPS
     an = (o.grads(g)[:, 0] if scalar else o.grads(g)[0]).copy()
     base = getattr(sc, g).astype(np.float64)
@@ -349,7 +352,7 @@ def test_p7_step_param_gradients_vs_fd(group):
         # one substep is piecewise LINEAR in the contact parameters (within a friction regime), so their central
         # difference is exact for any step that keeps the regimes; a larger step keeps round-off out of the tiny
         # stick-friction terms
-        h = (1e-3 if scalar else 1e-6) * (base[e] if group != "gravity" else 1.0)
+        h = (1e-3 if scalar else 1e-6) * (base[e] if group not in ABS_STEP else 1.0)
         vals = []
         for s in (+1, -1):
             p = base.copy(); p[e] += s * h
@@ -601,7 +604,7 @@ def test_p8_smooth_regime_strict():
             if g == "mass" and sc.pinned[e]:
                 assert an[e] == 0
                 continue
-            h = 1e-5 * (base[e] if g != "gravity" else 1.0)
+            h = 1e-5 * (base[e] if g not in ABS_STEP else 1.0)
             vals = []
             for sgn in (+1, -1):
                 p = base.copy(); p[e] += sgn * h
@@ -674,3 +677,131 @@ def test_openmp_thread_count_does_not_change_results():
         setattr(sc1, k, getattr(sc, k)[2:3])
     b = orc.Oracle(sc1).rollout(sc1.x0, sc1.v0, 20)["xT"]
     assert np.array_equal(a[2], b[0])  # env-parallel run == the same env alone (element-parallel run)
+
+
+# ---------------------------------------------------------------- actuation
+def test_actuation_closed_forms_tet_and_hinge():
+    """alpha of (J - alpha)^2 is "a per-element actuation value that allows the element to expand and
+    contract".  With reading A1, alpha = 1 + 3mu/(4 lambda) + act, at the rest shape F = I: P = -lambda act I, so the corner
+    tet with legs a (B = I/a, V = a^3/6) gets H = -V P B^T = (a^2 lambda act / 6) I -- outward for act > 0 -- and the
+    uniformly scaled shape x = s X is force-free where mu (1 - 1/(3s^2+1)) s + (lambda (s^3 - 1 - act) - 3mu/4) s^2 = 0.
+    PAPER.md:585-586: f_b = k_b sin(phi/2 + alpha) d: on the symmetric fold of test_hinge_force_closed_form the wing force is
+    k_b L |sin(theta/2 + alpha)| / h and vanishes at theta = -2 alpha ("flex inwards or outwards")."""
+    a, mu, lam = 0.25, 1.25e4, 2.0e4
+    X = np.array([[0, 0, 0], [a, 0, 0], [0, a, 0], [0, 0, a]], dtype=np.float64)
+    o = orc.Oracle(_free(scenes.custom_scene(X, tets=[[0, 1, 2, 3]], mu=mu, lam=lam, damp=0.0)))
+    for act in (0.125, -0.0625):
+        o.set_act_current(tet_act=[act])
+        f = o.forces(X, mask=orc.TETS)[0]
+        c = a * a * lam * act / 6
+        assert np.abs(f - np.vstack([np.full(3, -c), c * np.eye(3)])).max() <= 1e-12 * abs(c)
+        lo, hi = 0.5, 2.0  # root of the rest-stability polynomial by bisection
+        p = lambda s: mu * (1 - 1 / (3 * s * s + 1)) * s + (lam * (s ** 3 - 1 - act) - 0.75 * mu) * s * s
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            lo, hi = (mid, hi) if p(lo) * p(mid) > 0 else (lo, mid)
+        s_eq = 0.5 * (lo + hi)
+        assert (s_eq > 1) == (act > 0)
+        assert np.abs(o.forces(s_eq * X, mask=orc.TETS)[0]).max() <= 1e-9 * abs(c)
+    L, h, kb = 0.5, 0.25, 7.0
+    rest = np.array([[h, 0.0, L / 2], [-h, 0.0, L / 2], [0.0, 0.0, 0.0], [0.0, 0.0, L]])
+    oh = orc.Oracle(_free(scenes.custom_scene(rest, tris=[[2, 3, 0], [3, 2, 1]], hinges=[[0, 1, 2, 3]], kb=kb)))
+    # rotating wing 2 by +fold about the edge (as in the test above) is a signed dihedral theta = -fold (A13 orientation)
+    for alpha, fold in ((0.2, 0.3), (-0.15, 0.0), (0.1, 0.2)):
+        oh.set_act_current(hinge_act=[alpha])
+        x = rest.copy()
+        x[1] = [-h * np.cos(fold), h * np.sin(fold), L / 2]
+        f = oh.forces(x, mask=orc.HINGES)[0]
+        mag = kb * L * abs(np.sin(-fold / 2 + alpha)) / h
+        assert abs(np.linalg.norm(f[0]) - mag) <= 1e-12 * max(mag, 1.0) and abs(np.linalg.norm(f[1]) - mag) <= 1e-12 * max(mag, 1.0)
+    assert np.abs(f).max() <= 1e-12  # the last case sits at theta = -2 alpha: the actuated rest angle
+
+
+def test_actuation_forces_are_energy_gradients_and_conserve_momentum():
+    """With random activations on every tet and hinge: f = -grad U still holds (P3; U carries act / alpha as in the
+    oracle's header), internal forces still have zero net force and torque (P4)."""
+    rng = np.random.default_rng(21)
+    sc = _free(_mixed_scene(rng, damp=0.0, tri_damp=0.0))
+    o = orc.Oracle(sc)
+    o.set_act_current(tet_act=rng.uniform(-0.1, 0.1, sc.tets.shape[0]), hinge_act=rng.uniform(-0.3, 0.3, sc.hinges.shape[0]))
+    N = sc.n_particles
+    x = sc.x_rest.astype(np.float64) + 0.01 * rng.uniform(-1, 1, (N, 3))
+    mask = orc.TETS | orc.HINGES
+    f = o.forces(x, mask=mask)[0]
+    eps, g = 1e-6, np.zeros((N, 3))
+    for i in range(N):
+        for r in range(3):
+            d = np.zeros((N, 3)); d[i, r] = eps
+            g[i, r] = -(o.energy(x + d, mask=mask)[0] - o.energy(x - d, mask=mask)[0]) / (2 * eps)
+    assert np.abs(f - g).max() <= 1e-7 * np.abs(f).max()
+    assert np.abs(f.sum(0)).max() <= 1e-10 * np.abs(f).max()
+    assert np.abs(np.cross(x, f).sum(0)).max() <= 1e-10 * np.abs(f).max()
+
+
+def test_actuation_gradients_vs_fd_step_and_rollout():
+    """dL/d(act) per tet and per hinge: one substep against central FD (exact structure: P7), then a scheduled rollout
+    (frames of 8 substeps, airborne so that FD is valid at one fixed step: P8 strict), then the checkpointed backward
+    must reproduce the full-tape gradients bit for bit (P9) -- the replay has to reload each substep's frame."""
+    rng = np.random.default_rng(22)
+    sc = _mixed_scene(rng, n_substeps=40)
+    sc.plane_d = -1e6
+    o = orc.Oracle(sc)
+    M, Mh, N = sc.tets.shape[0], sc.hinges.shape[0], sc.n_particles
+    x = sc.x_rest.astype(np.float64)[None] + 0.004 * rng.uniform(-1, 1, (1, N, 3))
+    v = 0.3 * rng.normal(size=x.shape)
+    ta, ha = rng.uniform(-0.05, 0.05, (1, M)), rng.uniform(-0.2, 0.2, (1, Mh))
+    bx, bv = rng.normal(size=(N, 3)), rng.normal(size=(N, 3))
+    o.set_act_current(ta, ha)
+    o.zero_grads()
+    o.step_adjoint(x, v, bx, bv)
+    gt, gh = o.act_grads_current()
+
+    def phi():
+        xo, vo = o.step(x, v)
+        return (xo[0] * bx).sum() + (vo[0] * bv).sum()
+
+    for arr, g, setter in ((ta, gt, lambda a: o.set_act_current(tet_act=a)), (ha, gh, lambda a: o.set_act_current(hinge_act=a))):
+        assert np.abs(g).max() > 0
+        for e in range(arr.shape[1]):
+            vals = []
+            for sgn in (+1, -1):
+                p = arr.copy(); p[0, e] += sgn * 1e-6
+                setter(p); vals.append(phi())
+            setter(arr)
+            assert abs(g[0, e] - (vals[0] - vals[1]) / 2e-6) <= 1e-6 * np.abs(g).max(), e
+    # scheduled rollout: 5 frames of 8 substeps
+    T, stride, F = 40, 8, 5
+    st, sh = rng.uniform(-0.05, 0.05, (F, 1, M)), rng.uniform(-0.2, 0.2, (F, 1, Mh))
+    tgt = x.mean(1) + np.array([[0.1, -0.2, 0.05]])
+
+    def loss(st_, sh_, K=1):
+        o.set_act_schedule(stride, st_, sh_)
+        ro = o.rollout(x, v, T, K=K, rec_times=[T])
+        L, cot = orc.loss_and_cotangents("final_centroid", ro["rec_x"], tgt)
+        return L.sum(), ro, cot
+
+    L0, ro, cot = loss(st, sh)
+    o.zero_grads()
+    ax0, _ = o.rollout_backward(ro, [T], cot)
+    gst, gsh = o.act_schedule_grads()
+    gmu = o.grads("tet_mu").copy()
+    assert np.abs(gst[0]).max() > 0 and np.abs(gst[-1]).max() > 0 and np.abs(gsh).max() > 0
+    for arr, g, which in ((st, gst, 0), (sh, gsh, 1)):
+        for _ in range(6):
+            f_, e = int(rng.integers(F)), int(rng.integers(arr.shape[2]))
+            vals = []
+            for sgn in (+1, -1):
+                p = arr.copy(); p[f_, 0, e] += sgn * 1e-5
+                vals.append(loss(p if which == 0 else st, p if which == 1 else sh)[0])
+            assert abs(g[f_, 0, e] - (vals[0] - vals[1]) / 2e-5) <= 1e-5 * np.abs(g).max(), (which, f_, e)
+    for K in (7, 16):
+        _, rok, cotk = loss(st, sh, K=K)
+        o.zero_grads()
+        axk, _ = o.rollout_backward(rok, [T], cotk)
+        gk_t, gk_h = o.act_schedule_grads()
+        assert np.array_equal(axk, ax0) and np.array_equal(gk_t, gst) and np.array_equal(gk_h, gsh) and np.array_equal(o.grads("tet_mu"), gmu)
+    # no schedule and zero current activation: the passive model of every other test
+    o.set_act_schedule(1, None, None)
+    o.set_act_current(np.zeros((1, M)), np.zeros((1, Mh)))
+    o2 = orc.Oracle(sc)
+    assert np.array_equal(o.step(x, v)[0], o2.step(x, v)[0])
