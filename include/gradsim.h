@@ -64,8 +64,15 @@ enum gs_param_group {
                         per environment, arrays [E] (count = 1) */
     GS_GRAVITY = 12, /* gravity (Table 5 column "g", NEXT-2): ONE vector shared by all environments -- gs_set_params reads
                         d_values[0..2] (synchronises the stream; tapes re-capture their graphs at the next use);
-                        gs_param_grads returns dL/dg per environment, [E][3] (count = 3) */
-    GS_NUM_GROUPS = 13
+                        gs_param_grads returns dL/dg per environment, [E][3] (count = 3).  Off by default: the sum over
+                        all particles of every adjoint substep costs ~12 % of the particle adjoint kernel; gs_request_grads
+                        switches it on (before the backward pass), else gs_param_grads returns GS_ESTATE */
+    GS_HINGE_THETA0 = 13, /* rest angle per hinge (Table 5 column "rest": the rest configuration of the bending springs): one
+                        array [Mh] shared by all environments, as GS_HINGE_KB.  Its gradient is read from the hinge actuation
+                        gradients (theta0 and the per-edge actuation enter the same argument, PAPER.md:585-586:
+                        dL/dtheta0 = -1/2 sum over frames of dL/dalpha), so gs_param_grads needs an activation schedule
+                        attached (gs_actuation_create; one zero frame is enough), else GS_ESTATE */
+    GS_NUM_GROUPS = 14
 };
 
 /* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */
@@ -135,6 +142,28 @@ int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, 
 int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream stream);
 
 /*
+ * Actuation inputs.  PAPER.md:579: alpha of the volume term (J - alpha)^2 is "a per-element
+ * actuation value that allows the element to expand and contract" -- here alpha = 1 + 3 mu / (4 lambda) + act (DESIGN.md
+ * A1), act per tet; f_b = k_b sin(phi/2 + alpha) d with alpha "a per-edge actuation value that allows
+ * the mesh to flex inwards or outwards", per hinge.  Activations vary in time (App. E: a controller
+ * evaluated over simulation time produces them; the controller itself stays outside the library): a SCHEDULE of n_frames
+ * frames, frame f holding during substeps [f frame_stride, (f+1) frame_stride) of a rollout, the last frame to the end.
+ *   gs_actuation_create   attaches a schedule, all zeros (= passive), stored in d_mem (DEVICE, >= gs_actuation_bytes,
+ *                         256-byte aligned, must outlive the model or the next create); n_frames = 0 detaches.
+ *   gs_set_actuation      DEVICE values [n_frames][E][count] in caller element order (count = M or Mh).
+ *   gs_actuation_grads    dL/d(activation) [n_frames][E][count], accumulated by the adjoint substeps since gs_zero_grads
+ *                         (fp32 sums of frame_stride terms per entry).
+ *   gs_set_actuation_frame  the frame gs_step_forward / gs_step_backward use (default 0).
+ * Triangles carry no actuation.  Errors: GS_EINVAL, GS_ESTATE (no schedule attached), GS_ECUDA.
+ */
+enum gs_actuation_kind { GS_ACT_TET = 0, GS_ACT_HINGE = 1 };
+size_t gs_actuation_bytes(const gs_model *m, int n_frames);
+int gs_actuation_create(gs_model *m, int n_frames, int frame_stride, void *d_mem, size_t bytes, gs_stream stream);
+int gs_set_actuation(gs_model *m, int kind, const float *d_values, gs_stream stream);
+int gs_actuation_grads(gs_model *m, int kind, float *d_out, gs_stream stream);
+int gs_set_actuation_frame(gs_model *m, int frame);
+
+/*
  * One forward substep (PAPER.md:618-619 semi-implicit Euler; 763-764 Listing 1):
  *   f = tets + triangles + hinges + contact, all at the start-of-step state;
  *   v+ = v + (f w + g [w>0]) dt;  x+ = x + v+ dt.
@@ -178,6 +207,9 @@ int gs_tape_read(gs_model *m, gs_tape *t, int substep, float *d_x, float *d_v, g
 int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_stride, const float *d_adj_x_frames,
                         const float *d_adj_x_T, const float *d_adj_v_T, float *d_adj_x0, float *d_adj_v0, gs_stream stream);
 
+/* Switch a gradient that costs extra work per substep on or off (only GS_GRAVITY needs this; every other group is always
+   accumulated).  Tapes re-capture their graphs at the next use. */
+int gs_request_grads(gs_model *m, int group, int enable);
 int gs_zero_grads(gs_model *m, gs_stream stream);
 /* Accumulated dL/d(parameter) of one group, DEVICE out [E][count] fp32 in caller order.  For GS_MASS the
    gradient of a pinned particle is 0 (A11). */

@@ -92,6 +92,56 @@ extern "C" int gs_set_params(gs_model *m, int group, const float *d_values, gs_s
     return launch_set_params(m, group, d_values, (cudaStream_t)stream);
 }
 
+// ------------------------------------------------------------------------------------------ actuation inputs
+static size_t act_floats(const gs_model *m, int kind, int n_frames) {
+    const int t = kind == 0 ? T_TET : T_HINGE;
+    return m->counts[t] ? (size_t)n_frames * m->E * m->hes[t].cpad : 0;
+}
+static size_t al256f(size_t n) { return (n + 63) & ~(size_t)63; }  // floats, 256-byte granules
+extern "C" size_t gs_actuation_bytes(const gs_model *m, int n_frames) {
+    if (!m || n_frames < 1) return 0;
+    return 2 * (al256f(act_floats(m, 0, n_frames)) + al256f(act_floats(m, 1, n_frames))) * sizeof(float) + 256;
+}
+extern "C" int gs_actuation_create(gs_model *m, int n_frames, int frame_stride, void *d_mem, size_t bytes, gs_stream stream) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    m->epoch++;  // the frame pointers are kernel arguments: captured graphs are stale
+    m->act_cur = 0;
+    if (n_frames == 0) { m->act_frames = 0; m->d_act[0] = m->d_act[1] = m->d_gact[0] = m->d_gact[1] = nullptr; return GS_OK; }
+    GS_REQUIRE(n_frames >= 1 && frame_stride >= 1, GS_EINVAL, "n_frames and frame_stride must be >= 1");
+    GS_REQUIRE(d_mem && ((uintptr_t)d_mem & 255) == 0 && bytes >= gs_actuation_bytes(m, n_frames), GS_EINVAL, "actuation memory missing, misaligned or too small (%zu < %zu)",
+               bytes, gs_actuation_bytes(m, n_frames));
+    float *p = (float *)d_mem;
+    for (int k = 0; k < 2; k++) { m->d_act[k] = p; p += al256f(act_floats(m, k, n_frames)); m->d_gact[k] = p; p += al256f(act_floats(m, k, n_frames)); }
+    GS_CUDA(cudaMemsetAsync(d_mem, 0, gs_actuation_bytes(m, n_frames) - 256, (cudaStream_t)stream), "zero actuation memory");
+    m->act_frames = n_frames; m->act_stride = frame_stride;
+    return GS_OK;
+}
+extern "C" int gs_set_actuation(gs_model *m, int kind, const float *d_values, gs_stream stream) {
+    GS_REQUIRE(m && d_values, GS_EINVAL, "null argument");
+    GS_REQUIRE(kind == GS_ACT_TET || kind == GS_ACT_HINGE, GS_EINVAL, "unknown actuation kind %d", kind);
+    GS_REQUIRE(m->act_frames > 0, GS_ESTATE, "no activation schedule attached (gs_actuation_create)");
+    return launch_actuation_io(m, kind, d_values, nullptr, (cudaStream_t)stream);
+}
+extern "C" int gs_actuation_grads(gs_model *m, int kind, float *d_out, gs_stream stream) {
+    GS_REQUIRE(m && d_out, GS_EINVAL, "null argument");
+    GS_REQUIRE(kind == GS_ACT_TET || kind == GS_ACT_HINGE, GS_EINVAL, "unknown actuation kind %d", kind);
+    GS_REQUIRE(m->act_frames > 0, GS_ESTATE, "no activation schedule attached (gs_actuation_create)");
+    return launch_actuation_io(m, kind, nullptr, d_out, (cudaStream_t)stream);
+}
+extern "C" int gs_set_actuation_frame(gs_model *m, int frame) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    GS_REQUIRE(m->act_frames > 0 && frame >= 0 && frame < m->act_frames, GS_EINVAL, "frame %d outside the schedule of %d frames", frame, m->act_frames);
+    m->act_cur = frame;
+    return GS_OK;
+}
+
+extern "C" int gs_request_grads(gs_model *m, int group, int enable) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    GS_REQUIRE(group == GS_GRAVITY, GS_EINVAL, "group %d needs no request: only GS_GRAVITY is off by default", group);
+    if (m->dev.want_gravity != (enable != 0)) { m->dev.want_gravity = enable != 0; m->epoch++; }  // a by-value kernel argument
+    return GS_OK;
+}
+
 static int reset_bad(gs_model *m, cudaStream_t st) {
     GS_CUDA(cudaMemsetAsync(m->dev.bad, 0x7f, sizeof(int), st), "reset non-finite flag");
     return GS_OK;
@@ -102,7 +152,7 @@ extern "C" int gs_step_forward(gs_model *m, const float *d_x, const float *d_v, 
     cudaStream_t st = (cudaStream_t)stream;
     GS_TRY(reset_bad(m, st));
     GS_TRY(launch_pack(m, d_x, d_v, m->d_xs[0], m->d_vs[0], true, st));
-    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], 0, st));
+    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], -1, st));
     return launch_unpack(m, m->d_xs[1], m->d_vs[1], d_x_out, d_v_out, st);
 }
 
@@ -113,9 +163,9 @@ extern "C" int gs_step_backward(gs_model *m, const float *d_x, const float *d_v,
     GS_TRY(reset_bad(m, st));
     GS_TRY(launch_pack(m, d_x, d_v, m->d_xs[0], m->d_vs[0], true, st));
     // the end-of-step velocity enters the mass gradient: recompute the forward step
-    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], 0, st));
+    GS_TRY(stream_step_forward(m, m->d_xs[0], m->d_vs[0], m->d_xs[1], m->d_vs[1], -1, st));
     GS_TRY(launch_pack(m, d_adj_x_out, d_adj_v_out, m->d_adjx, m->d_adjv, false, st));
-    GS_TRY(stream_step_adjoint(m, m->d_xs[0], m->d_vs[0], m->d_vs[1], -1, st));
+    GS_TRY(stream_step_adjoint(m, m->d_xs[0], m->d_vs[0], m->d_vs[1], -1, -1, st));
     return launch_unpack(m, m->d_adjx, m->d_adjv, d_adj_x_in, d_adj_v_in, st);
 }
 
@@ -254,7 +304,7 @@ extern "C" int gs_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int fr
                     if (n_frames > 0 && (s + 1) % frame_stride == 0 && (s + 1) / frame_stride <= n_frames)
                         cot = (long long)((s + 1) / frame_stride - 1) * (long long)frame_elems;
                     const int a = t->slot_bwd(s), b = t->slot_bwd(s + 1);
-                    GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, q));
+                    GS_TRY(stream_step_adjoint(m, t->slot_x(a), t->slot_v(a), t->slot_v(b), cot, s, q));
                 }
             }
             return (int)GS_OK;
@@ -271,6 +321,7 @@ extern "C" int gs_zero_grads(gs_model *m, gs_stream stream) {
 extern "C" int gs_param_grads(gs_model *m, int group, float *d_out, gs_stream stream) {
     GS_REQUIRE(m && d_out, GS_EINVAL, "null argument");
     GS_REQUIRE(group >= 0 && group < GS_NUM_GROUPS, GS_EINVAL, "unknown parameter group %d", group);
+    GS_REQUIRE(group != GS_GRAVITY || m->dev.want_gravity, GS_ESTATE, "dL/dg was not requested before the backward pass (gs_request_grads)");
     return launch_get_grads(m, group, d_out, (cudaStream_t)stream);
 }
 
@@ -535,7 +586,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
     for (int k = 0; k < n_groups; k++) {
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
-        const int c = g == GS_MASS ? N : (g == GS_GRAVITY ? 3 : (g >= GS_CONTACT_KE ? 1 : (g == GS_HINGE_KB ? m->counts[T_HINGE] : m->counts[g / 3])));
+        const int c = g == GS_MASS ? N : (g == GS_GRAVITY ? 3 : (g == GS_HINGE_THETA0 || g == GS_HINGE_KB ? m->counts[T_HINGE] : (g >= GS_CONTACT_KE ? 1 : m->counts[g / 3])));
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
         // the staging buffer is reused: the copy is ordered before the next group's kernel on the same stream

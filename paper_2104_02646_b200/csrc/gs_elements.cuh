@@ -51,16 +51,17 @@ __device__ __forceinline__ void tet_kin(const vec3 &x0, const vec3 &x1, const ve
     k.J = dot(k.f1, k.c1);
 }
 
-// P = mu [s1 F - 3/4 cof F] + lambda (J - 1) cof F + k F sym(F^T Fdot),  s1 = 1 - 1/(I_C + 1)
+// P = mu [s1 F - 3/4 cof F] + lambda (J - 1 - act) cof F + k F sym(F^T Fdot),  s1 = 1 - 1/(I_C + 1)
+// act: the per-element actuation of PAPER.md:579 (0 = passive)
 // nodal forces H = -V P B^T; f[1..3] = columns of H, f[0] = -(sum)
-__device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], const float *b, float V, float mu, float lam, float kd, vec3 f[4]) {
+__device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], const float *b, float V, float mu, float lam, float kd, float act, vec3 f[4]) {
     TetKin k;
     tet_kin(x[0], x[1], x[2], x[3], b, k);
     vec3 g1, g2, g3;
     mat_cols_times_B(v[1] - v[0], v[2] - v[0], v[3] - v[0], b, g1, g2, g3);
     // -V is folded into the three scalar coefficients, so the columns below are those of -V P
     const float s1 = k.Ic * rcp_fast(k.Ic + 1.0f);
-    const float ce = -V * (lam * (k.J - 1.0f) - 0.75f * mu);  // lambda (J - alpha), alpha = 1 + 3mu/(4 lambda)  (A1)
+    const float ce = -V * (lam * ((k.J - 1.0f) - act) - 0.75f * mu);  // lambda (J - alpha), alpha = 1 + 3mu/(4 lambda) + act  (A1)
     const float ms = -V * mu * s1;
     const float kv = -V * kd, kh = 0.5f * kv;
     // kv S, S = sym(F^T Fdot)
@@ -79,8 +80,9 @@ __device__ __forceinline__ void tet_force(const vec3 x[4], const vec3 v[4], cons
 // parameter gradients of this element for this substep.
 // Everything downstream of A = adj_P = -V G B is linear in A, so the kernel works with A' = G B and folds -V into the
 // scalar coefficients; F:A = tr(F^T A) and (F S):A = S:sym(F^T A) reuse the entries of N = sym(F^T A').
-__device__ __forceinline__ void tet_adjoint(const vec3 x[4], const vec3 v[4], const vec3 a[4], const float *b, float V, float mu, float lam, float kd,
-                                            vec3 ax[4], vec3 av[4], float &gmu, float &glam, float &gk) {
+// gact = dL/d(act) of this substep: dP/d(act) = -lambda cof F
+__device__ __forceinline__ void tet_adjoint(const vec3 x[4], const vec3 v[4], const vec3 a[4], const float *b, float V, float mu, float lam, float kd, float act,
+                                            vec3 ax[4], vec3 av[4], float &gmu, float &glam, float &gk, float &gact) {
     TetKin k;
     tet_kin(x[0], x[1], x[2], x[3], b, k);
     vec3 g1, g2, g3;
@@ -103,11 +105,13 @@ __device__ __forceinline__ void tet_adjoint(const vec3 x[4], const vec3 v[4], co
     const float SN = fmaf(s11, n11, fmaf(s22, n22, s33 * n33)) + 2.0f * fmaf(s12, n12, fmaf(s13, n13, s23 * n23));
     // parameter gradients: P is linear in mu, lambda, k
     const float mV = -V;
+    const float Jm = (k.J - 1.0f) - act;
     gmu = mV * (s1 * FA - 0.75f * CA);
-    glam = mV * ((k.J - 1.0f) * CA);
+    glam = mV * (Jm * CA);
     gk = mV * SN;
+    gact = V * lam * CA;
     // adj_F = mu s1 A + 2 mu (F:A)/(Ic+1)^2 F + lambda (cof:A) cof + lambda (J - alpha) Dcof[A] + k (A S + Fdot N),  A = -V A'
-    const float ms = mV * mu * s1, q = mV * 2.0f * mu * FA * ip1 * ip1, lc = mV * lam * CA, ce = mV * (lam * (k.J - 1.0f) - 0.75f * mu);
+    const float ms = mV * mu * s1, q = mV * 2.0f * mu * FA * ip1 * ip1, lc = mV * lam * CA, ce = mV * (lam * Jm - 0.75f * mu);
     const float kv = mV * kd;
     const float t11 = kv * s11, t22 = kv * s22, t33 = kv * s33, t12 = kv * s12, t13 = kv * s13, t23 = kv * s23;  // kv S
     const float m11 = kv * n11, m22 = kv * n22, m33 = kv * n33, m12 = kv * n12, m13 = kv * n13, m23 = kv * n23;  // kv N
@@ -193,13 +197,14 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
 
 // ------------------------------------------------------------------------------------------ hinges
 // vertices: x[0], x[1] wings; x[2], x[3] the shared edge.  theta = signed dihedral (0 when flat);
-// f_i = k_b l0 sin((theta - theta0)/2) d_i, d_i = -d(theta)/dx_i (Bridson directions).
+// f_i = k_b l0 sin((theta - theta0)/2 + alpha) d_i, d_i = -d(theta)/dx_i (Bridson directions), alpha the per-edge actuation.
 // Rest constants per hinge: s0h = sin(theta0/2), c0h = cos(theta0/2), kl = k_b * l0 (fp64 on the host).
 struct HingeGeo {
     vec3 p13, p14, p23, p24, n1, n2, eh, m1, m2;
     float L, iL, i1, i2, c13, c14, c23, c24, sh, ch;  // sh, ch = sin, cos of (theta - theta0)/2
 };
-__device__ __forceinline__ void hinge_geo(const vec3 x[4], float s0h, float c0h, HingeGeo &h) {
+// sa, ca = sin, cos of the per-edge actuation alpha (sin(phi/2 + alpha)); (0, 1) = passive
+__device__ __forceinline__ void hinge_geo(const vec3 x[4], float s0h, float c0h, float sa, float ca, HingeGeo &h) {
     h.p13 = x[0] - x[2]; h.p14 = x[0] - x[3]; h.p23 = x[1] - x[2]; h.p24 = x[1] - x[3];
     h.n1 = cross(h.p13, h.p14); h.n2 = cross(h.p24, h.p23);
     const vec3 e = x[3] - x[2];
@@ -224,8 +229,9 @@ __device__ __forceinline__ void hinge_geo(const vec3 x[4], float s0h, float c0h,
         sht = copysignf(a, sn);
         cht = 0.5f * fabsf(sn) * rcp_fast(a);
     }
-    h.sh = sht * c0h - cht * s0h;
-    h.ch = cht * c0h + sht * s0h;
+    const float s1 = sht * c0h - cht * s0h, c1 = cht * c0h + sht * s0h;  // (theta - theta0)/2
+    h.sh = s1 * ca + c1 * sa;
+    h.ch = c1 * ca - s1 * sa;
 }
 __device__ __forceinline__ void hinge_dirs(const HingeGeo &h, vec3 d[4]) {
     d[0] = h.L * h.m1;
@@ -233,9 +239,9 @@ __device__ __forceinline__ void hinge_dirs(const HingeGeo &h, vec3 d[4]) {
     d[2] = madd(h.c14 * h.m1, h.c24, h.m2);
     d[3] = -madd(h.c13 * h.m1, h.c23, h.m2);
 }
-__device__ __forceinline__ void hinge_force(const vec3 x[4], float s0h, float c0h, float kl, vec3 f[4]) {
+__device__ __forceinline__ void hinge_force(const vec3 x[4], float s0h, float c0h, float kl, float sa, float ca, vec3 f[4]) {
     HingeGeo h;
-    hinge_geo(x, s0h, c0h, h);
+    hinge_geo(x, s0h, c0h, sa, ca, h);
     vec3 d[4];
     hinge_dirs(h, d);
     const float s = kl * h.sh;
@@ -243,9 +249,11 @@ __device__ __forceinline__ void hinge_force(const vec3 x[4], float s0h, float c0
 }
 // VJP = JVP (the force is conservative): ax_j = -E'' s d_j + E' Dd_j[a], s = sum_i d_i . a_i
 // gkb = dL/dk_b of this substep: the force is linear in k_b, dL/dk_b = l0 sin((theta - theta0)/2) sum_i d_i . a_i
-__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float s0h, float c0h, float kl, float l0, vec3 ax[4], float &gkb) {
+// gact = dL/d(alpha) of this substep = k_b l0 cos(ph) s (and dL/d(theta0) = -gact / 2: theta0 enters the same argument as -theta0/2)
+__device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], float s0h, float c0h, float kl, float l0, float sa, float ca, vec3 ax[4],
+                                              float &gkb, float &gact) {
     HingeGeo h;
-    hinge_geo(x, s0h, c0h, h);
+    hinge_geo(x, s0h, c0h, sa, ca, h);
     vec3 d[4];
     hinge_dirs(h, d);
     const vec3 q13 = a[0] - a[2], q14 = a[0] - a[3], q23 = a[1] - a[2], q24 = a[1] - a[3];
@@ -263,6 +271,7 @@ __device__ __forceinline__ void hinge_adjoint(const vec3 x[4], const vec3 a[4], 
     const float s = dot(h.m1, h.c13 * q14 - h.c14 * q13) + dot(h.m2, h.c23 * q24 - h.c24 * q23);
     const float E1 = kl * h.sh, E2s = 0.5f * kl * h.ch * s;
     gkb = l0 * h.sh * s;
+    gact = 2.0f * E2s;
     ax[0] = madd(-E2s * d[0], E1, madd(dL * h.m1, h.L, dm1));
     ax[1] = madd(-E2s * d[1], E1, madd(dL * h.m2, h.L, dm2));
     ax[2] = madd(-E2s * d[2], E1, madd(madd(madd(dc14 * h.m1, h.c14, dm1), dc24, h.m2), h.c24, dm2));

@@ -87,9 +87,18 @@ struct ModelDev {
                                       // three after every k_elements_fwd, k_particles_adj the adjoint three before every
                                       // k_elements_adj
     int *bad;                         // first non-finite substep (INT_MAX = none)
+    int want_gravity;                 // dL/dg requested (gs_request_grads): the particle adjoint reduces dt lv over all particles
     const float **frame_base;         // [1] base of the caller's frame-cotangent array of the running backward pass: read
                                       // through this slot (written by a one-thread kernel before the pass) so that the
                                       // captured backward graph does not depend on the caller's pointer
+};
+
+// Actuation inputs of ONE substep (PAPER.md:579 per-tet, 585-586 per-hinge): the frame of the
+// model's activation schedule that holds during this substep, internal element order [E][cpad]; null = passive.
+// Passed by value beside ModelDev to the element kernels.
+struct ActDev {
+    const float *tet, *hinge;  // activation values
+    float *g_tet, *g_hinge;    // dL/d(activation) accumulators of the same frame (adjoint kernels)
 };
 
 struct HostElemSet {
@@ -119,6 +128,19 @@ struct gs_model {
     bool pdl = true;                 // programmatic dependent launch of the hot-path kernels (small meshes only: configure_stream_kernels)
     long long elem_items = 0;        // work items (tile x environment) of the largest element type
     int step_counter = 0;  // substep index written to dev.bad on a non-finite state
+    // activation schedule (gs_actuation_create): n_frames frames of act_stride substeps, [F][E][cpad] per kind (0 tets, 1 hinges)
+    int act_frames = 0, act_stride = 1, act_cur = 0;  // act_cur: the frame single-substep calls use
+    float *d_act[2] = {nullptr, nullptr}, *d_gact[2] = {nullptr, nullptr};
+    gs::ActDev act_for(int substep) const {
+        gs::ActDev a = {nullptr, nullptr, nullptr, nullptr};
+        if (act_frames <= 0) return a;
+        int f = substep / act_stride;
+        f = f < act_frames ? f : act_frames - 1;
+        const size_t o0 = (size_t)f * E * hes[gs::T_TET].cpad, o1 = (size_t)f * E * hes[gs::T_HINGE].cpad;
+        if (counts[gs::T_TET]) { a.tet = d_act[0] + o0; a.g_tet = d_gact[0] + o0; }
+        if (counts[gs::T_HINGE]) { a.hinge = d_act[1] + o1; a.g_hinge = d_gact[1] + o1; }
+        return a;
+    }
     uint64_t epoch = 0;    // bumped when a by-value kernel argument changes (gravity): captured graphs of older epochs are stale
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
     void *res_host = nullptr;
@@ -194,7 +216,7 @@ int build_model(const gs_model_desc *desc, void *d_workspace, size_t bytes, cuda
 
 // gs_stream.cu: streaming plan launches
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st);
-int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, cudaStream_t st);
+int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, int substep, cudaStream_t st);
 int launch_set_frame_base(gs_model *m, const float *d_frames, cudaStream_t st);
 int launch_pack(gs_model *m, const float *x, const float *v, float4 *x4, float4 *v4, bool x_is_state, cudaStream_t st);
 int launch_unpack(gs_model *m, const float4 *x4, const float4 *v4, float *x, float *v, cudaStream_t st);
@@ -202,6 +224,7 @@ int launch_flush_grads(gs_model *m, cudaStream_t st);
 int launch_zero_grads(gs_model *m, cudaStream_t st);
 int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st);
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st);
+int launch_actuation_io(gs_model *m, int kind, const float *d_in, float *d_out, cudaStream_t st);  // caller order <-> internal schedule
 int configure_stream_kernels(gs_model *m);
 
 // gs_resident.cu: resident plan

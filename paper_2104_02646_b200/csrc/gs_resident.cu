@@ -44,6 +44,14 @@ struct ResDev {
     const uint16_t *csr_slots; // [4 M] slot = k * M + e
 };
 
+// activation schedule of the tets (gs_actuation_create), internal order [F][E][cpad]; used by the ACT kernel variants
+struct ResAct {
+    const float *tet;
+    float *g_tet;
+    int F, stride;
+    size_t fstride;  // E * cpad
+};
+
 struct ResHost {
     ResDev rd;
     int ept;
@@ -53,10 +61,11 @@ struct ResHost {
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
 // shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
-// adjoint only: per-particle fp64 accumulators of the per-environment totals (contact parameters, gravity), double[7][N]
+// adjoint only: per-particle accumulators of the per-environment totals (contact parameters, gravity): double[7][N] masters,
+// then float[4][N] chunks of the contact terms
 constexpr int kResAcc = 7;
 static size_t res_smem(int L, int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)kResAcc * N * 8) : 0) +
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + 4 * 4)) : 0) +
            al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)4 * M * 2);
 }
 
@@ -76,6 +85,7 @@ size_t resident_blob_bytes(const gs_model_desc *d) {
 // ------------------------------------------------------------------------------------------ kernels
 struct TetReg {
     float b[9], V, mu, lam, kd;
+    float act;  // this substep's actuation; 0 in the passive kernels
     ushort4 li;
     bool on;
 };
@@ -100,6 +110,7 @@ __device__ __forceinline__ void load_tets(const ModelDev &md, const ResDev &rd, 
         tr[j].lam = es.par[par_index(es.n_tiles, env, ee, 1)];
         tr[j].kd = es.par[par_index(es.n_tiles, env, ee, 2)];
         tr[j].li = rd.idx[ee];
+        tr[j].act = 0.0f;
     }
 }
 
@@ -136,8 +147,8 @@ __device__ __forceinline__ float group_sum(float v, int kpp) {
 }
 
 // forward: substeps [0, T), tape slot s = (x4, v4) at base + 2 s S (+ S for v), S = E N
-template <int EPT, int MAXT, int MINB>
-__global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, const ResDev rd, float4 *__restrict__ tape, size_t S, int T) {
+template <int EPT, int MAXT, int MINB, bool ACT>
+__global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, const ResDev rd, float4 *__restrict__ tape, size_t S, int T, const ResAct ra) {
     extern __shared__ float4 smem4[];
     const int N = rd.N, M = rd.M, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L;
@@ -161,6 +172,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
     __syncthreads();
     int bad = INT_MAX;
     for (int s = 0; s < T; s++) {
+        if (ACT && s % ra.stride == 0 && s / ra.stride < ra.F) {  // a new frame of the activation schedule begins
+#pragma unroll
+            for (int j = 0; j < EPT; j++)
+                if (tr[j].on) tr[j].act = ra.tet[(size_t)(s / ra.stride) * ra.fstride + (size_t)env * md.es[T_TET].cpad + tid + j * blockDim.x];
+        }
 #pragma unroll
         for (int j = 0; j < EPT; j++) {
             if (tr[j].on) {
@@ -168,7 +184,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
                 const vec3 x[4] = {vec3(sx[li.x]), vec3(sx[li.y]), vec3(sx[li.z]), vec3(sx[li.w])};
                 const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
                 vec3 f[4];
-                tet_force(x, v, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, f);
+                tet_force(x, v, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, tr[j].act, f);
                 const int e = tid + j * blockDim.x;
 #pragma unroll
                 for (int k = 0; k < 4; k++) sf[k * M + e] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
@@ -201,19 +217,20 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
 
 // adjoint: substeps T-1 .. 0.  adjx / adjv: [E][N] float4 in/out (dL/d(final state) -> dL/d(initial state)).
 // frames: caller-order [n_frames][E][N][3] cotangents of the states after (k+1) * stride substeps, or nullptr.
-template <int EPT, int MAXT, int MINB>
+template <int EPT, int MAXT, int MINB, bool ACT>
 __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, const ResDev rd, const float4 *__restrict__ tape, size_t S, int T,
                                                               float4 *__restrict__ adjx, float4 *__restrict__ adjv, const float *__restrict__ frames,
-                                                              int n_frames, int stride) {
+                                                              int n_frames, int stride, const ResAct ra) {
     extern __shared__ float4 smem4[];
     const int N = rd.N, M = rd.M, PL = 4 * M, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
     float4 *sf = smem4 + 3 * L;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
-    // dL/d(k_e, k_d, k_f, mu_c) and dL/dg: per-particle fp64 partial sums (only the particle's lead lane touches its
-    // entries; the contact terms are of mixed sign and cancel, so they are accumulated in fp64 from the start), summed in
-    // particle order at the end: deterministic
-    double *dgc = reinterpret_cast<double *>(sf + 2 * PL);  // [kResAcc][N]
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((kResAcc * N * 8 + 15) & ~15));
+    // dL/d(k_e, k_d, k_f, mu_c) and dL/dg: per-particle partial sums (only the particle's lead lane touches its entries):
+    // fp32 chunks of kFlushEvery substeps (contact: shared memory; gravity: registers) folded into fp64 masters (hazard
+    // H4), summed in particle order at the end: deterministic
+    double *dgc = reinterpret_cast<double *>(sf + 2 * PL);   // [kResAcc][N]
+    float *sgc = reinterpret_cast<float *>(dgc + kResAcc * N);  // [4][N]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((N * (kResAcc * 8 + 4 * 4) + 15) & ~15));
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
     uint16_t *s_slots = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
@@ -238,7 +255,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
     if (po.lead)
-        for (int q = 0; q < kResAcc; q++) dgc[q * N + po.p] = 0.0;
+        for (int q = 0; q < kResAcc; q++) { dgc[q * N + po.p] = 0.0; if (q < 4) sgc[q * N + po.p] = 0.f; }
     vec3 glv = zero3();  // sum over a chunk of substeps of lv (cotangent of v+): dL/dg = dt sum lv for a free particle
     const size_t frame_elems = (size_t)md.E * N * 3;
     const size_t gstride = (size_t)md.E * md.es[T_TET].cpad;
@@ -260,7 +277,20 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         dx = vec3(group_sum(ax, rd.kpp), group_sum(ay, rd.kpp), group_sum(az, rd.kpp));
         dv = vec3(group_sum(cx, rd.kpp), group_sum(cy, rd.kpp), group_sum(cz, rd.kpp));
     };
+    float gact[EPT];
+#pragma unroll
+    for (int j = 0; j < EPT; j++) gact[j] = 0.f;
+    int act_frame = -1;
     for (int s = T - 1; s >= 0; s--) {
+        if (ACT) {  // the frame of the activation schedule that holds during substep s
+            const int f = s / ra.stride < ra.F ? s / ra.stride : ra.F - 1;
+            if (f != act_frame) {
+                act_frame = f;
+#pragma unroll
+                for (int j = 0; j < EPT; j++)
+                    if (tr[j].on) tr[j].act = ra.tet[(size_t)f * ra.fstride + (size_t)env * md.es[T_TET].cpad + tid + j * blockDim.x];
+            }
+        }
         // prefetch the start state of the previous substep while this one is processed
         float4 xp = xq, vp = vq;
         if (po.lead && s > 0) { xp = tape[(size_t)(2 * (s - 1)) * S + poff]; vp = tape[(size_t)(2 * (s - 1) + 1) * S + poff]; }
@@ -282,13 +312,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             if (w > 0.0f) {
                 const vec3 dvf = (vec3(vnext) - v) - dt * g;
                 gm32 += -w * dot(dvf, lv);
-                glv += lv;
+                if (md.want_gravity) glv += lv;
             }
             float gp[4];
             contact_adjoint(cp, x, v, af, ax, av, gp);
             if (gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f) {
 #pragma unroll
-                for (int q = 0; q < 4; q++) dgc[q * N + po.p] += (double)gp[q];
+                for (int q = 0; q < 4; q++) sgc[q * N + po.p] += gp[q];
             }
             bx = ax; bv = av;
             sx[po.lp] = xq; sv[po.lp] = vq; sa[po.lp] = make_float4(af.x, af.y, af.z, 0.f);
@@ -303,9 +333,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
                 const vec3 a[4] = {vec3(sa[li.x]), vec3(sa[li.y]), vec3(sa[li.z]), vec3(sa[li.w])};
                 vec3 ax[4], av[4];
-                float gmu, glam, gk;
-                tet_adjoint(x, v, a, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, ax, av, gmu, glam, gk);
+                float gmu, glam, gk, ga;
+                tet_adjoint(x, v, a, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, tr[j].act, ax, av, gmu, glam, gk, ga);
                 g32[j][0] += gmu; g32[j][1] += glam; g32[j][2] += gk;
+                if (ACT) gact[j] += ga;
                 const int e = tid + j * blockDim.x;
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
@@ -314,8 +345,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 }
             }
         }
+        if (ACT && s % ra.stride == 0 && s / ra.stride < ra.F) {  // substep s was the first of its frame: the frame's gradient is complete
+#pragma unroll
+            for (int j = 0; j < EPT; j++) {
+                if (tr[j].on) ra.g_tet[(size_t)act_frame * ra.fstride + (size_t)env * md.es[T_TET].cpad + tid + j * blockDim.x] += gact[j];
+                gact[j] = 0.f;
+            }
+        }
         if ((s & (kFlushEvery - 1)) == 0) {  // fold the fp32 chunk into fp64 (hazard H4)
             if (po.lead) {
+#pragma unroll
+                for (int q = 0; q < 4; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
                 dgc[4 * N + po.p] += (double)(dt * glv.x); dgc[5 * N + po.p] += (double)(dt * glv.y); dgc[6 * N + po.p] += (double)(dt * glv.z);
                 glv = zero3();
             }
@@ -461,16 +501,17 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     rh->smem_adj = res_smem(Lsp, N, M, 2, true);
     m->res_host = rh;
     int rc = GS_OK;
-    if (rh->ept == 1 && rh->rd.nthreads <= 320) {
-        rc = set_smem(k_resident_fwd<1, 320, 3>, rh->smem_fwd);
-        if (rc == GS_OK) rc = set_smem(k_resident_adj<1, 320, 2>, rh->smem_adj);
-    } else if (rh->ept == 1) {
-        rc = set_smem(k_resident_fwd<1, 1024, 1>, rh->smem_fwd);
-        if (rc == GS_OK) rc = set_smem(k_resident_adj<1, 1024, 1>, rh->smem_adj);
-    } else {
-        rc = set_smem(k_resident_fwd<2, 1024, 1>, rh->smem_fwd);
-        if (rc == GS_OK) rc = set_smem(k_resident_adj<2, 1024, 1>, rh->smem_adj);
-    }
+#define GS_RES_SMEM(E_, T_, BF_, BA_)                                                                  \
+    do {                                                                                               \
+        rc = set_smem(k_resident_fwd<E_, T_, BF_, false>, rh->smem_fwd);                               \
+        if (rc == GS_OK) rc = set_smem(k_resident_fwd<E_, T_, BF_, true>, rh->smem_fwd);               \
+        if (rc == GS_OK) rc = set_smem(k_resident_adj<E_, T_, BA_, false>, rh->smem_adj);              \
+        if (rc == GS_OK) rc = set_smem(k_resident_adj<E_, T_, BA_, true>, rh->smem_adj);               \
+    } while (0)
+    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_SMEM(1, 320, 3, 2);
+    else if (rh->ept == 1) GS_RES_SMEM(1, 1024, 1, 1);
+    else GS_RES_SMEM(2, 1024, 1, 1);
+#undef GS_RES_SMEM
     if (rc != GS_OK) return rc;
     m->plan = GS_PLAN_RESIDENT;
     return GS_OK;
@@ -481,17 +522,27 @@ void resident_release(gs_model *m) {
     m->res_host = nullptr;
 }
 
+static ResAct res_act(const gs_model *m) {
+    ResAct ra = {m->d_act[0], m->d_gact[0], m->act_frames, m->act_stride, (size_t)m->E * m->hes[T_TET].cpad};
+    return ra;
+}
+
 int resident_rollout(gs_model *m, gs_tape *t, cudaStream_t st) {
     ResHost *rh = res_of(m);
     if (!rh) { set_error("resident plan unavailable"); return GS_ESTATE; }
     const dim3 grid(m->E), block(rh->rd.nthreads);
+    const ResAct ra = res_act(m);
+    const bool act = m->act_frames > 0;
     cudaEvent_t ta = m->timing ? timing_begin(m, st) : nullptr;
-    if (rh->ept == 1 && rh->rd.nthreads <= 320)
-        k_resident_fwd<1, 320, 3><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
-    else if (rh->ept == 1)
-        k_resident_fwd<1, 1024, 1><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
-    else
-        k_resident_fwd<2, 1024, 1><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T);
+#define GS_RES_FWD(E_, T_, B_)                                                                                                      \
+    do {                                                                                                                            \
+        if (act) k_resident_fwd<E_, T_, B_, true><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T, ra);      \
+        else k_resident_fwd<E_, T_, B_, false><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T, ra);         \
+    } while (0)
+    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_FWD(1, 320, 3);
+    else if (rh->ept == 1) GS_RES_FWD(1, 1024, 1);
+    else GS_RES_FWD(2, 1024, 1);
+#undef GS_RES_FWD
     GS_RES_CHECK("k_resident_fwd");
     if (ta) timing_end(m, GS_K_RESIDENT_FWD, ta, st);
     return GS_OK;
@@ -503,13 +554,18 @@ int resident_rollout_backward(gs_model *m, gs_tape *t, int n_frames, int frame_s
     const dim3 grid(m->E), block(rh->rd.nthreads);
     const float *fr = n_frames > 0 ? d_adj_x_frames : nullptr;
     const int stride = frame_stride > 0 ? frame_stride : 1;
+    const ResAct ra = res_act(m);
+    const bool act = m->act_frames > 0;
     cudaEvent_t ta = m->timing ? timing_begin(m, st) : nullptr;
-    if (rh->ept == 1 && rh->rd.nthreads <= 320)
-        k_resident_adj<1, 320, 2><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
-    else if (rh->ept == 1)
-        k_resident_adj<1, 1024, 1><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
-    else
-        k_resident_adj<2, 1024, 1><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride);
+#define GS_RES_ADJ(E_, T_, B_)                                                                                                                                   \
+    do {                                                                                                                                                         \
+        if (act) k_resident_adj<E_, T_, B_, true><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride, ra);  \
+        else k_resident_adj<E_, T_, B_, false><<<grid, block, rh->smem_adj, st>>>(m->dev, rh->rd, t->base, t->S, t->T, m->d_adjx, m->d_adjv, fr, n_frames, stride, ra);     \
+    } while (0)
+    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_ADJ(1, 320, 2);
+    else if (rh->ept == 1) GS_RES_ADJ(1, 1024, 1);
+    else GS_RES_ADJ(2, 1024, 1);
+#undef GS_RES_ADJ
     GS_RES_CHECK("k_resident_adj");
     if (ta) timing_end(m, GS_K_RESIDENT_ADJ, ta, st);
     return GS_OK;

@@ -198,11 +198,12 @@ struct ElemRegs {
     float4 c0, c1;
     float2 c2;
     float area, mu, lam, damp;
+    float act;  // this substep's actuation of the element (0 = passive)
 };
 
 // The persistent tile loop shared by the forward and adjoint kernels.  `compute(tv, tile, env, e_local)` evaluates one
 // element into the output slots; `emit(id, env, sums...)` is called once per tile-particle with its summed slots.
-template <int TYPE, bool ADJ>
+template <int TYPE, bool ADJ, bool ACT>
 struct TilePipe {
     using S = TileSmem<TYPE, ADJ>;
     const ElemDev &es;
@@ -213,9 +214,10 @@ struct TilePipe {
     float4 *out;
     uint64_t *bars;  // full[0..1], idfull[0..2]
     const float4 *x4, *v4, *a4;
+    const float *act;  // [E][cpad] actuation of this substep for this element type, or null
     uint64_t pol_stream, pol_keep;
-    __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_)
-        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_) {
+    __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_, const float *act_)
+        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_), act(act_) {
         idbuf = (int *)smem;
         locbuf = (uint16_t *)(smem + 3 * pmax * 4);
         bufs = smem + 3 * pmax * 4 + 2 * pmax * 2;
@@ -264,6 +266,7 @@ struct TilePipe {
             const float *q = es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems) + tid;
             er.mu = __ldcs(q); er.lam = __ldcs(q + kTileElems); er.damp = __ldcs(q + 2 * kTileElems);
         }
+        er.act = (ACT && TYPE != T_TRI) ? __ldcs(act + ((size_t)env * es.n_tiles + tile) * kTileElems + tid) : 0.0f;
     }
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
@@ -397,10 +400,11 @@ __device__ __forceinline__ void init_barriers(uint64_t *bars) {
     __syncthreads();
 }
 
-template <int TYPE>
-__device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
+template <int TYPE, bool ACT>
+__device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, float4 *__restrict__ f4) {
-    TilePipe<TYPE, false> pipe(md, smem, bars, x4, v4, nullptr);
+    const float *actp = TYPE == T_TET ? ad.tet : (TYPE == T_HINGE ? ad.hinge : nullptr);
+    TilePipe<TYPE, false, ACT> pipe(md, smem, bars, x4, v4, nullptr, actp);
     const int N = md.N;
     pipe.run(
         rot, md.tile_ctr + TYPE, next_slot,
@@ -414,7 +418,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
                 vec3 f[4];
-                tet_force(x, v, b, c2.y, er.mu, er.lam, er.damp, f);
+                tet_force(x, v, b, c2.y, er.mu, er.lam, er.damp, er.act, f);
 #pragma unroll
                 for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             } else if (TYPE == T_TRI) {
@@ -430,7 +434,9 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
                 const float4 c0 = er.c0;
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 vec3 f[4];
-                hinge_force(x, c0.x, c0.y, c0.z, f);
+                float sa = 0.0f, ca = 1.0f;
+                if (ACT) sincosf(er.act, &sa, &ca);
+                hinge_force(x, c0.x, c0.y, c0.z, sa, ca, f);
 #pragma unroll
                 for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             }
@@ -449,15 +455,16 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, char *smem, uint64
 
 // all element types of one substep in ONE persistent launch: a CTA walks its tets, then its triangles, then its
 // hinges (forces only meet in the global accumulator, so no grid-wide ordering is needed between the types)
-__global__ void __launch_bounds__(kTileElems) k_elements_fwd(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
+template <bool ACT>
+__global__ void __launch_bounds__(kTileElems) k_elements_fwd(const ModelDev md, const ActDev ad, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
                                                              float4 *__restrict__ f4) {
     extern __shared__ __align__(16) char smem[];
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_fwd<T_TET>(md, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_fwd<T_TRI>(md, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE>(md, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
+    if (md.es[T_TET].count) { tiles_fwd<T_TET, ACT>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_fwd<T_TRI, ACT>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE, ACT>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
 }
 
 // ------------------------------------------------------------------------------------------ forward particles
@@ -532,52 +539,58 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
             adjv[i] = make_float4(av.x, av.y, av.z, 0.f);
             adjf[i] = make_float4(af.x, af.y, af.z, 0.f);
         }
-        // per-environment totals (north_star (4): reduce with warp shuffles, then one reduction per value and warp into one
-        // of kConSlots fp64 slots): dL/dg = dt sum_i [w_i > 0] lv_i from every warp; dL/d(k_e, k_d, k_f, mu_c) from the warps
-        // that have a particle in contact.  The contact sums are sums of mixed-sign terms that cancel: they are
-        // shuffle-reduced in fp64.  Gravity terms are summed per warp in fp32 (32 terms) and accumulated in fp64.
-        const unsigned live = __ballot_sync(0xffffffffu, env >= 0);
+        // per-environment totals (north_star (4): reduce with warp shuffles): dL/d(k_e, k_d, k_f, mu_c) from the warps that
+        // have a particle in contact, and -- only when the model was asked for it (gs_request_grads: the extra reductions
+        // cost 12 % of this kernel on the 476k-particle scene) -- dL/dg = dt sum_i [w_i > 0] lv_i from every warp.  Warp sums
+        // in fp32 (32 terms), then one fp64 reduction per value and warp into one of kConSlots slots per environment.
+        const bool mine = gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f;
+        const unsigned act = __ballot_sync(0xffffffffu, mine);
+        const unsigned live = md.want_gravity ? __ballot_sync(0xffffffffu, env >= 0) : act;
         if (live) {
             const int env0 = __shfl_sync(0xffffffffu, env, __ffs(live) - 1);
             const bool uni = __all_sync(0xffffffffu, env < 0 || env == env0);  // false: the warp straddles two environments
-            const bool mine = gp[0] != 0.f || gp[1] != 0.f || gp[2] != 0.f || gp[3] != 0.f;
-            const unsigned act = __ballot_sync(0xffffffffu, mine);
             const int sl = blockIdx.x & (kConSlots - 1);
             if (uni) {
                 double *slot = md.gacc + ((size_t)env0 * kConSlots + sl) * kAccVals;
-#pragma unroll
-                for (int q = 0; q < 3; q++) {
-                    float t = gg[q];
-                    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                    if (lane == 0 && t != 0.f) red_add_f64(slot + 4 + q, (double)t);
-                }
                 if (act) {
 #pragma unroll
                     for (int q = 0; q < 4; q++) {
-                        double t = (double)gp[q];
+                        float t = gp[q];
                         for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                        if (lane == 0 && t != 0.0) red_add_f64(slot + q, t);
+                        if (lane == 0 && t != 0.f) red_add_f64(slot + q, (double)t);
+                    }
+                }
+                if (md.want_gravity) {
+#pragma unroll
+                    for (int q = 0; q < 3; q++) {
+                        float t = gg[q];
+                        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                        if (lane == 0 && t != 0.f) red_add_f64(slot + 4 + q, (double)t);
                     }
                 }
             } else if (env >= 0) {
                 double *slot = md.gacc + ((size_t)env * kConSlots + sl) * kAccVals;
 #pragma unroll
-                for (int q = 0; q < 3; q++)
-                    if (gg[q] != 0.f) red_add_f64(slot + 4 + q, (double)gg[q]);
-#pragma unroll
                 for (int q = 0; q < 4; q++)
                     if (gp[q] != 0.f) red_add_f64(slot + q, (double)gp[q]);
+                if (md.want_gravity) {
+#pragma unroll
+                    for (int q = 0; q < 3; q++)
+                        if (gg[q] != 0.f) red_add_f64(slot + 4 + q, (double)gg[q]);
+                }
             }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------ adjoint elements
-template <int TYPE>
-__device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
+template <int TYPE, bool ACT>
+__device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, const float4 *__restrict__ adjf, float4 *__restrict__ adjx,
                                           float4 *__restrict__ adjv) {
-    TilePipe<TYPE, true> pipe(md, smem, bars, x4, v4, adjf);
+    const float *actp = TYPE == T_TET ? ad.tet : (TYPE == T_HINGE ? ad.hinge : nullptr);
+    float *gactp = TYPE == T_TET ? ad.g_tet : (TYPE == T_HINGE ? ad.g_hinge : nullptr);
+    TilePipe<TYPE, true, ACT> pipe(md, smem, bars, x4, v4, adjf, actp);
     const int N = md.N;
     constexpr int PL = RecLayout<TYPE>::kArityT * kTileElems;  // second output plane: adj_v contributions
     const ElemDev &es = md.es[TYPE];
@@ -595,10 +608,11 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                 const vec3 v[4] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z]), vec3(tv.v[li.w])};
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4], av[4];
-                float gmu, glam, gk;
-                tet_adjoint(x, v, a, b, c2.y, er.mu, er.lam, er.damp, ax, av, gmu, glam, gk);
+                float gmu, glam, gk, ga;
+                tet_adjoint(x, v, a, b, c2.y, er.mu, er.lam, er.damp, er.act, ax, av, gmu, glam, gk, ga);
                 float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
                 red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
+                if (ACT) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
                     so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
@@ -625,9 +639,11 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4];
-                float gkb;
-                hinge_adjoint(x, a, c0.x, c0.y, c0.z, c0.w, ax, gkb);
+                float gkb, ga, sa = 0.0f, ca = 1.0f;
+                if (ACT) sincosf(er.act, &sa, &ca);
+                hinge_adjoint(x, a, c0.x, c0.y, c0.z, c0.w, sa, ca, ax, gkb, ga);
                 red_add_f32(es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid, gkb);
+                if (ACT) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
 #pragma unroll
                 for (int k = 0; k < 4; k++) so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
             }
@@ -646,15 +662,16 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, char *smem, uint64
         });
 }
 
-__global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
+template <bool ACT>
+__global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, const ActDev ad, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
                                                              const float4 *__restrict__ adjf, float4 *__restrict__ adjx, float4 *__restrict__ adjv) {
     extern __shared__ __align__(16) char smem[];
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_adj<T_TET>(md, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_adj<T_TRI>(md, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_adj<T_HINGE>(md, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
+    if (md.es[T_TET].count) { tiles_adj<T_TET, ACT>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_adj<T_TRI, ACT>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_adj<T_HINGE, ACT>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
 }
 
 // ------------------------------------------------------------------------------------------ layout conversion
@@ -788,8 +805,13 @@ int configure_stream_kernels(gs_model *m) {
     if (items == 0) return GS_OK;
     m->smem_fwd = fwd + kBarBytes;
     m->smem_adj = adj + kBarBytes;
-    int rc = tile_kernel_setup(k_elements_fwd, m->smem_fwd, &m->occ_fwd);
-    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj, m->smem_adj, &m->occ_adj);
+    // the actuated variants are set up first: the occupancy the launches use is that of the passive kernels, the actuated
+    // ones must fit the same grid (they use a few registers more; a persistent grid that is not co-resident is still correct)
+    int occ_a = 0;
+    int rc = tile_kernel_setup(k_elements_fwd<true>, m->smem_fwd, &occ_a);
+    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<true>, m->smem_adj, &occ_a);
+    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_fwd<false>, m->smem_fwd, &m->occ_fwd);
+    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<false>, m->smem_adj, &m->occ_adj);
     // Programmatic dependent launch pays where a kernel is a few microseconds long (20k tets, 157 tiles: -9 % per substep
     // pair): the next kernel's CTAs are resident and past their prologue when the predecessor drains.  It is neutral
     // from 350 to 650 tiles and costs beyond (250k tets +2.5 %, 490k tets +5 %): CTAs that launch into whatever slots
@@ -812,23 +834,77 @@ static inline int tile_grid(const gs_model *m, int occ) {
     return (int)(m->elem_items < cap ? m->elem_items : cap);
 }
 
+// substep < 0: a single-substep call (gs_step_forward / gs_step_backward): the activation frame is the model's current
+// one (gs_set_actuation_frame) and a non-finite state is reported as substep 0
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
-    if (m->elem_items > 0)
-        GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
-                 launch_pdl(m->pdl, k_elements_fwd, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, x, v, m->d_f));
-    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, substep));
+    const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
+    const int bad_idx = substep < 0 ? 0 : substep;
+    if (m->elem_items > 0) {
+        if (m->act_frames > 0)
+            GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
+                     launch_pdl(m->pdl, k_elements_fwd<true>, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
+        else
+            GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
+                     launch_pdl(m->pdl, k_elements_fwd<false>, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
+    }
+    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, bad_idx));
     return GS_OK;
 }
 
 // adjoint of the substep whose start state is (x, v) and whose end velocity is v_next; cotangents live in
 // m->d_adjx / m->d_adjv (updated in place); the frame cotangent at frame_off (caller order, < 0: none) is added to adj_x first.
-int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, cudaStream_t st) {
+int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, int substep, cudaStream_t st) {
+    const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
              launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
-    if (m->elem_items > 0)
-        GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                 launch_pdl(m->pdl, k_elements_adj, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+    if (m->elem_items > 0) {
+        if (m->act_frames > 0)
+            GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
+                     launch_pdl(m->pdl, k_elements_adj<true>, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+        else
+            GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
+                     launch_pdl(m->pdl, k_elements_adj<false>, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+    }
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
+    return GS_OK;
+}
+
+// activation schedules: caller order [F][E][count] <-> internal [F][E][cpad] (padding stays 0).  dir 0: ext -> internal
+// values; dir 1: internal gradients -> ext
+__global__ void k_actuation_io(float *__restrict__ internal, float *__restrict__ ext, const int *__restrict__ perm, int F, int E, int count, int cpad, int dir) {
+    const size_t total = (size_t)F * E * count;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t fe = i / count;
+        const int e = (int)(i - fe * count);
+        if (dir == 0) internal[fe * cpad + e] = ext[fe * count + perm[e]];
+        else ext[fe * count + perm[e]] = internal[fe * cpad + e];
+    }
+}
+// dL/d(theta0) = -1/2 sum_f dL/d(alpha_f): the rest angle enters sin((theta - theta0)/2 + alpha) as -theta0/2
+__global__ void k_theta0_grads(const float *__restrict__ gact, const int *__restrict__ perm, float *__restrict__ out, int F, int E, int count, int cpad) {
+    const size_t total = (size_t)E * count;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int env = (int)(i / count), e = (int)(i - (size_t)env * count);
+        double s = 0.0;
+        for (int f = 0; f < F; f++) s += (double)gact[((size_t)f * E + env) * cpad + e];
+        out[(size_t)env * count + perm[e]] = (float)(-0.5 * s);
+    }
+}
+// rest angles live in the hinge records as (sin(theta0/2), cos(theta0/2)) in c0.x, c0.y: row 0 of src
+__global__ void k_set_hinge_theta0(char *__restrict__ rec, int rec_bytes, const int *__restrict__ perm, const float *__restrict__ src, int count) {
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+        float4 *c0 = reinterpret_cast<float4 *>(rec + (size_t)(e / kTileElems) * rec_bytes + RecLayout<T_HINGE>::oC0) + (e % kTileElems);
+        const double h = 0.5 * (double)src[perm[e]];
+        c0->x = (float)sin(h); c0->y = (float)cos(h);
+    }
+}
+int launch_actuation_io(gs_model *m, int kind, const float *d_in, float *d_out, cudaStream_t st) {
+    const int t = kind == 0 ? T_TET : T_HINGE, c = m->counts[t];
+    if (c == 0) return GS_OK;
+    const size_t n = (size_t)m->act_frames * m->E * c;
+    if (d_in) k_actuation_io<<<grid_for(n), 256, 0, st>>>(m->d_act[kind], const_cast<float *>(d_in), m->dev.es[t].perm, m->act_frames, m->E, c, m->hes[t].cpad, 0);
+    else k_actuation_io<<<grid_for(n), 256, 0, st>>>(m->d_gact[kind], d_out, m->dev.es[t].perm, m->act_frames, m->E, c, m->hes[t].cpad, 1);
+    GS_LAUNCH_CHECK("k_actuation_io");
     return GS_OK;
 }
 
@@ -862,6 +938,12 @@ int launch_flush_grads(gs_model *m, cudaStream_t st) {
 }
 int launch_zero_grads(gs_model *m, cudaStream_t st) {
     m->steps_since_flush = 0;
+    for (int k = 0; k < 2; k++) {  // dL/d(activation) of every frame
+        const int t = k == 0 ? T_TET : T_HINGE;
+        if (m->act_frames <= 0 || !m->counts[t]) continue;
+        cudaError_t e = cudaMemsetAsync(m->d_gact[k], 0, sizeof(float) * (size_t)m->act_frames * m->E * m->hes[t].cpad, st);
+        if (e != cudaSuccess) return cuda_fail(e, "zero actuation gradients");
+    }
     for (int t = 0; t < N_TYPES; t++) {
         const size_t n = m->counts[t] ? kNumGrads[t] * (size_t)m->E * m->hes[t].cpad : 0;
         if (!n) continue;
@@ -880,6 +962,11 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
         k_get_contact<<<grid_for((size_t)m->E), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, group - GS_CONTACT_KE, 1);
     } else if (group == GS_GRAVITY) {
         k_get_contact<<<grid_for((size_t)m->E * 3), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, 4, 3);
+    } else if (group == GS_HINGE_THETA0) {
+        const int c = m->counts[T_HINGE];
+        if (c == 0) return GS_OK;
+        if (m->act_frames <= 0) { set_error("dL/d(theta0) is read from the hinge actuation gradients: attach an activation schedule first (gs_actuation_create; one zero frame is enough)"); return GS_ESTATE; }
+        k_theta0_grads<<<grid_for((size_t)m->E * c), 256, 0, st>>>(m->d_gact[1], m->dev.es[T_HINGE].perm, d_out, m->act_frames, m->E, c, m->hes[T_HINGE].cpad);
     } else {
         const int t = group == GS_HINGE_KB ? T_HINGE : group / 3, q = group == GS_HINGE_KB ? 0 : group % 3, c = m->counts[t];
         if (c == 0) return GS_OK;
@@ -906,6 +993,10 @@ int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_
     } else if (group >= GS_CONTACT_KE && group <= GS_CONTACT_MUC) {
         const float *dst[4] = {m->dev.ke, m->dev.kd, m->dev.kf, m->dev.muc};
         k_set_scalar<<<grid_for((size_t)m->E), 256, 0, st>>>(const_cast<float *>(dst[group - GS_CONTACT_KE]), d_values, m->E);
+    } else if (group == GS_HINGE_THETA0) {
+        const int c = m->counts[T_HINGE];
+        if (c == 0) return GS_OK;
+        k_set_hinge_theta0<<<grid_for((size_t)c), 256, 0, st>>>(const_cast<char *>(m->dev.es[T_HINGE].rec), m->dev.es[T_HINGE].rec_bytes, m->dev.es[T_HINGE].perm, d_values, c);
     } else if (group == GS_HINGE_KB) {
         const int c = m->counts[T_HINGE];
         if (c == 0) return GS_OK;

@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libgradsim.so")
 
 GS_OK, GS_EINVAL, GS_EMESH, GS_ENOMEM, GS_ECUDA, GS_ENONFINITE, GS_ESTATE = 0, -1, -2, -3, -4, -5, -6
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13}
+ACT_KINDS = {"tet": 0, "hinge": 1}
 GS_ELEM_PER_ENV, GS_MASS_PER_ENV, GS_CONTACT_PER_ENV = 1, 2, 4
 GS_PLAN_AUTO, GS_PLAN_STREAMING, GS_PLAN_RESIDENT = 0, 1, 2
 LOSS_KINDS = {"final_centroid": 0, "pos_mse_frames": 1, "centroid_traj": 2}
@@ -54,6 +55,11 @@ SIGNATURES = {
     "gs_model_plan": (_int, [_vp]),
     "gs_model_info": (_int, [_vp, _ip, _ip, _ip]),
     "gs_set_params": (_int, [_vp, _int, _vp, _vp]),
+    "gs_actuation_bytes": (_sz, [_vp, _int]),
+    "gs_actuation_create": (_int, [_vp, _int, _int, _vp, _sz, _vp]),
+    "gs_set_actuation": (_int, [_vp, _int, _vp, _vp]),
+    "gs_actuation_grads": (_int, [_vp, _int, _vp, _vp]),
+    "gs_set_actuation_frame": (_int, [_vp, _int]),
     "gs_step_forward": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "gs_step_backward": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "gs_tape_bytes": (_sz, [_vp, _int, _int]),
@@ -62,6 +68,7 @@ SIGNATURES = {
     "gs_rollout": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "gs_tape_read": (_int, [_vp, _vp, _int, _vp, _vp, _vp]),
     "gs_rollout_backward": (_int, [_vp, _vp, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "gs_request_grads": (_int, [_vp, _int, _int]),
     "gs_zero_grads": (_int, [_vp, _vp]),
     "gs_param_grads": (_int, [_vp, _int, _vp, _vp]),
     "gs_check_finite": (_int, [_vp, _vp, C.POINTER(_int)]),
@@ -232,6 +239,8 @@ class Model:
         self.n_elements = sum(self.counts.values())
         self.plan = L.gs_model_plan(self.h)
         self._scratch = None
+        self._act_mem, self.act_frames = None, 0
+        self._want_gravity = False
         del keep
 
     def __del__(self):
@@ -246,9 +255,9 @@ class Model:
         g = GROUPS[group] if isinstance(group, str) else int(group)
         if g == 12:
             return 3  # gravity: dL/dg per environment
-        if g >= 8:
+        if 8 <= g <= 11:
             return 1  # contact parameters: one value per environment
-        return self.N if g == 6 else (self.counts["hinge"] if g == 7 else (self.counts["tet"] if g < 3 else self.counts["tri"]))
+        return self.N if g == 6 else (self.counts["hinge"] if g in (7, 13) else (self.counts["tet"] if g < 3 else self.counts["tri"]))
 
     def new_state(self):
         return _torch().empty(self._shape(), dtype=_torch().float32, device=self.device)
@@ -269,6 +278,37 @@ class Model:
     def set_params(self, group, values):
         n = self.group_count(group)
         _check(lib().gs_set_params(self.h, GROUPS[group], _dp(_st(values, (self.E, n))), _stream()))
+
+    # ---- actuation inputs: a schedule of n_frames frames of frame_stride substeps
+    def actuation(self, n_frames, frame_stride=1):
+        """Attach an all-zero activation schedule (n_frames = 0 detaches).  The model keeps the torch block alive."""
+        L = lib()
+        if n_frames == 0:
+            _check(L.gs_actuation_create(self.h, 0, 1, None, 0, _stream()))
+            self._act_mem, self.act_frames = None, 0
+            return
+        nbytes = L.gs_actuation_bytes(self.h, int(n_frames))
+        mem = _aligned_bytes(nbytes, self.device)
+        _check(L.gs_actuation_create(self.h, int(n_frames), int(frame_stride), _dp(mem), nbytes, _stream()))
+        self._act_mem, self.act_frames = mem, int(n_frames)
+
+    def set_actuation(self, kind, values):
+        n = self.counts[kind]
+        _check(lib().gs_set_actuation(self.h, ACT_KINDS[kind], _dp(_st(values, (self.act_frames, self.E, n))), _stream()))
+
+    def actuation_grads(self, kind):
+        torch = _torch()
+        out = torch.zeros((self.act_frames, self.E, self.counts[kind]), dtype=torch.float32, device=self.device)
+        if out.numel():
+            _check(lib().gs_actuation_grads(self.h, ACT_KINDS[kind], _dp(out), _stream()))
+        return out
+
+    def set_actuation_frame(self, frame):
+        _check(lib().gs_set_actuation_frame(self.h, int(frame)))
+
+    def request_grads(self, group, enable=True):
+        _check(lib().gs_request_grads(self.h, GROUPS[group], int(bool(enable))))
+        self._want_gravity = bool(enable)
 
     def zero_grads(self):
         _check(lib().gs_zero_grads(self.h, _stream()))

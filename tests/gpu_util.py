@@ -29,9 +29,17 @@ def gpu_run_scene(sc, target, K=None, plan=gs.GS_PLAN_AUTO, model=None):
     """rollout + loss + backward on the GPU.  target: as oracle.truth_targets(sc) returns
     (final_centroid [E,3]; pos_mse_frames [n_t,E,N,3]; centroid_traj [n_t,E,3]), fp64 numpy."""
     m = gs.Model(sc, plan=plan) if model is None else model
+    m.request_grads("gravity")  # off by default (gradsim.h, GS_GRAVITY)
     K = sc.checkpoint_every if K is None else K
     T, s = sc.n_substeps, sc.frame_stride
     tape = m.tape(T, K)
+    act = getattr(sc, "act", None)  # optional activation schedule: dict(stride=, tet=[F,E,M] or None, hinge=[F,E,Mh] or None)
+    if act:
+        F = next(a.shape[0] for a in (act.get("tet"), act.get("hinge")) if a is not None)
+        m.actuation(F, act["stride"])
+        for kind in ("tet", "hinge"):
+            if act.get(kind) is not None:
+                m.set_actuation(kind, dev(act[kind]))
     m.zero_grads()
     xT, vT = tape.rollout(dev(sc.x0), dev(sc.v0))
     lt = sc.loss_times()
@@ -66,6 +74,10 @@ def gpu_run_scene(sc, target, K=None, plan=gs.GS_PLAN_AUTO, model=None):
     out.update(xT=host(xT), vT=host(vT), loss=host(loss), adj_x0=host(ax0), adj_v0=host(av0), bad=bad,
                rec_x=np.stack([host(r) for r in rec]))
     for g in gs.GROUPS:
+        if g == "hinge_theta0" and not m.act_frames:
+            continue  # read from the hinge actuation gradients: needs a schedule (gradsim.h, GS_HINGE_THETA0)
         out["g_" + g] = host(m.param_grads(g))
+    if act:
+        out["g_act_tet"], out["g_act_hinge"] = host(m.actuation_grads("tet")), host(m.actuation_grads("hinge"))
     out["model"] = m
     return out
