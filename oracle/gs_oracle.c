@@ -23,6 +23,7 @@
  *                               "triangular structure ... computed explicitly")
  *   rollout, rollout_backward   PAPER.md:613 (reverse mode stores the input state of every step);
  *                               checkpoint + replay per BASELINE.json configs[2]
+ *   aero_force / aero_adjoint   PAPER.md:586 (lift / drag of the air on the cloth faces); reading A21
  *   actuation inputs            PAPER.md:579 (per-tet alpha of (J - alpha)^2), 585-586 (per-edge alpha of sin(phi/2 + alpha)),
  *                               777 (App. E: activations produced in time by a controller); SURVEY.md 8(f) NEXT-1
  * Readings A1..A20 are listed in DESIGN.md ("Readings of the paper").
@@ -52,6 +53,11 @@ typedef struct {
     double *hinge_theta0, *hinge_l0, *hinge_kb; /* [Mh] */
     double g[3], dt, n[3], d, r;
     double *ke, *kd, *kf, *mu_c; /* [E] */
+    /* lift / drag of the surrounding air on the cloth triangles ("We also include a lift/drag model that
+       approximates the effect of the surrounding air on the surface of mesh"; reading A21: the paper gives no formula) */
+    double *k_drag, *k_lift;     /* [E], 0 = none */
+    double wind[3];              /* velocity of the air */
+    double *g_kdrag, *g_klift;   /* [E] dL/dk_drag, dL/dk_lift */
     /* incident lists: for particle i, entries inc_ptr[i]..inc_ptr[i+1] of inc_slot index
        the per-element-vertex slot arrays (tets: 4 slots, then tris: 3, then hinges: 4) */
     int *inc_ptr, *inc_slot;
@@ -148,7 +154,7 @@ void orc_destroy(orc_model *m) {
     free(m->inc_ptr); free(m->inc_slot);
     free(m->g_tet_mu); free(m->g_tet_lambda); free(m->g_tet_damp);
     free(m->g_tri_mu); free(m->g_tri_lambda); free(m->g_tri_damp); free(m->g_mass); free(m->g_hinge_kb); free(m->g_ke); free(m->g_kd); free(m->g_kf); free(m->g_muc);
-    free(m->g_gravity); free(m->g_con_abs);
+    free(m->g_gravity); free(m->g_con_abs); free(m->k_drag); free(m->k_lift); free(m->g_kdrag); free(m->g_klift);
     free(m->tet_act); free(m->hinge_act); free(m->g_tet_act); free(m->g_hinge_act); free(m->sched_tet); free(m->sched_hinge);
     free(m->g_sched_tet); free(m->g_sched_hinge); free(m->g_hinge_theta0);
     free(m);
@@ -212,6 +218,7 @@ orc_model *orc_create(int N, int M, int Mt, int Mh, int E, const double *x_rest,
     m->g_hinge_kb = zeros_d((size_t)E * Mh);
     m->g_ke = zeros_d((size_t)E); m->g_kd = zeros_d((size_t)E); m->g_kf = zeros_d((size_t)E); m->g_muc = zeros_d((size_t)E);
     m->g_gravity = zeros_d((size_t)E * 3); m->g_con_abs = zeros_d((size_t)E * 4);
+    m->k_drag = zeros_d(E); m->k_lift = zeros_d(E); m->g_kdrag = zeros_d(E); m->g_klift = zeros_d(E);
     m->tet_act = zeros_d((size_t)E * M); m->hinge_act = zeros_d((size_t)E * Mh);
     m->g_tet_act = zeros_d((size_t)E * M); m->g_hinge_act = zeros_d((size_t)E * Mh); m->g_hinge_theta0 = zeros_d((size_t)E * Mh);
 
@@ -291,6 +298,9 @@ int orc_set_params(orc_model *m, int group, const double *v) {
     }
     if (group == 12) { m->g[0] = v[0]; m->g[1] = v[1]; m->g[2] = v[2]; return 0; } /* gravity: one vector for all environments */
     if (group == 13) { memcpy(m->hinge_theta0, v, sizeof(double) * m->Mh); return 0; } /* rest angles: one array for all environments */
+    if (group == 14) { memcpy(m->k_drag, v, sizeof(double) * m->E); return 0; }        /* one value per environment */
+    if (group == 15) { memcpy(m->k_lift, v, sizeof(double) * m->E); return 0; }
+    if (group == 16) { m->wind[0] = v[0]; m->wind[1] = v[1]; m->wind[2] = v[2]; return 0; } /* one vector for all environments; no gradient */
     if (group < 0 || group > 6) return -1;
     memcpy(dst[group], v, sizeof(double) * n[group] * m->E);
     return 0;
@@ -305,6 +315,8 @@ int orc_get_grads(const orc_model *m, int group, double *out) {
     }
     if (group == 12) { memcpy(out, m->g_gravity, sizeof(double) * 3 * m->E); return 0; } /* [E][3] */
     if (group == 13) { memcpy(out, m->g_hinge_theta0, sizeof(double) * m->Mh * m->E); return 0; } /* [E][Mh] */
+    if (group == 14) { memcpy(out, m->g_kdrag, sizeof(double) * m->E); return 0; }
+    if (group == 15) { memcpy(out, m->g_klift, sizeof(double) * m->E); return 0; }
     if (group == 100) { memcpy(out, m->g_con_abs, sizeof(double) * 4 * m->E); return 0; } /* [E][4] diagnostic */
     if (group < 0 || group > 7) return -1;
     memcpy(out, src[group], sizeof(double) * n[group] * m->E);
@@ -318,6 +330,7 @@ void orc_zero_grads(orc_model *m) {
     memset(m->g_hinge_kb, 0, sizeof(double) * E * m->Mh);
     memset(m->g_ke, 0, sizeof(double) * E); memset(m->g_kd, 0, sizeof(double) * E); memset(m->g_kf, 0, sizeof(double) * E); memset(m->g_muc, 0, sizeof(double) * E);
     memset(m->g_gravity, 0, sizeof(double) * E * 3); memset(m->g_con_abs, 0, sizeof(double) * E * 4);
+    memset(m->g_kdrag, 0, sizeof(double) * E); memset(m->g_klift, 0, sizeof(double) * E);
     memset(m->g_tet_act, 0, sizeof(double) * E * m->M); memset(m->g_hinge_act, 0, sizeof(double) * E * m->Mh);
     memset(m->g_hinge_theta0, 0, sizeof(double) * E * m->Mh);
     if (m->g_sched_tet) memset(m->g_sched_tet, 0, sizeof(double) * m->act_frames * E * m->M);
@@ -492,6 +505,51 @@ static void tri_adjoint(const double *x[3], const double *v[3], const double *a[
     }
 }
 
+/* ---------------------------------------------------------------- lift / drag on triangles (reading A21) */
+/* Thin-plate model, quadratic in the speed: with c = (x1-x0) x (x2-x0), area A = |c|/2, unit normal n = c/|c|, relative
+   velocity vb = (v0+v1+v2)/3 - wind, s = sqrt(|vb|^2 + eps^2) (eps = 1e-6 m/s keeps the model smooth at rest), v_n = n.vb:
+       F = -A s (k_drag vb + k_lift v_n n)
+   an isotropic drag plus a pressure term along the face normal (the part of it perpendicular to the flow is the lift of an
+   inclined face); F is shared equally by the three vertices.  Dissipative: F.vb = -A s (k_drag |vb|^2 + k_lift v_n^2) <= 0. */
+#define ORC_AERO_EPS 1e-6
+static void aero_force(const double *x[3], const double *v[3], const double *wind, double kdrag, double klift, double f[3][3]) {
+    double e1[3], e2[3], c[3], vb[3];
+    v_sub(x[1], x[0], e1); v_sub(x[2], x[0], e2); v_cross(e1, e2, c);
+    double L = sqrt(v_dot(c, c));
+    for (int r = 0; r < 3; r++) vb[r] = (v[0][r] + v[1][r] + v[2][r]) / 3.0 - wind[r];
+    double s = sqrt(v_dot(vb, vb) + ORC_AERO_EPS * ORC_AERO_EPS), A = 0.5 * L, vn = v_dot(c, vb) / L;
+    for (int r = 0; r < 3; r++) {
+        double F = -A * s * (kdrag * vb[r] + klift * vn * c[r] / L);
+        f[0][r] = f[1][r] = f[2][r] = F / 3.0;
+    }
+}
+/* VJP: a_k = dL/df_k.  Adds to ax, av and to the parameter gradients.  With ab = (a0+a1+a2)/3, L = |c|, u = c.vb,
+   P = k_drag L vb + k_lift u c / L (F = -s P / 2):
+     dL/dvb = -(ab.P)/(2 s) vb - (s/2) k_drag L ab - (s/2) k_lift (ab.c)/L c                       (shared: each dL/dv_k gets a third)
+     dL/dc  = -(s/2) k_drag (ab.vb) n - (s/2) k_lift [ (ab.c)/L vb + (u/L) ab - u (ab.c)/L^2 n ]
+     dL/de1 = e2 x dL/dc, dL/de2 = dL/dc x e1 */
+static void aero_adjoint(const double *x[3], const double *v[3], const double *a[3], const double *wind, double kdrag, double klift,
+                         double ax[3][3], double av[3][3], double *g_kdrag, double *g_klift) {
+    double e1[3], e2[3], c[3], vb[3], ab[3], n[3], P[3], gv[3], gc[3], t1[3], t2[3];
+    v_sub(x[1], x[0], e1); v_sub(x[2], x[0], e2); v_cross(e1, e2, c);
+    double L = sqrt(v_dot(c, c));
+    for (int r = 0; r < 3; r++) { vb[r] = (v[0][r] + v[1][r] + v[2][r]) / 3.0 - wind[r]; ab[r] = (a[0][r] + a[1][r] + a[2][r]) / 3.0; n[r] = c[r] / L; }
+    double s = sqrt(v_dot(vb, vb) + ORC_AERO_EPS * ORC_AERO_EPS), u = v_dot(c, vb), ac = v_dot(ab, c), avb = v_dot(ab, vb);
+    for (int r = 0; r < 3; r++) P[r] = kdrag * L * vb[r] + klift * u * c[r] / L;
+    double aP = v_dot(ab, P);
+    *g_kdrag += -0.5 * s * L * avb;
+    *g_klift += -0.5 * s * u * ac / L;
+    for (int r = 0; r < 3; r++) {
+        gv[r] = -0.5 * aP / s * vb[r] - 0.5 * s * kdrag * L * ab[r] - 0.5 * s * klift * ac / L * c[r];
+        gc[r] = -0.5 * s * kdrag * avb * n[r] - 0.5 * s * klift * (ac / L * vb[r] + u / L * ab[r] - u * ac / (L * L) * n[r]);
+    }
+    v_cross(e2, gc, t1); v_cross(gc, e1, t2);
+    for (int r = 0; r < 3; r++) {
+        ax[1][r] += t1[r]; ax[2][r] += t2[r]; ax[0][r] -= t1[r] + t2[r];
+        av[0][r] += gv[r] / 3.0; av[1][r] += gv[r] / 3.0; av[2][r] += gv[r] / 3.0;
+    }
+}
+
 /* ---------------------------------------------------------------- hinges (A5, A6) */
 /* E_b = 2 k_b l0 (1 - cos((theta - theta0)/2)),  f_i = k_b l0 sin((theta - theta0)/2) d_i */
 static double hinge_energy(const double *x[4], double theta0, double l0, double kb, double act) {
@@ -622,6 +680,11 @@ static void env_forces(const orc_model *m, int env, const double *x, const doubl
             for (int k = 0; k < 3; k++) { xe[k] = x + 3 * t[k]; ve[k] = v + 3 * t[k]; }
             double fe[3][3];
             tri_force(xe, ve, m->tri_B + 4 * e, m->tri_A[e], m->tri_mu[(size_t)env * Mt + e], m->tri_lambda[(size_t)env * Mt + e], m->tri_damp[(size_t)env * Mt + e], fe);
+            if (m->k_drag[env] != 0.0 || m->k_lift[env] != 0.0) { /* lift / drag of the air on this face */
+                double fa[3][3];
+                aero_force(xe, ve, m->wind, m->k_drag[env], m->k_lift[env], fa);
+                for (int k = 0; k < 3; k++) v_axpy(1.0, fa[k], fe[k]);
+            }
             memcpy(slots + 3 * (4 * (size_t)M + 3 * (size_t)e), fe, sizeof fe);
         }
     }
@@ -760,6 +823,8 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         memcpy(slots + 3 * (4 * (size_t)e), cx, sizeof cx);
         memcpy(slots_v + 3 * (4 * (size_t)e), cv, sizeof cv);
     }
+    const int aero = m->k_drag[env] != 0.0 || m->k_lift[env] != 0.0;
+    double *gaero = aero ? zeros_d(2 * (size_t)Mt) : NULL; /* per-triangle terms of dL/dk_drag, dL/dk_lift, summed in element order below */
 #pragma omp parallel for if (par) schedule(static)
     for (int e = 0; e < Mt; e++) {
         const int *t = m->tris + 3 * e;
@@ -769,8 +834,13 @@ static void env_step_adjoint(orc_model *m, int env, const double *x, const doubl
         size_t pe = (size_t)env * Mt + e;
         tri_adjoint(xe, ve, ae, m->tri_B + 4 * e, m->tri_A[e], m->tri_mu[pe], m->tri_lambda[pe], m->tri_damp[pe], cx, cv,
                     &m->g_tri_mu[pe], &m->g_tri_lambda[pe], &m->g_tri_damp[pe]);
+        if (aero) aero_adjoint(xe, ve, ae, m->wind, m->k_drag[env], m->k_lift[env], cx, cv, &gaero[2 * (size_t)e], &gaero[2 * (size_t)e + 1]);
         memcpy(slots + 3 * (4 * (size_t)M + 3 * (size_t)e), cx, sizeof cx);
         memcpy(slots_v + 3 * (4 * (size_t)M + 3 * (size_t)e), cv, sizeof cv);
+    }
+    if (aero) {
+        for (int e = 0; e < Mt; e++) { m->g_kdrag[env] += gaero[2 * (size_t)e]; m->g_klift[env] += gaero[2 * (size_t)e + 1]; }
+        free(gaero);
     }
 #pragma omp parallel for if (par) schedule(static)
     for (int e = 0; e < Mh; e++) {

@@ -24,7 +24,7 @@ _LIB = os.path.join(_HERE, "libgs_oracle.so")
 
 TETS, TRIS, HINGES, CONTACT, ALL = 1, 2, 4, 8, 15
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13, "k_drag": 14, "k_lift": 15}
 
 
 def build(force: bool = False) -> str:
@@ -95,6 +95,13 @@ class Oracle:
             raise ValueError("oracle: invalid mesh: " + L.orc_last_error().decode())
         self.h = C.c_void_p(h)
         self.dt = float(sc.dt)
+        # lift / drag of the air (reading A21): optional scene attributes, zero when absent
+        for g, code in (("k_drag", 14), ("k_lift", 15)):
+            val = getattr(sc, g, None)
+            if val is not None:
+                assert L.orc_set_params(self.h, C.c_int(code), _p(_d(np.broadcast_to(_d(val).ravel(), (E,))))) == 0
+        if getattr(sc, "wind", None) is not None:
+            assert L.orc_set_params(self.h, C.c_int(16), _p(_d(sc.wind))) == 0
 
     def __del__(self):
         if getattr(self, "h", None) is not None and _lib is not None:

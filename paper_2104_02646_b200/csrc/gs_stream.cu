@@ -203,7 +203,9 @@ struct ElemRegs {
 
 // The persistent tile loop shared by the forward and adjoint kernels.  `compute(tv, tile, env, e_local)` evaluates one
 // element into the output slots; `emit(id, env, sums...)` is called once per tile-particle with its summed slots.
-template <int TYPE, bool ADJ, bool ACT>
+// ME: the model has more than one environment (work item = tile x environment).  The single-environment kernels (the large
+// meshes) carry none of the item -> (tile, env) divisions and environment offsets.
+template <int TYPE, bool ADJ, bool ACT, bool ME>
 struct TilePipe {
     using S = TileSmem<TYPE, ADJ>;
     const ElemDev &es;
@@ -227,7 +229,7 @@ struct TilePipe {
     }
     // work item -> (tile, env); single-environment models (the large meshes) skip the division
     __device__ __forceinline__ void split(int item, unsigned &tile, unsigned &env) const {
-        if (E == 1) { tile = (unsigned)item; env = 0u; }
+        if (!ME) { tile = (unsigned)item; env = 0u; }
         else { env = (unsigned)item / (unsigned)es.n_tiles; tile = (unsigned)item - env * (unsigned)es.n_tiles; }
     }
     // ids of the CTA's j-th item go to id buffer `slot` = j % 3, its staging indices to loc buffer `par` = j % 2
@@ -345,6 +347,8 @@ struct TilePipe {
         const bool queue = kQueue && 2 * G < n_items;  // otherwise the static items cover everything
         int item = first, item_n = first + G;  // items i, i+1 (all threads)
         int claimed = n_items;                 // kQueue: item i+2, thread 0 only until published through next_slot
+        int ticket = -1;                       // raw result of the queue's atomicAdd for item i+3 (< 0: none): converted one
+                                               // iteration later, so that the atomic's round trip is not waited on
         if (tid == 0) {
             load_ids(first, 0, 0);
             if (item_n < n_items) load_ids(item_n, 1, 1);
@@ -393,18 +397,18 @@ struct TilePipe {
 constexpr int kBarBytes = 128;  // 15 mbarriers at the start of shared memory (5 per element type) + the queue hand-over slot
 
 __device__ __forceinline__ void init_barriers(uint64_t *bars) {
-    if (threadIdx.x == 0) {
-        for (int k = 0; k < 15; k++) mbar_init(bars + k, 1);
+    if (threadIdx.x < 15) {  // one barrier per lane of the first warp: one instruction instead of 15 in a row
+        mbar_init(bars + threadIdx.x, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 }
 
-template <int TYPE, bool ACT>
+template <int TYPE, bool ACT, bool ME>
 __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, float4 *__restrict__ f4) {
     const float *actp = TYPE == T_TET ? ad.tet : (TYPE == T_HINGE ? ad.hinge : nullptr);
-    TilePipe<TYPE, false, ACT> pipe(md, smem, bars, x4, v4, nullptr, actp);
+    TilePipe<TYPE, false, ACT, ME> pipe(md, smem, bars, x4, v4, nullptr, actp);
     const int N = md.N;
     pipe.run(
         rot, md.tile_ctr + TYPE, next_slot,
@@ -455,16 +459,16 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
 
 // all element types of one substep in ONE persistent launch: a CTA walks its tets, then its triangles, then its
 // hinges (forces only meet in the global accumulator, so no grid-wide ordering is needed between the types)
-template <bool ACT>
-__global__ void __launch_bounds__(kTileElems) k_elements_fwd(const ModelDev md, const ActDev ad, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
+template <bool ACT, bool ME>
+__global__ void __launch_bounds__(kTileElems, 9) k_elements_fwd(const ModelDev md, const ActDev ad, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
                                                              float4 *__restrict__ f4) {
     extern __shared__ __align__(16) char smem[];
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_fwd<T_TET, ACT>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_fwd<T_TRI, ACT>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE, ACT>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
+    if (md.es[T_TET].count) { tiles_fwd<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_fwd<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_fwd<T_HINGE, ACT, ME>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
 }
 
 // ------------------------------------------------------------------------------------------ forward particles
@@ -584,13 +588,13 @@ __global__ void __launch_bounds__(256) k_particles_adj(const ModelDev md, const 
 }
 
 // ------------------------------------------------------------------------------------------ adjoint elements
-template <int TYPE, bool ACT>
+template <int TYPE, bool ACT, bool ME>
 __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, char *smem, uint64_t *bars, int *next_slot, int rot, const float4 *__restrict__ x4,
                                           const float4 *__restrict__ v4, const float4 *__restrict__ adjf, float4 *__restrict__ adjx,
                                           float4 *__restrict__ adjv) {
     const float *actp = TYPE == T_TET ? ad.tet : (TYPE == T_HINGE ? ad.hinge : nullptr);
     float *gactp = TYPE == T_TET ? ad.g_tet : (TYPE == T_HINGE ? ad.g_hinge : nullptr);
-    TilePipe<TYPE, true, ACT> pipe(md, smem, bars, x4, v4, adjf, actp);
+    TilePipe<TYPE, true, ACT, ME> pipe(md, smem, bars, x4, v4, adjf, actp);
     const int N = md.N;
     constexpr int PL = RecLayout<TYPE>::kArityT * kTileElems;  // second output plane: adj_v contributions
     const ElemDev &es = md.es[TYPE];
@@ -662,16 +666,16 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
         });
 }
 
-template <bool ACT>
+template <bool ACT, bool ME>
 __global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, const ActDev ad, const float4 *__restrict__ x4, const float4 *__restrict__ v4,
                                                              const float4 *__restrict__ adjf, float4 *__restrict__ adjx, float4 *__restrict__ adjv) {
     extern __shared__ __align__(16) char smem[];
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_adj<T_TET, ACT>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_adj<T_TRI, ACT>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_HINGE].count) tiles_adj<T_HINGE, ACT>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
+    if (md.es[T_TET].count) { tiles_adj<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_adj<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_HINGE].count) tiles_adj<T_HINGE, ACT, ME>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
 }
 
 // ------------------------------------------------------------------------------------------ layout conversion
@@ -808,10 +812,18 @@ int configure_stream_kernels(gs_model *m) {
     // the actuated variants are set up first: the occupancy the launches use is that of the passive kernels, the actuated
     // ones must fit the same grid (they use a few registers more; a persistent grid that is not co-resident is still correct)
     int occ_a = 0;
-    int rc = tile_kernel_setup(k_elements_fwd<true>, m->smem_fwd, &occ_a);
-    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<true>, m->smem_adj, &occ_a);
-    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_fwd<false>, m->smem_fwd, &m->occ_fwd);
-    if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<false>, m->smem_adj, &m->occ_adj);
+    int rc = GS_OK;
+    if (m->E > 1) {
+        rc = tile_kernel_setup(k_elements_fwd<true, true>, m->smem_fwd, &occ_a);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<true, true>, m->smem_adj, &occ_a);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_fwd<false, true>, m->smem_fwd, &m->occ_fwd);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<false, true>, m->smem_adj, &m->occ_adj);
+    } else {
+        rc = tile_kernel_setup(k_elements_fwd<true, false>, m->smem_fwd, &occ_a);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<true, false>, m->smem_adj, &occ_a);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_fwd<false, false>, m->smem_fwd, &m->occ_fwd);
+        if (rc == GS_OK) rc = tile_kernel_setup(k_elements_adj<false, false>, m->smem_adj, &m->occ_adj);
+    }
     // Programmatic dependent launch pays where a kernel is a few microseconds long (20k tets, 157 tiles: -9 % per substep
     // pair): the next kernel's CTAs are resident and past their prologue when the predecessor drains.  It is neutral
     // from 350 to 650 tiles and costs beyond (250k tets +2.5 %, 490k tets +5 %): CTAs that launch into whatever slots
@@ -840,12 +852,9 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
     const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     const int bad_idx = substep < 0 ? 0 : substep;
     if (m->elem_items > 0) {
-        if (m->act_frames > 0)
-            GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
-                     launch_pdl(m->pdl, k_elements_fwd<true>, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
-        else
-            GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd",
-                     launch_pdl(m->pdl, k_elements_fwd<false>, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
+        const bool act = m->act_frames > 0, me = m->E > 1;
+        auto kern = act ? (me ? k_elements_fwd<true, true> : k_elements_fwd<true, false>) : (me ? k_elements_fwd<false, true> : k_elements_fwd<false, false>);
+        GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", launch_pdl(m->pdl, kern, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
     }
     GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, bad_idx));
     return GS_OK;
@@ -858,12 +867,10 @@ int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const flo
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
              launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0) {
-        if (m->act_frames > 0)
-            GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                     launch_pdl(m->pdl, k_elements_adj<true>, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
-        else
-            GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
-                     launch_pdl(m->pdl, k_elements_adj<false>, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+        const bool act = m->act_frames > 0, me = m->E > 1;
+        auto kern = act ? (me ? k_elements_adj<true, true> : k_elements_adj<true, false>) : (me ? k_elements_adj<false, true> : k_elements_adj<false, false>);
+        GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
+                 launch_pdl(m->pdl, kern, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
     }
     if (++m->steps_since_flush >= kFlushEvery) return launch_flush_grads(m, st);
     return GS_OK;

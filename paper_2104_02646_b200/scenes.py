@@ -152,6 +152,16 @@ class Scene:
     loss: str = "final_centroid"  # | "pos_mse_frames" | "centroid_traj"
     target: Optional[np.ndarray] = None  # final_centroid: [E,3]
     truth: dict = field(default_factory=dict)  # truth-stream parameters (configs 2, 3)
+    k_drag: Optional[np.ndarray] = None  # [E] lift / drag of the air on the cloth faces (A21); None = zeros
+    k_lift: Optional[np.ndarray] = None  # [E]
+    wind: tuple = (0.0, 0.0, 0.0)
+    act: Optional[dict] = None  # activation schedule: dict(stride=, tet=[F,E,M] or None, hinge=[F,E,Mh] or None)
+
+    def __post_init__(self):
+        if self.k_drag is None:
+            self.k_drag = np.zeros(self.n_envs, np.float32)
+        if self.k_lift is None:
+            self.k_lift = np.zeros(self.n_envs, np.float32)
 
     @property
     def n_particles(self):
@@ -448,7 +458,7 @@ def perturbed_state(sc: Scene, amp_x=0.1, amp_v=0.5, seed=0):
 def custom_scene(x, tets=None, tris=None, hinges=None, n_envs=1, mass=0.1, mu=1e4, lam=1e4, damp=1.0,
                  tri_mu=1e3, tri_lam=1e3, tri_damp=1.0, kb=10.0, pinned=None, v0=None, x0=None, gravity=(0.0, -9.8, 0.0),
                  dt=1.0 / 1920.0, ke=1e4, kd=10.0, kf=50.0, mu_c=0.5, n_substeps=1, checkpoint_every=1,
-                 plane_n=(0.0, 1.0, 0.0), plane_d=0.0, radius=0.0, name="custom", config=9):
+                 plane_n=(0.0, 1.0, 0.0), plane_d=0.0, radius=0.0, name="custom", config=9, k_drag=0.0, k_lift=0.0, wind=(0.0, 0.0, 0.0)):
     """Free-form scene for unit tests.  Scalars broadcast; arrays are taken as given ([E,n] or [n])."""
     x = _f32(x)
     N, E = x.shape[0], n_envs
@@ -478,6 +488,7 @@ def custom_scene(x, tets=None, tris=None, hinges=None, n_envs=1, mass=0.1, mu=1e
         hinges=hinges, hinge_kb=_f32(np.broadcast_to(np.asarray(kb, np.float64).ravel(), (Mh,))),
         ke=e1(ke), kd=e1(kd), kf=e1(kf), mu_c=e1(mu_c), gravity=tuple(gravity), dt=dt, plane_n=tuple(plane_n),
         plane_d=plane_d, radius=radius, n_substeps=n_substeps, checkpoint_every=checkpoint_every,
+        k_drag=e1(k_drag), k_lift=e1(k_lift), wind=tuple(wind),
     )
     sc.target = _final_centroid_target(config, sc.x0)
     return sc

@@ -13,7 +13,7 @@ import copy
 import numpy as np
 
 # per-environment arrays of a scene (leading axis E)
-_ENV_FIELDS = ("x0", "v0", "mass", "tet_mu", "tet_lambda", "tet_damp", "tri_mu", "tri_lambda", "tri_damp", "ke", "kd", "kf", "mu_c")
+_ENV_FIELDS = ("x0", "v0", "mass", "tet_mu", "tet_lambda", "tet_damp", "tri_mu", "tri_lambda", "tri_damp", "ke", "kd", "kf", "mu_c", "k_drag", "k_lift")
 
 
 def env_block(n_envs: int, world: int, rank: int) -> tuple[int, int]:

@@ -39,9 +39,10 @@ def _rot(rng):
 
 
 def _free(sc):
-    """no gravity, contact plane far away"""
+    """no gravity, contact plane far away, no air"""
     sc.gravity = (0.0, 0.0, 0.0)
     sc.plane_d = -1e6
+    sc.k_drag, sc.k_lift = 0 * sc.k_drag, 0 * sc.k_lift
     return sc
 
 
@@ -56,12 +57,13 @@ def _mixed_scene(rng, **kw):
         mass=rng.uniform(0.05, 0.2, x.shape[0]), mu=rng.uniform(5e3, 2e4, M), lam=rng.uniform(5e3, 2e4, M),
         damp=rng.uniform(0.5, 2.0, M), tri_mu=rng.uniform(5e2, 2e3, Mt), tri_lam=rng.uniform(5e2, 2e3, Mt),
         tri_damp=rng.uniform(0.5, 2.0, Mt), kb=rng.uniform(5, 20, hinges.shape[0]),
+        k_drag=0.3, k_lift=0.2, wind=(0.5, -0.2, 0.3),  # lift / drag of the air on the cloth patch (reading A21)
     )
     args.update(kw)
     return scenes.custom_scene(x, tets=tets, tris=tris + n0, hinges=hinges + n0, **args)
 
 
-SCALAR_GROUPS = ("ke", "kd", "kf", "mu_c")  # one value per environment
+SCALAR_GROUPS = ("ke", "kd", "kf", "mu_c", "k_drag", "k_lift")  # one value per environment
 ABS_STEP = ("gravity", "hinge_theta0")       # parameters whose value may be 0: absolute FD steps
 
 
@@ -352,7 +354,10 @@ def test_p7_step_param_gradients_vs_fd(group):
         # one substep is piecewise LINEAR in the contact parameters (within a friction regime), so their central
         # difference is exact for any step that keeps the regimes; a larger step keeps round-off out of the tiny
         # stick-friction terms
-        h = (1e-3 if scalar else 1e-6) * (base[e] if group not in ABS_STEP else 1.0)
+        # (the substep is also exactly affine in mu, lambda, k_damp, k_b -- the stress is linear in them -- so the larger
+        # step is exact for those groups too and keeps round-off of the O(1) functional out of their small gradients)
+        affine = scalar or group.startswith(("tet_", "tri_")) or group == "hinge_kb"
+        h = (1e-3 if affine else 1e-6) * (base[e] if group not in ABS_STEP else 1.0)
         vals = []
         for s in (+1, -1):
             p = base.copy(); p[e] += s * h
@@ -604,7 +609,9 @@ def test_p8_smooth_regime_strict():
             if g == "mass" and sc.pinned[e]:
                 assert an[e] == 0
                 continue
-            h = 1e-5 * (base[e] if g not in ABS_STEP else 1.0)
+            # (the air coefficients barely move this loss: |dL/dk| ~ 1e-8 against L ~ 0.05, so their step is larger to keep
+            # the difference of the two losses above round-off)
+            h = (1e-3 if g in ("k_drag", "k_lift") else 1e-5) * (base[e] if g not in ABS_STEP else 1.0)
             vals = []
             for sgn in (+1, -1):
                 p = base.copy(); p[e] += sgn * h
@@ -805,3 +812,42 @@ def test_actuation_gradients_vs_fd_step_and_rollout():
     o.set_act_current(np.zeros((1, M)), np.zeros((1, Mh)))
     o2 = orc.Oracle(sc)
     assert np.array_equal(o.step(x, v)[0], o2.step(x, v)[0])
+
+
+# ---------------------------------------------------------------- lift / drag on cloth faces
+def test_aero_closed_forms_and_dissipation():
+    """PAPER.md:586 ("a lift/drag model that approximates the effect of the surrounding air on the surface of mesh") with
+    reading A21: F = -A s (k_drag vb + k_lift (n.vb) n), s = |vb|, vb = mean vertex velocity - wind, shared equally by the
+    three vertices.  Right triangle with legs a in the xz-plane (A = a^2/2, n = +y), elastic terms switched off:
+      moving along its normal at speed u   ->  F = -A u^2 (k_drag + k_lift) n
+      moving in its own plane at speed u   ->  F = -A u^2 k_drag t         (no pressure term: n.vb = 0)
+      at rest in still air                 ->  F = 0
+      at rest in a wind w                  ->  F = +A |w| (k_drag w + k_lift (n.w) n)
+    and for any state F.vb = -A s (k_drag |vb|^2 + k_lift (n.vb)^2) <= 0: the air only dissipates."""
+    a, kd_, kl_ = 0.25, 0.75, 0.5
+    X = np.array([[0, 0, 0], [a, 0, 0], [0, 0, -a]], dtype=np.float64)  # normal +y
+    A, n = a * a / 2, np.array([0.0, 1.0, 0.0])
+
+    def force(v, wind=(0.0, 0.0, 0.0)):
+        sc = scenes.custom_scene(X, tris=[[0, 1, 2]], hinges=np.zeros((0, 4), np.int32), tri_mu=0.0, tri_lam=1.0, tri_damp=0.0,
+                                 k_drag=kd_, k_lift=kl_, wind=wind, gravity=(0, 0, 0), plane_d=-1e6)
+        return orc.Oracle(sc).forces(X, v=np.broadcast_to(np.asarray(v, np.float64), (3, 3)), mask=orc.TRIS)[0]
+
+    u = 1.5
+    f = force(u * n)
+    assert np.abs(f.sum(0) - (-A * u * u * (kd_ + kl_) * n)).max() <= 1e-12 and np.abs(f[0] - f[1]).max() == 0 and np.abs(f[0] - f[2]).max() == 0
+    t = np.array([0.6, 0.0, -0.8])
+    assert np.abs(force(u * t).sum(0) - (-A * u * u * kd_ * t)).max() <= 1e-12
+    assert np.abs(force(np.zeros(3))).max() <= 1e-12  # eps = 1e-6 m/s regularisation: |F| <= A eps * 0 = 0 at vb = 0
+    w = np.array([0.5, -0.25, 0.125])  # exact in fp32 (A19)
+    assert np.abs(force(np.zeros(3), wind=tuple(w)).sum(0) - A * np.linalg.norm(w) * (kd_ * w + kl_ * (n @ w) * n)).max() <= 1e-9
+    rng = np.random.default_rng(31)
+    for _ in range(20):  # deformed, tumbling triangle: compare against the formula evaluated here and check dissipation
+        x = X + 0.05 * rng.normal(size=(3, 3)); v = rng.normal(size=(3, 3))
+        sc = scenes.custom_scene(X, tris=[[0, 1, 2]], hinges=np.zeros((0, 4), np.int32), tri_mu=0.0, tri_lam=1.0, tri_damp=0.0,
+                                 k_drag=kd_, k_lift=kl_, gravity=(0, 0, 0), plane_d=-1e6)
+        F = orc.Oracle(sc).forces(x, v=v, mask=orc.TRIS)[0].sum(0)
+        vb = v.mean(0)
+        assert F @ vb < 0
+        c = np.cross(x[1] - x[0], x[2] - x[0]); Ac = 0.5 * np.linalg.norm(c); nc = c / np.linalg.norm(c)
+        assert abs(F @ vb + Ac * np.linalg.norm(vb) * (kd_ * vb @ vb + kl_ * (nc @ vb) ** 2)) <= 1e-9
