@@ -72,7 +72,10 @@ enum gs_param_group {
                         gradients (theta0 and the per-edge actuation enter the same argument, PAPER.md:585-586:
                         dL/dtheta0 = -1/2 sum over frames of dL/dalpha), so gs_param_grads needs an activation schedule
                         attached (gs_actuation_create; one zero frame is enough), else GS_ESTATE */
-    GS_NUM_GROUPS = 14
+    GS_AERO_DRAG = 14, GS_AERO_LIFT = 15, /* k_drag, k_lift of the lift / drag model (NEXT-3): one value per environment, [E] */
+    GS_WIND = 16,    /* velocity of the air: ONE vector for all environments, set like GS_GRAVITY; it has no gradient
+                        (gs_param_grads returns GS_EINVAL) */
+    GS_NUM_GROUPS = 17
 };
 
 /* bit flags of gs_model_desc.param_layout: which parameter arrays carry a leading [E] axis */
@@ -99,6 +102,9 @@ enum gs_plan {
  *   tets must be positively oriented (det D_m > 0), else GS_EMESH.
  *   hinges[h] = (wing1, wing2, edge_a, edge_b): the two vertices opposite the shared edge, then the edge.
  *   pinned[i] != 0 => inverse mass 0 (step(inv_mass)).
+ *   Air ("a lift/drag model that approximates the effect of the surrounding air on the surface of mesh";
+ *   DESIGN.md A21, the paper gives no formula): every triangle with area A, unit normal n and relative velocity
+ *   vb = mean vertex velocity - wind gets F = -A |vb| (k_drag vb + k_lift (n.vb) n), a third on each vertex.
  *   Contact: plane n.x = d, threshold particle_radius, stiffness ke, damping kd,
  *   friction stiffness kf, friction coefficient mu_c (A7-A9).
  */
@@ -121,6 +127,8 @@ typedef struct {
     float particle_radius;
     const float *ke, *kd, *kf, *mu_c; /* [E] or [1] */
     int32_t plan;          /* gs_plan */
+    const float *k_drag, *k_lift; /* [E] or [1] (GS_CONTACT_PER_ENV), or NULL = 0: lift / drag of the air on the triangles */
+    float wind[3];         /* velocity of the air */
 } gs_model_desc;
 
 /* Upper bound of the device workspace a model of this description needs (bytes).  0 on a bad desc. */

@@ -321,6 +321,7 @@ extern "C" int gs_zero_grads(gs_model *m, gs_stream stream) {
 extern "C" int gs_param_grads(gs_model *m, int group, float *d_out, gs_stream stream) {
     GS_REQUIRE(m && d_out, GS_EINVAL, "null argument");
     GS_REQUIRE(group >= 0 && group < GS_NUM_GROUPS, GS_EINVAL, "unknown parameter group %d", group);
+    GS_REQUIRE(group != GS_WIND, GS_EINVAL, "the wind has no gradient");
     GS_REQUIRE(group != GS_GRAVITY || m->dev.want_gravity, GS_ESTATE, "dL/dg was not requested before the backward pass (gs_request_grads)");
     return launch_get_grads(m, group, d_out, (cudaStream_t)stream);
 }
@@ -587,6 +588,7 @@ extern "C" int gs_rollout_loss_backward_host(gs_model *m, gs_tape *t, const floa
         const int g = groups[k];
         GS_REQUIRE(g >= 0 && g < GS_NUM_GROUPS && h_grads[k], GS_EINVAL, "bad group %d", g);
         const int c = g == GS_MASS ? N : (g == GS_GRAVITY ? 3 : (g == GS_HINGE_THETA0 || g == GS_HINGE_KB ? m->counts[T_HINGE] : (g >= GS_CONTACT_KE ? 1 : m->counts[g / 3])));
+        GS_REQUIRE(g != GS_WIND, GS_EINVAL, "the wind has no gradient");
         if (c == 0) continue;
         GS_TRY(gs_param_grads(m, g, d_g, stream));
         // the staging buffer is reused: the copy is ordered before the next group's kernel on the same stream

@@ -195,6 +195,42 @@ __device__ __forceinline__ void tri_adjoint(const vec3 x[3], const vec3 v[3], co
     av[1] = madd(b[0] * aG1, b[1], aG2); av[2] = madd(b[2] * aG1, b[3], aG2); av[0] = -(av[1] + av[2]);
 }
 
+// ------------------------------------------------------------------------------------------ lift / drag on triangles
+// PAPER.md:586 ("a lift/drag model that approximates the effect of the surrounding air on the surface of mesh"); DESIGN.md
+// A21: F = -A s (k_drag vb + k_lift (n.vb) n), c = (x1-x0) x (x2-x0), A = |c|/2, n = c/|c|, vb = mean vertex velocity -
+// wind, s = sqrt(|vb|^2 + eps^2); a third of F on each vertex.  Written with L = |c|, u = c.vb: F = -(s/2) (k_drag L vb + k_lift u c / L).
+constexpr float kAeroEps2 = 1e-12f;  // (1e-6 m/s)^2
+__device__ __forceinline__ void aero_force_add(const vec3 x[3], const vec3 v[3], const vec3 &wind, float kdrag, float klift, vec3 f[3]) {
+    const vec3 e1 = x[1] - x[0], e2 = x[2] - x[0];
+    const vec3 c = cross(e1, e2);
+    const vec3 vb = (1.0f / 3.0f) * (v[0] + v[1] + v[2]) - wind;
+    const float L2 = dot(c, c), iL = rsqrtf(L2), L = L2 * iL;
+    const float s = sqrtf(dot(vb, vb) + kAeroEps2), u = dot(c, vb);
+    const vec3 F3 = (-s * (1.0f / 6.0f)) * madd((kdrag * L) * vb, klift * u * iL, c);  // F / 3
+    f[0] += F3; f[1] += F3; f[2] += F3;
+}
+// VJP (a_k = dL/df_k): adds to ax, av; gd, gl = this substep's dL/dk_drag, dL/dk_lift of the triangle.  With ab = mean a_k,
+// P = k_drag L vb + k_lift u c / L:  dL/dvb = -(ab.P)/(2s) vb - (s/2) k_drag L ab - (s/2) k_lift (ab.c)/L c;
+// dL/dc = -(s/2) k_drag (ab.vb) n - (s/2) k_lift [(ab.c)/L vb + (u/L) ab - u (ab.c)/L^2 n]; dL/de1 = e2 x dL/dc, dL/de2 = dL/dc x e1
+__device__ __forceinline__ void aero_adjoint_add(const vec3 x[3], const vec3 v[3], const vec3 a[3], const vec3 &wind, float kdrag, float klift,
+                                                 vec3 ax[3], vec3 av[3], float &gd, float &gl) {
+    const vec3 e1 = x[1] - x[0], e2 = x[2] - x[0];
+    const vec3 c = cross(e1, e2);
+    const vec3 vb = (1.0f / 3.0f) * (v[0] + v[1] + v[2]) - wind;
+    const vec3 ab = (1.0f / 3.0f) * (a[0] + a[1] + a[2]);
+    const float L2 = dot(c, c), iL = rsqrtf(L2), L = L2 * iL;
+    const vec3 n = iL * c;
+    const float s = sqrtf(dot(vb, vb) + kAeroEps2), hs = 0.5f * s, u = dot(c, vb), ac = dot(ab, c), avb = dot(ab, vb);
+    gd = -hs * L * avb;
+    gl = -hs * u * ac * iL;
+    const float aP = kdrag * L * avb + klift * u * iL * ac;
+    const vec3 gv = (1.0f / 3.0f) * madd(madd((-0.5f * aP / s) * vb, -hs * kdrag * L, ab), -hs * klift * ac * iL, c);
+    const vec3 gc = madd((-hs * kdrag * avb) * n, -hs * klift, madd(madd((ac * iL) * vb, u * iL, ab), -u * ac * iL * iL, n));
+    const vec3 t1 = cross(e2, gc), t2 = cross(gc, e1);
+    ax[1] += t1; ax[2] += t2; ax[0] -= t1 + t2;
+    av[0] += gv; av[1] += gv; av[2] += gv;
+}
+
 // ------------------------------------------------------------------------------------------ hinges
 // vertices: x[0], x[1] wings; x[2], x[3] the shared edge.  theta = signed dihedral (0 when flat);
 // f_i = k_b l0 sin((theta - theta0)/2 + alpha) d_i, d_i = -d(theta)/dx_i (Bridson directions), alpha the per-edge actuation.

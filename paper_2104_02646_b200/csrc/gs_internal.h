@@ -13,11 +13,12 @@ namespace gs {
 
 enum { T_TET = 0, T_TRI = 1, T_HINGE = 2, N_TYPES = 3 };
 static const int kArity[N_TYPES] = {4, 3, 4};
-static const int kNumGrads[N_TYPES] = {3, 3, 1};  // accumulated parameter gradients per element: (mu, lambda, k_damp) x2, k_b
+static const int kNumGrads[N_TYPES] = {3, 5, 1};  // accumulated parameter gradients per element: tets (mu, lambda, k_damp); triangles the
+                                                  // same plus the element's terms of dL/dk_drag, dL/dk_lift (summed per environment on read); hinges k_b
 
 constexpr int kTileElems = 128;      // elements per tile = threads per CTA of the streaming element kernels
 constexpr int kConSlots = 64;        // accumulator slots per environment for the per-environment gradient totals
-constexpr int kAccVals = 8;          // values per slot: dL/d(k_e, k_d, k_f, mu_c), dL/dg (3), one pad
+constexpr int kAccVals = 12;         // values per slot: dL/d(k_e, k_d, k_f, mu_c), dL/dg (3), dL/d(k_drag, k_lift), pad
 constexpr int kFlushEvery = 32;      // substeps between fp32 -> fp64 parameter-gradient flushes (hazard H4)
 
 // Byte layout of one tile's RECORD: everything static a tile of kTileElems elements needs, packed contiguously so
@@ -74,6 +75,9 @@ struct ModelDev {
     float gx, gy, gz, dt;
     float nx, ny, nz, pd, pr;
     const float *ke, *kd, *kf, *muc;  // [E]
+    const float *kdrag, *klift;       // [E] lift / drag coefficients of the air (A21)
+    float wx, wy, wz;                 // wind
+    int aero;                         // some environment has a non-zero air coefficient: the extended element kernels run
     const int *perm_p;                // [N] internal -> caller particle index
     const float *inv_mass;            // [E][N] internal order (0 = pinned)
     float *gmass32;                   // [E][N]
@@ -141,6 +145,7 @@ struct gs_model {
         if (counts[gs::T_HINGE]) { a.hinge = d_act[1] + o1; a.g_hinge = d_gact[1] + o1; }
         return a;
     }
+    bool aero_host = false;  // build_model: some air coefficient is non-zero
     uint64_t epoch = 0;    // bumped when a by-value kernel argument changes (gravity): captured graphs of older epochs are stale
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
     void *res_host = nullptr;

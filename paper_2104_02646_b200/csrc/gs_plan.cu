@@ -56,7 +56,7 @@ struct Layout {
     float *par[N_TYPES], *g32[N_TYPES];
     double *g64[N_TYPES];
     int *perm_p, *bad;
-    float *inv_mass, *gmass32, *ke, *kd, *kf, *muc;
+    float *inv_mass, *gmass32, *ke, *kd, *kf, *muc, *kdrag, *klift;
     double *gmass64, *gcon64, *gacc;
     int *tile_ctr;
     const float **frame_base;
@@ -75,8 +75,8 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
         L.tile_parts[t] = b.take<int>(2 * a * cp);  // 6 bytes per entry (id + local index), upper bound
         if (t != T_HINGE) {
             L.par[t] = b.take<float>(3 * E * cp);
-            L.g32[t] = b.take<float>(3 * E * cp);
-            L.g64[t] = b.take<double>(3 * E * cp);
+            L.g32[t] = b.take<float>(kNumGrads[t] * E * cp);
+            L.g64[t] = b.take<double>(kNumGrads[t] * E * cp);
         } else {
             L.par[t] = nullptr;
             L.g32[t] = b.take<float>(E * cp);
@@ -93,6 +93,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
     L.tile_ctr = b.take<int>(8);
     L.frame_base = b.take<const float *>(1);
     L.ke = b.take<float>(E); L.kd = b.take<float>(E); L.kf = b.take<float>(E); L.muc = b.take<float>(E);
+    L.kdrag = b.take<float>(E); L.klift = b.take<float>(E);
     L.bad = b.take<int>(1);
     L.f = b.take<float4>(EN);
     for (int i = 0; i < 2; i++) { L.xs[i] = b.take<float4>(EN); L.vs[i] = b.take<float4>(EN); }
@@ -193,6 +194,17 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         for (int q = 0; q < 4; q++) {
             for (int env = 0; env < E; env++) s[env] = (d->param_layout & GS_CONTACT_PER_ENV) ? src[q][env] : src[q][0];
             UP(dst[q], s);
+        }
+        const float *asrc[2] = {d->k_drag, d->k_lift};
+        float *adst[2] = {L.kdrag, L.klift};
+        m->aero_host = false;
+        for (int q = 0; q < 2; q++) {
+            for (int env = 0; env < E; env++) {
+                s[env] = asrc[q] ? ((d->param_layout & GS_CONTACT_PER_ENV) ? asrc[q][env] : asrc[q][0]) : 0.0f;
+                if (!std::isfinite(s[env]) || s[env] < 0.0f) { set_error("k_drag / k_lift must be finite and >= 0"); return GS_EINVAL; }
+                if (s[env] != 0.0f) m->aero_host = true;
+            }
+            UP(adst[q], s);
         }
     }
 
@@ -396,8 +408,8 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                     }
             UP(L.par[t], v);
             if (c > 0) {  // an empty set owns one placeholder element only
-                cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * 3 * (size_t)E * cp, stream);
-                if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * 3 * (size_t)E * cp, stream);
+                cudaError_t ce = cudaMemsetAsync(L.g32[t], 0, sizeof(float) * kNumGrads[t] * (size_t)E * cp, stream);
+                if (ce == cudaSuccess) ce = cudaMemsetAsync(L.g64[t], 0, sizeof(double) * kNumGrads[t] * (size_t)E * cp, stream);
                 if (ce != cudaSuccess) return cuda_fail(ce, "memset grads");
             }
         }
@@ -422,6 +434,8 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     }
     dev.pd = d->plane_d; dev.pr = d->particle_radius;
     dev.ke = L.ke; dev.kd = L.kd; dev.kf = L.kf; dev.muc = L.muc;
+    dev.kdrag = L.kdrag; dev.klift = L.klift; dev.wx = d->wind[0]; dev.wy = d->wind[1]; dev.wz = d->wind[2];
+    dev.aero = (m->aero_host && counts[T_TRI] > 0) ? 1 : 0;
     dev.perm_p = L.perm_p; dev.inv_mass = L.inv_mass; dev.gmass32 = L.gmass32; dev.gmass64 = L.gmass64; dev.gacc = L.gacc; dev.gcon64 = L.gcon64; dev.tile_ctr = L.tile_ctr; dev.bad = L.bad; dev.frame_base = L.frame_base;
     m->N = N; m->E = E;
     m->d_f = L.f; m->d_xs[0] = L.xs[0]; m->d_xs[1] = L.xs[1]; m->d_vs[0] = L.vs[0]; m->d_vs[1] = L.vs[1];

@@ -25,6 +25,7 @@
 // a1-a10 of SURVEY.md 8(a); citations of the formulas are in gs_elements.cuh.
 #include <algorithm>
 #include <climits>
+#include <vector>
 #include <cstdio>
 #include <cstdlib>
 
@@ -203,6 +204,8 @@ struct ElemRegs {
 
 // The persistent tile loop shared by the forward and adjoint kernels.  `compute(tv, tile, env, e_local)` evaluates one
 // element into the output slots; `emit(id, env, sums...)` is called once per tile-particle with its summed slots.
+// ACT: the EXTENDED kernels: activation schedules and / or the lift / drag of the air on triangles
+// (PAPER.md:586), each checked at run time inside; the plain kernels (ACT = false) carry neither.
 // ME: the model has more than one environment (work item = tile x environment).  The single-environment kernels (the large
 // meshes) carry none of the item -> (tile, env) divisions and environment offsets.
 template <int TYPE, bool ADJ, bool ACT, bool ME>
@@ -268,7 +271,7 @@ struct TilePipe {
             const float *q = es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems) + tid;
             er.mu = __ldcs(q); er.lam = __ldcs(q + kTileElems); er.damp = __ldcs(q + 2 * kTileElems);
         }
-        er.act = (ACT && TYPE != T_TRI) ? __ldcs(act + ((size_t)env * es.n_tiles + tile) * kTileElems + tid) : 0.0f;
+        er.act = (ACT && TYPE != T_TRI && act) ? __ldcs(act + ((size_t)env * es.n_tiles + tile) * kTileElems + tid) : 0.0f;
     }
     __device__ __forceinline__ void gather(int item, int slot, int b) {  // all threads
         unsigned tile, env;
@@ -412,7 +415,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
     const int N = md.N;
     pipe.run(
         rot, md.tile_ctr + TYPE, next_slot,
-        [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int, float4 *sf) {
+        [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int env, float4 *sf) {
             const int tid = threadIdx.x;
             const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
             if (TYPE == T_TET) {
@@ -432,6 +435,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
                 const vec3 v[3] = {vec3(tv.v[li.x]), vec3(tv.v[li.y]), vec3(tv.v[li.z])};
                 vec3 f[3];
                 tri_force(x, v, b, er.area, er.mu, er.lam, er.damp, f);
+                if (ACT && md.aero) aero_force_add(x, v, vec3(md.wx, md.wy, md.wz), md.kdrag[env], md.klift[env], f);
 #pragma unroll
                 for (int k = 0; k < 3; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
             } else {
@@ -439,7 +443,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
                 const vec3 x[4] = {vec3(tv.x[li.x]), vec3(tv.x[li.y]), vec3(tv.x[li.z]), vec3(tv.x[li.w])};
                 vec3 f[4];
                 float sa = 0.0f, ca = 1.0f;
-                if (ACT) sincosf(er.act, &sa, &ca);
+                if (ACT && actp) sincosf(er.act, &sa, &ca);
                 hinge_force(x, c0.x, c0.y, c0.z, sa, ca, f);
 #pragma unroll
                 for (int k = 0; k < 4; k++) sf[k * kTileElems + tid] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
@@ -616,7 +620,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
                 tet_adjoint(x, v, a, b, c2.y, er.mu, er.lam, er.damp, er.act, ax, av, gmu, glam, gk, ga);
                 float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
                 red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
-                if (ACT) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
+                if (ACT && gactp) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
                     so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
@@ -633,6 +637,11 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
                 tri_adjoint(x, v, a, b, er.area, er.mu, er.lam, er.damp, ax, av, gmu, glam, gk);
                 float *g = es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid;
                 red_add_f32(g, gmu); red_add_f32(g + gstride, glam); red_add_f32(g + 2 * gstride, gk);
+                if (ACT && md.aero) {  // the triangle's terms of dL/dk_drag, dL/dk_lift go to rows 3, 4 of its gradient block
+                    float gd, gl;
+                    aero_adjoint_add(x, v, a, vec3(md.wx, md.wy, md.wz), md.kdrag[env], md.klift[env], ax, av, gd, gl);
+                    red_add_f32(g + 3 * gstride, gd); red_add_f32(g + 4 * gstride, gl);
+                }
 #pragma unroll
                 for (int k = 0; k < 3; k++) {
                     so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
@@ -644,10 +653,10 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
                 const vec3 a[4] = {vec3(tv.a[li.x]), vec3(tv.a[li.y]), vec3(tv.a[li.z]), vec3(tv.a[li.w])};
                 vec3 ax[4];
                 float gkb, ga, sa = 0.0f, ca = 1.0f;
-                if (ACT) sincosf(er.act, &sa, &ca);
+                if (ACT && actp) sincosf(er.act, &sa, &ca);
                 hinge_adjoint(x, a, c0.x, c0.y, c0.z, c0.w, sa, ca, ax, gkb, ga);
                 red_add_f32(es.g32 + (size_t)env * es.cpad + tile * kTileElems + tid, gkb);
-                if (ACT) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
+                if (ACT && gactp) red_add_f32(gactp + (size_t)env * es.cpad + tile * kTileElems + tid, ga);
 #pragma unroll
                 for (int k = 0; k < 4; k++) so[k * kTileElems + tid] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
             }
@@ -715,6 +724,21 @@ __global__ void k_get_grads(const double *__restrict__ g64, const int *__restric
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const int env = (int)(i / count), e = (int)(i - (size_t)env * count);
         out[(size_t)env * count + perm[e]] = (float)g64[(size_t)env * stride + e];
+    }
+}
+// out[env] = sum over the elements of one row of a per-element gradient block (the air coefficients: one value per environment)
+__global__ void k_sum_grad_row(const double *__restrict__ row, float *__restrict__ out, int count, int stride) {
+    __shared__ double red[32];
+    const int env = blockIdx.x;
+    double s = 0.0;
+    for (int e = threadIdx.x; e < count; e += blockDim.x) s += row[(size_t)env * stride + e];
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) t += red[w];
+        out[env] = (float)t;
     }
 }
 // q < 0: dst is the [E][count] inverse-mass array; else dst is ElemDev::par and q the parameter (0 mu, 1 lambda, 2 damp)
@@ -852,7 +876,7 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
     const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     const int bad_idx = substep < 0 ? 0 : substep;
     if (m->elem_items > 0) {
-        const bool act = m->act_frames > 0, me = m->E > 1;
+        const bool act = m->act_frames > 0 || m->dev.aero, me = m->E > 1;
         auto kern = act ? (me ? k_elements_fwd<true, true> : k_elements_fwd<true, false>) : (me ? k_elements_fwd<false, true> : k_elements_fwd<false, false>);
         GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", launch_pdl(m->pdl, kern, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
     }
@@ -867,7 +891,7 @@ int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const flo
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
              launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0) {
-        const bool act = m->act_frames > 0, me = m->E > 1;
+        const bool act = m->act_frames > 0 || m->dev.aero, me = m->E > 1;
         auto kern = act ? (me ? k_elements_adj<true, true> : k_elements_adj<true, false>) : (me ? k_elements_adj<false, true> : k_elements_adj<false, false>);
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
                  launch_pdl(m->pdl, kern, tile_grid(m, m->occ_adj), kTileElems, m->smem_adj, st, m->dev, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
@@ -969,6 +993,10 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
         k_get_contact<<<grid_for((size_t)m->E), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, group - GS_CONTACT_KE, 1);
     } else if (group == GS_GRAVITY) {
         k_get_contact<<<grid_for((size_t)m->E * 3), 256, 0, st>>>(m->dev.gcon64, d_out, m->E, 4, 3);
+    } else if (group == GS_AERO_DRAG || group == GS_AERO_LIFT) {
+        const int c = m->counts[T_TRI], cp = m->hes[T_TRI].cpad;
+        if (c == 0) { cudaMemsetAsync(d_out, 0, sizeof(float) * m->E, st); return GS_OK; }
+        k_sum_grad_row<<<m->E, 256, 0, st>>>(m->dev.es[T_TRI].g64 + (size_t)(group == GS_AERO_DRAG ? 3 : 4) * m->E * cp, d_out, c, cp);
     } else if (group == GS_HINGE_THETA0) {
         const int c = m->counts[T_HINGE];
         if (c == 0) return GS_OK;
@@ -983,15 +1011,39 @@ int launch_get_grads(gs_model *m, int group, float *d_out, cudaStream_t st) {
     return GS_OK;
 }
 int launch_set_params(gs_model *m, int group, const float *d_values, cudaStream_t st) {
-    if (group == GS_GRAVITY) {
-        // gravity is a by-value kernel argument (ModelDev): read the three floats back (synchronises the stream) and
+    if (group == GS_AERO_DRAG || group == GS_AERO_LIFT) {
+        // the extended kernels run iff some coefficient is non-zero: read the values back (synchronises the stream)
+        std::vector<float> h(m->E);
+        float *dst = const_cast<float *>(group == GS_AERO_DRAG ? m->dev.kdrag : m->dev.klift);
+        const float *other = group == GS_AERO_DRAG ? m->dev.klift : m->dev.kdrag;
+        cudaError_t e = cudaMemcpyAsync(h.data(), d_values, sizeof(float) * m->E, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "read air coefficients");
+        bool any = false;
+        for (float q : h) {
+            if (!(q >= 0.0f) || !(q <= 3.0e38f)) { set_error("k_drag / k_lift must be finite and >= 0"); return GS_EINVAL; }
+            any = any || q != 0.0f;
+        }
+        std::vector<float> o(m->E);
+        e = cudaMemcpyAsync(o.data(), other, sizeof(float) * m->E, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dst, d_values, sizeof(float) * m->E, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "set air coefficients");
+        for (float q : o) any = any || q != 0.0f;
+        const int aero = (any && m->counts[T_TRI] > 0) ? 1 : 0;
+        if (aero != m->dev.aero) { m->dev.aero = aero; m->epoch++; }
+        return GS_OK;
+    }
+    if (group == GS_GRAVITY || group == GS_WIND) {
+        // gravity / wind are by-value kernel arguments (ModelDev): read the three floats back (synchronises the stream) and
         // bump the epoch so that tapes re-capture their graphs
         float g[3];
         cudaError_t e = cudaMemcpyAsync(g, d_values, sizeof g, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) return cuda_fail(e, "read gravity");
-        if (!(fabsf(g[0]) <= 3.0e38f) || !(fabsf(g[1]) <= 3.0e38f) || !(fabsf(g[2]) <= 3.0e38f)) { set_error("gravity must be finite"); return GS_EINVAL; }
-        m->dev.gx = g[0]; m->dev.gy = g[1]; m->dev.gz = g[2];
+        if (!(fabsf(g[0]) <= 3.0e38f) || !(fabsf(g[1]) <= 3.0e38f) || !(fabsf(g[2]) <= 3.0e38f)) { set_error("gravity / wind must be finite"); return GS_EINVAL; }
+        if (group == GS_GRAVITY) { m->dev.gx = g[0]; m->dev.gy = g[1]; m->dev.gz = g[2]; }
+        else { m->dev.wx = g[0]; m->dev.wy = g[1]; m->dev.wz = g[2]; }
         m->epoch++;
         return GS_OK;
     }

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgradsim.so")
 
 GS_OK, GS_EINVAL, GS_EMESH, GS_ENOMEM, GS_ECUDA, GS_ENONFINITE, GS_ESTATE = 0, -1, -2, -3, -4, -5, -6
 GROUPS = {"tet_mu": 0, "tet_lambda": 1, "tet_damp": 2, "tri_mu": 3, "tri_lambda": 4, "tri_damp": 5, "mass": 6, "hinge_kb": 7,
-          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13}
+          "ke": 8, "kd": 9, "kf": 10, "mu_c": 11, "gravity": 12, "hinge_theta0": 13, "k_drag": 14, "k_lift": 15, "wind": 16}
 ACT_KINDS = {"tet": 0, "hinge": 1}
 GS_ELEM_PER_ENV, GS_MASS_PER_ENV, GS_CONTACT_PER_ENV = 1, 2, 4
 GS_PLAN_AUTO, GS_PLAN_STREAMING, GS_PLAN_RESIDENT = 0, 1, 2
@@ -42,6 +42,7 @@ class gs_model_desc(C.Structure):
         ("plane_n", C.c_float * 3), ("plane_d", C.c_float), ("particle_radius", C.c_float),
         ("ke", _fp), ("kd", _fp), ("kf", _fp), ("mu_c", _fp),
         ("plan", C.c_int32),
+        ("k_drag", _fp), ("k_lift", _fp), ("wind", C.c_float * 3),
     ]
 
 
@@ -208,6 +209,10 @@ def fill_desc(sc, plan=GS_PLAN_AUTO):
     layout |= GS_CONTACT_PER_ENV
     for name in ("ke", "kd", "kf", "mu_c"):
         setattr(d, name, f(np.broadcast_to(np.asarray(getattr(sc, name), np.float32).ravel(), (E,))))
+    for name in ("k_drag", "k_lift"):
+        val = getattr(sc, name, None)
+        setattr(d, name, f(np.broadcast_to(np.zeros(1, np.float32) if val is None else np.asarray(val, np.float32).ravel(), (E,))))
+    d.wind = (C.c_float * 3)(*[float(g) for g in getattr(sc, "wind", (0.0, 0.0, 0.0))])
     d.param_layout = layout
     d.gravity = (C.c_float * 3)(*[float(g) for g in sc.gravity])
     d.dt = float(sc.dt)
@@ -253,8 +258,10 @@ class Model:
 
     def group_count(self, group):
         g = GROUPS[group] if isinstance(group, str) else int(group)
-        if g == 12:
-            return 3  # gravity: dL/dg per environment
+        if g in (12, 16):
+            return 3  # gravity: dL/dg per environment; wind: one vector
+        if g in (14, 15):
+            return 1  # air coefficients: one value per environment
         if 8 <= g <= 11:
             return 1  # contact parameters: one value per environment
         return self.N if g == 6 else (self.counts["hinge"] if g in (7, 13) else (self.counts["tet"] if g < 3 else self.counts["tri"]))

@@ -74,7 +74,7 @@ def gpu_run_scene(sc, target, K=None, plan=gs.GS_PLAN_AUTO, model=None):
     out.update(xT=host(xT), vT=host(vT), loss=host(loss), adj_x0=host(ax0), adj_v0=host(av0), bad=bad,
                rec_x=np.stack([host(r) for r in rec]))
     for g in gs.GROUPS:
-        if g == "hinge_theta0" and not m.act_frames:
+        if g == "wind" or (g == "hinge_theta0" and not m.act_frames):
             continue  # read from the hinge actuation gradients: needs a schedule (gradsim.h, GS_HINGE_THETA0)
         out["g_" + g] = host(m.param_grads(g))
     if act:

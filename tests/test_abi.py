@@ -64,7 +64,7 @@ def test_param_group_enum_matches_binding():
     enum = {k: int(v) for k, v in re.findall(r"(GS_[A-Z0-9_]+)\s*=\s*(\d+)", body)}
     names = {"GS_TET_MU": "tet_mu", "GS_TET_LAMBDA": "tet_lambda", "GS_TET_DAMP": "tet_damp", "GS_TRI_MU": "tri_mu", "GS_TRI_LAMBDA": "tri_lambda",
              "GS_TRI_DAMP": "tri_damp", "GS_MASS": "mass", "GS_HINGE_KB": "hinge_kb", "GS_CONTACT_KE": "ke", "GS_CONTACT_KD": "kd",
-             "GS_CONTACT_KF": "kf", "GS_CONTACT_MUC": "mu_c", "GS_GRAVITY": "gravity", "GS_HINGE_THETA0": "hinge_theta0"}
+             "GS_CONTACT_KF": "kf", "GS_CONTACT_MUC": "mu_c", "GS_GRAVITY": "gravity", "GS_HINGE_THETA0": "hinge_theta0", "GS_AERO_DRAG": "k_drag", "GS_AERO_LIFT": "k_lift", "GS_WIND": "wind"}
     assert enum.pop("GS_NUM_GROUPS") == len(gs.GROUPS) == len(names)
     assert {names[k]: v for k, v in enum.items()} == gs.GROUPS
 

@@ -599,3 +599,70 @@ def test_actuation_scheduled_rollout_and_gradients(config, plan, K):
     back = gpu_run_scene(passive, ref["target"], K=K, model=m)
     pref = orc.run_scene(passive, target=ref["target"])
     assert np.abs(back["xT"] - pref["xT"]).max() <= TOL_ROLLOUT * sc.extent()
+
+
+# ------------------------------------------------------------------------------------------ lift / drag (NEXT-3)
+def _with_air(sc, kd_=300.0, kl_=200.0, wind=(0.5, -0.25, 0.125)):  # (heavy 0.1 kg particles on 1 cm faces, A15: physical coefficients ~0.5 would be invisible)
+    sc = copy.copy(sc)
+    sc.k_drag = np.full(sc.n_envs, kd_, np.float32)
+    sc.k_lift = np.full(sc.n_envs, kl_, np.float32)
+    sc.wind = wind
+    return sc
+
+
+@pytest.mark.parametrize("config", [1, 4])
+def test_aero_one_substep_forward_and_adjoint(config):
+    """Lift / drag of the air on the cloth faces (reading A21) on one substep: state, cotangents, every
+    gradient incl. dL/dk_drag, dL/dk_lift against the oracle; then the coefficients are switched off and on again through
+    gs_set_params (the plain and the extended kernels are different instantiations)."""
+    sc = _with_air(scenes.make_scene(config, small=True))
+    x, v = scenes.perturbed_state(sc)
+    o = orc.Oracle(sc)
+    xo, vo = o.step(x, v)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert np.abs(host(xg) - xo).max() <= TOL_STEP * sc.extent()
+    assert rel_inf(host(vg), vo) <= 2e-5
+    still = copy.copy(sc); still.k_drag, still.k_lift = 0 * sc.k_drag, 0 * sc.k_lift
+    xs, vs = orc.Oracle(still).step(x, v)
+    assert rel_inf(vs, vo) > 1e-5  # the air is visible in the result
+    r = scenes.rng_for(config, "misc", 79)
+    bx, bv = r.normal(size=x.shape).astype(np.float32), r.normal(size=x.shape).astype(np.float32)
+    o.zero_grads()
+    ax, av = o.step_adjoint(x, v, bx, bv)
+    m.zero_grads()
+    axg, avg = m.step_backward(dev(x), dev(v), dev(bx), dev(bv))
+    assert rel_inf(host(axg), ax) <= 1e-4 and rel_inf(host(avg), av) <= 1e-4
+    for g in _grad_groups(sc) + ["k_drag", "k_lift"]:
+        assert np.abs(o.grads(g)).max() > 0
+        assert rel_inf(host(m.param_grads(g)), o.grads(g)) <= TOL_GRAD, g
+    zero = dev(np.zeros((sc.n_envs, 1), np.float32))
+    m.set_params("k_drag", zero); m.set_params("k_lift", zero)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert np.abs(host(xg) - xs).max() <= TOL_STEP * sc.extent() and rel_inf(host(vg), vs) <= 2e-5
+    m.set_params("k_drag", dev(sc.k_drag[:, None])); m.set_params("k_lift", dev(sc.k_lift[:, None]))
+    m.set_params("wind", dev(np.broadcast_to(np.float32([0.0, 0.5, 0.0]), (sc.n_envs, 3)).copy()))
+    s2 = copy.copy(sc); s2.wind = (0.0, 0.5, 0.0)
+    x2, v2 = orc.Oracle(s2).step(x, v)
+    xg, vg = m.step_forward(dev(x), dev(v))
+    assert np.abs(host(xg) - x2).max() <= TOL_STEP * sc.extent() and rel_inf(host(vg), v2) <= 2e-5
+
+
+@pytest.mark.parametrize("config", [1, 4])
+def test_aero_rollout_and_gradients(config):
+    """A sheet tumbling through a wind (airborne: no contact-branch flips, A20) for a whole rollout + backward: final
+    state, every gradient and dL/dk_drag, dL/dk_lift against the oracle; the control-cloth workload of the paper
+    (optimise the initial velocity "under nonlinear lift/drag forces") reads dL/dv0 from the same pass."""
+    sc = _with_air(scenes.make_scene(config, small=True), wind=(1.0, 0.5, -0.5))
+    sc.plane_d = -1e6
+    sc.v0 = (sc.v0 + scenes.rng_for(config, "misc", 80).normal(0.0, 0.3, sc.v0.shape)).astype(np.float32)
+    sc.v0[:, sc.pinned.astype(bool)] = 0
+    ref = orc.run_scene(sc)
+    got = gpu_run_scene(sc, ref["target"])
+    assert got["bad"] == -1
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * sc.extent()
+    still = copy.copy(sc); still.k_drag, still.k_lift = 0 * sc.k_drag, 0 * sc.k_lift
+    assert np.abs(orc.run_scene(still, target=ref["target"])["xT"] - ref["xT"]).max() > 1e-4 * sc.extent()
+    for k in ["adj_x0", "adj_v0"] + ["g_" + g for g in _grad_groups(sc) + ["k_drag", "k_lift"]]:
+        assert np.abs(ref[k]).max() > 0, k
+        assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
