@@ -76,6 +76,14 @@ struct EmitPlan {
         keep[0] = (bb & 1u) ? 0.f : 1.f; keep[1] = (bb & 2u) ? 0.f : 1.f; keep[2] = (bb & 4u) ? 0.f : 1.f;
         idp = ids + (dsc & 1023u);
     }
+    // checked build: every slot inside the output plane, every flushed run inside the tile's particle list with a valid id
+    __device__ __forceinline__ bool in_range(int n_slots, int first, int pmax, int N) const {
+        bool ok = (int)s[0] < n_slots && (int)s[1] < n_slots && (int)s[2] < n_slots && (int)s[3] < n_slots;
+#pragma unroll
+        for (int k = 0; k < 4; k++)
+            if (fl & (1u << k)) ok = ok && first + (int)r[k] < pmax && idp[r[k]] >= 0 && idp[r[k]] < N;
+        return ok;
+    }
     // running sums a[k] of the runs; a[k] is final where bit k of fl is set
     __device__ __forceinline__ void sums(const float4 *src, float3 a[4]) const {
         const float4 c0 = src[s[0]], c1 = src[s[1]], c2 = src[s[2]], c3 = src[s[3]];
@@ -152,6 +160,17 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
         : "memory");
 }
 
+// Checked build (python -m paper_2104_02646_b200.build --checked, -DGS_CHECKED): every index the tile pipeline takes from
+// the packed tile data is range-checked before use; a violation raises the model's flag with a code >= kCheckBase (reported
+// by gs_check_finite as "substep" kCheckBase + code) and the access is skipped.  compute-sanitizer is not available on this
+// pool, so the GPU parity tests are run once against this build instead (profiles/r2_sanitizers.md).
+constexpr int kCheckBase = 0x7e000000;
+#ifdef GS_CHECKED
+#define GS_CHECK_IDX(cond, code, md_bad) ((cond) ? true : (atomicMin((md_bad), kCheckBase + (code)), false))
+#else
+#define GS_CHECK_IDX(cond, code, md_bad) (true)
+#endif
+
 // ------------------------------------------------------------------------------------------ tile pipeline
 // Shared memory of one CTA of a tile kernel (ADJ adds the gathered adj_f and a second output plane):
 //   ids   int[3][pmax]                      particle ids of tiles i, i+1, i+2      (bulk copy, two tiles ahead)
@@ -220,9 +239,10 @@ struct TilePipe {
     uint64_t *bars;  // full[0..1], idfull[0..2]
     const float4 *x4, *v4, *a4;
     const float *act;  // [E][cpad] actuation of this substep for this element type, or null
+    int *bad;          // the model's flag (checked build)
     uint64_t pol_stream, pol_keep;
     __device__ __forceinline__ TilePipe(const ModelDev &md, char *smem, uint64_t *bars_, const float4 *x4_, const float4 *v4_, const float4 *a4_, const float *act_)
-        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_), act(act_) {
+        : es(md.es[TYPE]), N(md.N), E(md.E), pmax(md.es[TYPE].pmax), lmax(md.es[TYPE].lmax), bb(S::buf_bytes(md.es[TYPE].lmax)), bars(bars_), x4(x4_), v4(v4_), a4(a4_), act(act_), bad(md.bad) {
         idbuf = (int *)smem;
         locbuf = (uint16_t *)(smem + 3 * pmax * 4);
         bufs = smem + 3 * pmax * 4 + 2 * pmax * 2;
@@ -284,6 +304,7 @@ struct TilePipe {
             const int id = ids[p];
             if (id >= 0) {
                 const int l = loc[p];
+                if (!GS_CHECK_IDX(id < N && l < lmax, 1, bad)) continue;
                 cp_async16_hint(tv.x + l, x4 + eoff + id, pol_keep);
                 if (S::kHasV) cp_async16_hint(tv.v + l, v4 + eoff + id, pol_keep);
                 if (ADJ) cp_async16_hint(tv.a + l, a4 + eoff + id, pol_keep);
@@ -418,6 +439,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
         [&](const TileView<TYPE, false> &tv, const ElemRegs<TYPE> &er, int, int env, float4 *sf) {
             const int tid = threadIdx.x;
             const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
+            if (!GS_CHECK_IDX(li.x < pipe.lmax && li.y < pipe.lmax && li.z < pipe.lmax && (TYPE == T_TRI || li.w < pipe.lmax), 2, md.bad)) return;
             if (TYPE == T_TET) {
                 const float4 c0 = er.c0, c1 = er.c1;
                 const float2 c2 = er.c2;
@@ -455,6 +477,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
             const unsigned dsc = tv.slot_desc[threadIdx.x];
             if ((dsc >> 13) == 0u) return;
             const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
+            if (!GS_CHECK_IDX(ep.in_range(RecLayout<TYPE>::kArityT * kTileElems, (int)(dsc & 1023u), pipe.pmax, N), 3, md.bad)) return;
             float3 a[4];
             ep.sums(sf, a);
             ep.flush(f4 + (size_t)env * N, a);
@@ -608,6 +631,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
         [&](const TileView<TYPE, true> &tv, const ElemRegs<TYPE> &er, int tile, int env, float4 *so) {
             const int tid = threadIdx.x;
             const ushort4 li = make_ushort4((unsigned short)(er.li.x & 0xFFFFu), (unsigned short)(er.li.x >> 16), (unsigned short)(er.li.y & 0xFFFFu), (unsigned short)(er.li.y >> 16));
+            if (!GS_CHECK_IDX(li.x < pipe.lmax && li.y < pipe.lmax && li.z < pipe.lmax && (TYPE == T_TRI || li.w < pipe.lmax), 2, md.bad)) return;
             if (TYPE == T_TET) {
                 const float4 c0 = er.c0, c1 = er.c1;
                 const float2 c2 = er.c2;
@@ -665,6 +689,7 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
             const unsigned dsc = tv.slot_desc[threadIdx.x];
             if ((dsc >> 13) == 0u) return;
             const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
+            if (!GS_CHECK_IDX(ep.in_range(RecLayout<TYPE>::kArityT * kTileElems, (int)(dsc & 1023u), pipe.pmax, N), 3, md.bad)) return;
             float3 a[4];
             ep.sums(so, a);
             ep.flush(adjx + (size_t)env * N, a);
