@@ -40,8 +40,17 @@ struct ResDev {
                                // particles one quarter-warp reads for the same vertex fall into different 16-byte bank
                                // groups (conflict-free LDS.128), as in the streaming plan
     const uint16_t *owner;     // [N] particle served by particle slot q, most incident tets first
-    const uint16_t *csr_ptr;   // [N + 1]
-    const uint16_t *csr_slots; // [4 M] slot = k * M + e
+    const uint16_t *csr_ptr;   // [N + 1] incidences per internal particle (prefix sums): valence = ptr[p + 1] - ptr[p]
+    // Scatter as a TRANSPOSED gather list.  Particle slots are sorted by valence (most incident tets first), and the j-th
+    // incidence of the particle in slot q lives at entry row[j] + q of the contribution plane: row j holds the j-th
+    // incidence of every particle that has one (slots 0 .. count_j - 1).  The lanes of a warp serve consecutive slots, so
+    // their LDS.128 of one row are consecutive, conflict-free, and need no index load; with kpp lanes per particle the lanes
+    // of a group take rows j0, j0 + kpp, ..., and row starts are padded to 8 / kpp modulo 8 entries so that the rows a
+    // quarter-warp reads at once fall into different 16-byte bank groups.  Element threads keep the four destinations of
+    // their tet in two registers.
+    const ushort4 *dest;       // [M] entry of each tet vertex's contribution
+    const uint16_t *row;       // [maxval + 1] first entry of row j
+    int maxval, Ltot;          // rows; entries of one contribution plane (padded)
 };
 
 // activation schedule of the tets (gs_actuation_create), internal order [F][E][cpad]; used by the ACT kernel variants
@@ -60,33 +69,64 @@ struct ResHost {
 
 static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 
-// shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), slots [planes][4M] float4, csr_ptr, owner, csr_slots
+// shared memory: sx[N] float4, sv[N] float4, (adjoint: sa[N] float4), contributions [planes][Ltot] float4, csr_ptr, owner, row
 // adjoint only: per-particle accumulators of the per-environment totals (contact parameters, gravity): double[7][N] masters,
-// then float[4][N] chunks of the contact terms
+// then float[7][N] chunks
 constexpr int kResAcc = 7;
-static size_t res_smem(int L, int N, int M, int planes, bool adj) {
-    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * 4 * M * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + 4 * 4)) : 0) +
-           al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)4 * M * 2);
+static size_t res_smem(int L, int N, int Ltot, int maxval, int planes, bool adj) {
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * Ltot * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + kResAcc * 4)) : 0) +
+           al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)(maxval + 1) * 2);
+}
+static int res_threads(int M) { const int ept = M > kResMaxThreads ? 2 : 1; return ((M + ept - 1) / ept + 31) / 32 * 32; }
+static int res_kpp(int nthreads, int N) { return nthreads >= 4 * N ? 4 : (nthreads >= 2 * N ? 2 : 1); }
+// rows of the transposed gather list from the valences (any order): row[j] (maxval + 1 entries); returns the padded total
+static int res_rows(std::vector<int> val, int kpp, std::vector<uint16_t> *row) {
+    std::sort(val.begin(), val.end(), [](int a, int b) { return a > b; });
+    const int maxval = val.empty() ? 0 : val[0], want = (8 / kpp) & 7;  // row stride modulo 8 (kpp = 1: no constraint)
+    int off = 0;
+    if (row) row->assign(maxval + 1, 0);
+    for (int j = 0; j < maxval; j++) {
+        int cnt = 0;
+        while (cnt < (int)val.size() && val[cnt] > j) cnt++;
+        if (row) (*row)[j] = (uint16_t)off;
+        int stride = cnt;
+        if (kpp > 1) while ((stride & 7) != want) stride++;
+        off += stride;
+    }
+    if (row) (*row)[maxval] = (uint16_t)off;
+    return off;
+}
+static std::vector<int> res_valences(const gs_model_desc *d) {
+    std::vector<int> val(d->n_particles, 0);
+    for (size_t i = 0; i < (size_t)d->n_tets * 4; i++) {
+        const int p = d->tets[i];
+        if (p >= 0 && p < d->n_particles) val[p]++;
+    }
+    return val;
 }
 
 static bool resident_fits(const gs_model_desc *d) {
     if (d->n_tris > 0 || d->n_hinges > 0 || d->n_tets < 1 || d->n_tets > kResMaxTets) return false;
-    const int ept = d->n_tets > kResMaxThreads ? 2 : 1;
-    const int nthreads = ((d->n_tets + ept - 1) / ept + 31) / 32 * 32;
-    if (d->n_particles > nthreads) return false;
-    return res_smem(d->n_particles + 24, d->n_particles, d->n_tets, 2, true) <= 200 * 1024;
+    const int nthreads = res_threads(d->n_tets);
+    if (d->n_particles > nthreads || !d->tets) return false;
+    const std::vector<int> val = res_valences(d);
+    const int maxval = *std::max_element(val.begin(), val.end());
+    const int Ltot = res_rows(val, res_kpp(nthreads, d->n_particles), nullptr);
+    if (Ltot > 65535) return false;
+    return res_smem(d->n_particles + 24, d->n_particles, Ltot, maxval, 2, true) <= 200 * 1024;
 }
 
 size_t resident_blob_bytes(const gs_model_desc *d) {
     if (!resident_fits(d)) return 0;
-    return 256 * 6 + (size_t)d->n_tets * sizeof(ushort4) + (size_t)(3 * d->n_particles + 1) * 2 + (size_t)4 * d->n_tets * 2;
+    return 256 * 8 + 2 * (size_t)d->n_tets * sizeof(ushort4) + (size_t)(3 * d->n_particles + 1) * 2 + (size_t)(4 * d->n_tets + 2) * 2;
 }
 
 // ------------------------------------------------------------------------------------------ kernels
 struct TetReg {
     float b[9], V, mu, lam, kd;
     float act;  // this substep's actuation; 0 in the passive kernels
-    ushort4 li;
+    ushort4 li;   // staging indices of the four particles
+    ushort4 dst;  // entries of the four per-vertex contributions (ResDev::dest)
     bool on;
 };
 
@@ -110,14 +150,15 @@ __device__ __forceinline__ void load_tets(const ModelDev &md, const ResDev &rd, 
         tr[j].lam = es.par[par_index(es.n_tiles, env, ee, 1)];
         tr[j].kd = es.par[par_index(es.n_tiles, env, ee, 2)];
         tr[j].li = rd.idx[ee];
+        tr[j].dst = rd.dest[ee];
         tr[j].act = 0.0f;
     }
 }
 
-__device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint16_t *s_owner, uint16_t *s_slots) {
+__device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint16_t *s_owner, uint16_t *s_row) {
     for (int i = threadIdx.x; i <= rd.N; i += blockDim.x) s_ptr[i] = rd.csr_ptr[i];
     for (int i = threadIdx.x; i < rd.N; i += blockDim.x) s_owner[i] = rd.owner[i];
-    for (int i = threadIdx.x; i < 4 * rd.M; i += blockDim.x) s_slots[i] = rd.csr_slots[i];
+    for (int i = threadIdx.x; i <= rd.maxval; i += blockDim.x) s_row[i] = rd.row[i];
 }
 
 // Particle ownership: particle slot q = tid / kpp is served by kpp adjacent lanes (kpp = 1, 2 or 4, the largest that
@@ -126,7 +167,8 @@ __device__ __forceinline__ void load_csr(const ResDev &rd, uint16_t *s_ptr, uint
 // lane 0 (the "lead") holds the particle's state in registers for the whole rollout.
 struct PartOwn {
     bool is_p, lead;
-    int p, lp, beg, end;  // particle, its staging index, this lane's part of its slot run
+    int p, lp;          // particle, its staging index
+    int q, j0, val;     // particle slot; this lane takes rows j0, j0 + kpp, ... < val of the particle's incidences
 };
 __device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_ptr, const uint16_t *s_owner) {
     PartOwn o;
@@ -135,9 +177,8 @@ __device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_
     o.lead = o.is_p && j == 0;
     o.p = o.is_p ? s_owner[q] : 0;
     o.lp = rd.rloc[o.p];
-    const int b = s_ptr[o.p], len = o.is_p ? s_ptr[o.p + 1] - b : 0;
-    o.beg = b + (len * j) / rd.kpp;
-    o.end = b + (len * (j + 1)) / rd.kpp;
+    o.q = q; o.j0 = j;
+    o.val = o.is_p ? s_ptr[o.p + 1] - s_ptr[o.p] : 0;
     return o;
 }
 __device__ __forceinline__ float group_sum(float v, int kpp) {
@@ -152,14 +193,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
     extern __shared__ float4 smem4[];
     const int N = rd.N, M = rd.M, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L;
-    float4 *sf = smem4 + 2 * L;  // [4 M] per element-vertex force
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + 4 * M);
+    float4 *sf = smem4 + 2 * L;  // [Ltot] per element-vertex force, transposed gather layout
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(sf + rd.Ltot);
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
-    uint16_t *s_slots = s_owner + ((N + 7) & ~7);
+    uint16_t *s_row = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
     TetReg tr[EPT];
     load_tets<EPT>(md, rd, env, tr);
-    load_csr(rd, s_ptr, s_owner, s_slots);
+    load_csr(rd, s_ptr, s_owner, s_row);
     __syncthreads();
     const PartOwn po = part_own(rd, s_ptr, s_owner);
     const size_t poff = (size_t)env * N + po.p;
@@ -171,6 +212,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
     const vec3 g(md.gx, md.gy, md.gz);
     __syncthreads();
     int bad = INT_MAX;
+    float4 *tpf = tape + poff;  // this particle's entry of the current tape slot (x; v is S further)
     for (int s = 0; s < T; s++) {
         if (ACT && s % ra.stride == 0 && s / ra.stride < ra.F) {  // a new frame of the activation schedule begins
 #pragma unroll
@@ -185,15 +227,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
                 const vec3 v[4] = {vec3(sv[li.x]), vec3(sv[li.y]), vec3(sv[li.z]), vec3(sv[li.w])};
                 vec3 f[4];
                 tet_force(x, v, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, tr[j].act, f);
-                const int e = tid + j * blockDim.x;
-#pragma unroll
-                for (int k = 0; k < 4; k++) sf[k * M + e] = make_float4(f[k].x, f[k].y, f[k].z, 0.f);
+                const ushort4 ds = tr[j].dst;
+                sf[ds.x] = make_float4(f[0].x, f[0].y, f[0].z, 0.f); sf[ds.y] = make_float4(f[1].x, f[1].y, f[1].z, 0.f);
+                sf[ds.z] = make_float4(f[2].x, f[2].y, f[2].z, 0.f); sf[ds.w] = make_float4(f[3].x, f[3].y, f[3].z, 0.f);
             }
         }
         __syncthreads();
         float ax = 0.f, ay = 0.f, az = 0.f;
-        for (int q = po.beg; q < po.end; q++) {
-            const float4 c = sf[s_slots[q]];
+        for (int j = po.j0; j < po.val; j += rd.kpp) {
+            const float4 c = sf[s_row[j] + po.q];
             ax += c.x; ay += c.y; az += c.z;
         }
         ax = group_sum(ax, rd.kpp); ay = group_sum(ay, rd.kpp); az = group_sum(az, rd.kpp);
@@ -205,8 +247,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_fwd(const ModelDev md, 
             xq = make_float4(x1.x, x1.y, x1.z, xq.w);
             vq = make_float4(v1.x, v1.y, v1.z, 0.f);
             sx[po.lp] = xq; sv[po.lp] = vq;
-            float4 *slot = tape + (size_t)(2 * (s + 1)) * S;
-            slot[poff] = xq; slot[S + poff] = vq;
+            tpf += 2 * S;
+            tpf[0] = xq; tpf[S] = vq;
             const float chk = x1.x + x1.y + x1.z + v1.x + v1.y + v1.z;
             if (!(fabsf(chk) <= 3.0e38f) && bad == INT_MAX) bad = s;
         }
@@ -222,21 +264,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                                                               float4 *__restrict__ adjx, float4 *__restrict__ adjv, const float *__restrict__ frames,
                                                               int n_frames, int stride, const ResAct ra) {
     extern __shared__ float4 smem4[];
-    const int N = rd.N, M = rd.M, PL = 4 * M, L = rd.L;
+    const int N = rd.N, PL = rd.Ltot, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
-    float4 *sf = smem4 + 3 * L;  // [2][4 M]: adj_x contributions, then adj_v contributions, per element-vertex
+    float4 *sf = smem4 + 3 * L;  // [2][Ltot]: adj_x contributions, then adj_v contributions, per element-vertex (transposed gather layout)
     // dL/d(k_e, k_d, k_f, mu_c) and dL/dg: per-particle partial sums (only the particle's lead lane touches its entries):
-    // fp32 chunks of kFlushEvery substeps (contact: shared memory; gravity: registers) folded into fp64 masters (hazard
-    // H4), summed in particle order at the end: deterministic
+    // fp32 chunks of kFlushEvery substeps in shared memory (no registers held across the element phase) folded into fp64
+    // masters (hazard H4), summed in particle order at the end: deterministic
     double *dgc = reinterpret_cast<double *>(sf + 2 * PL);   // [kResAcc][N]
-    float *sgc = reinterpret_cast<float *>(dgc + kResAcc * N);  // [4][N]
-    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((N * (kResAcc * 8 + 4 * 4) + 15) & ~15));
+    float *sgc = reinterpret_cast<float *>(dgc + kResAcc * N);  // [kResAcc][N]
+    uint16_t *s_ptr = reinterpret_cast<uint16_t *>(reinterpret_cast<char *>(dgc) + ((N * (kResAcc * 8 + kResAcc * 4) + 15) & ~15));
     uint16_t *s_owner = s_ptr + (((N + 1) + 7) & ~7);
-    uint16_t *s_slots = s_owner + ((N + 7) & ~7);
+    uint16_t *s_row = s_owner + ((N + 7) & ~7);
     const int tid = threadIdx.x, env = blockIdx.x;
     TetReg tr[EPT];
     load_tets<EPT>(md, rd, env, tr);
-    load_csr(rd, s_ptr, s_owner, s_slots);
+    load_csr(rd, s_ptr, s_owner, s_row);
     __syncthreads();
     const PartOwn po = part_own(rd, s_ptr, s_owner);
     const size_t poff = (size_t)env * N + po.p;
@@ -255,8 +297,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
     if (po.lead)
-        for (int q = 0; q < kResAcc; q++) { dgc[q * N + po.p] = 0.0; if (q < 4) sgc[q * N + po.p] = 0.f; }
-    vec3 glv = zero3();  // sum over a chunk of substeps of lv (cotangent of v+): dL/dg = dt sum lv for a free particle
+        for (int q = 0; q < kResAcc; q++) { dgc[q * N + po.p] = 0.0; sgc[q * N + po.p] = 0.f; }
     const size_t frame_elems = (size_t)md.E * N * 3;
     const size_t gstride = (size_t)md.E * md.es[T_TET].cpad;
     float gm32 = 0.f;
@@ -268,8 +309,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     // the summed element contributions of the previous element phase, for this thread's particle (lead lane holds them)
     auto gather = [&](vec3 &dx, vec3 &dv) {
         float ax = 0.f, ay = 0.f, az = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;
-        for (int q = po.beg; q < po.end; q++) {
-            const int sl = s_slots[q];
+        for (int j = po.j0; j < po.val; j += rd.kpp) {
+            const int sl = s_row[j] + po.q;
             const float4 c = sf[sl], d = sf[PL + sl];
             ax += c.x; ay += c.y; az += c.z;
             cx += d.x; cy += d.y; cz += d.z;
@@ -281,6 +322,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
 #pragma unroll
     for (int j = 0; j < EPT; j++) gact[j] = 0.f;
     int act_frame = -1;
+    // running pointers / counters instead of per-substep 64-bit index products and divisions by the frame stride
+    const float4 *tp = tape + (size_t)(2 * (T - 1)) * S + poff;  // state slot of substep s - 1 is tp - 2 S
+    const size_t S2 = 2 * S;
+    // frame boundary bookkeeping: the state after substep s is frame (s + 1) / stride - 1 when stride divides s + 1
+    int fr_left = (T % stride);              // substeps until the next (lower) frame boundary: 0 = state T is one
+    int fr_idx = T / stride - 1;             // index of that frame
     for (int s = T - 1; s >= 0; s--) {
         if (ACT) {  // the frame of the activation schedule that holds during substep s
             const int f = s / ra.stride < ra.F ? s / ra.stride : ra.F - 1;
@@ -293,15 +340,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
         }
         // prefetch the start state of the previous substep while this one is processed
         float4 xp = xq, vp = vq;
-        if (po.lead && s > 0) { xp = tape[(size_t)(2 * (s - 1)) * S + poff]; vp = tape[(size_t)(2 * (s - 1) + 1) * S + poff]; }
+        tp -= S2;
+        if (po.lead && s > 0) { xp = tp[0]; vp = tp[S]; }
         if (s != T - 1) {  // contributions of the element phase of substep s + 1 (all lanes: the sums meet by shuffle)
             vec3 dx, dv;
             gather(dx, dv);
             bx += dx; bv += dv;
         }
         if (po.lead) {
-            if (cot && (s + 1) % stride == 0 && (s + 1) / stride <= n_frames) {
-                const float *c = cot + (size_t)((s + 1) / stride - 1) * frame_elems;
+            if (cot && fr_left == 0 && fr_idx < n_frames) {
+                const float *c = cot + (size_t)fr_idx * frame_elems;
                 bx += vec3(c[0], c[1], c[2]);
             }
             const float w = xq.w;
@@ -312,7 +360,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
             if (w > 0.0f) {
                 const vec3 dvf = (vec3(vnext) - v) - dt * g;
                 gm32 += -w * dot(dvf, lv);
-                if (md.want_gravity) glv += lv;
+                if (md.want_gravity) {  // dL/dg = dt sum lv over the free particles
+                    sgc[4 * N + po.p] += dt * lv.x; sgc[5 * N + po.p] += dt * lv.y; sgc[6 * N + po.p] += dt * lv.z;
+                }
             }
             float gp[4];
             contact_adjoint(cp, x, v, af, ax, av, gp);
@@ -337,11 +387,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 tet_adjoint(x, v, a, tr[j].b, tr[j].V, tr[j].mu, tr[j].lam, tr[j].kd, tr[j].act, ax, av, gmu, glam, gk, ga);
                 g32[j][0] += gmu; g32[j][1] += glam; g32[j][2] += gk;
                 if (ACT) gact[j] += ga;
-                const int e = tid + j * blockDim.x;
+                const ushort4 ds = tr[j].dst;
+                const unsigned dk[4] = {ds.x, ds.y, ds.z, ds.w};
 #pragma unroll
                 for (int k = 0; k < 4; k++) {
-                    sf[k * M + e] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
-                    sf[PL + k * M + e] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
+                    sf[dk[k]] = make_float4(ax[k].x, ax[k].y, ax[k].z, 0.f);
+                    sf[PL + dk[k]] = make_float4(av[k].x, av[k].y, av[k].z, 0.f);
                 }
             }
         }
@@ -352,12 +403,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                 gact[j] = 0.f;
             }
         }
+        if (fr_left == 0) { fr_left = stride; fr_idx--; }
+        fr_left--;
         if ((s & (kFlushEvery - 1)) == 0) {  // fold the fp32 chunk into fp64 (hazard H4)
             if (po.lead) {
 #pragma unroll
-                for (int q = 0; q < 4; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
-                dgc[4 * N + po.p] += (double)(dt * glv.x); dgc[5 * N + po.p] += (double)(dt * glv.y); dgc[6 * N + po.p] += (double)(dt * glv.z);
-                glv = zero3();
+                for (int q = 0; q < kResAcc; q++) { dgc[q * N + po.p] += (double)sgc[q * N + po.p]; sgc[q * N + po.p] = 0.f; }
             }
             // the fp64 masters live in global memory (each thread owns its entries; one update per kFlushEvery substeps),
             // which keeps 8 registers free for the element VJP
@@ -420,7 +471,7 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     std::vector<int> inv_p(N);
     for (int i = 0; i < N; i++) inv_p[m->perm_p[i]] = i;
     std::vector<ushort4> idx(M);
-    std::vector<uint16_t> ptr(N + 1, 0), slots((size_t)4 * M);
+    std::vector<uint16_t> ptr(N + 1, 0);
     std::vector<int> cnt(N + 1, 0);
     for (int e = 0; e < M; e++) {
         const int32_t *ix = d->tets + (size_t)m->hes[T_TET].perm[e] * 4;
@@ -430,11 +481,7 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     }
     for (int p = 0; p < N; p++) cnt[p + 1] += cnt[p];
     for (int p = 0; p <= N; p++) ptr[p] = (uint16_t)cnt[p];
-    std::vector<int> pos(cnt.begin(), cnt.end() - 1);
-    for (int e = 0; e < M; e++) {
-        const unsigned short li[4] = {idx[e].x, idx[e].y, idx[e].z, idx[e].w};
-        for (int k = 0; k < 4; k++) slots[pos[li[k]]++] = (uint16_t)(k * M + e);
-    }
+    const std::vector<ushort4> pid = idx;  // internal particle ids of every tet (idx becomes staging indices below)
     // staging indices by greedy 8-colouring of the (quarter-warp, vertex) read groups
     std::vector<uint16_t> rloc(N);
     int Lsp = 8;
@@ -476,29 +523,67 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     auto take = [&](size_t n) { char *q = p; p += (n + 255) & ~(size_t)255; return q; };
     ushort4 *d_idx = (ushort4 *)take(idx.size() * sizeof(ushort4));
     uint16_t *d_ptr = (uint16_t *)take(ptr.size() * 2);
-    uint16_t *d_slots = (uint16_t *)take(slots.size() * 2);
+
     // particle slots: most incident tets first (stable), so the lanes of a warp run near-equal gather loops
     std::vector<uint16_t> owner(N);
     for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
     std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
+    // transposed gather list (ResDev::dest / row): the j-th incidence (element order) of the particle in slot q -> row[j] + q
+    const int nthreads_ = res_threads(M), kpp_ = res_kpp(nthreads_, N);
+    std::vector<int> val(N);
+    for (int i = 0; i < N; i++) val[i] = cnt[i + 1] - cnt[i];
+    std::vector<uint16_t> row;
+    const int Ltot = res_rows(val, kpp_, &row);
+    const int maxval = (int)row.size() - 1;
+    std::vector<int> slot_of(N);
+    for (int q = 0; q < N; q++) slot_of[owner[q]] = q;
+    // Which of a particle's rows an incidence takes is free: pick it so that the eight lanes of a quarter-warp (eight
+    // consecutive tets, same vertex position) store into different 16-byte bank groups where possible (STS.128 is served
+    // a quarter-warp at a time); greedy, lowest free row first among the rows whose bank group is still unused.
+    std::vector<std::vector<char>> used(N);
+    for (int i = 0; i < N; i++) used[i].assign(val[i], 0);
+    std::vector<ushort4> dest(M);
+    for (int e0 = 0; e0 < M; e0 += 8) {
+        for (int k = 0; k < 4; k++) {
+            unsigned banks = 0;
+            for (int e = e0; e < std::min(M, e0 + 8); e++) {
+                const int pk = k == 0 ? pid[e].x : (k == 1 ? pid[e].y : (k == 2 ? pid[e].z : pid[e].w));
+                int pick = -1, fallback = -1;
+                for (int j = 0; j < val[pk]; j++) {
+                    if (used[pk][j]) continue;
+                    if (fallback < 0) fallback = j;
+                    if (!(banks >> ((row[j] + slot_of[pk]) & 7) & 1u)) { pick = j; break; }
+                }
+                if (pick < 0) pick = fallback;
+                used[pk][pick] = 1;
+                const unsigned short dk = (unsigned short)(row[pick] + slot_of[pk]);
+                banks |= 1u << (dk & 7);
+                if (k == 0) dest[e].x = dk; else if (k == 1) dest[e].y = dk; else if (k == 2) dest[e].z = dk; else dest[e].w = dk;
+            }
+        }
+    }
+    ushort4 *d_dest = (ushort4 *)take(dest.size() * sizeof(ushort4));
+    uint16_t *d_row = (uint16_t *)take(row.size() * 2);
     uint16_t *d_owner = (uint16_t *)take(owner.size() * 2);
     uint16_t *d_rloc = (uint16_t *)take(rloc.size() * 2);
     cudaError_t ce = cudaMemcpyAsync(d_owner, owner.data(), owner.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_rloc, rloc.data(), rloc.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * 2, cudaMemcpyHostToDevice, st);
-    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_slots, slots.data(), slots.size() * 2, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_dest, dest.data(), dest.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_row, row.data(), row.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
     if (ce != cudaSuccess) return cuda_fail(ce, "resident upload");
     ResHost *rh = new ResHost();
     rh->ept = M > kResMaxThreads ? 2 : 1;
     rh->rd.M = M; rh->rd.N = N;
-    rh->rd.nthreads = ((M + rh->ept - 1) / rh->ept + 31) / 32 * 32;
-    rh->rd.kpp = rh->rd.nthreads >= 4 * N ? 4 : (rh->rd.nthreads >= 2 * N ? 2 : 1);
+    rh->rd.nthreads = nthreads_;
+    rh->rd.kpp = kpp_;
     rh->rd.L = Lsp; rh->rd.rloc = d_rloc;
-    rh->rd.idx = d_idx; rh->rd.owner = d_owner; rh->rd.csr_ptr = d_ptr; rh->rd.csr_slots = d_slots;
-    rh->smem_fwd = res_smem(Lsp, N, M, 1, false);
-    rh->smem_adj = res_smem(Lsp, N, M, 2, true);
+    rh->rd.idx = d_idx; rh->rd.owner = d_owner; rh->rd.csr_ptr = d_ptr;
+    rh->rd.dest = d_dest; rh->rd.row = d_row; rh->rd.maxval = maxval; rh->rd.Ltot = Ltot;
+    rh->smem_fwd = res_smem(Lsp, N, Ltot, maxval, 1, false);
+    rh->smem_adj = res_smem(Lsp, N, Ltot, maxval, 2, true);
     m->res_host = rh;
     int rc = GS_OK;
 #define GS_RES_SMEM(E_, T_, BF_, BA_)                                                                  \
