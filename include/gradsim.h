@@ -241,6 +241,34 @@ int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_re
                 float *d_loss, float *d_adj_x, gs_stream stream);
 
 /*
+ * Soft silhouette rasteriser on a headless device buffer, and its adjoint: the image-space loss of
+ * the paper's pixels-to-parameters loop.  PAPER.md:168-172 (section 2.2: "replace discontinuous triangle mesh edges with
+ * smooth sigmoids"); the formula is the SoftRas silhouette as SPEC.md:251 states it (A22):
+ *   D_j(p) = sigmoid(delta d^2(p, boundary of triangle j) / sigma), delta = +1 inside / -1 outside, distances in NDC;
+ *   S(p) = 1 - prod_j (1 - D_j(p));   gs_loss_silhouette: L_e (+)= scale sum_p (S_e(p) - target_e(p))^2.
+ * Camera (HOST struct, read during the call): p_cam = R x + t (R row-major), a triangle is drawn iff all three vertices
+ * have z_cam > near_z, NDC (u, v) = (fx X / Z, fy Y / Z), pixel (i, j) centre at u = 2 (i + 1/2) / W - 1, v = 2 (j + 1/2) / H - 1.
+ * d_x [E][N][3] caller order (e.g. a state from gs_rollout / gs_tape_read); d_tris [n_tris][3] DEVICE int32 indices into
+ * the particles (any surface mesh: the cloth triangles, or the boundary faces of a tet mesh); images [E][H][W] fp32.
+ * gs_loss_silhouette: d_loss [E] (overwritten unless accumulate), d_adj_x [E][N][3] = dL/dx overwritten (may be NULL),
+ * d_image optional.  The result feeds gs_rollout_backward as d_adj_x_T or a frame cotangent.  d_scratch: DEVICE block of
+ * >= gs_raster_scratch_bytes, 256-byte aligned.  Silhouette channel only: colour / texture shading is not built.
+ */
+typedef struct {
+    float R[9], t[3];      /* world -> camera */
+    float fx, fy;          /* focal lengths in NDC units (1 / tan(fov / 2)) */
+    int32_t width, height;
+    float sigma;           /* edge blur, in squared NDC units */
+    float near_z;
+} gs_camera;
+size_t gs_raster_scratch_bytes(int n_envs, int n_particles, int n_tris);
+int gs_render_silhouette(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const gs_camera *cam,
+                         float *d_image, void *d_scratch, size_t scratch_bytes, gs_stream stream);
+int gs_loss_silhouette(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const gs_camera *cam,
+                       const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x, float *d_image,
+                       void *d_scratch, size_t scratch_bytes, gs_stream stream);
+
+/*
  * End-to-end convenience with HOST buffers (bench.py's e2e leg): ONE call uploads x0, v0 [E][N][3] and the loss
  * targets, runs gs_rollout, the loss, gs_rollout_backward, and downloads loss [E], dL/dx0, dL/dv0 [E][N][3] (each may
  * be NULL) and the parameter gradients listed in groups[] into h_grads[k] ([E][count] each).  Zeroes the model's

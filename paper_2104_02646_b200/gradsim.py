@@ -46,6 +46,19 @@ class gs_model_desc(C.Structure):
     ]
 
 
+class gs_camera(C.Structure):
+    _fields_ = [("R", C.c_float * 9), ("t", C.c_float * 3), ("fx", C.c_float), ("fy", C.c_float), ("width", C.c_int32), ("height", C.c_int32),
+                ("sigma", C.c_float), ("near_z", C.c_float)]
+
+
+def make_camera(R, t, fx, fy, width, height, sigma, near_z=1e-3):
+    c = gs_camera()
+    c.R = (C.c_float * 9)(*[float(v) for v in np.asarray(R, np.float64).reshape(9)])
+    c.t = (C.c_float * 3)(*[float(v) for v in np.asarray(t, np.float64).reshape(3)])
+    c.fx, c.fy, c.width, c.height, c.sigma, c.near_z = float(fx), float(fy), int(width), int(height), float(sigma), float(near_z)
+    return c
+
+
 # name -> (restype, argtypes); the list tests/test_abi.py checks against include/gradsim.h
 _vp, _sz, _int = C.c_void_p, C.c_size_t, C.c_int
 _descp = C.POINTER(gs_model_desc)
@@ -75,6 +88,9 @@ SIGNATURES = {
     "gs_check_finite": (_int, [_vp, _vp, C.POINTER(_int)]),
     "gs_loss_centroid": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
     "gs_loss_pos": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
+    "gs_raster_scratch_bytes": (_sz, [_int, _int, _int]),
+    "gs_render_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, _vp, _sz, _vp]),
+    "gs_loss_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gs_host_scratch_bytes": (_sz, [_vp, _vp, _int, _int]),
     "gs_rollout_loss_backward_host": (_int, [_vp, _vp, _vp, _vp, _int, _int, _vp, _vp, _vp, _vp, _int, C.POINTER(_int), C.POINTER(_vp), _vp, _sz, _vp]),
     "gs_launch_count": (C.c_uint64, []),
@@ -445,3 +461,35 @@ def loss_pos(x, ref, scale=1.0, loss=None, accumulate=False, want_adj=True):
     adj = torch.empty_like(x) if want_adj else None
     _check(lib().gs_loss_pos(E, N, _dp(x), _dp(_st(ref, (E, N, 3))), float(scale), int(accumulate), _dp(loss), _dp(adj), _stream()))
     return loss, adj
+
+
+# ------------------------------------------------------------------------------------------ soft silhouette rasteriser
+def _raster_args(x, tris):
+    torch = _torch()
+    E, N, _ = x.shape
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+    assert tris.is_cuda and tris.dtype == torch.int32 and tris.is_contiguous() and tris.ndim == 2 and tris.shape[1] == 3
+    nbytes = lib().gs_raster_scratch_bytes(E, N, int(tris.shape[0]))
+    return E, N, int(tris.shape[0]), _aligned_bytes(nbytes, x.device), nbytes
+
+
+def render_silhouette(x, tris, cam):
+    """x [E, N, 3] cuda fp32, tris [Mt, 3] cuda int32, cam a gs_camera -> silhouette images [E, H, W]."""
+    torch = _torch()
+    E, N, Mt, scratch, nbytes = _raster_args(x, tris)
+    img = torch.empty((E, cam.height, cam.width), dtype=torch.float32, device=x.device)
+    _check(lib().gs_render_silhouette(E, N, _dp(x), Mt, _dp(tris), C.byref(cam), _dp(img), _dp(scratch), nbytes, _stream()))
+    return img
+
+
+def loss_silhouette(x, tris, cam, target, scale=None, loss=None, accumulate=False, want_adj=True, want_image=False):
+    """L_e (+)= scale sum_p (S_e(p) - target_e(p))^2 (scale defaults to 1 / (W H): the pixelwise mean) and dL/dx."""
+    torch = _torch()
+    E, N, Mt, scratch, nbytes = _raster_args(x, tris)
+    scale = 1.0 / (cam.width * cam.height) if scale is None else float(scale)
+    loss = torch.zeros(E, dtype=torch.float32, device=x.device) if loss is None else loss
+    adj = torch.empty_like(x) if want_adj else None
+    img = torch.empty((E, cam.height, cam.width), dtype=torch.float32, device=x.device) if want_image else None
+    _check(lib().gs_loss_silhouette(E, N, _dp(x), Mt, _dp(tris), C.byref(cam), _dp(_st(target, (E, cam.height, cam.width))), scale, int(accumulate),
+                                    _dp(loss), _dp(adj), _dp(img), _dp(scratch), nbytes, _stream()))
+    return loss, adj, img
