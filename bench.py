@@ -481,6 +481,68 @@ def measure(args, config, rank, world, local, dist, with_cpu):
     }
 
 
+RASTER_FLOPS_FWD, RASTER_FLOPS_BWD = 95, 325  # per evaluated (pixel, triangle) pair: 3 point-segment distances, 3 edge functions,
+# a sigmoid (forward); the adjoint walks the pairs twice and adds the closest-edge weights
+
+
+def raster_record(devs, steps):
+    """the soft silhouette rasteriser + adjoint on E = 64 deformed copies of config 1's 32 x 32 cloth
+    (1922 triangles), 256 x 256 pixels.  ALU-bound: flops = evaluated (pixel, triangle) pairs (those the tile culling
+    keeps, counted here from the oracle's projection) x the per-pair counts above."""
+    import torch
+
+    from oracle import raster_oracle as ro
+    from paper_2104_02646_b200 import gradsim as gs
+    from paper_2104_02646_b200 import scenes
+
+    sc = scenes.make_scene(1)
+    E, W, H, sigma = 64, 256, 256, 1e-4
+    r = scenes.rng_for(1, "misc", 123)
+    x = (sc.x0[0][None] + 0.003 * r.normal(size=(E,) + sc.x0[0].shape)).astype(np.float32)
+    th = 0.4
+    R = np.array([[1, 0, 0], [0, np.cos(-1.0), -np.sin(-1.0)], [0, np.sin(-1.0), np.cos(-1.0)]]) @ np.array([[np.cos(th), 0, np.sin(th)], [0, 1, 0], [-np.sin(th), 0, np.cos(th)]])
+    cam_args = (R, np.array([-0.15, 0.1, 0.6]), 2.0, 2.0, W, H, sigma)
+    cg, co = gs.make_camera(*cam_args), ro.Camera(*cam_args)
+    xd = torch.as_tensor(x, device=devs)
+    tris = torch.as_tensor(np.ascontiguousarray(sc.tris, dtype=np.int32), device=devs)
+    target = gs.render_silhouette(torch.as_tensor(x + np.float32(0.004), device=devs), tris, cg)
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    ms_f = timed(lambda: gs.render_silhouette(xd, tris, cg))
+    ms_b = timed(lambda: gs.loss_silhouette(xd, tris, cg, target))
+    # evaluated pairs: triangles whose grown bounding box meets a 16 x 16 tile, x 256 pixels (environment 0, scaled by E)
+    ndc, z = ro.project(x[0].astype(np.float64), co)
+    q = ndc[sc.tris]
+    m = np.sqrt(40.0 * sigma)
+    lo, hi = q.min(1) - m, q.max(1) + m
+    tu0 = np.arange(0, W, 16) * 2.0 / W - 1.0
+    tv0 = np.arange(0, H, 16) * 2.0 / H - 1.0
+    nx = ((lo[:, None, 0] <= tu0[None] + 32.0 / W) & (hi[:, None, 0] >= tu0[None])).sum(1)
+    ny = ((lo[:, None, 1] <= tv0[None] + 32.0 / H) & (hi[:, None, 1] >= tv0[None])).sum(1)
+    pairs = float((nx * ny).sum()) * 256 * E
+    t0 = time.perf_counter()
+    ro.silhouette(x[0], sc.tris, co)
+    t_cpu = time.perf_counter() - t0
+    return {"workload": f"config1 cloth 32x32 ({sc.tris.shape[0]} triangles) x {E} environments, {W}x{H} pixels, sigma {sigma}",
+            "ms_render": ms_f, "ms_loss_and_adjoint": ms_b, "evaluated_pairs": pairs,
+            "roofline": {"bound": "alu", "kernel": "k_rs_forward", "achieved": pairs * RASTER_FLOPS_FWD / (ms_f * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "frac": pairs * RASTER_FLOPS_FWD / (ms_f * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                         "adjoint_frac": pairs * RASTER_FLOPS_BWD / (ms_b * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                         "note": "ms_render includes projection + triangle packing; flops per pair counted from csrc/gs_raster.cu"},
+            "cpu_baseline": {"kind": "oracle", "seconds_per_image": t_cpu, "sample": "one environment, forward only, fp64 numpy", "images_per_s_gpu": E / (ms_f * 1e-3)}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -520,6 +582,7 @@ def main():
         sub = measure(args, 3, rank, world, local, dist, with_cpu)
     if rank == 0:
         line["config3"] = sub
+        line["raster"] = raster_record(f"cuda:{local}", args.steps) if (with_cpu and args.config == 4 and not args.small and not args.substeps) else None
         line["paper_context"] = "Table 4-right: 3721 Hz fwd / 1429 Hz bwd at 10k tets (3.7e7 / 1.4e7 tet-steps/s), hardware unstated (PAPER.md:464-478)"
         print(json.dumps(line))
     if dist is not None:
