@@ -26,8 +26,6 @@
 #include <algorithm>
 #include <climits>
 #include <vector>
-#include <cstdio>
-#include <cstdlib>
 
 #include "gs_elements.cuh"
 #include "gs_internal.h"
@@ -879,13 +877,6 @@ int configure_stream_kernels(gs_model *m) {
     // free up first are placed unevenly over the SMs.  The rule keeps the launch attribute while the largest type has
     // at most two tiles per SM.
     m->pdl = items <= 2LL * sms;
-    // experiment overrides (not part of the interface)
-    if (const char *q = getenv("GS_PDL")) m->pdl = atoi(q) != 0;
-    if (const char *q = getenv("GS_OCC_FWD")) m->occ_fwd = std::min(m->occ_fwd, std::max(1, atoi(q)));
-    if (const char *q = getenv("GS_OCC_ADJ")) m->occ_adj = std::min(m->occ_adj, std::max(1, atoi(q)));
-    if (getenv("GS_DEBUG"))
-        fprintf(stderr, "gradsim: element kernels smem fwd %d adj %d bytes, CTAs/SM fwd %d adj %d, pmax %d/%d/%d lmax %d/%d/%d\n", m->smem_fwd, m->smem_adj,
-                m->occ_fwd, m->occ_adj, es[0].pmax, es[1].pmax, es[2].pmax, es[0].lmax, es[1].lmax, es[2].lmax);
     return rc;
 }
 
