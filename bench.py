@@ -77,12 +77,12 @@ def resident_stream_bytes(sc, adjoint):
 # kernels were captured at 64 substeps: bytes per substep of the launch, scaled by the rollout length.
 NCU_TRAFFIC = {
     "config4-large-1000000tets-522242tris": {
-        "source": "profiles/r1d_ncu_config4_streaming.md (kernels of commit 0aaa43c)",
-        "k_elements_fwd": ("per_launch", 161568256), "k_particles_fwd": ("per_launch", 22874368),
-        "k_elements_adj": ("per_launch", 204752896), "k_particles_adj": ("per_launch", 40113664),
+        "source": "profiles/r2_ncu_config4_streaming.md (round-2 kernels; k_particles_adj still from profiles/r1d_ncu_config4_streaming.md)",
+        "k_elements_fwd": ("per_launch", 161725952), "k_particles_fwd": ("per_launch", 24154368),
+        "k_elements_adj": ("per_launch", 205242880), "k_particles_adj": ("per_launch", 40113664),
     },
-    "config3-sysid-E1024": {"source": "profiles/r1d_ncu_config3_resident.md (kernels of commit 0aaa43c)",
-                            "k_resident_fwd": ("per_substep", 3468752), "k_resident_adj": ("per_substep", 4660056)},
+    "config3-sysid-E1024": {"source": "profiles/r2_ncu_config3_resident.md (round-2 kernels, 64-substep capture gpurun_out/r2_ncu_res.ncu-rep)",
+                            "k_resident_fwd": ("per_substep", 3495948), "k_resident_adj": ("per_substep", 4730524)},
 }
 
 
