@@ -124,7 +124,7 @@ def _env_scene(sc, e):
     """environment e of a batched scene as a scene of its own (inputs only)."""
     s1 = copy.copy(sc)
     s1.n_envs = 1
-    for k in ("x0", "v0", "mass", "tet_mu", "tet_lambda", "tet_damp", "tri_mu", "tri_lambda", "tri_damp", "ke", "kd", "kf", "mu_c"):
+    for k in ("x0", "v0", "mass", "tet_mu", "tet_lambda", "tet_damp", "tri_mu", "tri_lambda", "tri_damp", "ke", "kd", "kf", "mu_c", "k_drag", "k_lift"):
         setattr(s1, k, getattr(sc, k)[e:e + 1])
     s1.truth = {k: v[e:e + 1] for k, v in sc.truth.items()}
     return s1
