@@ -262,6 +262,8 @@ struct TilePipe {
         bulk_g2s(idbuf + slot * pmax, blk, pmax * 4, bars + 2 + slot, pol_stream);
         bulk_g2s(locbuf + par * pmax, blk + pmax * 4, pmax * 2, bars + 2 + slot, pol_stream);
     }
+    // The producer work of a tile is dealt to lane 0 of three different warps (load_ids: warp 0, the gather-list copy:
+    // warp 1, the L2 prefetches: warp 2), so that no warp is a tile's worth of issue slots behind the others at the barrier.
     __device__ __forceinline__ void load_static(int item, int b) {  // one thread
         unsigned tile, env;
         split(item, tile, env);
@@ -269,6 +271,11 @@ struct TilePipe {
         const char *rec = es.rec + (size_t)tile * es.rec_bytes;
         mbar_expect_tx(bars + b, S::kEmitBytes);
         bulk_g2s(tv.emit, rec + S::R::oSlots, S::kEmitBytes, bars + b, pol_stream);
+    }
+    __device__ __forceinline__ void prefetch_static(int item) {  // one thread
+        unsigned tile, env;
+        split(item, tile, env);
+        const char *rec = es.rec + (size_t)tile * es.rec_bytes;
         // the thread-private part of the record goes to L2 now and to registers (load_regs) one tile later
         bulk_prefetch_l2(rec, S::R::oSlots, pol_stream);
         if (S::kPar) bulk_prefetch_l2(es.par + ((size_t)env * es.n_tiles + tile) * (3 * kTileElems), S::kPar, pol_stream);
@@ -321,8 +328,9 @@ struct TilePipe {
         if (tid == 0) {
             load_ids(first, 0, 0);
             if (cnt > 1) load_ids(first + G, 1, 1);
-            load_static(first, 0);
         }
+        if (tid == 32) load_static(first, 0);
+        if (tid == 64) prefetch_static(first);
         ElemRegs<TYPE> er;
         load_regs(first, er);
         mbar_wait(bars + 2, 0);
@@ -336,10 +344,9 @@ struct TilePipe {
             mbar_wait(bars + (i & 1), (i >> 1) & 1);
             if (i + 1 < cnt) mbar_wait(bars + 2 + s3n, (q3 + (s3n == 0 ? 1 : 0)) & 1);
             __syncthreads();
-            if (tid == 0) {
-                if (i + 2 < cnt) load_ids(item + 2 * G, s3nn, i & 1);
-                if (i + 1 < cnt) load_static(item + G, (i + 1) & 1);
-            }
+            if (tid == 0 && i + 2 < cnt) load_ids(item + 2 * G, s3nn, i & 1);
+            if (tid == 32 && i + 1 < cnt) load_static(item + G, (i + 1) & 1);
+            if (tid == 64 && i + 1 < cnt) prefetch_static(item + G);
             if (i + 1 < cnt) gather(item + G, s3n, (i + 1) & 1);
             unsigned tile, env;
             split(item, tile, env);
@@ -374,8 +381,9 @@ struct TilePipe {
         if (tid == 0) {
             load_ids(first, 0, 0);
             if (item_n < n_items) load_ids(item_n, 1, 1);
-            load_static(first, 0);
         }
+        if (tid == 32) load_static(first, 0);
+        if (tid == 64) prefetch_static(first);
         ElemRegs<TYPE> er;
         load_regs(first, er);
         mbar_wait(bars + 2, 0);
@@ -394,9 +402,10 @@ struct TilePipe {
                 const int item_nn = kQueue ? claimed : item_n + G;  // item i+2
                 if (kQueue) *next_slot = claimed;                   // read by everybody after the next barrier
                 if (has_n && item_nn < n_items) load_ids(item_nn, s3nn, i & 1);
-                if (has_n) load_static(item_n, (i + 1) & 1);
                 if (kQueue) claimed = (queue && claimed < n_items) ? 2 * G + atomicAdd(ctr, 1) : n_items;  // item i+3
             }
+            if (tid == 32 && has_n) load_static(item_n, (i + 1) & 1);
+            if (tid == 64 && has_n) prefetch_static(item_n);
             if (has_n) gather(item_n, s3n, (i + 1) & 1);
             unsigned tile, env;
             split(item, tile, env);
