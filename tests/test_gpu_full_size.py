@@ -290,3 +290,37 @@ def test_config4_full_rollout_properties():
     g2 = m.param_grads("tet_mu")
     assert rel_inf(host(a2), 2 * host(a1)) <= 1e-4
     assert rel_inf(host(g2), 2 * host(g1)) <= 1e-4
+
+
+@pytest.mark.parametrize("n,T", [(32, 512), (512, 96)])
+def test_contact_rich_rollout_with_smooth_contact_is_strict(n, T):
+    """A contact-rich scene whose contact force is SMOOTH, held to the stated tolerances with no relaxed branch (ADVICE
+    round 1).  The sheet starts in resting contact at the equilibrium penetration c = -m g / k_e = -9.8e-5 m with seeded
+    in-plane velocities (0.1 m/s) and 1e-3 m/s of vertical noise (oscillation amplitude 3e-6 m: no particle ever leaves the
+    plane), with k_d = 0 (no normal damping, whose switch at v_n = 0 is a kink of the force) and mu_c = 1e3 (always the stick
+    branch: f_f = -k_f v_t).  Then f_contact = -k_e c n - k_f v_t on every particle at every substep, linear in the state,
+    and the whole rollout is smooth: measured with the oracle alone, 1e-7 m of noise on x0 moves dL/dx0 by 5e-9 here, against
+    21 % with k_d = 10 (every particle crosses v_n = 0 every ~19 substeps, and backpropagation through a kink of a C0
+    force is discontinuous in the state: "these forces are only C0 continuous").  Compared strictly: xT, loss,
+    dL/dx0, dL/dv0, dL/dm, dL/dk_e, dL/dk_f -- the contact adjoint carries all of them.  The elastic gradients are not
+    compared here: stick friction freezes the sheet, so they are zero up to noise in the oracle itself (their strict
+    comparisons are the airborne and small-variant tests).  32 x 32 over 512 substeps, and config 4's 512 x 512 sheet
+    (262 144 particles) over 96 substeps."""
+    sc = scenes.cloth_scene(config=1, n=n, n_substeps=T, y0=-0.1 * 9.8 / 1e4, pins=(n == 32))
+    r = scenes.rng_for(1, "misc", 500 + n)
+    v0 = r.normal(0.0, 0.1, sc.v0.shape)
+    v0[..., 1] = r.normal(0.0, 1e-3, sc.v0.shape[:2])
+    v0[:, sc.pinned.astype(bool)] = 0.0
+    sc.v0 = v0.astype(np.float32)
+    sc.kd[:] = 0.0
+    sc.mu_c[:] = 1e3
+    ref = orc.run_scene(sc)
+    assert ref["xT"][..., 1].max() < 0 and np.abs(ref["g_kf"]).max() > 0 and np.abs(ref["g_mu_c"]).max() == 0  # in contact, stick only
+    got = gpu_run_scene(sc, ref["target"])
+    assert got["bad"] == -1
+    assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * sc.extent()
+    assert rel_inf(got["loss"], ref["loss"]) <= TOL_GRAD
+    errs = {k: rel_inf(got[k], ref[k]) for k in list(STATE_GRADS) + ["g_mass", "g_ke", "g_kf"]}
+    _report({"test": f"smooth_contact_{n}x{n}", "errors": errs, "relaxed": {}})
+    for k, e in errs.items():
+        assert e <= TOL_GRAD, (k, e)
