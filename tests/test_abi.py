@@ -82,6 +82,18 @@ def test_argument_errors_without_a_device(lib_path):
     d = gs.gs_model_desc()
     d.n_particles, d.n_envs = 0, 1
     assert L.gs_model_workspace_bytes(C.byref(d)) == 0
+    # round-2 entry points: null handles / bad sizes come back as codes
+    assert L.gs_actuation_bytes(None, 4) == 0
+    assert L.gs_actuation_create(None, 4, 8, None, 0, None) == gs.GS_EINVAL
+    assert L.gs_set_actuation(None, 0, None, None) == gs.GS_EINVAL
+    assert L.gs_actuation_grads(None, 0, None, None) == gs.GS_EINVAL
+    assert L.gs_set_actuation_frame(None, 0) == gs.GS_EINVAL
+    assert L.gs_request_grads(None, gs.GROUPS["gravity"], 1) == gs.GS_EINVAL
+    assert L.gs_host_scratch_bytes(None, None, 0, 1) == 0
+    assert L.gs_raster_scratch_bytes(0, 10, 3) == 0 and L.gs_raster_scratch_bytes(1, 10, 3) > 0
+    cam = gs.make_camera([1, 0, 0, 0, 1, 0, 0, 0, 1], [0, 0, 1], 1.0, 1.0, 8, 8, 1e-3)
+    assert L.gs_render_silhouette(1, 4, None, 0, None, C.byref(cam), None, None, 0, None) == gs.GS_EINVAL  # image is null
+    assert L.gs_loss_silhouette(1, 4, None, 0, None, C.byref(cam), None, 1.0, 0, None, None, None, None, 0, None) == gs.GS_EINVAL
 
 
 def test_product_path_does_not_import_the_oracle():

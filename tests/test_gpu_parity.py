@@ -666,3 +666,41 @@ def test_aero_rollout_and_gradients(config):
     for k in ["adj_x0", "adj_v0"] + ["g_" + g for g in _grad_groups(sc) + ["k_drag", "k_lift"]]:
         assert np.abs(ref[k]).max() > 0, k
         assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
+
+
+def test_error_paths_of_the_round2_entry_points():
+    sc = scenes.make_scene(1, small=True)
+    m = gs.Model(sc)
+    L = gs.lib()
+    z = torch.zeros((2, 1, sc.tris.shape[0]), device="cuda:0")
+    assert L.gs_set_actuation(m.h, 1, gs._dp(z), gs._stream()) == gs.GS_ESTATE              # no schedule attached
+    with pytest.raises(gs.GradSimError) as e:
+        m.param_grads("hinge_theta0")                                                          # read from the actuation accumulators
+    assert e.value.code == gs.GS_ESTATE
+    with pytest.raises(gs.GradSimError) as e:
+        m.param_grads("wind")
+    assert e.value.code == gs.GS_EINVAL
+    with pytest.raises(gs.GradSimError) as e:
+        m.request_grads("mass")
+    assert e.value.code == gs.GS_EINVAL
+    mem = torch.empty(1024, dtype=torch.uint8, device="cuda:0")
+    assert L.gs_actuation_create(m.h, 4, 8, gs._dp(mem), 1024, gs._stream()) == gs.GS_EINVAL  # block too small
+    m.actuation(3, 8)
+    with pytest.raises(gs.GradSimError) as e:
+        m.set_actuation_frame(3)
+    assert e.value.code == gs.GS_EINVAL
+    assert L.gs_set_actuation(m.h, 7, gs._dp(z), gs._stream()) == gs.GS_EINVAL               # unknown kind
+    with pytest.raises(gs.GradSimError) as e:
+        m.set_params("k_drag", dev(np.full((1, 1), -1.0, np.float32)))
+    assert e.value.code == gs.GS_EINVAL
+    # the host entry point refuses a frame stride a checkpointed tape cannot serve, and a scratch block that is too small
+    tape = m.tape(64, 16)
+    hx = torch.as_tensor(sc.x0).pin_memory()
+    with pytest.raises(gs.GradSimError) as e:
+        m.rollout_loss_backward_host(tape, hx, hx, torch.zeros((8, 1, 3)).pin_memory(), loss="centroid_traj", frame_stride=8)
+    assert e.value.code == gs.GS_EINVAL
+    x = dev(sc.x0)
+    tris = torch.as_tensor(np.ascontiguousarray(sc.tris, dtype=np.int32), device="cuda:0")
+    cam = gs.make_camera(np.eye(3), [0, 0, 1], 1.0, 1.0, 16, 16, 1e-3)
+    img = torch.empty((1, 16, 16), device="cuda:0")
+    assert L.gs_render_silhouette(1, sc.n_particles, gs._dp(x), int(tris.shape[0]), gs._dp(tris), gs.C.byref(cam), gs._dp(img), gs._dp(mem), 1024, gs._stream()) == gs.GS_EINVAL
