@@ -79,19 +79,24 @@ static size_t res_smem(int L, int N, int Ltot, int maxval, int planes, bool adj)
 }
 static int res_threads(int M) { const int ept = M > kResMaxThreads ? 2 : 1; return ((M + ept - 1) / ept + 31) / 32 * 32; }
 static int res_kpp(int nthreads, int N) { return nthreads >= 4 * N ? 4 : (nthreads >= 2 * N ? 2 : 1); }
-// rows of the transposed gather list from the valences (any order): row[j] (maxval + 1 entries); returns the padded total
+// rows of the transposed gather list from the valences (any order): row[j] (maxval + 1 entries); returns the padded total.
+// Row starts are placed at prescribed residues modulo 8 (the 16-byte bank group of entry row[j] + q is (row[j] + q) mod 8):
+// the rows a lane group reads in the same iteration (kpp = 2: rows 2i, 2i + 1; kpp = 4: rows 4i .. 4i + 3) must differ by
+// 8 / kpp so that a quarter-warp's LDS.128 is conflict-free, and beyond that the residues cycle through all eight values,
+// which gives the store side (res_dest) up to eight bank groups to choose from for every incidence of a particle.
 static int res_rows(std::vector<int> val, int kpp, std::vector<uint16_t> *row) {
+    static const int kRes2[8] = {0, 4, 1, 5, 2, 6, 3, 7}, kRes4[8] = {0, 2, 4, 6, 1, 3, 5, 7};
     std::sort(val.begin(), val.end(), [](int a, int b) { return a > b; });
-    const int maxval = val.empty() ? 0 : val[0], want = (8 / kpp) & 7;  // row stride modulo 8 (kpp = 1: no constraint)
+    const int maxval = val.empty() ? 0 : val[0];
     int off = 0;
     if (row) row->assign(maxval + 1, 0);
     for (int j = 0; j < maxval; j++) {
+        const int want = kpp == 2 ? kRes2[j & 7] : (kpp == 4 ? kRes4[j & 7] : (j & 7));
+        while ((off & 7) != want) off++;
         int cnt = 0;
         while (cnt < (int)val.size() && val[cnt] > j) cnt++;
         if (row) (*row)[j] = (uint16_t)off;
-        int stride = cnt;
-        if (kpp > 1) while ((stride & 7) != want) stride++;
-        off += stride;
+        off += cnt;
     }
     if (row) (*row)[maxval] = (uint16_t)off;
     return off;
@@ -514,6 +519,33 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
         };
         for (int e = 0; e < M; e++) { assign(idx[e].x); assign(idx[e].y); assign(idx[e].z); assign(idx[e].w); }
         for (int q = 0; q < N; q++) assign(q);  // particles no tet touches
+        // local search: a quarter-warp's LDS.128 of vertex k takes as many wavefronts as its fullest bank group holds
+        // DISTINCT particles; move single particles to another colour while that lowers the total (a few sweeps)
+        auto group_cost = [&](int g) {
+            int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0}, mx = 0;
+            for (int r : groups[g]) mx = std::max(mx, ++cnt[colour[r]]);
+            return mx;
+        };
+        for (int sweep = 0; sweep < 8; sweep++) {
+            bool improved = false;
+            for (int q = 0; q < N; q++) {
+                if (of_part[q].empty()) continue;
+                int base = 0;
+                for (int g : of_part[q]) base += group_cost(g);
+                const int c0 = colour[q];
+                int best = c0, best_cost = base;
+                for (int cc = 0; cc < 8; cc++) {
+                    if (cc == c0 || csize[cc] >= cap) continue;
+                    colour[q] = cc;
+                    int cost = 0;
+                    for (int g : of_part[q]) cost += group_cost(g);
+                    if (cost < best_cost) { best_cost = cost; best = cc; }
+                }
+                colour[q] = best;
+                if (best != c0) { csize[c0]--; csize[best]++; improved = true; }
+            }
+            if (!improved) break;
+        }
         std::fill(csize.begin(), csize.end(), 0);
         for (int q = 0; q < N; q++) { rloc[q] = (uint16_t)(colour[q] + 8 * csize[colour[q]]); csize[colour[q]]++; }
         for (int cc = 0; cc < 8; cc++) Lsp = std::max(Lsp, 8 * csize[cc]);
@@ -528,8 +560,26 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     std::vector<uint16_t> owner(N);
     for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
     std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
-    // transposed gather list (ResDev::dest / row): the j-th incidence (element order) of the particle in slot q -> row[j] + q
     const int nthreads_ = res_threads(M), kpp_ = res_kpp(nthreads_, N);
+    {
+        // within a class of equal valence the order is free: arrange it so that the lead lanes of a quarter-warp (8 / kpp
+        // particle slots) own particles in different 16-byte bank groups of the staging arrays -- their STS.128 of x, v
+        // (and adj_f) after the particle phase are then conflict-free where the class is large enough
+        const int per = 8 / kpp_;
+        for (int a = 0; a < N;) {
+            int b = a;
+            const int va = cnt[owner[a] + 1] - cnt[owner[a]];
+            while (b < N && cnt[owner[b] + 1] - cnt[owner[b]] == va) b++;
+            for (int i = a; i < b; i++) {
+                unsigned banks = 0;
+                for (int j = i - i % per; j < i; j++) banks |= 1u << (rloc[owner[j]] & 7);
+                for (int j = i; j < b; j++)
+                    if (!(banks >> (rloc[owner[j]] & 7) & 1u)) { std::swap(owner[i], owner[j]); break; }
+            }
+            a = b;
+        }
+    }
+    // transposed gather list (ResDev::dest / row): the j-th incidence (element order) of the particle in slot q -> row[j] + q
     std::vector<int> val(N);
     for (int i = 0; i < N; i++) val[i] = cnt[i + 1] - cnt[i];
     std::vector<uint16_t> row;
@@ -560,6 +610,36 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
                 banks |= 1u << (dk & 7);
                 if (k == 0) dest[e].x = dk; else if (k == 1) dest[e].y = dk; else if (k == 2) dest[e].z = dk; else dest[e].w = dk;
             }
+        }
+    }
+    {
+        // local search on the store side: a quarter-warp's STS.128 of vertex k takes as many wavefronts as its fullest
+        // bank group holds entries; swap the rows of two incidences of one particle while that lowers the total
+        auto dk = [&](int e, int k) -> unsigned short & { return k == 0 ? dest[e].x : (k == 1 ? dest[e].y : (k == 2 ? dest[e].z : dest[e].w)); };
+        auto grp_cost = [&](int e, int k) {
+            int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0}, mx = 0;
+            const int e0 = e & ~7;
+            for (int f = e0; f < std::min(M, e0 + 8); f++) mx = std::max(mx, ++cnt[dk(f, k) & 7]);
+            return mx;
+        };
+        std::vector<std::vector<std::pair<int, int>>> inc(N);
+        for (int e = 0; e < M; e++) {
+            const unsigned short pk[4] = {pid[e].x, pid[e].y, pid[e].z, pid[e].w};
+            for (int k = 0; k < 4; k++) inc[pk[k]].push_back({e, k});
+        }
+        for (int sweep = 0; sweep < 8; sweep++) {
+            bool improved = false;
+            for (int q = 0; q < N; q++)
+                for (size_t a = 0; a < inc[q].size(); a++)
+                    for (size_t b = a + 1; b < inc[q].size(); b++) {
+                        const int ea = inc[q][a].first, ka = inc[q][a].second, eb = inc[q][b].first, kb = inc[q][b].second;
+                        if ((ea & ~7) == (eb & ~7) && ka == kb) continue;  // same store instruction of the same quarter-warp
+                        const int before = grp_cost(ea, ka) + grp_cost(eb, kb);
+                        std::swap(dk(ea, ka), dk(eb, kb));
+                        if (grp_cost(ea, ka) + grp_cost(eb, kb) < before) improved = true;
+                        else std::swap(dk(ea, ka), dk(eb, kb));
+                    }
+            if (!improved) break;
         }
     }
     ushort4 *d_dest = (ushort4 *)take(dest.size() * sizeof(ushort4));
