@@ -74,7 +74,7 @@ static inline size_t al16(size_t n) { return (n + 15) & ~(size_t)15; }
 // then float[7][N] chunks
 constexpr int kResAcc = 7;
 static size_t res_smem(int L, int N, int Ltot, int maxval, int planes, bool adj) {
-    return (size_t)(adj ? 7 : 2) * L * sizeof(float4) + (size_t)planes * Ltot * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + kResAcc * 4)) : 0) +
+    return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * Ltot * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + kResAcc * 4)) : 0) +
            al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)(maxval + 1) * 2);
 }
 static int res_threads(int M) { const int ept = M > kResMaxThreads ? 2 : 1; return ((M + ept - 1) / ept + 31) / 32 * 32; }
@@ -186,11 +186,6 @@ __device__ __forceinline__ PartOwn part_own(const ResDev &rd, const uint16_t *s_
     o.val = o.is_p ? s_ptr[o.p + 1] - s_ptr[o.p] : 0;
     return o;
 }
-__device__ __forceinline__ void res_cp_async16(void *smem_dst, const void *gmem_src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void res_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void res_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ float group_sum(float v, int kpp) {
     if (kpp >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
     if (kpp >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
@@ -276,11 +271,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     extern __shared__ float4 smem4[];
     const int N = rd.N, PL = rd.Ltot, L = rd.L;
     float4 *sx = smem4, *sv = smem4 + L, *sa = smem4 + 2 * L;
-    // the particle state of the adjoint lives in shared memory between particle phases, so that no register of it is held
-    // across the element phase (the VJP of a tet needs ~90): running cotangents sbx, sbv and the prefetched start state of
-    // the previous substep sxn, svn (cp.async, one substep ahead)
-    float4 *sbx = smem4 + 3 * L, *sbv = smem4 + 4 * L, *sxn = smem4 + 5 * L, *svn = smem4 + 6 * L;
-    float4 *sf = smem4 + 7 * L;  // [2][Ltot]: adj_x contributions, then adj_v contributions, per element-vertex (transposed gather layout)
+    float4 *sf = smem4 + 3 * L;  // [2][Ltot]: adj_x contributions, then adj_v contributions, per element-vertex (transposed gather layout)
     // dL/d(k_e, k_d, k_f, mu_c) and dL/dg: per-particle partial sums (only the particle's lead lane touches its entries):
     // fp32 chunks of kFlushEvery substeps in shared memory (no registers held across the element phase) folded into fp64
     // masters (hazard H4), summed in particle order at the end: deterministic
@@ -301,13 +292,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     cp.ke = md.ke[env]; cp.kd = md.kd[env]; cp.kf = md.kf[env]; cp.mu = md.muc[env];
     const vec3 g(md.gx, md.gy, md.gz);
     const float dt = md.dt;
+    vec3 bx = zero3(), bv = zero3();       // running cotangents of the lead thread's particle
+    float4 xq = make_float4(0.f, 0.f, 0.f, 0.f), vq = xq, vnext = xq;
     const float *cot = nullptr;
     if (po.lead) {
-        sbx[po.lp] = adjx[poff]; sbv[po.lp] = adjv[poff];
-        sv[po.lp] = tape[(size_t)(2 * T + 1) * S + poff];  // v after the last substep: "v+" of the first adjoint substep
-        res_cp_async16(sxn + po.lp, tape + (size_t)(2 * (T - 1)) * S + poff);
-        res_cp_async16(svn + po.lp, tape + (size_t)(2 * (T - 1) + 1) * S + poff);
-        res_cp_async_commit();
+        bx = vec3(adjx[poff]); bv = vec3(adjv[poff]);
+        vnext = tape[(size_t)(2 * T + 1) * S + poff];
+        xq = tape[(size_t)(2 * (T - 1)) * S + poff]; vq = tape[(size_t)(2 * (T - 1) + 1) * S + poff];
         if (frames) cot = frames + ((size_t)env * N + md.perm_p[po.p]) * 3;
     }
     if (po.lead)
@@ -352,15 +343,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
                     if (tr[j].on) tr[j].act = ra.tet[(size_t)f * ra.fstride + (size_t)env * md.es[T_TET].cpad + tid + j * blockDim.x];
             }
         }
+        // prefetch the start state of the previous substep while this one is processed
+        float4 xp = xq, vp = vq;
         tp -= S2;
-        vec3 dx = zero3(), dv = zero3();
-        if (s != T - 1) gather(dx, dv);  // contributions of the element phase of substep s + 1 (all lanes: the sums meet by shuffle)
+        if (po.lead && s > 0) { xp = tp[0]; vp = tp[S]; }
+        if (s != T - 1) {  // contributions of the element phase of substep s + 1 (all lanes: the sums meet by shuffle)
+            vec3 dx, dv;
+            gather(dx, dv);
+            bx += dx; bv += dv;
+        }
         if (po.lead) {
-            res_cp_async_wait_all();
-            const float4 xq = sxn[po.lp], vq = svn[po.lp], vnext = sv[po.lp];  // sv still holds v of state s + 1
-            // prefetch the start state of the previous substep while this one is processed
-            if (s > 0) { res_cp_async16(sxn + po.lp, tp); res_cp_async16(svn + po.lp, tp + S); res_cp_async_commit(); }
-            vec3 bx = vec3(sbx[po.lp]) + dx, bv = vec3(sbv[po.lp]) + dv;
             if (cot && fr_left == 0 && fr_idx < n_frames) {
                 const float *c = cot + (size_t)fr_idx * frame_elems;
                 bx += vec3(c[0], c[1], c[2]);
@@ -383,8 +375,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
 #pragma unroll
                 for (int q = 0; q < 4; q++) sgc[q * N + po.p] += gp[q];
             }
-            sbx[po.lp] = make_float4(ax.x, ax.y, ax.z, 0.f); sbv[po.lp] = make_float4(av.x, av.y, av.z, 0.f);
+            bx = ax; bv = av;
             sx[po.lp] = xq; sv[po.lp] = vq; sa[po.lp] = make_float4(af.x, af.y, af.z, 0.f);
+            vnext = vq; xq = xp; vq = vp;
         }
         __syncthreads();
 #pragma unroll
@@ -439,11 +432,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_resident_adj(const ModelDev md, 
     {
         vec3 dx, dv;
         gather(dx, dv);
-        if (po.lead) {
-            const vec3 bx = vec3(sbx[po.lp]) + dx, bv = vec3(sbv[po.lp]) + dv;
-            adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
-            adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
-        }
+        bx += dx; bv += dv;
+    }
+    if (po.lead) {
+        adjx[poff] = make_float4(bx.x, bx.y, bx.z, 0.f);
+        adjv[poff] = make_float4(bv.x, bv.y, bv.z, 0.f);
     }
     __syncthreads();
     if (tid < kResAcc) {
