@@ -239,6 +239,15 @@ int gs_loss_centroid(int n_envs, int n_particles, const float *d_x, const float 
                      float *d_loss, float *d_adj_x, gs_stream stream);
 int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const float *d_ref, float scale, int accumulate,
                 float *d_loss, float *d_adj_x, gs_stream stream);
+/*
+ * Centroid-trajectory loss of a rollout (BASELINE.json configs[3]; PAPER.md:365 a centre-of-mass loss "at each time step"):
+ *   L_e = 1/n_t sum_f || c_e(t_f) - target_{f,e} ||^2,  t_f = (f+1) frame_stride, n_t = T / frame_stride frames,
+ * read from the tape of the last gs_rollout.  d_targets [n_t][E][3]; d_loss [E] overwritten; d_adj_x_frames [n_t][E][N][3]
+ * overwritten with dL/dx(t_f) in the layout gs_rollout_backward takes (may be NULL); d_scratch_x: DEVICE [E][N][3].
+ * A checkpointed tape needs K | frame_stride.  Errors: GS_EINVAL, GS_ESTATE (no rollout on the tape).
+ */
+int gs_loss_centroid_traj(gs_model *m, gs_tape *t, int frame_stride, const float *d_targets, float *d_loss,
+                          float *d_adj_x_frames, float *d_scratch_x, gs_stream stream);
 
 /*
  * Soft silhouette rasteriser on a headless device buffer, and its adjoint: the image-space loss of

@@ -504,6 +504,23 @@ extern "C" int gs_loss_pos(int n_envs, int n_particles, const float *d_x, const 
     return GS_OK;
 }
 
+// centroid-trajectory loss over the frames of a rollout (SURVEY.md 8(b) gs_loss_centroid_traj_mse; BASELINE.json configs[3])
+extern "C" int gs_loss_centroid_traj(gs_model *m, gs_tape *t, int frame_stride, const float *d_targets, float *d_loss, float *d_adj_x_frames,
+                                     float *d_scratch_x, gs_stream stream) {
+    GS_REQUIRE(m && t && t->m == m && d_targets && d_loss && d_scratch_x, GS_EINVAL, "null argument or foreign tape");
+    GS_REQUIRE(t->has_rollout, GS_ESTATE, "the tape holds no rollout yet");
+    GS_REQUIRE(frame_stride >= 1 && frame_stride <= t->T, GS_EINVAL, "frame_stride must be in [1, T]");
+    GS_REQUIRE(t->K == 1 || frame_stride % t->K == 0, GS_EINVAL, "a checkpointed tape holds multiples of %d only", t->K);
+    const int n_t = t->T / frame_stride;
+    const size_t per = (size_t)m->E * m->N * 3;
+    for (int f = 0; f < n_t; f++) {
+        GS_TRY(gs_tape_read(m, t, (f + 1) * frame_stride, d_scratch_x, nullptr, stream));
+        GS_TRY(gs_loss_centroid(m->E, m->N, d_scratch_x, d_targets + (size_t)f * m->E * 3, 1.0f / (float)n_t, f > 0, d_loss,
+                                d_adj_x_frames ? d_adj_x_frames + (size_t)f * per : nullptr, stream));
+    }
+    return GS_OK;
+}
+
 // ------------------------------------------------------------------------------------------ host-buffer end-to-end
 static size_t al256(size_t n) { return (n + 255) & ~(size_t)255; }
 

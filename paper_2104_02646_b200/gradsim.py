@@ -88,6 +88,7 @@ SIGNATURES = {
     "gs_check_finite": (_int, [_vp, _vp, C.POINTER(_int)]),
     "gs_loss_centroid": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
     "gs_loss_pos": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
+    "gs_loss_centroid_traj": (_int, [_vp, _vp, _int, _vp, _vp, _vp, _vp, _vp]),
     "gs_raster_scratch_bytes": (_sz, [_int, _int, _int]),
     "gs_render_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, _vp, _sz, _vp]),
     "gs_loss_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _sz, _vp]),
@@ -428,6 +429,16 @@ class Tape:
         v = m.new_state() if want_v else None
         _check(lib().gs_tape_read(m.h, self.h, int(substep), _dp(x), _dp(v), _stream()))
         return x, v
+
+    def loss_centroid_traj(self, frame_stride, targets, want_adj=True):
+        """gs_loss_centroid_traj: (loss [E], dL/dx of the frames [n_t, E, N, 3]) from the tape of the last rollout."""
+        torch = _torch()
+        m = self.model
+        n_t = self.T // int(frame_stride)
+        loss = torch.zeros(m.E, dtype=torch.float32, device=m.device)
+        adj = torch.empty((n_t,) + m._shape(), dtype=torch.float32, device=m.device) if want_adj else None
+        _check(lib().gs_loss_centroid_traj(m.h, self.h, int(frame_stride), _dp(_st(targets, (n_t, m.E, 3))), _dp(loss), _dp(adj), _dp(m.new_state()), _stream()))
+        return loss, adj
 
     def backward(self, adj_x_T=None, adj_v_T=None, adj_x_frames=None, frame_stride=1, want_out=True):
         m = self.model

@@ -704,3 +704,23 @@ def test_error_paths_of_the_round2_entry_points():
     cam = gs.make_camera(np.eye(3), [0, 0, 1], 1.0, 1.0, 16, 16, 1e-3)
     img = torch.empty((1, 16, 16), device="cuda:0")
     assert L.gs_render_silhouette(1, sc.n_particles, gs._dp(x), int(tris.shape[0]), gs._dp(tris), gs.C.byref(cam), gs._dp(img), gs._dp(mem), 1024, gs._stream()) == gs.GS_EINVAL
+
+
+def test_loss_centroid_traj_call_matches_the_oracle():
+    """gs_loss_centroid_traj (the third loss of SURVEY.md 8(b)): loss and frame cotangents of config 3's loss in one call,
+    against the oracle's loss and, through gs_rollout_backward, its gradients; on a full and on a checkpointed tape."""
+    sc = scenes.make_scene(3, small=True)
+    ref = orc.run_scene(sc)
+    for K in (1, 32):
+        m = gs.Model(sc)
+        tape = m.tape(sc.n_substeps, K)
+        m.zero_grads()
+        tape.rollout(dev(sc.x0), dev(sc.v0))
+        loss, cot = tape.loss_centroid_traj(sc.frame_stride, dev(ref["target"]))
+        assert rel_inf(host(loss), ref["loss"]) <= 5e-3
+        ax0, av0 = tape.backward(adj_x_frames=cot, frame_stride=sc.frame_stride)
+        assert rel_inf(host(ax0), ref["adj_x0"]) <= TOL_GRAD and rel_inf(host(av0), ref["adj_v0"]) <= TOL_GRAD
+        assert rel_inf(host(m.param_grads("tet_mu")), ref["g_tet_mu"]) <= TOL_GRAD
+    with pytest.raises(gs.GradSimError) as e:
+        gs.Model(sc).tape(64).loss_centroid_traj(32, dev(ref["target"][:2]))  # no rollout on this tape yet
+    assert e.value.code == gs.GS_ESTATE
