@@ -257,6 +257,14 @@ def test_config4_full_rollout_vs_oracle():
     assert np.abs(got["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * ext
     assert rel_inf(got["vT"], ref["vT"]) <= 1e-2  # velocities are not part of the stated tolerances: sanity bound
     assert rel_inf(got["loss"], ref["loss"]) <= TOL_GRAD
+    # the 1M-tet solid and the sheet do not interact (A16): the solid's share of every per-particle array is held to 2e-3
+    # flat (norm of its own slice); the relaxed branch below is needed by the sheet's entries only (and by dL/dk_damp of the
+    # few tets next to a bottom particle whose contact branch flipped)
+    Ns = int(sc.tets.max()) + 1
+    solid = {k: rel_inf(got[k][:, :Ns], ref[k][:, :Ns]) for k in ("adj_x0", "adj_v0", "g_mass")}
+    _report({"test": "config4_solid_particles", "errors": solid, "relaxed": {}})
+    for k, e in solid.items():
+        assert e <= TOL_GRAD, (k, e)
     _compare_gradients("config4", sc, ref, got, draws=1)
 
 
