@@ -140,6 +140,17 @@ size_t gs_model_workspace_bytes(const gs_model_desc *desc);
 int gs_model_create(const gs_model_desc *desc, void *d_workspace, size_t bytes, gs_stream stream, gs_model **out);
 void gs_model_destroy(gs_model *m);
 
+/*
+ * Deterministic mode of the streaming plan (SURVEY.md 8(c) hazard H6: "a coloured-scatter debug mode makes runs
+ * repeatable"; north_star (3): atomic or graph-coloured scatter).  The tiles of all element types are coloured at model
+ * creation so that no two tiles of a colour share a particle; with the mode on, the element kernels are launched once per
+ * colour, so every particle's force / cotangent sum is formed in a fixed order and states, dL/dx0, dL/dv0 and the
+ * per-element / per-particle gradients are bitwise reproducible run to run (the per-environment totals of the contact,
+ * gravity and air parameters are fp64 atomic sums and may differ in the last bit).  Slower (about one launch per colour:
+ * 10-20 per substep); the resident plan is deterministic as it is.  GS_ESTATE if the mesh needs more than 64 colours.
+ */
+int gs_set_deterministic(gs_model *m, int enable);
+
 /* Which plan the model runs (gs_plan value), and basic sizes. */
 int gs_model_plan(const gs_model *m);
 int gs_model_info(const gs_model *m, int32_t *n_particles, int32_t *n_elements, int32_t *n_envs);

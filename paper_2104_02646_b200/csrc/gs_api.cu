@@ -142,6 +142,13 @@ extern "C" int gs_request_grads(gs_model *m, int group, int enable) {
     return GS_OK;
 }
 
+extern "C" int gs_set_deterministic(gs_model *m, int enable) {
+    GS_REQUIRE(m, GS_EINVAL, "model is null");
+    GS_REQUIRE(!enable || m->det_colours > 0, GS_ESTATE, "the mesh's tiles need more than 64 colours: no deterministic mode for this model");
+    if (m->det != (enable != 0)) { m->det = enable != 0; m->epoch++; }
+    return GS_OK;
+}
+
 static int reset_bad(gs_model *m, cudaStream_t st) {
     GS_CUDA(cudaMemsetAsync(m->dev.bad, 0x7f, sizeof(int), st), "reset non-finite flag");
     return GS_OK;

@@ -63,6 +63,8 @@ struct ElemDev {
     float *g32;                 // [kNumGrads][E][cpad] per-substep fp32 accumulators (mu, lambda, damp; hinges: k_b)
     double *g64;                // [kNumGrads][E][cpad] fp64 masters
     const int *perm;            // [count] internal -> caller element index
+    const int *det_list;        // deterministic mode (gs_set_deterministic): the tiles of ONE colour class this launch walks
+    int det_n;                  //   (no two tiles of a class share a particle); null / 0 in the normal mode
 };
 // index of parameter q (0 mu, 1 lambda, 2 damp) of internal element e of environment env inside ElemDev::par
 __host__ __device__ inline size_t par_index(int n_tiles, int env, int e, int q) {
@@ -146,6 +148,12 @@ struct gs_model {
         return a;
     }
     bool aero_host = false;  // build_model: some air coefficient is non-zero
+    // deterministic mode: tiles of all element types coloured so that tiles of one colour share no particle; the element
+    // kernels are then launched once per colour, and every particle's sum is formed in colour order
+    bool det = false;
+    int det_colours = 0;
+    int *d_det[gs::N_TYPES] = {nullptr, nullptr, nullptr};  // [n_tiles] tile indices sorted by colour
+    std::vector<int> det_off[gs::N_TYPES];                  // [det_colours + 1] offsets of the colour classes
     uint64_t epoch = 0;    // bumped when a by-value kernel argument changes (gravity): captured graphs of older epochs are stale
     // resident plan (gs_resident.cu): host descriptor, null when the model runs the streaming plan
     void *res_host = nullptr;

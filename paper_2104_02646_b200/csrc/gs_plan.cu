@@ -52,7 +52,7 @@ struct Bump {
 struct Layout {
     // per type
     char *rec[N_TYPES];
-    int *tile_parts[N_TYPES], *perm[N_TYPES];
+    int *tile_parts[N_TYPES], *perm[N_TYPES], *det[N_TYPES];
     float *par[N_TYPES], *g32[N_TYPES];
     double *g64[N_TYPES];
     int *perm_p, *bad;
@@ -83,6 +83,7 @@ static Layout make_layout(void *base, int N, int E, const int counts[N_TYPES]) {
             L.g64[t] = b.take<double>(E * cp);
         }
         L.perm[t] = b.take<int>(c);
+        L.det[t] = b.take<int>(nt);
     }
     L.perm_p = b.take<int>(N);
     L.inv_mass = b.take<float>(EN);
@@ -211,6 +212,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
     // ---- elements: rest quantities, Morton order, tiles
     ModelDev &dev = m->dev;
     memset(&dev, 0, sizeof dev);
+    std::vector<std::vector<int>> all_tids[N_TYPES];  // particles of every tile, kept for the tile colouring below
     for (int t = 0; t < N_TYPES; t++) {
         const int c = counts[t], a = kArity[t];
         const int nt = (c + kTileElems - 1) / kTileElems;
@@ -392,6 +394,7 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
                 if (t == T_TRI) qa[e - e0] = r1[hs.perm[e]].x;
             }
         }
+        all_tids[t] = tids;
         UP(L.rec[t], rec); UP(L.tile_parts[t], tparts);
         UP(L.perm[t], hs.perm);
         // per-env element parameters: [E][n_tiles][3][kTileElems] (padding holds harmless finite values)
@@ -424,6 +427,40 @@ int build_model(const gs_model_desc *d, void *d_workspace, size_t bytes, cudaStr
         ed.g32 = L.g32[t]; ed.g64 = L.g64[t];
         ed.perm = L.perm[t];
         m->counts[t] = c;
+    }
+    {
+        // deterministic mode: greedy colouring of the tiles of all types (tets, then triangles, then hinges, in tile order):
+        // a tile takes the lowest colour none of its particles has seen; per colour class no two tiles share a particle
+        std::vector<uint64_t> seen(N, 0);
+        std::vector<int> colour[N_TYPES];
+        int nc = 0;
+        bool ok = true;
+        for (int t = 0; t < N_TYPES && ok; t++) {
+            colour[t].assign(all_tids[t].size(), 0);
+            for (size_t j = 0; j < all_tids[t].size(); j++) {
+                uint64_t used = 0;
+                for (int pi : all_tids[t][j]) used |= seen[pi];
+                int c = 0;
+                while (c < 64 && (used >> c & 1ull)) c++;
+                if (c == 64) { ok = false; break; }
+                colour[t][j] = c;
+                nc = std::max(nc, c + 1);
+                for (int pi : all_tids[t][j]) seen[pi] |= 1ull << c;
+            }
+        }
+        m->det_colours = ok ? nc : 0;
+        for (int t = 0; t < N_TYPES; t++) {
+            const int nt = (int)all_tids[t].size();
+            std::vector<int> order(nt);
+            std::iota(order.begin(), order.end(), 0);
+            if (ok) std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return colour[t][a] < colour[t][b]; });
+            m->det_off[t].assign(nc + 1, 0);
+            if (ok)
+                for (int j = 0; j < nt; j++) m->det_off[t][colour[t][j] + 1]++;
+            for (int c = 0; c < nc; c++) m->det_off[t][c + 1] += m->det_off[t][c];
+            UP(L.det[t], order);
+            m->d_det[t] = L.det[t];
+        }
     }
     dev.N = N; dev.E = E;
     dev.gx = d->gravity[0]; dev.gy = d->gravity[1]; dev.gz = d->gravity[2]; dev.dt = d->dt;

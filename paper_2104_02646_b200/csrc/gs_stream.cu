@@ -95,6 +95,43 @@ struct EmitPlan {
         for (int k = 0; k < 4; k++) red_add_v4_if(fl & (1u << k), dst + idp[r[k]], a[k].x, a[k].y, a[k].z);
     }
 };
+// Deterministic emit (gs_set_deterministic): as the plain emit, but a run of equal particles that crosses the 4-entry
+// chunks of several threads is summed by the thread that owns its START, in entry order, and leaves as ONE reduction --
+// the plain emit issues one per chunk, whose order at the L2 is not fixed.  A thread whose first run continues the previous
+// thread's last run publishes that run's partial sum in `plane` (the output plane, free once every thread has read its
+// entries: two extra CTA barriers); w = 1: the run ends inside the chunk, 2: the whole chunk belongs to the run.
+// All threads of the CTA must call it.
+__device__ __forceinline__ void emit_det(const uint16_t *slot_desc, const uint16_t *slots, const int *ids, float4 *plane, float4 *dst) {
+    const int tid = threadIdx.x;
+    const unsigned dsc = slot_desc[tid], nv = dsc >> 13;
+    const bool has = nv > 0u;
+    bool cont = false;
+    if (has && tid > 0) {
+        const unsigned dp = slot_desc[tid - 1];
+        cont = (dp >> 13) > 0u && (dp & 1023u) + (unsigned)__popc((dp >> 10) & 7u) == (dsc & 1023u);
+    }
+    const EmitPlan ep(has ? reinterpret_cast<const uint2 *>(slots)[tid] : make_uint2(0u, 0u), has ? dsc : (1u << 13), ids);
+    float3 a[4];
+    ep.sums(plane, a);
+    const int k0 = __ffs(ep.fl) - 1;  // entry at which my first run ends
+    __syncthreads();
+    plane[tid] = (has && cont) ? make_float4(a[k0].x, a[k0].y, a[k0].z, k0 == (int)nv - 1 ? 2.f : 1.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+    if (!has) return;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        if (!(ep.fl & (1u << k)) || (k == k0 && cont)) continue;
+        float3 tot = a[k];
+        if (k == (int)nv - 1)
+            for (int u = tid + 1; u < kTileElems; u++) {
+                const float4 c = plane[u];
+                if (c.w == 0.f) break;
+                tot.x += c.x; tot.y += c.y; tot.z += c.z;
+                if (c.w != 2.f) break;
+            }
+        red_add_v4(dst + ep.idp[ep.r[k]], tot.x, tot.y, tot.z);
+    }
+}
 __device__ __forceinline__ void red_add_f32(float *addr, float a) {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
 }
@@ -249,9 +286,12 @@ struct TilePipe {
         pol_keep = l2_policy_evict_last();
     }
     // work item -> (tile, env); single-environment models (the large meshes) skip the division
+    // tiles this launch walks per environment: all of them, or (extended kernels, deterministic mode) one colour class
+    __device__ __forceinline__ int n_walk() const { return (ACT && es.det_list) ? es.det_n : es.n_tiles; }
     __device__ __forceinline__ void split(int item, unsigned &tile, unsigned &env) const {
         if (!ME) { tile = (unsigned)item; env = 0u; }
-        else { env = (unsigned)item / (unsigned)es.n_tiles; tile = (unsigned)item - env * (unsigned)es.n_tiles; }
+        else { const unsigned nw = (unsigned)n_walk(); env = (unsigned)item / nw; tile = (unsigned)item - env * nw; }
+        if (ACT && es.det_list) tile = (unsigned)es.det_list[tile];
     }
     // ids of the CTA's j-th item go to id buffer `slot` = j % 3, its staging indices to loc buffer `par` = j % 2
     __device__ __forceinline__ void load_ids(int item, int slot, int par) {  // one thread
@@ -321,7 +361,7 @@ struct TilePipe {
     // types of one launch, so their remainders do not pile onto the same CTAs
     template <class Compute, class Emit>
     __device__ __forceinline__ void run_static(int rot, Compute compute, Emit emit) {
-        const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
+        const int n_items = n_walk() * E, G = gridDim.x, tid = threadIdx.x;
         const int first = (int)((blockIdx.x + (unsigned)G - (unsigned)rot % (unsigned)G) % (unsigned)G);  // item j of this type -> CTA (j + rot) mod G
         if (first >= n_items) return;
         const int cnt = (n_items - first + G - 1) / G;
@@ -370,10 +410,12 @@ struct TilePipe {
     template <class Compute, class Emit>
     __device__ __forceinline__ void run(int rot, int *ctr, int *next_slot, Compute compute, Emit emit) {
         if (!kQueue) { run_static(rot, compute, emit); return; }
-        const int n_items = es.n_tiles * E, G = gridDim.x, tid = threadIdx.x;
+        const int n_items = n_walk() * E, G = gridDim.x, tid = threadIdx.x;
         const int first = (int)((blockIdx.x + (unsigned)G - (unsigned)rot % (unsigned)G) % (unsigned)G);  // item j of this type -> CTA (j + rot) mod G
         if (first >= n_items) return;
-        const bool queue = kQueue && 2 * G < n_items;  // otherwise the static items cover everything
+        // otherwise the static items cover everything; the deterministic mode launches several times per substep between
+        // two resets of the queue counters, so it deals statically
+        const bool queue = kQueue && 2 * G < n_items && !(ACT && es.det_list);
         int item = first, item_n = first + G;  // items i, i+1 (all threads)
         int claimed = n_items;                 // kQueue: item i+2, thread 0 only until published through next_slot
         int ticket = -1;                       // raw result of the queue's atomicAdd for item i+3 (< 0: none): converted one
@@ -423,6 +465,9 @@ struct TilePipe {
         }
     }
 };
+
+template <bool ACT>
+__device__ __forceinline__ int walked(const ElemDev &es) { return (ACT && es.det_list) ? es.det_n : es.n_tiles; }
 
 // ------------------------------------------------------------------------------------------ forward elements
 constexpr int kBarBytes = 128;  // 15 mbarriers at the start of shared memory (5 per element type) + the queue hand-over slot
@@ -481,6 +526,7 @@ __device__ __forceinline__ void tiles_fwd(const ModelDev &md, const ActDev &ad, 
         [&](const TileView<TYPE, false> &tv, const int *ids, int env, const float4 *sf) {
             // thread t sums gather-list entries 4t .. 4t+3 (sorted by tile-particle) and issues one vector reduction per
             // run of equal particles: balanced over all lanes, no loop, no branch, no shared-memory atomics
+            if (ACT && md.es[TYPE].det_list) { emit_det(tv.slot_desc, tv.slots, ids, const_cast<float4 *>(sf), f4 + (size_t)env * N); return; }
             const unsigned dsc = tv.slot_desc[threadIdx.x];
             if ((dsc >> 13) == 0u) return;
             const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
@@ -500,8 +546,8 @@ __global__ void __launch_bounds__(kTileElems, 9) k_elements_fwd(const ModelDev m
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_fwd<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_fwd<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TET].count) { tiles_fwd<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, f4); rot += walked<ACT>(md.es[T_TET]) * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_fwd<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, f4); rot += walked<ACT>(md.es[T_TRI]) * md.E; __syncthreads(); }
     if (md.es[T_HINGE].count) tiles_fwd<T_HINGE, ACT, ME>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, f4);
 }
 
@@ -693,6 +739,11 @@ __device__ __forceinline__ void tiles_adj(const ModelDev &md, const ActDev &ad, 
             }
         },
         [&](const TileView<TYPE, true> &tv, const int *ids, int env, const float4 *so) {
+            if (ACT && md.es[TYPE].det_list) {
+                emit_det(tv.slot_desc, tv.slots, ids, const_cast<float4 *>(so), adjx + (size_t)env * N);
+                if (TYPE != T_HINGE) emit_det(tv.slot_desc, tv.slots, ids, const_cast<float4 *>(so) + PL, adjv + (size_t)env * N);
+                return;
+            }
             const unsigned dsc = tv.slot_desc[threadIdx.x];
             if ((dsc >> 13) == 0u) return;
             const EmitPlan ep(reinterpret_cast<const uint2 *>(tv.slots)[threadIdx.x], dsc, ids);
@@ -714,8 +765,8 @@ __global__ void __launch_bounds__(kTileElems) k_elements_adj(const ModelDev md, 
     uint64_t *bars = (uint64_t *)smem;
     init_barriers(bars);
     int rot = 0;
-    if (md.es[T_TET].count) { tiles_adj<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TET].n_tiles * md.E; __syncthreads(); }
-    if (md.es[T_TRI].count) { tiles_adj<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += md.es[T_TRI].n_tiles * md.E; __syncthreads(); }
+    if (md.es[T_TET].count) { tiles_adj<T_TET, ACT, ME>(md, ad, smem + kBarBytes, bars, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += walked<ACT>(md.es[T_TET]) * md.E; __syncthreads(); }
+    if (md.es[T_TRI].count) { tiles_adj<T_TRI, ACT, ME>(md, ad, smem + kBarBytes, bars + 5, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv); rot += walked<ACT>(md.es[T_TRI]) * md.E; __syncthreads(); }
     if (md.es[T_HINGE].count) tiles_adj<T_HINGE, ACT, ME>(md, ad, smem + kBarBytes, bars + 10, (int *)(smem + 120), rot, x4, v4, adjf, adjx, adjv);
 }
 
@@ -895,12 +946,34 @@ static inline int tile_grid(const gs_model *m, int occ) {
     return (int)(m->elem_items < cap ? m->elem_items : cap);
 }
 
+// deterministic mode: point the model description at colour class c; returns the largest item count of a type in it
+static long long det_class(const gs_model *m, int c, ModelDev &md) {
+    long long items = 0;
+    for (int t = 0; t < N_TYPES; t++) {
+        if (!m->counts[t]) continue;
+        md.es[t].det_list = m->d_det[t] + m->det_off[t][c];
+        md.es[t].det_n = m->det_off[t][c + 1] - m->det_off[t][c];
+        items = std::max(items, (long long)md.es[t].det_n * m->E);
+    }
+    return items;
+}
+
 // substep < 0: a single-substep call (gs_step_forward / gs_step_backward): the activation frame is the model's current
 // one (gs_set_actuation_frame) and a non-finite state is reported as substep 0
 int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *xo, float4 *vo, int substep, cudaStream_t st) {
     const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     const int bad_idx = substep < 0 ? 0 : substep;
-    if (m->elem_items > 0) {
+    if (m->elem_items > 0 && m->det) {
+        // deterministic mode: one launch of the extended kernel per colour class of tiles
+        auto kern = m->E > 1 ? k_elements_fwd<true, true> : k_elements_fwd<true, false>;
+        for (int c = 0; c < m->det_colours; c++) {
+            ModelDev md = m->dev;
+            long long items = det_class(m, c, md);
+            if (items == 0) continue;
+            const long long cap = (long long)m->n_sms * m->occ_fwd;
+            GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", launch_pdl(false, kern, (int)std::min(items, cap), kTileElems, m->smem_fwd, st, md, ad, x, v, m->d_f));
+        }
+    } else if (m->elem_items > 0) {
         const bool act = m->act_frames > 0 || m->dev.aero, me = m->E > 1;
         auto kern = act ? (me ? k_elements_fwd<true, true> : k_elements_fwd<true, false>) : (me ? k_elements_fwd<false, true> : k_elements_fwd<false, false>);
         GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", launch_pdl(m->pdl, kern, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
@@ -915,7 +988,17 @@ int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const flo
     const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
              launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
-    if (m->elem_items > 0) {
+    if (m->elem_items > 0 && m->det) {
+        auto kern = m->E > 1 ? k_elements_adj<true, true> : k_elements_adj<true, false>;
+        for (int c = 0; c < m->det_colours; c++) {
+            ModelDev md = m->dev;
+            long long items = det_class(m, c, md);
+            if (items == 0) continue;
+            const long long cap = (long long)m->n_sms * m->occ_adj;
+            GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",
+                     launch_pdl(false, kern, (int)std::min(items, cap), kTileElems, m->smem_adj, st, md, ad, x, v, m->d_adjf, m->d_adjx, m->d_adjv));
+        }
+    } else if (m->elem_items > 0) {
         const bool act = m->act_frames > 0 || m->dev.aero, me = m->E > 1;
         auto kern = act ? (me ? k_elements_adj<true, true> : k_elements_adj<true, false>) : (me ? k_elements_adj<false, true> : k_elements_adj<false, false>);
         GS_TIMED(m, GS_K_ELEMENTS_ADJ, st, "k_elements_adj",

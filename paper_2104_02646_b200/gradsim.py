@@ -83,6 +83,7 @@ SIGNATURES = {
     "gs_tape_read": (_int, [_vp, _vp, _int, _vp, _vp, _vp]),
     "gs_rollout_backward": (_int, [_vp, _vp, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
     "gs_request_grads": (_int, [_vp, _int, _int]),
+    "gs_set_deterministic": (_int, [_vp, _int]),
     "gs_zero_grads": (_int, [_vp, _vp]),
     "gs_param_grads": (_int, [_vp, _int, _vp, _vp]),
     "gs_check_finite": (_int, [_vp, _vp, C.POINTER(_int)]),
@@ -329,6 +330,9 @@ class Model:
 
     def set_actuation_frame(self, frame):
         _check(lib().gs_set_actuation_frame(self.h, int(frame)))
+
+    def set_deterministic(self, enable=True):
+        _check(lib().gs_set_deterministic(self.h, int(bool(enable))))
 
     def request_grads(self, group, enable=True):
         _check(lib().gs_request_grads(self.h, GROUPS[group], int(bool(enable))))

@@ -89,6 +89,8 @@ def test_argument_errors_without_a_device(lib_path):
     assert L.gs_actuation_grads(None, 0, None, None) == gs.GS_EINVAL
     assert L.gs_set_actuation_frame(None, 0) == gs.GS_EINVAL
     assert L.gs_request_grads(None, gs.GROUPS["gravity"], 1) == gs.GS_EINVAL
+    assert L.gs_set_deterministic(None, 1) == gs.GS_EINVAL
+    assert L.gs_loss_centroid_traj(None, None, 1, None, None, None, None, None) == gs.GS_EINVAL
     assert L.gs_host_scratch_bytes(None, None, 0, 1) == 0
     assert L.gs_raster_scratch_bytes(0, 10, 3) == 0 and L.gs_raster_scratch_bytes(1, 10, 3) > 0
     cam = gs.make_camera([1, 0, 0, 0, 1, 0, 0, 0, 1], [0, 0, 1], 1.0, 1.0, 8, 8, 1e-3)

@@ -724,3 +724,31 @@ def test_loss_centroid_traj_call_matches_the_oracle():
     with pytest.raises(gs.GradSimError) as e:
         gs.Model(sc).tape(64).loss_centroid_traj(32, dev(ref["target"][:2]))  # no rollout on this tape yet
     assert e.value.code == gs.GS_ESTATE
+
+
+@pytest.mark.parametrize("config", [2, 4])
+def test_deterministic_mode_is_bitwise_reproducible(config):
+    """gs_set_deterministic (hazard H6): with the coloured scatter two runs of rollout + backward agree BITWISE on the
+    states, the cotangents and the per-element / per-particle gradients (the default mode's atomics reorder the sums: a
+    few ulp per substep), the result still matches the oracle, and switching the mode off restores the fast path."""
+    sc = scenes.make_scene(config, small=True)
+    ref = orc.run_scene(sc)
+    m = gs.Model(sc, plan=gs.GS_PLAN_STREAMING)
+    m.set_deterministic(True)
+    a = gpu_run_scene(sc, ref["target"], model=m)
+    b = gpu_run_scene(sc, ref["target"], model=m)
+    keys = ["xT", "vT", "adj_x0", "adj_v0"] + ["g_" + g for g in _grad_groups(sc)]
+    for k in keys:
+        assert np.array_equal(a[k], b[k]), k
+    assert np.abs(a["xT"] - ref["xT"]).max() <= TOL_ROLLOUT * sc.extent()
+    for k in keys[2:]:
+        assert rel_inf(a[k], ref[k]) <= TOL_GRAD, k
+    L = gs.lib()
+    n0 = L.gs_launch_count()
+    m.set_deterministic(False)
+    c = gpu_run_scene(sc, ref["target"], model=m)
+    n1 = L.gs_launch_count()
+    assert np.abs(c["xT"] - a["xT"]).max() <= 1e-5 * sc.extent() and rel_inf(c["adj_x0"], a["adj_x0"]) <= 1e-4
+    m.set_deterministic(True)
+    gpu_run_scene(sc, ref["target"], model=m)
+    assert L.gs_launch_count() - n1 > n1 - n0  # one element launch per colour class and substep
