@@ -61,9 +61,12 @@ struct ResAct {
     size_t fstride;  // E * cpad
 };
 
+// The forward and the adjoint kernel may use different layouts of the particle phase (the tape is indexed by particle, so the
+// two need not agree): the lean forward kernel runs best with two tets per thread and half the threads where the particles
+// still fit, the adjoint with one tet per thread.  rd_fwd shares idx / rloc / csr_ptr with rd; owner / dest / row are its own.
 struct ResHost {
-    ResDev rd;
-    int ept;
+    ResDev rd, rd_fwd;
+    int ept, ept_fwd;
     size_t smem_fwd, smem_adj;
 };
 
@@ -77,7 +80,10 @@ static size_t res_smem(int L, int N, int Ltot, int maxval, int planes, bool adj)
     return (size_t)(adj ? 3 : 2) * L * sizeof(float4) + (size_t)planes * Ltot * sizeof(float4) + (adj ? al16((size_t)N * (kResAcc * 8 + kResAcc * 4)) : 0) +
            al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)(maxval + 1) * 2);
 }
-static int res_threads(int M) { const int ept = M > kResMaxThreads ? 2 : 1; return ((M + ept - 1) / ept + 31) / 32 * 32; }
+static int res_ept(int M) { return M > kResMaxThreads ? 2 : 1; }
+// forward: two tets per thread as soon as half the threads still hold one particle each
+static int res_ept_fwd(int M, int N) { return (M > kResMaxThreads || ((M + 1) / 2 + 31) / 32 * 32 >= N) ? 2 : 1; }
+static int res_threads(int M, int ept) { return ((M + ept - 1) / ept + 31) / 32 * 32; }
 static int res_kpp(int nthreads, int N) { return nthreads >= 4 * N ? 4 : (nthreads >= 2 * N ? 2 : 1); }
 // rows of the transposed gather list from the valences (any order): row[j] (maxval + 1 entries); returns the padded total.
 // Row starts are placed at prescribed residues modulo 8 (the 16-byte bank group of entry row[j] + q is (row[j] + q) mod 8):
@@ -112,18 +118,22 @@ static std::vector<int> res_valences(const gs_model_desc *d) {
 
 static bool resident_fits(const gs_model_desc *d) {
     if (d->n_tris > 0 || d->n_hinges > 0 || d->n_tets < 1 || d->n_tets > kResMaxTets) return false;
-    const int nthreads = res_threads(d->n_tets);
+    const int nthreads = res_threads(d->n_tets, res_ept(d->n_tets));
     if (d->n_particles > nthreads || !d->tets) return false;
     const std::vector<int> val = res_valences(d);
     const int maxval = *std::max_element(val.begin(), val.end());
     const int Ltot = res_rows(val, res_kpp(nthreads, d->n_particles), nullptr);
-    if (Ltot > 65535) return false;
-    return res_smem(d->n_particles + 24, d->n_particles, Ltot, maxval, 2, true) <= 200 * 1024;
+    const int nthreads_f = res_threads(d->n_tets, res_ept_fwd(d->n_tets, d->n_particles));
+    const int Ltot_f = res_rows(val, res_kpp(nthreads_f, d->n_particles), nullptr);
+    if (Ltot > 65535 || Ltot_f > 65535) return false;
+    return res_smem(d->n_particles + 24, d->n_particles, Ltot, maxval, 2, true) <= 200 * 1024 &&
+           res_smem(d->n_particles + 24, d->n_particles, Ltot_f, maxval, 1, false) <= 200 * 1024;
 }
 
 size_t resident_blob_bytes(const gs_model_desc *d) {
     if (!resident_fits(d)) return 0;
-    return 256 * 8 + 2 * (size_t)d->n_tets * sizeof(ushort4) + (size_t)(3 * d->n_particles + 1) * 2 + (size_t)(4 * d->n_tets + 2) * 2;
+    // idx, csr_ptr, rloc once; dest, row, owner per layout (adjoint, forward)
+    return 256 * 12 + 3 * (size_t)d->n_tets * sizeof(ushort4) + (size_t)(4 * d->n_particles + 1) * 2 + 2 * (size_t)(4 * d->n_tets + 2) * 2;
 }
 
 // ------------------------------------------------------------------------------------------ kernels
@@ -556,126 +566,138 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     ushort4 *d_idx = (ushort4 *)take(idx.size() * sizeof(ushort4));
     uint16_t *d_ptr = (uint16_t *)take(ptr.size() * 2);
 
-    // particle slots: most incident tets first (stable), so the lanes of a warp run near-equal gather loops
-    std::vector<uint16_t> owner(N);
-    for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
-    std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
-    const int nthreads_ = res_threads(M), kpp_ = res_kpp(nthreads_, N);
-    {
-        // within a class of equal valence the order is free: arrange it so that the lead lanes of a quarter-warp (8 / kpp
-        // particle slots) own particles in different 16-byte bank groups of the staging arrays -- their STS.128 of x, v
-        // (and adj_f) after the particle phase are then conflict-free where the class is large enough
-        const int per = 8 / kpp_;
-        for (int a = 0; a < N;) {
-            int b = a;
-            const int va = cnt[owner[a] + 1] - cnt[owner[a]];
-            while (b < N && cnt[owner[b] + 1] - cnt[owner[b]] == va) b++;
-            for (int i = a; i < b; i++) {
-                unsigned banks = 0;
-                for (int j = i - i % per; j < i; j++) banks |= 1u << (rloc[owner[j]] & 7);
-                for (int j = i; j < b; j++)
-                    if (!(banks >> (rloc[owner[j]] & 7) & 1u)) { std::swap(owner[i], owner[j]); break; }
-            }
-            a = b;
-        }
-    }
-    // transposed gather list (ResDev::dest / row): the j-th incidence (element order) of the particle in slot q -> row[j] + q
-    std::vector<int> val(N);
-    for (int i = 0; i < N; i++) val[i] = cnt[i + 1] - cnt[i];
-    std::vector<uint16_t> row;
-    const int Ltot = res_rows(val, kpp_, &row);
-    const int maxval = (int)row.size() - 1;
-    std::vector<int> slot_of(N);
-    for (int q = 0; q < N; q++) slot_of[owner[q]] = q;
-    // Which of a particle's rows an incidence takes is free: pick it so that the eight lanes of a quarter-warp (eight
-    // consecutive tets, same vertex position) store into different 16-byte bank groups where possible (STS.128 is served
-    // a quarter-warp at a time); greedy, lowest free row first among the rows whose bank group is still unused.
-    std::vector<std::vector<char>> used(N);
-    for (int i = 0; i < N; i++) used[i].assign(val[i], 0);
-    std::vector<ushort4> dest(M);
-    for (int e0 = 0; e0 < M; e0 += 8) {
-        for (int k = 0; k < 4; k++) {
-            unsigned banks = 0;
-            for (int e = e0; e < std::min(M, e0 + 8); e++) {
-                const int pk = k == 0 ? pid[e].x : (k == 1 ? pid[e].y : (k == 2 ? pid[e].z : pid[e].w));
-                int pick = -1, fallback = -1;
-                for (int j = 0; j < val[pk]; j++) {
-                    if (used[pk][j]) continue;
-                    if (fallback < 0) fallback = j;
-                    if (!(banks >> ((row[j] + slot_of[pk]) & 7) & 1u)) { pick = j; break; }
-                }
-                if (pick < 0) pick = fallback;
-                used[pk][pick] = 1;
-                const unsigned short dk = (unsigned short)(row[pick] + slot_of[pk]);
-                banks |= 1u << (dk & 7);
-                if (k == 0) dest[e].x = dk; else if (k == 1) dest[e].y = dk; else if (k == 2) dest[e].z = dk; else dest[e].w = dk;
-            }
-        }
-    }
-    {
-        // local search on the store side: a quarter-warp's STS.128 of vertex k takes as many wavefronts as its fullest
-        // bank group holds entries; swap the rows of two incidences of one particle while that lowers the total
-        auto dk = [&](int e, int k) -> unsigned short & { return k == 0 ? dest[e].x : (k == 1 ? dest[e].y : (k == 2 ? dest[e].z : dest[e].w)); };
-        auto grp_cost = [&](int e, int k) {
-            int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0}, mx = 0;
-            const int e0 = e & ~7;
-            for (int f = e0; f < std::min(M, e0 + 8); f++) mx = std::max(mx, ++cnt[dk(f, k) & 7]);
-            return mx;
-        };
-        std::vector<std::vector<std::pair<int, int>>> inc(N);
-        for (int e = 0; e < M; e++) {
-            const unsigned short pk[4] = {pid[e].x, pid[e].y, pid[e].z, pid[e].w};
-            for (int k = 0; k < 4; k++) inc[pk[k]].push_back({e, k});
-        }
-        for (int sweep = 0; sweep < 8; sweep++) {
-            bool improved = false;
-            for (int q = 0; q < N; q++)
-                for (size_t a = 0; a < inc[q].size(); a++)
-                    for (size_t b = a + 1; b < inc[q].size(); b++) {
-                        const int ea = inc[q][a].first, ka = inc[q][a].second, eb = inc[q][b].first, kb = inc[q][b].second;
-                        if ((ea & ~7) == (eb & ~7) && ka == kb) continue;  // same store instruction of the same quarter-warp
-                        const int before = grp_cost(ea, ka) + grp_cost(eb, kb);
-                        std::swap(dk(ea, ka), dk(eb, kb));
-                        if (grp_cost(ea, ka) + grp_cost(eb, kb) < before) improved = true;
-                        else std::swap(dk(ea, ka), dk(eb, kb));
-                    }
-            if (!improved) break;
-        }
-    }
-    ushort4 *d_dest = (ushort4 *)take(dest.size() * sizeof(ushort4));
-    uint16_t *d_row = (uint16_t *)take(row.size() * 2);
-    uint16_t *d_owner = (uint16_t *)take(owner.size() * 2);
+    // One layout of the particle phase and of the transposed gather list for a CTA of nthreads_ threads (owner / row / dest
+    // depend on the lanes per particle); uploaded into the workspace, pointers and sizes into rd.
+    cudaError_t ce = cudaSuccess;
     uint16_t *d_rloc = (uint16_t *)take(rloc.size() * 2);
-    cudaError_t ce = cudaMemcpyAsync(d_owner, owner.data(), owner.size() * 2, cudaMemcpyHostToDevice, st);
+    auto build_layout = [&](int nthreads_, ResDev &rd) {
+        // particle slots: most incident tets first (stable), so the lanes of a warp run near-equal gather loops
+        std::vector<uint16_t> owner(N);
+        for (int i = 0; i < N; i++) owner[i] = (uint16_t)i;
+        std::stable_sort(owner.begin(), owner.end(), [&](uint16_t x, uint16_t y) { return cnt[x + 1] - cnt[x] > cnt[y + 1] - cnt[y]; });
+        const int kpp_ = res_kpp(nthreads_, N);
+        {
+            // within a class of equal valence the order is free: arrange it so that the lead lanes of a quarter-warp (8 / kpp
+            // particle slots) own particles in different 16-byte bank groups of the staging arrays -- their STS.128 of x, v
+            // (and adj_f) after the particle phase are then conflict-free where the class is large enough
+            const int per = 8 / kpp_;
+            for (int a = 0; a < N;) {
+                int b = a;
+                const int va = cnt[owner[a] + 1] - cnt[owner[a]];
+                while (b < N && cnt[owner[b] + 1] - cnt[owner[b]] == va) b++;
+                for (int i = a; i < b; i++) {
+                    unsigned banks = 0;
+                    for (int j = i - i % per; j < i; j++) banks |= 1u << (rloc[owner[j]] & 7);
+                    for (int j = i; j < b; j++)
+                        if (!(banks >> (rloc[owner[j]] & 7) & 1u)) { std::swap(owner[i], owner[j]); break; }
+                }
+                a = b;
+            }
+        }
+        // transposed gather list (ResDev::dest / row): the j-th incidence (element order) of the particle in slot q -> row[j] + q
+        std::vector<int> val(N);
+        for (int i = 0; i < N; i++) val[i] = cnt[i + 1] - cnt[i];
+        std::vector<uint16_t> row;
+        const int Ltot = res_rows(val, kpp_, &row);
+        const int maxval = (int)row.size() - 1;
+        std::vector<int> slot_of(N);
+        for (int q = 0; q < N; q++) slot_of[owner[q]] = q;
+        // Which of a particle's rows an incidence takes is free: pick it so that the eight lanes of a quarter-warp (eight
+        // consecutive tets, same vertex position) store into different 16-byte bank groups where possible (STS.128 is served
+        // a quarter-warp at a time); greedy, lowest free row first among the rows whose bank group is still unused.
+        std::vector<std::vector<char>> used(N);
+        for (int i = 0; i < N; i++) used[i].assign(val[i], 0);
+        std::vector<ushort4> dest(M);
+        for (int e0 = 0; e0 < M; e0 += 8) {
+            for (int k = 0; k < 4; k++) {
+                unsigned banks = 0;
+                for (int e = e0; e < std::min(M, e0 + 8); e++) {
+                    const int pk = k == 0 ? pid[e].x : (k == 1 ? pid[e].y : (k == 2 ? pid[e].z : pid[e].w));
+                    int pick = -1, fallback = -1;
+                    for (int j = 0; j < val[pk]; j++) {
+                        if (used[pk][j]) continue;
+                        if (fallback < 0) fallback = j;
+                        if (!(banks >> ((row[j] + slot_of[pk]) & 7) & 1u)) { pick = j; break; }
+                    }
+                    if (pick < 0) pick = fallback;
+                    used[pk][pick] = 1;
+                    const unsigned short dk = (unsigned short)(row[pick] + slot_of[pk]);
+                    banks |= 1u << (dk & 7);
+                    if (k == 0) dest[e].x = dk; else if (k == 1) dest[e].y = dk; else if (k == 2) dest[e].z = dk; else dest[e].w = dk;
+                }
+            }
+        }
+        {
+            // local search on the store side: a quarter-warp's STS.128 of vertex k takes as many wavefronts as its fullest
+            // bank group holds entries; swap the rows of two incidences of one particle while that lowers the total
+            auto dk = [&](int e, int k) -> unsigned short & { return k == 0 ? dest[e].x : (k == 1 ? dest[e].y : (k == 2 ? dest[e].z : dest[e].w)); };
+            auto grp_cost = [&](int e, int k) {
+                int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0}, mx = 0;
+                const int e0 = e & ~7;
+                for (int f = e0; f < std::min(M, e0 + 8); f++) mx = std::max(mx, ++cnt[dk(f, k) & 7]);
+                return mx;
+            };
+            std::vector<std::vector<std::pair<int, int>>> inc(N);
+            for (int e = 0; e < M; e++) {
+                const unsigned short pk[4] = {pid[e].x, pid[e].y, pid[e].z, pid[e].w};
+                for (int k = 0; k < 4; k++) inc[pk[k]].push_back({e, k});
+            }
+            for (int sweep = 0; sweep < 8; sweep++) {
+                bool improved = false;
+                for (int q = 0; q < N; q++)
+                    for (size_t a = 0; a < inc[q].size(); a++)
+                        for (size_t b = a + 1; b < inc[q].size(); b++) {
+                            const int ea = inc[q][a].first, ka = inc[q][a].second, eb = inc[q][b].first, kb = inc[q][b].second;
+                            if ((ea & ~7) == (eb & ~7) && ka == kb) continue;  // same store instruction of the same quarter-warp
+                            const int before = grp_cost(ea, ka) + grp_cost(eb, kb);
+                            std::swap(dk(ea, ka), dk(eb, kb));
+                            if (grp_cost(ea, ka) + grp_cost(eb, kb) < before) improved = true;
+                            else std::swap(dk(ea, ka), dk(eb, kb));
+                        }
+                if (!improved) break;
+            }
+        }
+        ushort4 *d_dest = (ushort4 *)take(dest.size() * sizeof(ushort4));
+        uint16_t *d_row = (uint16_t *)take(row.size() * 2);
+        uint16_t *d_owner = (uint16_t *)take(owner.size() * 2);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_owner, owner.data(), owner.size() * 2, cudaMemcpyHostToDevice, st);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_dest, dest.data(), dest.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_row, row.data(), row.size() * 2, cudaMemcpyHostToDevice, st);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);  // the host vectors die with this call
+        rd.M = M; rd.N = N;
+        rd.nthreads = nthreads_;
+        rd.kpp = kpp_;
+        rd.L = Lsp; rd.rloc = d_rloc;
+        rd.idx = d_idx; rd.owner = d_owner; rd.csr_ptr = d_ptr;
+        rd.dest = d_dest; rd.row = d_row; rd.maxval = maxval; rd.Ltot = Ltot;
+    };
+    ResHost *rh = new ResHost();
+    rh->ept = res_ept(M);
+    rh->ept_fwd = res_ept_fwd(M, N);
+    build_layout(res_threads(M, rh->ept), rh->rd);
+    if (rh->ept_fwd == rh->ept) rh->rd_fwd = rh->rd;
+    else build_layout(res_threads(M, rh->ept_fwd), rh->rd_fwd);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_rloc, rloc.data(), rloc.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_idx, idx.data(), idx.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * 2, cudaMemcpyHostToDevice, st);
-    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_dest, dest.data(), dest.size() * sizeof(ushort4), cudaMemcpyHostToDevice, st);
-    if (ce == cudaSuccess) ce = cudaMemcpyAsync(d_row, row.data(), row.size() * 2, cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-    if (ce != cudaSuccess) return cuda_fail(ce, "resident upload");
-    ResHost *rh = new ResHost();
-    rh->ept = M > kResMaxThreads ? 2 : 1;
-    rh->rd.M = M; rh->rd.N = N;
-    rh->rd.nthreads = nthreads_;
-    rh->rd.kpp = kpp_;
-    rh->rd.L = Lsp; rh->rd.rloc = d_rloc;
-    rh->rd.idx = d_idx; rh->rd.owner = d_owner; rh->rd.csr_ptr = d_ptr;
-    rh->rd.dest = d_dest; rh->rd.row = d_row; rh->rd.maxval = maxval; rh->rd.Ltot = Ltot;
-    rh->smem_fwd = res_smem(Lsp, N, Ltot, maxval, 1, false);
-    rh->smem_adj = res_smem(Lsp, N, Ltot, maxval, 2, true);
+    if (ce != cudaSuccess) { delete rh; return cuda_fail(ce, "resident upload"); }
+    rh->smem_fwd = res_smem(Lsp, N, rh->rd_fwd.Ltot, rh->rd_fwd.maxval, 1, false);
+    rh->smem_adj = res_smem(Lsp, N, rh->rd.Ltot, rh->rd.maxval, 2, true);
     m->res_host = rh;
     int rc = GS_OK;
-#define GS_RES_SMEM(E_, T_, BF_, BA_)                                                                  \
-    do {                                                                                               \
-        rc = set_smem(k_resident_fwd<E_, T_, BF_, false>, rh->smem_fwd);                               \
-        if (rc == GS_OK) rc = set_smem(k_resident_fwd<E_, T_, BF_, true>, rh->smem_fwd);               \
-        if (rc == GS_OK) rc = set_smem(k_resident_adj<E_, T_, BA_, false>, rh->smem_adj);              \
-        if (rc == GS_OK) rc = set_smem(k_resident_adj<E_, T_, BA_, true>, rh->smem_adj);               \
+#define GS_RES_SMEM(K_, E_, T_, B_, BYTES_)                                  \
+    do {                                                                     \
+        if (rc == GS_OK) rc = set_smem(K_<E_, T_, B_, false>, BYTES_);       \
+        if (rc == GS_OK) rc = set_smem(K_<E_, T_, B_, true>, BYTES_);        \
     } while (0)
-    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_SMEM(1, 320, 3, 2);
-    else if (rh->ept == 1) GS_RES_SMEM(1, 1024, 1, 1);
-    else GS_RES_SMEM(2, 1024, 1, 1);
+    if (rh->ept_fwd == 2 && rh->rd_fwd.nthreads <= 160) GS_RES_SMEM(k_resident_fwd, 2, 160, 4, rh->smem_fwd);
+    else if (rh->ept_fwd == 1 && rh->rd_fwd.nthreads <= 320) GS_RES_SMEM(k_resident_fwd, 1, 320, 3, rh->smem_fwd);
+    else if (rh->ept_fwd == 1) GS_RES_SMEM(k_resident_fwd, 1, 1024, 1, rh->smem_fwd);
+    else GS_RES_SMEM(k_resident_fwd, 2, 1024, 1, rh->smem_fwd);
+    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_SMEM(k_resident_adj, 1, 320, 2, rh->smem_adj);
+    else if (rh->ept == 1) GS_RES_SMEM(k_resident_adj, 1, 1024, 1, rh->smem_adj);
+    else GS_RES_SMEM(k_resident_adj, 2, 1024, 1, rh->smem_adj);
 #undef GS_RES_SMEM
     if (rc != GS_OK) return rc;
     m->plan = GS_PLAN_RESIDENT;
@@ -695,17 +717,18 @@ static ResAct res_act(const gs_model *m) {
 int resident_rollout(gs_model *m, gs_tape *t, cudaStream_t st) {
     ResHost *rh = res_of(m);
     if (!rh) { set_error("resident plan unavailable"); return GS_ESTATE; }
-    const dim3 grid(m->E), block(rh->rd.nthreads);
+    const dim3 grid(m->E), block(rh->rd_fwd.nthreads);
     const ResAct ra = res_act(m);
     const bool act = m->act_frames > 0;
     cudaEvent_t ta = m->timing ? timing_begin(m, st) : nullptr;
 #define GS_RES_FWD(E_, T_, B_)                                                                                                      \
     do {                                                                                                                            \
-        if (act) k_resident_fwd<E_, T_, B_, true><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T, ra);      \
-        else k_resident_fwd<E_, T_, B_, false><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd, t->base, t->S, t->T, ra);         \
+        if (act) k_resident_fwd<E_, T_, B_, true><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd_fwd, t->base, t->S, t->T, ra);      \
+        else k_resident_fwd<E_, T_, B_, false><<<grid, block, rh->smem_fwd, st>>>(m->dev, rh->rd_fwd, t->base, t->S, t->T, ra);         \
     } while (0)
-    if (rh->ept == 1 && rh->rd.nthreads <= 320) GS_RES_FWD(1, 320, 3);
-    else if (rh->ept == 1) GS_RES_FWD(1, 1024, 1);
+    if (rh->ept_fwd == 2 && rh->rd_fwd.nthreads <= 160) GS_RES_FWD(2, 160, 4);
+    else if (rh->ept_fwd == 1 && rh->rd_fwd.nthreads <= 320) GS_RES_FWD(1, 320, 3);
+    else if (rh->ept_fwd == 1) GS_RES_FWD(1, 1024, 1);
     else GS_RES_FWD(2, 1024, 1);
 #undef GS_RES_FWD
     GS_RES_CHECK("k_resident_fwd");
