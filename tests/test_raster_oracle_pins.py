@@ -84,3 +84,113 @@ def test_silhouette_loss_gradient_vs_fd():
     assert np.abs(g - fd).max() <= 1e-6 * np.abs(fd).max()
     # and L is what its definition says
     assert abs(L - ((ro.silhouette(x, tris, cam) - target) ** 2).mean()) <= 1e-18
+
+
+# ------------------------------------------------------------------------------------------ colour channel (reading A22b)
+def _sh(gamma=0.05, eps=1e-3, far=10.0, bg=(0.1, 0.2, 0.3)):
+    return ro.Shading(gamma, eps, far, bg)
+
+
+def test_rgb_values_the_definition_fixes():
+    """no triangles -> rgb = background; one fronto-parallel triangle of one colour: the two-term softmax in
+    closed form, with D = 1 deep inside and D = 1/2 at a pixel centre on an edge; a triangle farther than the cut
+    (s < -40 sigma) leaves the pixel at the background exactly."""
+    cam = _cam(W=4, H=4, sigma=1e-4)
+    sh = _sh()
+    bg = sh.background
+    x = np.array([[-20.0, -10.0, 0.0], [20.0, -10.0, 0.0], [0.0, 30.0, 0.0]])
+    col = np.tile([0.9, 0.5, 0.2], (3, 1))
+    I0 = ro.rgb(x, np.zeros((0, 3), int), col, cam, sh)
+    assert all(np.all(I0[c] == bg[c]) for c in range(3))
+    zbar = (sh.far - 5.0) / (sh.far - cam.near)
+    a, b = np.exp(zbar / sh.gamma), np.exp(sh.eps / sh.gamma)
+    I = ro.rgb(x, [[0, 1, 2]], col, cam, sh)
+    for c in range(3):
+        assert np.allclose(I[c], (a * col[0, c] + b * bg[c]) / (a + b), rtol=1e-12)
+    xe = np.array([[-10.0, -1.25, 0.0], [10.0, -1.25, 0.0], [0.0, 10.0, 0.0]])  # edge through the centre of pixel (i=2, j=1)
+    Ie = ro.rgb(xe, [[0, 1, 2]], col, _cam(W=4, H=4, sigma=1e-2), sh)
+    for c in range(3):
+        assert abs(Ie[c, 1, 2] - (0.5 * a * col[0, c] + b * bg[c]) / (0.5 * a + b)) < 1e-12
+    # the row below the edge is 0.5 NDC away: s = -0.25 < -40 * 1e-4 -> not in the sum at all
+    If = ro.rgb(xe, [[0, 1, 2]], col, cam, sh)
+    assert all(np.all(If[c, 0, :] == bg[c]) for c in range(3))
+
+
+def test_rgb_barycentric_interpolation_and_clamping():
+    """With the background weight at zero (eps / gamma = -inf in effect) one triangle's pixel is its own C_j: an affine
+    colour field over the vertices is reproduced at every interior pixel (wrong vertex / weight pairing fails), any vertex
+    order gives the same image, and an exterior pixel beyond the edge opposite vertex k gets none of vertex k's colour."""
+    cam = _cam(W=16, H=12, sigma=5e-2)
+    sh = _sh(eps=-1e4)
+    x = np.array([[-3.5, -3.0, 0.3], [4.0, -2.0, -0.2], [0.5, 3.5, 0.1]])
+    ndc, _ = ro.project(x, cam)
+    A, b0 = np.array([[0.3, -0.2], [0.1, 0.4], [-0.25, 0.15]]), np.array([0.5, 0.4, 0.6])
+    col = ndc @ A.T + b0
+    I = ro.rgb(x, [[0, 1, 2]], col, cam, sh)
+    pu, pv = ro.pixel_centres(cam)
+    inside = ro.hard_silhouette(x, [[0, 1, 2]], cam)
+    assert inside.sum() > 20
+    for c in range(3):
+        assert np.allclose(I[c][inside], (A[c, 0] * pu + A[c, 1] * pv + b0[c])[inside], atol=1e-12)
+    for perm in ([1, 2, 0], [2, 1, 0]):
+        assert np.allclose(ro.rgb(x, [perm], col, cam, sh), I, atol=1e-13)
+    rgbc = np.eye(3)
+    Ic = ro.rgb(x, [[0, 1, 2]], rgbc, cam, sh)
+    lam, _ = ro._bary(pu, pv, ndc)
+    for k in range(3):
+        beyond = lam[k] < 0
+        assert beyond.any() and np.all(Ic[k][beyond] == 0.0)
+    assert np.allclose(Ic.sum(0), 1.0, atol=1e-13)  # the clamped weights are renormalised
+
+
+def test_rgb_depth_softmax_limits():
+    """Two fronto-parallel triangles over the same pixels: gamma -> 0 shows the nearer one, gamma -> infinity the plain mean
+    of the two and the background (all D = 1); the image is a convex combination of the colours throughout."""
+    cam = _cam(W=6, H=6, sigma=1e-6)
+    x = np.array([[-20.0, -10.0, 0.0], [20.0, -10.0, 0.0], [0.0, 30.0, 0.0], [-20.0, -10.0, 1.0], [20.0, -10.0, 1.0], [0.0, 30.0, 1.0]])
+    col = np.array([[1.0, 0.0, 0.0]] * 3 + [[0.0, 1.0, 0.0]] * 3)
+    tris = [[3, 4, 5], [0, 1, 2]]
+    near = ro.rgb(x, tris, col, cam, _sh(gamma=1e-4))
+    assert np.allclose(near[0], 1.0, atol=1e-12) and np.allclose(near[1], 0.0, atol=1e-12)
+    flat = ro.rgb(x, tris, col, cam, _sh(gamma=1e9))
+    for c, want in enumerate([(1.0 + 0.1) / 3, (1.0 + 0.2) / 3, 0.3 / 3]):
+        assert np.allclose(flat[c], want, atol=1e-8)
+    mid = ro.rgb(x, tris, col, cam, _sh(gamma=0.05))
+    zb = [(10.0 - 5.0) / (10.0 - cam.near), (10.0 - 6.0) / (10.0 - cam.near)]
+    wts = np.array([np.exp(zb[0] / 0.05), np.exp(zb[1] / 0.05), np.exp(1e-3 / 0.05)])
+    for c, cols in enumerate([(1.0, 0.0, 0.1), (0.0, 1.0, 0.2), (0.0, 0.0, 0.3)]):  # (near, far, background) per channel
+        assert np.allclose(mid[c], (wts * np.array(cols)).sum() / wts.sum(), rtol=1e-12)
+    rng = np.random.default_rng(11)
+    xr = np.concatenate([rng.uniform(-3, 3, (12, 2)), rng.uniform(-0.5, 0.5, (12, 1))], 1)
+    cr = rng.uniform(0.2, 0.9, (12, 3))
+    Ir = ro.rgb(xr, [[0, 1, 2], [3, 4, 5], [6, 7, 8], [9, 10, 11]], cr, _cam(sigma=3e-3), _sh())
+    assert Ir.min() >= 0.1 - 1e-12 and Ir.max() <= 0.9 + 1e-12
+
+
+def test_rgb_loss_gradients_vs_fd():
+    """dL/dx and dL/dcolours of the pixelwise RGB MSE (hand-written chain rule through coverage, depth softmax and the
+    clamped barycentrics) against central differences: rotated off-axis camera (vertex depths differ), overlapping
+    triangles, many exterior pixels inside the 40 sigma cut."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([rng.uniform(-2.5, 2.5, (9, 2)), rng.uniform(-0.4, 0.4, (9, 1))], 1)
+    tris = np.array([[0, 1, 2], [2, 3, 4], [4, 5, 6], [6, 7, 8], [1, 5, 8]])
+    th = 0.3
+    R = np.array([[np.cos(th), 0, np.sin(th)], [0, 1, 0], [-np.sin(th), 0, np.cos(th)]]) @ np.array([[1, 0, 0], [0, np.cos(0.2), -np.sin(0.2)], [0, np.sin(0.2), np.cos(0.2)]])
+    cam = ro.Camera(R, (0.2, -0.1, 6.0), 1.7, 1.9, 40, 30, 2e-2)
+    sh = _sh()
+    col = rng.uniform(0, 1, (9, 3))
+    target = ro.rgb(x + 0.15 * rng.normal(size=x.shape), tris, rng.uniform(0, 1, (9, 3)), cam, sh)
+    L, gx, gc = ro.rgb_loss_and_grads(x, tris, col, cam, sh, target)
+    assert abs(L - ((ro.rgb(x, tris, col, cam, sh) - target) ** 2).mean()) <= 1e-18
+    f = lambda xx, cc: ro.rgb_loss_and_grads(xx, tris, cc, cam, sh, target)[0]
+    eps = 1e-6
+    fdx, fdc = np.zeros_like(x), np.zeros_like(col)
+    for i in range(9):
+        for r in range(3):
+            d = np.zeros_like(x); d[i, r] = eps
+            fdx[i, r] = (f(x + d, col) - f(x - d, col)) / (2 * eps)
+            fdc[i, r] = (f(x, col + d) - f(x, col - d)) / (2 * eps)
+    assert np.abs(gx).max() > 0 and np.abs(gx - fdx).max() <= 1e-6 * np.abs(fdx).max()
+    assert np.abs(gc).max() > 0 and np.abs(gc - fdc).max() <= 1e-6 * np.abs(fdc).max()
+    # depth matters: the gradient with respect to a pure camera-depth shift of one triangle is not zero
+    assert np.abs(gx @ R[2]).max() > 1e-6
