@@ -483,6 +483,8 @@ def measure(args, config, rank, world, local, dist, with_cpu):
 
 RASTER_FLOPS_FWD, RASTER_FLOPS_BWD = 95, 325  # per evaluated (pixel, triangle) pair: 3 point-segment distances, 3 edge functions,
 # a sigmoid (forward); the adjoint walks the pairs twice and adds the closest-edge weights
+RASTER_FLOPS_FWD_RGB, RASTER_FLOPS_BWD_RGB = 175, 590  # colour channel: + barycentrics, clamp, depth, colour, two exp, the running
+# softmax (forward); the adjoint walks twice, adds the chain through the barycentrics and 18 warp sums
 
 
 def raster_record(devs, steps):
@@ -521,6 +523,12 @@ def raster_record(devs, steps):
 
     ms_f = timed(lambda: gs.render_silhouette(xd, tris, cg))
     ms_b = timed(lambda: gs.loss_silhouette(xd, tris, cg, target))
+    # colour channel (A22b): random vertex colours, depth softmax gamma = 0.05
+    sg = gs.make_shading(0.05, 1e-3, 3.0, (0.1, 0.2, 0.3))
+    cold = torch.as_tensor(r.uniform(0.0, 1.0, x.shape).astype(np.float32), device=devs)
+    target_rgb = gs.render_rgb(torch.as_tensor(x + np.float32(0.004), device=devs), tris, cold, cg, sg)
+    ms_fc = timed(lambda: gs.render_rgb(xd, tris, cold, cg, sg))
+    ms_bc = timed(lambda: gs.loss_rgb(xd, tris, cold, cg, sg, target_rgb))
     # evaluated pairs: triangles whose grown bounding box meets a 16 x 16 tile, x 256 pixels (environment 0, scaled by E)
     ndc, z = ro.project(x[0].astype(np.float64), co)
     q = ndc[sc.tris]
@@ -536,6 +544,10 @@ def raster_record(devs, steps):
     t_cpu = time.perf_counter() - t0
     return {"workload": f"config1 cloth 32x32 ({sc.tris.shape[0]} triangles) x {E} environments, {W}x{H} pixels, sigma {sigma}",
             "ms_render": ms_f, "ms_loss_and_adjoint": ms_b, "evaluated_pairs": pairs,
+            "rgb": {"ms_render": ms_fc, "ms_loss_and_adjoint": ms_bc, "gamma": 0.05,
+                    "alu_frac_upper": pairs * RASTER_FLOPS_FWD_RGB / (ms_fc * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                    "adjoint_alu_frac_upper": pairs * RASTER_FLOPS_BWD_RGB / (ms_bc * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                    "note": "upper bounds: flops per pair as if every culled-in pair passed the per-pixel 40 sigma cut"},
             "roofline": {"bound": "alu", "kernel": "k_rs_forward", "achieved": pairs * RASTER_FLOPS_FWD / (ms_f * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": pairs * RASTER_FLOPS_FWD / (ms_f * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
                          "adjoint_frac": pairs * RASTER_FLOPS_BWD / (ms_b * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,

@@ -272,7 +272,7 @@ int gs_loss_centroid_traj(gs_model *m, gs_tape *t, int frame_stride, const float
  * the particles (any surface mesh: the cloth triangles, or the boundary faces of a tet mesh); images [E][H][W] fp32.
  * gs_loss_silhouette: d_loss [E] (overwritten unless accumulate), d_adj_x [E][N][3] = dL/dx overwritten (may be NULL),
  * d_image optional.  The result feeds gs_rollout_backward as d_adj_x_T or a frame cotangent.  d_scratch: DEVICE block of
- * >= gs_raster_scratch_bytes, 256-byte aligned.  Silhouette channel only: colour / texture shading is not built.
+ * >= gs_raster_scratch_bytes, 256-byte aligned.  The colour channel is gs_render_rgb / gs_loss_rgb below.
  */
 typedef struct {
     float R[9], t[3];      /* world -> camera */
@@ -287,6 +287,36 @@ int gs_render_silhouette(int n_envs, int n_particles, const float *d_x, int n_tr
 int gs_loss_silhouette(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const gs_camera *cam,
                        const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x, float *d_image,
                        void *d_scratch, size_t scratch_bytes, gs_stream stream);
+
+/*
+ * Colour channel of the soft rasteriser and its adjoint (SURVEY.md 8(f) NEXT-4 "silhouette/colour"; A22b).
+ * PAPER.md:168-172 blurs the edges, PAPER.md:495 names the "only colour" shading; the aggregation is the one SPEC.md:251
+ * states ("depth-softmax aggregation ... weights proportional to D_j exp(zbar_j / gamma) plus a background term, normalized;
+ * ... barycentric interpolation of ... vertex colors, barycentrics clamped for exterior pixels"):
+ *   lam_k(p) screen-space (NDC) barycentrics of pixel centre p in triangle j;  w = clip(lam, 0, 1) / sum clip(lam, 0, 1);
+ *   z_j = sum_k w_k Z_k (camera depth),  zbar_j = (far_z - z_j) / (far_z - near_z);  C_j = sum_k w_k c_k;
+ *   I(p) = (sum_j D_j e^{zbar_j / gamma} C_j + e^{eps / gamma} background) / (sum_j D_j e^{zbar_j / gamma} + e^{eps / gamma})
+ * over the drawn triangles with |2 area| > 1e-5 x (longest edge)^2 in NDC (no slivers) and signed squared distance s_j(p) >= -40 sigma; D_j, camera and pixel
+ * grid as for the silhouette.  gs_loss_rgb: L_e (+)= scale sum_p sum_c (I_{e,c}(p) - target_{e,c}(p))^2.
+ * d_colour [E][N][3] per-vertex colours (no lighting); images and targets planar [E][3][H][W] fp32.  d_adj_x [E][N][3] = dL/dx and
+ * d_adj_colour [E][N][3] = dL/dcolour are overwritten (each may be NULL); d_image optional in gs_loss_rgb.  gs_shading is a
+ * HOST struct read during the call.  d_scratch: DEVICE block of >= gs_raster_rgb_scratch_bytes, 256-byte aligned.
+ * Errors: GS_EINVAL (null / misaligned / too small a block, gamma <= 0, far_z <= near_z), GS_ECUDA.
+ */
+typedef struct {
+    float gamma;          /* depth softmax temperature, in units of the normalised depth */
+    float eps;            /* normalised depth of the background term */
+    float far_z;          /* camera depth mapped to zbar = 0 (near_z of the camera maps to 1) */
+    float background[3];
+} gs_shading;
+size_t gs_raster_rgb_scratch_bytes(int n_envs, int n_particles, int n_tris);
+int gs_render_rgb(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const float *d_colour,
+                  const gs_camera *cam, const gs_shading *shading, float *d_image, void *d_scratch, size_t scratch_bytes,
+                  gs_stream stream);
+int gs_loss_rgb(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const float *d_colour,
+                const gs_camera *cam, const gs_shading *shading, const float *d_target, float scale, int accumulate,
+                float *d_loss, float *d_adj_x, float *d_adj_colour, float *d_image, void *d_scratch, size_t scratch_bytes,
+                gs_stream stream);
 
 /*
  * End-to-end convenience with HOST buffers (bench.py's e2e leg): ONE call uploads x0, v0 [E][N][3] and the loss

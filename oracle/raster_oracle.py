@@ -148,11 +148,13 @@ def hard_silhouette(x, tris, cam):
 #   z_j(p)     = sum_k w_k Z_k (camera depths),  zbar_j = (far - z_j) / (far - near)  (nearer = larger)
 #   C_j(p)     = sum_k w_k c_k  (vertex colours c_k in R^3: the "only colour" shading of PAPER.md:495, no lighting)
 #   I(p)       = (sum_j D_j e^{zbar_j / gamma} C_j + e^{eps / gamma} C_b) / (sum_j D_j e^{zbar_j / gamma} + e^{eps / gamma})
-# the sums over the drawn triangles with |2 area| > 1e-12 whose signed squared distance s_j(p) >= -40 sigma (beyond that
+# the sums over the drawn triangles that are not slivers (|2 area| > 1e-5 x the squared longest edge, in NDC: a collinear
+# triangle has no barycentrics, and the threshold sits where fp32 and fp64 still agree on which side a triangle is) whose
+# signed squared distance s_j(p) >= -40 sigma (beyond that
 # D_j < e^-40; the cut is part of the definition, as SoftRas's distance threshold is).  Loss: pixelwise MSE over the three
 # channels, L = mean_{p, c} (I_c(p) - I*_c(p))^2.
 K_CULL = 40.0
-AREA_MIN = 1e-12
+SLIVER = 1e-5
 
 
 class Shading:
@@ -183,7 +185,7 @@ def _rgb_terms(x, tris, cam, sh):
             continue
         q = ndc[tr]
         A2c = (q[1][0] - q[0][0]) * (q[2][1] - q[0][1]) - (q[1][1] - q[0][1]) * (q[2][0] - q[0][0])
-        if abs(A2c) <= AREA_MIN:
+        if abs(A2c) <= SLIVER * max(((q[(k + 1) % 3] - q[k]) ** 2).sum() for k in range(3)):
             continue
         s, best, t, du, dv = _tri_terms(pu, pv, q)
         on = s >= -K_CULL * cam.sigma

@@ -235,6 +235,285 @@ __global__ void k_rs_project_adj(CamDev cam, int E, int N, const float *__restri
     }
 }
 
+// ------------------------------------------------------------------------------------------ colour channel (A22b)
+// depth-softmax aggregation of barycentric vertex colours ("only colour" shading):
+//   lam_k screen-space barycentrics, w = clip(lam, 0, 1) renormalised, z_j = sum w_k Z_k, zbar_j = (far - z_j) / (far - near),
+//   C_j = sum w_k c_k,  I = (sum_j D_j e^{zbar_j / gamma} C_j + e^{eps / gamma} C_b) / (sum_j D_j e^{zbar_j / gamma} + e^{eps / gamma})
+// over the drawn triangles with |2 area| > 1e-5 x (longest edge)^2 (no slivers) and s_j(p) >= -40 sigma.  The exponents are taken relative to a running
+// maximum m (it cancels in the quotient); images are planar [E][3][H][W].
+struct ShadeDev {
+    float inv_gamma, eps_g, far_z, inv_range, bg[3], s_cut;
+};
+struct TriCol { float4 v0, v1, v2; };  // per vertex (Z, r, g, b)
+
+__global__ void k_rs_pack_rgb(int E, int N, int Mt, const int *__restrict__ tris, const float4 *__restrict__ ndc, const float *__restrict__ colour,
+                              TriRec *__restrict__ rec, TriCol *__restrict__ col) {
+    const size_t total = (size_t)E * Mt;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int env = (int)(i / Mt), j = (int)(i - (size_t)env * Mt);
+        const size_t i0 = (size_t)env * N + tris[3 * j], i1 = (size_t)env * N + tris[3 * j + 1], i2 = (size_t)env * N + tris[3 * j + 2];
+        const float4 p0 = ndc[i0], p1 = ndc[i1], p2 = ndc[i2];
+        const float A2 = (p1.x - p0.x) * (p2.y - p0.y) - (p1.y - p0.y) * (p2.x - p0.x);
+        const float l01 = (p1.x - p0.x) * (p1.x - p0.x) + (p1.y - p0.y) * (p1.y - p0.y), l12 = (p2.x - p1.x) * (p2.x - p1.x) + (p2.y - p1.y) * (p2.y - p1.y),
+                    l20 = (p0.x - p2.x) * (p0.x - p2.x) + (p0.y - p2.y) * (p0.y - p2.y);
+        rec[i].b.w = fabsf(A2) > 1e-5f * fmaxf(l01, fmaxf(l12, l20)) ? 1.0f : 0.0f;  // rec[i].a, .box and .b.xyz are k_rs_pack's
+        TriCol c;
+        c.v0 = make_float4(p0.z, colour[3 * i0], colour[3 * i0 + 1], colour[3 * i0 + 2]);
+        c.v1 = make_float4(p1.z, colour[3 * i1], colour[3 * i1 + 1], colour[3 * i1 + 2]);
+        c.v2 = make_float4(p2.z, colour[3 * i2], colour[3 * i2 + 1], colour[3 * i2 + 2]);
+        col[i] = c;
+    }
+}
+
+// as stage_tris, with the colour records of the survivors
+__device__ __forceinline__ int stage_tris_rgb(const TriRec *__restrict__ rec, const TriCol *__restrict__ col, int j0, int Mt, float tu0, float tv0, float tu1,
+                                              float tv1, float4 *sa, float4 *sb, float4 *sc, int *sj, int *s_cnt) {
+    const int tid = threadIdx.y * kRsTile + threadIdx.x, j = j0 + tid;
+    if (tid == 0) *s_cnt = 0;
+    __syncthreads();
+    bool hit = false;
+    TriRec r;
+    if (j < Mt) {
+        r = rec[j];
+        hit = r.b.z > 0.f && r.b.w > 0.f && r.box.x <= tu1 && r.box.z >= tu0 && r.box.y <= tv1 && r.box.w >= tv0;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    int base = 0;
+    if ((tid & 31) == 0 && m) base = atomicAdd(s_cnt, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (hit) {
+        const int o = base + __popc(m & ((1u << (tid & 31)) - 1u));
+        const TriCol c = col[j];
+        sa[o] = r.a; sb[o] = r.b; sj[o] = j;
+        sc[3 * o] = c.v0; sc[3 * o + 1] = c.v1; sc[3 * o + 2] = c.v2;
+    }
+    __syncthreads();
+    return *s_cnt;
+}
+
+// one pixel x one triangle of the colour channel
+struct RgbTerm {
+    float s, D, omD, t, du, dv, lam[3], w[3], isu, iA, e, C[3];  // omD = 1 - D
+    int k;
+    bool on;
+};
+__device__ __forceinline__ void rgb_term(const CamDev &cam, const ShadeDev &sh, float pu, float pv, const float4 &a, const float4 &b, const float4 *c, RgbTerm &r) {
+    r.s = tri_signed_d2(pu, pv, a, b, r.k, r.t, r.du, r.dv);
+    r.on = r.s >= sh.s_cut;
+    if (!r.on) return;
+    // D multiplies e^{zbar / gamma}: its tail must be accurate in RELATIVE terms (the tanh form of the silhouette rounds
+    // D < 6e-8 to zero); s / sigma >= -40 keeps e^{-s / sigma} finite
+    const float ex = expf(-r.s * cam.inv_sigma);
+    r.D = 1.0f / (1.0f + ex);
+    r.omD = ex * r.D;
+    const float e0 = (a.z - a.x) * (pv - a.y) - (a.w - a.y) * (pu - a.x);
+    const float e1 = (b.x - a.z) * (pv - a.w) - (b.y - a.w) * (pu - a.z);
+    const float e2 = (a.x - b.x) * (pv - b.y) - (a.y - b.y) * (pu - b.x);
+    r.iA = 1.0f / (e0 + e1 + e2);
+    r.lam[0] = e1 * r.iA; r.lam[1] = e2 * r.iA; r.lam[2] = e0 * r.iA;
+    const float u0 = fminf(fmaxf(r.lam[0], 0.f), 1.f), u1 = fminf(fmaxf(r.lam[1], 0.f), 1.f), u2 = fminf(fmaxf(r.lam[2], 0.f), 1.f);
+    r.isu = 1.0f / (u0 + u1 + u2);
+    r.w[0] = u0 * r.isu; r.w[1] = u1 * r.isu; r.w[2] = u2 * r.isu;
+    const float z = r.w[0] * c[0].x + r.w[1] * c[1].x + r.w[2] * c[2].x;
+    r.e = (sh.far_z - z) * sh.inv_range * sh.inv_gamma;
+    r.C[0] = r.w[0] * c[0].y + r.w[1] * c[1].y + r.w[2] * c[2].y;
+    r.C[1] = r.w[0] * c[0].z + r.w[1] * c[1].z + r.w[2] * c[2].z;
+    r.C[2] = r.w[0] * c[0].w + r.w[1] * c[1].w + r.w[2] * c[2].w;
+}
+// running softmax sums of one pixel: m = largest exponent so far, den / num relative to it
+struct RgbAcc {
+    float m, den, num[3];
+    __device__ __forceinline__ RgbAcc(const ShadeDev &sh) : m(sh.eps_g), den(1.0f) { num[0] = sh.bg[0]; num[1] = sh.bg[1]; num[2] = sh.bg[2]; }
+    __device__ __forceinline__ void add(const RgbTerm &r) {
+        if (r.e > m) {
+            const float f = expf(m - r.e);
+            den *= f; num[0] *= f; num[1] *= f; num[2] *= f;
+            m = r.e;
+        }
+        const float a = r.D * expf(r.e - m);
+        den += a; num[0] += a * r.C[0]; num[1] += a * r.C[1]; num[2] += a * r.C[2];
+    }
+};
+
+// grid (tiles_x, tiles_y, E).  image [E][3][H][W] out (may be null); target likewise / loss [E] (atomicAdd) optional.
+__global__ void __launch_bounds__(kRsTile *kRsTile) k_rs_forward_rgb(CamDev cam, ShadeDev sh, int Mt, const TriRec *__restrict__ rec, const TriCol *__restrict__ col,
+                                                                      float *__restrict__ image, const float *__restrict__ target, float scale,
+                                                                      float *__restrict__ loss) {
+    __shared__ float4 sa[kRsChunk], sb[kRsChunk], sc[3 * kRsChunk];
+    __shared__ int sj[kRsChunk], s_cnt;
+    __shared__ float red[8];
+    const int env = blockIdx.z, pi = blockIdx.x * kRsTile + threadIdx.x, pj = blockIdx.y * kRsTile + threadIdx.y;
+    const float su = 2.0f / cam.W, sv = 2.0f / cam.H;
+    const float pu = (pi + 0.5f) * su - 1.0f, pv = (pj + 0.5f) * sv - 1.0f;
+    const float tu0 = blockIdx.x * kRsTile * su - 1.0f, tv0 = blockIdx.y * kRsTile * sv - 1.0f, tu1 = tu0 + kRsTile * su, tv1 = tv0 + kRsTile * sv;
+    RgbAcc acc(sh);
+    for (int j0 = 0; j0 < Mt; j0 += kRsChunk) {
+        const int n = stage_tris_rgb(rec + (size_t)env * Mt, col + (size_t)env * Mt, j0, Mt, tu0, tv0, tu1, tv1, sa, sb, sc, sj, &s_cnt);
+        for (int q = 0; q < n; q++) {
+            RgbTerm r;
+            rgb_term(cam, sh, pu, pv, sa[q], sb[q], sc + 3 * q, r);
+            if (r.on) acc.add(r);
+        }
+        __syncthreads();
+    }
+    const bool in = pi < cam.W && pj < cam.H;
+    const size_t plane = (size_t)cam.H * cam.W, o = (size_t)env * 3 * plane + (size_t)pj * cam.W + pi;
+    const float iden = 1.0f / acc.den;
+    float d = 0.f;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const float I = acc.num[c] * iden;
+        if (in && image) image[o + c * plane] = I;
+        if (in && target) { const float dd = I - target[o + c * plane]; d += dd * dd; }
+    }
+    if (target) {
+        for (int w = 16; w > 0; w >>= 1) d += __shfl_xor_sync(0xffffffffu, d, w);
+        const int tid = threadIdx.y * kRsTile + threadIdx.x;
+        if ((tid & 31) == 0) red[tid >> 5] = d;
+        __syncthreads();
+        if (tid == 0) {
+            float tot = 0.f;
+            for (int w = 0; w < 8; w++) tot += red[w];
+            atomicAdd(loss + env, scale * tot);
+        }
+    }
+}
+
+// dL/d(NDC u, v and camera depth Z of the vertices) [E][N] float4 (x, y, z; zero on entry) and dL/dcolour [E][N][3] (zero on
+// entry, may be null) of L = scale sum_{p, c} (I_c - I*_c)^2.  Pass 1 rebuilds the pixel's softmax sums; pass 2, per surviving
+// triangle:  a = D e^{e - m},  g_a = sum_c gI_c (C_c - I_c) / W,  gC_c = gI_c a / W;  through the coverage ds as in the
+// silhouette with dL/ds = g_a a (1 - D) / sigma;  through depth g_z = -g_a a / (gamma (far - near));  g_w_k = g_z Z_k +
+// sum_c gC_c c_kc;  through w = u / sum u, u = clip(lam): g_lam_k = (g_w_k - sum_i g_w_i w_i) / sum u where 0 < lam_k < 1;
+// through lam = (e_1, e_2, e_0) / (e_0 + e_1 + e_2) and the edge functions to the vertices.  The 18 per-vertex components
+// are summed over the warp by shuffles; lane 0 issues the atomics.
+__global__ void __launch_bounds__(kRsTile *kRsTile) k_rs_backward_rgb(CamDev cam, ShadeDev sh, int N, int Mt, const int *__restrict__ tris,
+                                                                       const TriRec *__restrict__ rec, const TriCol *__restrict__ col,
+                                                                       const float *__restrict__ target, float scale, float4 *__restrict__ g_ndc,
+                                                                       float *__restrict__ g_colour) {
+    __shared__ float4 sa[kRsChunk], sb[kRsChunk], sc[3 * kRsChunk];
+    __shared__ int sj[kRsChunk], s_cnt;
+    const int env = blockIdx.z, pi = blockIdx.x * kRsTile + threadIdx.x, pj = blockIdx.y * kRsTile + threadIdx.y;
+    const float su = 2.0f / cam.W, sv = 2.0f / cam.H;
+    const float pu = (pi + 0.5f) * su - 1.0f, pv = (pj + 0.5f) * sv - 1.0f;
+    const float tu0 = blockIdx.x * kRsTile * su - 1.0f, tv0 = blockIdx.y * kRsTile * sv - 1.0f, tu1 = tu0 + kRsTile * su, tv1 = tv0 + kRsTile * sv;
+    const TriRec *re = rec + (size_t)env * Mt;
+    const TriCol *ce = col + (size_t)env * Mt;
+    const bool in = pi < cam.W && pj < cam.H;
+    const int lane = (threadIdx.y * kRsTile + threadIdx.x) & 31;
+    RgbAcc acc(sh);
+    for (int j0 = 0; j0 < Mt; j0 += kRsChunk) {
+        const int n = stage_tris_rgb(re, ce, j0, Mt, tu0, tv0, tu1, tv1, sa, sb, sc, sj, &s_cnt);
+        for (int q = 0; q < n; q++) {
+            RgbTerm r;
+            rgb_term(cam, sh, pu, pv, sa[q], sb[q], sc + 3 * q, r);
+            if (r.on) acc.add(r);
+        }
+        __syncthreads();
+    }
+    const size_t plane = (size_t)cam.H * cam.W, o = (size_t)env * 3 * plane + (size_t)pj * cam.W + pi;
+    const float iW = 1.0f / acc.den;
+    float I[3], gI[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        I[c] = acc.num[c] * iW;
+        gI[c] = in ? 2.0f * scale * (I[c] - target[o + c * plane]) : 0.f;
+    }
+    const bool live = gI[0] != 0.f || gI[1] != 0.f || gI[2] != 0.f;
+    for (int j0 = 0; j0 < Mt; j0 += kRsChunk) {
+        const int n = stage_tris_rgb(re, ce, j0, Mt, tu0, tv0, tu1, tv1, sa, sb, sc, sj, &s_cnt);
+        for (int q = 0; q < n; q++) {
+            RgbTerm r;
+            const float4 a4 = sa[q], b4 = sb[q];
+            const float4 *cq = sc + 3 * q;
+            rgb_term(cam, sh, pu, pv, a4, b4, cq, r);
+            const bool use = live && r.on;
+            if (!__any_sync(0xffffffffu, use)) continue;
+            float g[18];  // NDC (u, v) of vertices 0, 1, 2; Z of 0, 1, 2; colour (r, g, b) of 0, 1, 2
+#pragma unroll
+            for (int i = 0; i < 18; i++) g[i] = 0.f;
+            if (use) {
+                const float a = r.D * expf(r.e - acc.m);
+                const float g_a = (gI[0] * (r.C[0] - I[0]) + gI[1] * (r.C[1] - I[1]) + gI[2] * (r.C[2] - I[2])) * iW;
+                const float gC[3] = {gI[0] * a * iW, gI[1] * a * iW, gI[2] * a * iW};
+                // coverage: closest edge r.k -> r.k + 1
+                const float gs = g_a * a * r.omD * cam.inv_sigma * (r.s >= 0.f ? 1.0f : -1.0f);
+                const float wa = -2.0f * (1.0f - r.t) * gs, wb = -2.0f * r.t * gs;
+                const int ka = r.k, kb = r.k == 2 ? 0 : r.k + 1;
+#pragma unroll
+                for (int v = 0; v < 3; v++) {
+                    const float w = (v == ka ? wa : 0.f) + (v == kb ? wb : 0.f);
+                    g[2 * v] = w * r.du; g[2 * v + 1] = w * r.dv;
+                }
+                // depth and colour through the clamped barycentrics
+                const float g_z = -(g_a * a * sh.inv_gamma) * sh.inv_range;
+                float g_w[3], dot = 0.f;
+#pragma unroll
+                for (int v = 0; v < 3; v++) {
+                    g_w[v] = g_z * cq[v].x + gC[0] * cq[v].y + gC[1] * cq[v].z + gC[2] * cq[v].w;
+                    dot += g_w[v] * r.w[v];
+                    g[6 + v] = g_z * r.w[v];
+                    g[9 + 3 * v] = gC[0] * r.w[v]; g[10 + 3 * v] = gC[1] * r.w[v]; g[11 + 3 * v] = gC[2] * r.w[v];
+                }
+                float g_lam[3], g_A2 = 0.f;
+#pragma unroll
+                for (int v = 0; v < 3; v++) {
+                    g_lam[v] = (r.lam[v] > 0.f && r.lam[v] < 1.f) ? (g_w[v] - dot) * r.isu : 0.f;
+                    g_A2 -= g_lam[v] * r.lam[v];
+                }
+                g_A2 *= r.iA;
+                const float g_e[3] = {g_lam[2] * r.iA + g_A2, g_lam[0] * r.iA + g_A2, g_lam[1] * r.iA + g_A2};
+                const float qu[3] = {a4.x, a4.z, b4.x}, qv[3] = {a4.y, a4.w, b4.y};
+#pragma unroll
+                for (int v = 0; v < 3; v++) {  // e_v = (qb_u - qa_u)(p_v - qa_v) - (qb_v - qa_v)(p_u - qa_u), qa = q_v, qb = q_{v+1}
+                    const int vb = v == 2 ? 0 : v + 1;
+                    g[2 * v] += g_e[v] * (qv[vb] - pv); g[2 * v + 1] += g_e[v] * (pu - qu[vb]);
+                    g[2 * vb] += g_e[v] * (pv - qv[v]); g[2 * vb + 1] -= g_e[v] * (pu - qu[v]);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 18; i++)
+                for (int w = 16; w > 0; w >>= 1) g[i] += __shfl_xor_sync(0xffffffffu, g[i], w);
+            if (lane == 0) {
+                const int *tr = tris + 3 * (size_t)sj[q];
+#pragma unroll
+                for (int v = 0; v < 3; v++) {
+                    float4 *gn = g_ndc + (size_t)env * N + tr[v];
+                    if (g[2 * v] != 0.f) atomicAdd(&gn->x, g[2 * v]);
+                    if (g[2 * v + 1] != 0.f) atomicAdd(&gn->y, g[2 * v + 1]);
+                    if (g[6 + v] != 0.f) atomicAdd(&gn->z, g[6 + v]);
+                    if (g_colour) {
+                        float *gc = g_colour + 3 * ((size_t)env * N + tr[v]);
+#pragma unroll
+                        for (int c = 0; c < 3; c++)
+                            if (g[9 + 3 * v + c] != 0.f) atomicAdd(gc + c, g[9 + 3 * v + c]);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// as k_rs_project_adj with the cotangent of the camera depth added: g = (dL/du, dL/dv, dL/dZ, -)
+__global__ void k_rs_project_adj_rgb(CamDev cam, int E, int N, const float *__restrict__ x, const float4 *__restrict__ g_ndc, float *__restrict__ adj_x) {
+    const size_t total = (size_t)E * N;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const float px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2];
+        const float X = cam.R[0] * px + cam.R[1] * py + cam.R[2] * pz + cam.t[0];
+        const float Y = cam.R[3] * px + cam.R[4] * py + cam.R[5] * pz + cam.t[1];
+        const float Z = cam.R[6] * px + cam.R[7] * py + cam.R[8] * pz + cam.t[2];
+        float gx = 0.f, gy = 0.f, gz = 0.f;
+        if (Z > cam.near_z) {
+            const float4 g = g_ndc[i];
+            const float iz = 1.0f / Z;
+            gx = g.x * cam.fx * iz; gy = g.y * cam.fy * iz; gz = -(g.x * cam.fx * X + g.y * cam.fy * Y) * iz * iz + g.z;
+        }
+        adj_x[3 * i] = cam.R[0] * gx + cam.R[3] * gy + cam.R[6] * gz;
+        adj_x[3 * i + 1] = cam.R[1] * gx + cam.R[4] * gy + cam.R[7] * gz;
+        adj_x[3 * i + 2] = cam.R[2] * gx + cam.R[5] * gy + cam.R[8] * gz;
+    }
+}
+
 static int grid1(size_t n) { size_t g = (n + 255) / 256; return (int)(g < 1 ? 1 : (g > 148 * 16 ? 148 * 16 : g)); }
 static size_t al256r(size_t n) { return (n + 255) & ~(size_t)255; }
 
@@ -301,4 +580,79 @@ extern "C" int gs_loss_silhouette(int n_envs, int n_particles, const float *d_x,
     if (!d_target || !d_loss) { set_error("target and loss are required"); return GS_EINVAL; }
     return raster_run(n_envs, n_particles, d_x, n_tris, d_tris, cam, d_image, d_target, scale, accumulate, d_loss, d_adj_x, d_scratch, scratch_bytes,
                       (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------ colour channel: entry points
+static int shade_dev(const gs_shading *s, const gs_camera *c, ShadeDev *d) {
+    if (!s) { set_error("shading is null"); return GS_EINVAL; }
+    if (!(s->gamma > 0.f) || !(s->far_z > c->near_z)) { set_error("bad shading: gamma > 0, far_z > near_z"); return GS_EINVAL; }
+    d->inv_gamma = 1.0f / s->gamma;
+    d->eps_g = s->eps / s->gamma;
+    d->far_z = s->far_z;
+    d->inv_range = 1.0f / (s->far_z - c->near_z);
+    for (int i = 0; i < 3; i++) d->bg[i] = s->background[i];
+    d->s_cut = -kRsCull * c->sigma;
+    return GS_OK;
+}
+
+extern "C" size_t gs_raster_rgb_scratch_bytes(int n_envs, int n_particles, int n_tris) {
+    if (n_envs < 1 || n_particles < 1 || n_tris < 0) return 0;
+    const size_t mt = n_tris ? n_tris : 1;
+    return 2 * al256r((size_t)n_envs * n_particles * sizeof(float4)) + al256r((size_t)n_envs * mt * sizeof(TriRec)) +
+           al256r((size_t)n_envs * mt * sizeof(TriCol)) + 256;
+}
+
+static int raster_run_rgb(int E, int N, const float *d_x, int Mt, const int32_t *d_tris, const float *d_colour, const gs_camera *cam, const gs_shading *shading,
+                          float *d_image, const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x, float *d_adj_colour,
+                          void *d_scratch, size_t bytes, cudaStream_t st) {
+    CamDev cd;
+    ShadeDev sd;
+    int rc = cam_dev(cam, &cd);
+    if (rc == GS_OK) rc = shade_dev(shading, cam, &sd);
+    if (rc != GS_OK) return rc;
+    if (E < 1 || N < 1 || Mt < 0 || !d_x || !d_colour || (Mt > 0 && !d_tris) || !d_scratch) { set_error("bad argument"); return GS_EINVAL; }
+    if (bytes < gs_raster_rgb_scratch_bytes(E, N, Mt) || ((uintptr_t)d_scratch & 255)) { set_error("raster scratch too small or misaligned"); return GS_EINVAL; }
+    if (E > 65535) { set_error("at most 65535 environments per render call"); return GS_EINVAL; }
+    char *p = (char *)d_scratch;
+    float4 *ndc = (float4 *)p; p += al256r((size_t)E * N * sizeof(float4));
+    float4 *g_ndc = (float4 *)p; p += al256r((size_t)E * N * sizeof(float4));
+    TriRec *rec = (TriRec *)p; p += al256r((size_t)E * (Mt ? Mt : 1) * sizeof(TriRec));
+    TriCol *col = (TriCol *)p;
+    const dim3 grid((cd.W + kRsTile - 1) / kRsTile, (cd.H + kRsTile - 1) / kRsTile, E), block(kRsTile, kRsTile);
+    k_rs_project<<<grid1((size_t)E * N), 256, 0, st>>>(cd, E, N, d_x, ndc);
+    count_launch();
+    if (Mt > 0) {
+        k_rs_pack<<<grid1((size_t)E * Mt), 256, 0, st>>>(cd, E, N, Mt, d_tris, ndc, rec);
+        k_rs_pack_rgb<<<grid1((size_t)E * Mt), 256, 0, st>>>(E, N, Mt, d_tris, ndc, d_colour, rec, col);
+        count_launch(2);
+    }
+    cudaError_t e = cudaSuccess;
+    if (d_loss && !accumulate) e = cudaMemsetAsync(d_loss, 0, sizeof(float) * E, st);
+    if (e != cudaSuccess) return cuda_fail(e, "zero loss");
+    k_rs_forward_rgb<<<grid, block, 0, st>>>(cd, sd, Mt, rec, col, d_image, d_target, scale, d_loss);
+    count_launch();
+    if (d_adj_x || d_adj_colour) {
+        e = cudaMemsetAsync(g_ndc, 0, sizeof(float4) * (size_t)E * N, st);
+        if (e == cudaSuccess && d_adj_colour) e = cudaMemsetAsync(d_adj_colour, 0, sizeof(float) * 3 * (size_t)E * N, st);
+        if (e != cudaSuccess) return cuda_fail(e, "zero raster gradients");
+        if (Mt > 0) { k_rs_backward_rgb<<<grid, block, 0, st>>>(cd, sd, N, Mt, d_tris, rec, col, d_target, scale, g_ndc, d_adj_colour); count_launch(); }
+        if (d_adj_x) { k_rs_project_adj_rgb<<<grid1((size_t)E * N), 256, 0, st>>>(cd, E, N, d_x, g_ndc, d_adj_x); count_launch(); }
+    }
+    e = cudaGetLastError();
+    return e == cudaSuccess ? GS_OK : cuda_fail(e, "raster kernels");
+}
+
+extern "C" int gs_render_rgb(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const float *d_colour, const gs_camera *cam,
+                             const gs_shading *shading, float *d_image, void *d_scratch, size_t scratch_bytes, gs_stream stream) {
+    if (!d_image) { set_error("image is null"); return GS_EINVAL; }
+    return raster_run_rgb(n_envs, n_particles, d_x, n_tris, d_tris, d_colour, cam, shading, d_image, nullptr, 0.f, 0, nullptr, nullptr, nullptr, d_scratch,
+                          scratch_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int gs_loss_rgb(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const float *d_colour, const gs_camera *cam,
+                           const gs_shading *shading, const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x,
+                           float *d_adj_colour, float *d_image, void *d_scratch, size_t scratch_bytes, gs_stream stream) {
+    if (!d_target || !d_loss) { set_error("target and loss are required"); return GS_EINVAL; }
+    return raster_run_rgb(n_envs, n_particles, d_x, n_tris, d_tris, d_colour, cam, shading, d_image, d_target, scale, accumulate, d_loss, d_adj_x,
+                          d_adj_colour, d_scratch, scratch_bytes, (cudaStream_t)stream);
 }

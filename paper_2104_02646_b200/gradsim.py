@@ -59,6 +59,17 @@ def make_camera(R, t, fx, fy, width, height, sigma, near_z=1e-3):
     return c
 
 
+class gs_shading(C.Structure):
+    _fields_ = [("gamma", C.c_float), ("eps", C.c_float), ("far_z", C.c_float), ("background", C.c_float * 3)]
+
+
+def make_shading(gamma, eps, far_z, background):
+    s = gs_shading()
+    s.gamma, s.eps, s.far_z = float(gamma), float(eps), float(far_z)
+    s.background = (C.c_float * 3)(*[float(v) for v in np.asarray(background, np.float64).reshape(3)])
+    return s
+
+
 # name -> (restype, argtypes); the list tests/test_abi.py checks against include/gradsim.h
 _vp, _sz, _int = C.c_void_p, C.c_size_t, C.c_int
 _descp = C.POINTER(gs_model_desc)
@@ -93,6 +104,10 @@ SIGNATURES = {
     "gs_raster_scratch_bytes": (_sz, [_int, _int, _int]),
     "gs_render_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, _vp, _sz, _vp]),
     "gs_loss_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "gs_raster_rgb_scratch_bytes": (_sz, [_int, _int, _int]),
+    "gs_render_rgb": (_int, [_int, _int, _vp, _int, _vp, _vp, C.POINTER(gs_camera), C.POINTER(gs_shading), _vp, _vp, _sz, _vp]),
+    "gs_loss_rgb": (_int, [_int, _int, _vp, _int, _vp, _vp, C.POINTER(gs_camera), C.POINTER(gs_shading), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _vp,
+                           _sz, _vp]),
     "gs_host_scratch_bytes": (_sz, [_vp, _vp, _int, _int]),
     "gs_rollout_loss_backward_host": (_int, [_vp, _vp, _vp, _vp, _int, _int, _vp, _vp, _vp, _vp, _int, C.POINTER(_int), C.POINTER(_vp), _vp, _sz, _vp]),
     "gs_launch_count": (C.c_uint64, []),
@@ -508,3 +523,34 @@ def loss_silhouette(x, tris, cam, target, scale=None, loss=None, accumulate=Fals
     _check(lib().gs_loss_silhouette(E, N, _dp(x), Mt, _dp(tris), C.byref(cam), _dp(_st(target, (E, cam.height, cam.width))), scale, int(accumulate),
                                     _dp(loss), _dp(adj), _dp(img), _dp(scratch), nbytes, _stream()))
     return loss, adj, img
+
+
+def _raster_rgb_args(x, tris, colour):
+    torch = _torch()
+    E, N, Mt, _, _ = _raster_args(x, tris)
+    assert colour.is_cuda and colour.dtype == torch.float32 and colour.is_contiguous() and tuple(colour.shape) == (E, N, 3)
+    nbytes = lib().gs_raster_rgb_scratch_bytes(E, N, Mt)
+    return E, N, Mt, _aligned_bytes(nbytes, x.device), nbytes
+
+
+def render_rgb(x, tris, colour, cam, shading):
+    """x, colour [E, N, 3] cuda fp32, tris [Mt, 3] cuda int32 -> colour images [E, 3, H, W] (A22b)."""
+    torch = _torch()
+    E, N, Mt, scratch, nbytes = _raster_rgb_args(x, tris, colour)
+    img = torch.empty((E, 3, cam.height, cam.width), dtype=torch.float32, device=x.device)
+    _check(lib().gs_render_rgb(E, N, _dp(x), Mt, _dp(tris), _dp(colour), C.byref(cam), C.byref(shading), _dp(img), _dp(scratch), nbytes, _stream()))
+    return img
+
+
+def loss_rgb(x, tris, colour, cam, shading, target, scale=None, loss=None, accumulate=False, want_adj=True, want_adj_colour=True, want_image=False):
+    """L_e (+)= scale sum_{p, c} (I_e(p, c) - target_e(p, c))^2 (scale defaults to 1 / (3 W H): the mean), dL/dx, dL/dcolour."""
+    torch = _torch()
+    E, N, Mt, scratch, nbytes = _raster_rgb_args(x, tris, colour)
+    scale = 1.0 / (3 * cam.width * cam.height) if scale is None else float(scale)
+    loss = torch.zeros(E, dtype=torch.float32, device=x.device) if loss is None else loss
+    adj = torch.empty_like(x) if want_adj else None
+    adj_c = torch.empty_like(colour) if want_adj_colour else None
+    img = torch.empty((E, 3, cam.height, cam.width), dtype=torch.float32, device=x.device) if want_image else None
+    _check(lib().gs_loss_rgb(E, N, _dp(x), Mt, _dp(tris), _dp(colour), C.byref(cam), C.byref(shading), _dp(_st(target, (E, 3, cam.height, cam.width))), scale,
+                             int(accumulate), _dp(loss), _dp(adj), _dp(adj_c), _dp(img), _dp(scratch), nbytes, _stream()))
+    return loss, adj, adj_c, img

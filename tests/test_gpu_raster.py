@@ -104,3 +104,105 @@ def test_pixels_to_parameters_gradient_through_the_rollout():
     assert rel_inf(host(loss), np.array([L])) <= 1e-3
     assert rel_inf(host(av0g), av0) <= 2e-3 and rel_inf(host(ax0g), ax0) <= 2e-3
     assert rel_inf(host(m.param_grads("tri_mu")), o.grads("tri_mu")) <= 2e-3
+
+
+# ------------------------------------------------------------------------------------------ colour channel (reading A22b)
+SHADE = (0.05, 1e-3, 3.0, (0.1, 0.2, 0.3))  # gamma, eps, far, background
+
+
+@pytest.mark.parametrize("W,H,sigma", [(64, 48, 3e-4), (45, 37, 3e-3)])
+def test_rgb_image_and_gradients_match_the_oracle(W, H, sigma):
+    """The wrinkled 12 x 12 sheet of the silhouette test with random vertex colours, two environments: image <= 1e-4
+    absolute per channel (a weight D_j e^{zbar_j / gamma} carries the fp32 rounding of s_j / sigma, up to 40 x 1e-6 relative), loss <= 1e-4 relative, dL/dx and dL/dcolour <= 2e-3 (A18 norm), image sizes that are not multiples
+    of the tile, overlapping projections (the depth softmax decides), many exterior pixels inside the 40 sigma cut."""
+    sc = scenes.make_scene(1, small=True)
+    r = scenes.rng_for(1, "misc", 93)
+    x = np.stack([sc.x0[0] + 0.004 * r.normal(size=sc.x0[0].shape), sc.x0[0] + 0.004 * r.normal(size=sc.x0[0].shape)]).astype(np.float32)
+    x[:, :, 1] += 0.02 * np.sin(40 * x[:, :, 0])
+    col = r.uniform(0.0, 1.0, x.shape).astype(np.float32)
+    cam_args = _camera(W, H, sigma)
+    co, cg = ro.Camera(*cam_args), gs.make_camera(*cam_args)
+    so, sg = ro.Shading(*SHADE), gs.make_shading(*SHADE)
+    tris = sc.tris
+    img = host(gs.render_rgb(dev(x), _itris(tris), dev(col), cg, sg))
+    ref = np.stack([ro.rgb(x[e], tris, col[e], co, so) for e in range(2)])
+    assert img.shape == ref.shape == (2, 3, H, W)
+    assert np.abs(ref - np.array(SHADE[3])[None, :, None, None]).max() > 0.3  # the sheet is visible
+    assert np.abs(img - ref).max() <= 1e-4
+    target = np.stack([ro.rgb(x[e] + 0.01 * r.normal(size=x[e].shape), tris, r.uniform(0, 1, col[e].shape), co, so) for e in range(2)]).astype(np.float32)
+    loss, adj, adj_c, im2 = gs.loss_rgb(dev(x), _itris(tris), dev(col), cg, sg, dev(target), want_image=True)
+    Lg = [ro.rgb_loss_and_grads(x[e], tris, col[e], co, so, target[e]) for e in range(2)]
+    assert rel_inf(host(loss), np.array([l[0] for l in Lg])) <= 1e-4
+    gx, gc = np.stack([l[1] for l in Lg]), np.stack([l[2] for l in Lg])
+    assert np.abs(gx).max() > 0 and np.abs(gc).max() > 0
+    assert rel_inf(host(adj), gx) <= 2e-3
+    assert rel_inf(host(adj_c), gc) <= 2e-3
+    assert np.abs(host(im2) - ref).max() <= 1e-4
+    # accumulate + explicit scale; gradients on request only
+    loss2, a2, c2, _ = gs.loss_rgb(dev(x), _itris(tris), dev(col), cg, sg, dev(target), scale=0.5 / (3 * W * H), loss=loss, accumulate=True, want_adj=False,
+                                   want_adj_colour=False)
+    assert a2 is None and c2 is None
+    assert rel_inf(host(loss2), 1.5 * np.array([l[0] for l in Lg])) <= 1e-4
+
+
+def test_rgb_small_gamma_and_edge_cases():
+    """A sharp depth softmax (gamma = 2e-3: exponents of several hundred, held by the running maximum) still matches; no
+    triangles -> the background exactly; a degenerate triangle and one behind the near plane are skipped; bad shading
+    parameters come back as codes."""
+    sc = scenes.make_scene(1, small=True)
+    r = scenes.rng_for(1, "misc", 94)
+    x = (sc.x0[:1] + 0.004 * r.normal(size=sc.x0[:1].shape)).astype(np.float32)
+    x[:, :, 1] += 0.02 * np.sin(40 * x[:, :, 0])
+    col = r.uniform(0.0, 1.0, x.shape).astype(np.float32)
+    cam_args = _camera(80, 56, 1e-3)
+    co, cg = ro.Camera(*cam_args), gs.make_camera(*cam_args)
+    sharp = (2e-3, 1e-3, 3.0, (0.0, 0.0, 0.0))
+    img = host(gs.render_rgb(dev(x), _itris(sc.tris), dev(col), cg, gs.make_shading(*sharp)))
+    ref = ro.rgb(x[0], sc.tris, col[0], co, ro.Shading(*sharp))[None]
+    # zbar / gamma ~ 350: an fp32 rounding of zbar moves a weight by ~ 4e-5 relative per ulp -- 1e-3 absolute on the image
+    assert np.abs(img - ref).max() <= 1e-3 and np.abs(img - ref).mean() <= 2e-5
+    sg, so = gs.make_shading(*SHADE), ro.Shading(*SHADE)
+    img0 = host(gs.render_rgb(dev(x), _itris(np.zeros((0, 3))), dev(col), cg, sg))
+    assert all(np.all(img0[0, c] == np.float32(SHADE[3][c])) for c in range(3))
+    x4 = np.array([[[0.0, 0.0, 0.0], [0.2, 0.0, 0.0], [0.0, 0.0, 0.2], [0.1, 0.3, -5.0], [0.1, 0.0, 0.0]]], np.float32)
+    c4 = r.uniform(0, 1, x4.shape).astype(np.float32)
+    tris = np.array([[0, 1, 2], [0, 1, 3], [0, 4, 1]])  # drawn, behind the near plane, collinear
+    img4 = host(gs.render_rgb(dev(x4), _itris(tris), dev(c4), cg, sg))
+    assert np.abs(img4[0] - ro.rgb(x4[0], tris, c4[0], co, so)).max() <= 2e-5
+    assert np.abs(img4[0] - ro.rgb(x4[0], tris[:1], c4[0], co, so)).max() <= 2e-5
+    for bad in [(0.0, 1e-3, 3.0, (0, 0, 0)), (0.05, 1e-3, 1e-4, (0, 0, 0))]:
+        with pytest.raises(gs.GradSimError) as e:
+            gs.render_rgb(dev(x4), _itris(tris), dev(c4), cg, gs.make_shading(*bad))
+        assert e.value.code == gs.GS_EINVAL
+
+
+def test_colour_pixels_to_parameters_gradient_through_the_rollout():
+    """PAPER.md:216 with the colour image: unroll the airborne sheet, render x_T in colour, pixelwise MSE, and back through
+    rasteriser and physics: dL/dv0, dL/dx0 and dL/dk_mu against the two oracles chained the same way; dL/dcolour at x_T."""
+    sc = scenes.make_scene(1, small=True)
+    sc.plane_d = -1e6
+    sc.v0 = (sc.v0 + scenes.rng_for(1, "misc", 95).normal(0, 0.2, sc.v0.shape)).astype(np.float32)
+    sc.v0[:, sc.pinned.astype(bool)] = 0
+    T = sc.n_substeps
+    cam_args = _camera(96, 64, 1e-3)
+    co, cg = ro.Camera(*cam_args), gs.make_camera(*cam_args)
+    so, sg = ro.Shading(*SHADE), gs.make_shading(*SHADE)
+    r = scenes.rng_for(1, "misc", 96)
+    col = r.uniform(0.0, 1.0, sc.x0.shape).astype(np.float32)
+    o = orc.Oracle(sc)
+    rollo = o.rollout(sc.x0, sc.v0, T, rec_times=[T])
+    xT = rollo["xT"]
+    target = ro.rgb(xT[0] + np.array([0.01, 0.0, 0.005]), sc.tris, r.uniform(0, 1, col[0].shape), co, so).astype(np.float32)[None]
+    L, gx, gc = ro.rgb_loss_and_grads(xT[0], sc.tris, col[0], co, so, target[0].astype(np.float64))
+    o.zero_grads()
+    ax0, av0 = o.rollout_backward(rollo, [T], gx[None, None])
+    m = gs.Model(sc)
+    tape = m.tape(T)
+    m.zero_grads()
+    xTg, _ = tape.rollout(dev(sc.x0), dev(sc.v0))
+    loss, adj, adj_c, _ = gs.loss_rgb(xTg, _itris(sc.tris), dev(col), cg, sg, dev(target))
+    ax0g, av0g = tape.backward(adj_x_T=adj)
+    assert rel_inf(host(loss), np.array([L])) <= 1e-3
+    assert rel_inf(host(adj_c), gc[None]) <= 2e-3
+    assert rel_inf(host(av0g), av0) <= 2e-3 and rel_inf(host(ax0g), ax0) <= 2e-3
+    assert rel_inf(host(m.param_grads("tri_mu")), o.grads("tri_mu")) <= 2e-3

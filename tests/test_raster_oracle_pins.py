@@ -194,3 +194,14 @@ def test_rgb_loss_gradients_vs_fd():
     assert np.abs(gc).max() > 0 and np.abs(gc - fdc).max() <= 1e-6 * np.abs(fdc).max()
     # depth matters: the gradient with respect to a pure camera-depth shift of one triangle is not zero
     assert np.abs(gx @ R[2]).max() > 1e-6
+
+
+def test_rgb_slivers_and_hidden_triangles_are_skipped():
+    """A collinear triangle (no barycentrics) and one with a vertex behind the near plane add nothing to the colour image."""
+    cam = _cam(W=12, H=10, sigma=1e-2)
+    x = np.array([[-2.0, -1.5, 0.0], [2.0, -1.0, 0.2], [0.0, 2.0, -0.1], [1.0, -1.25, 0.1], [0.3, 0.2, -9.0]])
+    col = np.random.default_rng(2).uniform(0, 1, (5, 3))
+    base = ro.rgb(x, [[0, 1, 2]], col, cam, _sh())
+    assert np.abs(base - _sh().background[:, None, None]).max() > 0.1
+    x[3] = 0.25 * x[0] + 0.75 * x[1]  # on the segment 0-1, hence collinear in the image too
+    assert np.array_equal(ro.rgb(x, [[0, 1, 2], [0, 3, 1], [0, 1, 4]], col, cam, _sh()), base)
