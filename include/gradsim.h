@@ -261,6 +261,22 @@ int gs_loss_centroid_traj(gs_model *m, gs_tape *t, int frame_stride, const float
                           float *d_adj_x_frames, float *d_scratch_x, gs_stream stream);
 
 /*
+ * The open-loop MPC controller that produces an activation schedule, and its weight gradient.
+ * "N phase-shifted sinusoidal signals ... passed to a fully-connected layer (zero-bias), and a final activation
+ * layer.  The output is a vector of per-element activation values"; tanh, 8 signals.  DESIGN.md A23b:
+ *   s_i(t) = sin(omega t + 2 pi i / n_signals);  act[f][e][k] = amplitude tanh(sum_i W[e][k][i] s_i(f frame_dt));
+ *   g_W[e][k][i] = sum_f g_act[f][e][k] amplitude (1 - tanh^2) s_i(f frame_dt).
+ * All arrays DEVICE fp32, caller order: d_W, d_g_W [n_envs][count][n_signals]; d_act [n_frames][n_envs][count] is what
+ * gs_set_actuation takes, d_g_act what gs_actuation_grads writes (frame_dt = frame_stride x dt of that schedule).  Pure
+ * functions of their arguments: no model is touched.  Both overwrite their output.  Errors: GS_EINVAL (sizes < 1,
+ * n_signals > 8192, frame_dt <= 0, null array), GS_ECUDA.
+ */
+int gs_controller_schedule(int n_frames, int n_envs, int count, int n_signals, float omega, float frame_dt, float amplitude,
+                           const float *d_W, float *d_act, gs_stream stream);
+int gs_controller_grads(int n_frames, int n_envs, int count, int n_signals, float omega, float frame_dt, float amplitude,
+                        const float *d_W, const float *d_g_act, float *d_g_W, gs_stream stream);
+
+/*
  * Soft silhouette rasteriser on a headless device buffer, and its adjoint: the image-space loss of
  * the paper's pixels-to-parameters loop.  PAPER.md:168-172 (section 2.2: "replace discontinuous triangle mesh edges with
  * smooth sigmoids"); the formula is the SoftRas silhouette as SPEC.md:251 states it (A22):

@@ -13,7 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgradsim.so")
-SOURCES = ["gs_plan.cu", "gs_stream.cu", "gs_resident.cu", "gs_api.cu", "gs_raster.cu"]
+SOURCES = ["gs_plan.cu", "gs_stream.cu", "gs_resident.cu", "gs_api.cu", "gs_raster.cu", "gs_controller.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",

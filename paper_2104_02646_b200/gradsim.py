@@ -101,6 +101,8 @@ SIGNATURES = {
     "gs_loss_centroid": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
     "gs_loss_pos": (_int, [_int, _int, _vp, _vp, C.c_float, _int, _vp, _vp, _vp]),
     "gs_loss_centroid_traj": (_int, [_vp, _vp, _int, _vp, _vp, _vp, _vp, _vp]),
+    "gs_controller_schedule": (_int, [_int, _int, _int, _int, C.c_float, C.c_float, C.c_float, _vp, _vp, _vp]),
+    "gs_controller_grads": (_int, [_int, _int, _int, _int, C.c_float, C.c_float, C.c_float, _vp, _vp, _vp, _vp]),
     "gs_raster_scratch_bytes": (_sz, [_int, _int, _int]),
     "gs_render_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, _vp, _sz, _vp]),
     "gs_loss_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _sz, _vp]),
@@ -554,3 +556,24 @@ def loss_rgb(x, tris, colour, cam, shading, target, scale=None, loss=None, accum
     _check(lib().gs_loss_rgb(E, N, _dp(x), Mt, _dp(tris), _dp(colour), C.byref(cam), C.byref(shading), _dp(_st(target, (E, 3, cam.height, cam.width))), scale,
                              int(accumulate), _dp(loss), _dp(adj), _dp(adj_c), _dp(img), _dp(scratch), nbytes, _stream()))
     return loss, adj, adj_c, img
+
+
+# ------------------------------------------------------------------------------------------ MPC controller (A23b)
+def controller_schedule(W, n_frames, frame_dt, omega, amplitude=1.0):
+    """W [E, M, N] cuda fp32 -> activation schedule [F, E, M] (the array Model.set_actuation takes)."""
+    torch = _torch()
+    assert W.is_cuda and W.dtype == torch.float32 and W.is_contiguous() and W.ndim == 3
+    E, M, N = W.shape
+    act = torch.empty((int(n_frames), E, M), dtype=torch.float32, device=W.device)
+    _check(lib().gs_controller_schedule(int(n_frames), E, M, N, float(omega), float(frame_dt), float(amplitude), _dp(W), _dp(act), _stream()))
+    return act
+
+
+def controller_grads(W, g_act, frame_dt, omega, amplitude=1.0):
+    """dL/dW [E, M, N] from dL/dact [F, E, M] (what Model.actuation_grads returns)."""
+    torch = _torch()
+    E, M, N = W.shape
+    F = int(g_act.shape[0])
+    g_W = torch.empty_like(W)
+    _check(lib().gs_controller_grads(F, E, M, N, float(omega), float(frame_dt), float(amplitude), _dp(W), _dp(_st(g_act, (F, E, M))), _dp(g_W), _stream()))
+    return g_W
