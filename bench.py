@@ -483,8 +483,8 @@ def measure(args, config, rank, world, local, dist, with_cpu):
 
 RASTER_FLOPS_FWD, RASTER_FLOPS_BWD = 95, 325  # per evaluated (pixel, triangle) pair: 3 point-segment distances, 3 edge functions,
 # a sigmoid (forward); the adjoint walks the pairs twice and adds the closest-edge weights
-RASTER_FLOPS_FWD_RGB, RASTER_FLOPS_BWD_RGB = 175, 590  # colour channel: + barycentrics, clamp, depth, colour, two exp, the running
-# softmax (forward); the adjoint walks twice, adds the chain through the barycentrics and 18 warp sums
+RASTER_FLOPS_FWD_RGB, RASTER_FLOPS_BWD_RGB = 175, 530  # colour channel: + barycentrics, clamp, depth, colour, two exp, the running
+# softmax (forward); the adjoint walks twice, adds the chain through the barycentrics and a transposing warp sum of the 18 vertex components
 
 
 def raster_record(devs, steps):

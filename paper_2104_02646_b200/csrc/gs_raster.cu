@@ -379,6 +379,26 @@ __global__ void __launch_bounds__(kRsTile *kRsTile) k_rs_forward_rgb(CamDev cam,
     }
 }
 
+// Transposing warp sum: every lane brings K <= 32 values g[0..K) (the rest of the 32 slots count as zero); afterwards lane L
+// holds the warp's total of component L.  Halving exchanges (16 + 8 + 4 + 2 + 1 = 31 shuffles instead of 5 K).
+template <int K>
+__device__ __forceinline__ float warp_transpose_sum(const float *g, int lane) {
+    float h[16], q[8], r4[4], r2[2];
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2, b0 = lane & 1;
+#pragma unroll
+    for (int i = 0; i < 16; i++) {
+        const float lo = i < K ? g[i] : 0.f, hi = 16 + i < K ? g[16 + i] : 0.f;
+        h[i] = (b4 ? hi : lo) + __shfl_xor_sync(0xffffffffu, b4 ? lo : hi, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) q[i] = (b3 ? h[8 + i] : h[i]) + __shfl_xor_sync(0xffffffffu, b3 ? h[i] : h[8 + i], 8);
+#pragma unroll
+    for (int i = 0; i < 4; i++) r4[i] = (b2 ? q[4 + i] : q[i]) + __shfl_xor_sync(0xffffffffu, b2 ? q[i] : q[4 + i], 4);
+#pragma unroll
+    for (int i = 0; i < 2; i++) r2[i] = (b1 ? r4[2 + i] : r4[i]) + __shfl_xor_sync(0xffffffffu, b1 ? r4[i] : r4[2 + i], 2);
+    return (b0 ? r2[1] : r2[0]) + __shfl_xor_sync(0xffffffffu, b0 ? r2[0] : r2[1], 1);
+}
+
 // dL/d(NDC u, v and camera depth Z of the vertices) [E][N] float4 (x, y, z; zero on entry) and dL/dcolour [E][N][3] (zero on
 // entry, may be null) of L = scale sum_{p, c} (I_c - I*_c)^2.  Pass 1 rebuilds the pixel's softmax sums; pass 2, per surviving
 // triangle:  a = D e^{e - m},  g_a = sum_c gI_c (C_c - I_c) / W,  gC_c = gI_c a / W;  through the coverage ds as in the
@@ -470,23 +490,18 @@ __global__ void __launch_bounds__(kRsTile *kRsTile) k_rs_backward_rgb(CamDev cam
                     g[2 * vb] += g_e[v] * (pv - qv[v]); g[2 * vb + 1] -= g_e[v] * (pu - qu[v]);
                 }
             }
-#pragma unroll
-            for (int i = 0; i < 18; i++)
-                for (int w = 16; w > 0; w >>= 1) g[i] += __shfl_xor_sync(0xffffffffu, g[i], w);
-            if (lane == 0) {
+            // lane L ends up with the warp's total of component L (0-5 NDC, 6-8 depth, 9-17 colour) and issues its own atomic
+            const float tot = warp_transpose_sum<18>(g, lane);
+            if (lane < 18 && tot != 0.f) {
                 const int *tr = tris + 3 * (size_t)sj[q];
-#pragma unroll
-                for (int v = 0; v < 3; v++) {
-                    float4 *gn = g_ndc + (size_t)env * N + tr[v];
-                    if (g[2 * v] != 0.f) atomicAdd(&gn->x, g[2 * v]);
-                    if (g[2 * v + 1] != 0.f) atomicAdd(&gn->y, g[2 * v + 1]);
-                    if (g[6 + v] != 0.f) atomicAdd(&gn->z, g[6 + v]);
-                    if (g_colour) {
-                        float *gc = g_colour + 3 * ((size_t)env * N + tr[v]);
-#pragma unroll
-                        for (int c = 0; c < 3; c++)
-                            if (g[9 + 3 * v + c] != 0.f) atomicAdd(gc + c, g[9 + 3 * v + c]);
-                    }
+                if (lane < 6) {
+                    float4 *gn = g_ndc + (size_t)env * N + tr[lane >> 1];
+                    atomicAdd((lane & 1) ? &gn->y : &gn->x, tot);
+                } else if (lane < 9) {
+                    atomicAdd(&g_ndc[(size_t)env * N + tr[lane - 6]].z, tot);
+                } else if (g_colour) {
+                    const int v = (lane - 9) / 3, c = (lane - 9) - 3 * v;
+                    atomicAdd(g_colour + 3 * ((size_t)env * N + tr[v]) + c, tot);
                 }
             }
         }
