@@ -57,6 +57,32 @@ def test_desc_struct_matches_header_field_order():
     assert fields == [f[0] for f in gs.gs_model_desc._fields_]
 
 
+def _struct_fields(name):
+    src = open(os.path.join(ROOT, "include", "gradsim.h")).read()
+    body = re.search(r"typedef struct \{((?:(?!typedef struct).)*?)\} %s;" % name, src, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if not decl:
+            continue
+        ctype = re.match(r"(const\s+)?(int32_t|uint32_t|uint8_t|float)", decl).group(2)
+        decl = re.sub(r"^(const\s+)?(int32_t|uint32_t|uint8_t|float)\s*", "", decl)
+        for part in decl.split(","):
+            dim = re.search(r"\[(\d+)\]", part)
+            fields.append((re.sub(r"[\*\s]|\[\d+\]", "", part), ctype, int(dim.group(1)) if dim else 0))
+    return fields
+
+
+@pytest.mark.parametrize("name,cls", [("gs_camera", gs.gs_camera), ("gs_shading", gs.gs_shading)])
+def test_host_structs_of_the_rasteriser_match_the_header(name, cls):
+    """field order, scalar type and array length of the HOST structs the rasteriser calls read"""
+    ctype = {"float": C.c_float, "int32_t": C.c_int32}
+    want = [(n, ctype[t] * d if d else ctype[t]) for n, t, d in _struct_fields(name)]
+    assert [(f[0], f[1]) for f in cls._fields_] == want
+    assert C.sizeof(cls) == sum(C.sizeof(t) for _, t in want)  # no padding: all members are 4-byte scalars
+
+
 def test_param_group_enum_matches_binding():
     src = open(os.path.join(ROOT, "include", "gradsim.h")).read()
     body = re.search(r"enum gs_param_group \{(.*?)\};", src, flags=re.S).group(1)
@@ -78,6 +104,12 @@ def test_argument_errors_without_a_device(lib_path):
     assert b"desc" in L.gs_last_error()
     assert L.gs_tape_bytes(None, 10, 1) == 0
     assert L.gs_zero_grads(None, None) == gs.GS_EINVAL
+    # rasteriser colour channel and controller: sizes and null arguments are rejected before any launch
+    assert L.gs_raster_rgb_scratch_bytes(0, 10, 10) == 0 and L.gs_raster_rgb_scratch_bytes(2, 10, 0) > 0
+    assert L.gs_render_rgb(1, 3, None, 1, None, None, None, None, None, None, 0, None) == gs.GS_EINVAL
+    assert L.gs_controller_schedule(0, 1, 1, 8, 1.0, 0.1, 1.0, None, None, None) == gs.GS_EINVAL
+    assert b"controller" in L.gs_last_error()
+    assert L.gs_controller_grads(4, 1, 1, 8, 1.0, -0.1, 1.0, None, None, None, None) == gs.GS_EINVAL
     assert L.gs_step_forward(None, None, None, None, None, None) == gs.GS_EINVAL
     d = gs.gs_model_desc()
     d.n_particles, d.n_envs = 0, 1
