@@ -165,8 +165,8 @@ int gs_set_params(gs_model *m, int group, const float *d_values, gs_stream strea
  * actuation value that allows the element to expand and contract" -- here alpha = 1 + 3 mu / (4 lambda) + act (DESIGN.md
  * A1), act per tet; f_b = k_b sin(phi/2 + alpha) d with alpha "a per-edge actuation value that allows
  * the mesh to flex inwards or outwards", per hinge.  Activations vary in time (App. E: a controller
- * evaluated over simulation time produces them; the controller itself stays outside the library): a SCHEDULE of n_frames
- * frames, frame f holding during substeps [f frame_stride, (f+1) frame_stride) of a rollout, the last frame to the end.
+ * evaluated over simulation time produces them; that controller is gs_controller_schedule / gs_controller_grads below): a
+ * SCHEDULE of n_frames frames, frame f holding during substeps [f frame_stride, (f+1) frame_stride) of a rollout, the last frame to the end.
  *   gs_actuation_create   attaches a schedule, all zeros (= passive), stored in d_mem (DEVICE, >= gs_actuation_bytes,
  *                         256-byte aligned, must outlive the model or the next create); n_frames = 0 detaches.
  *   gs_set_actuation      DEVICE values [n_frames][E][count] in caller element order (count = M or Mh).

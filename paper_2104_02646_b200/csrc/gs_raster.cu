@@ -6,7 +6,7 @@
 //     D_j(p) = sigmoid(delta_j(p) d^2(p, boundary of triangle j) / sigma),  delta = +1 inside, -1 outside (NDC distances)
 //     S(p)   = 1 - prod_j (1 - D_j(p));     loss ("pixelwise MSE")  L = scale sum_p (S(p) - S*(p))^2
 // Camera: pinhole, p_cam = R x + t, drawn iff z_cam > near for all three vertices, NDC (u, v) = (fx X / Z, fy Y / Z), pixel
-// (i, j) centre at u = 2 (i + 1/2) / W - 1, v = 2 (j + 1/2) / H - 1.  Silhouette channel only (no colour / texture shading).
+// (i, j) centre at u = 2 (i + 1/2) / W - 1, v = 2 (j + 1/2) / H - 1.  The colour channel (A22b) is in the second half of this file.
 //
 // Kernels (plain fp32 ALU work, no tensor cores: per pixel x per triangle distance evaluations):
 //   k_rs_project      particles -> NDC
