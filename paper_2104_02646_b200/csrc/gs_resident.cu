@@ -81,8 +81,13 @@ static size_t res_smem(int L, int N, int Ltot, int maxval, int planes, bool adj)
            al16((size_t)(N + 1) * 2) + al16((size_t)N * 2) + al16((size_t)(maxval + 1) * 2);
 }
 static int res_ept(int M) { return M > kResMaxThreads ? 2 : 1; }
-// forward: two tets per thread as soon as half the threads still hold one particle each
-static int res_ept_fwd(int M, int N) { return (M > kResMaxThreads || ((M + 1) / 2 + 31) / 32 * 32 >= N) ? 2 : 1; }
+// forward: two tets per thread where half the threads still hold one particle each AND the batch fills the GPU (more than two
+// CTAs per SM: throughput-bound).  A small batch is latency-bound per CTA and runs faster with one tet per thread
+// (config 0, one environment: forward 2.6 ms against 3.2 ms).
+constexpr int kResBatchEnvs = 2 * 148;
+static int res_ept_fwd(int M, int N, int E) {
+    return (M > kResMaxThreads || (E > kResBatchEnvs && ((M + 1) / 2 + 31) / 32 * 32 >= N)) ? 2 : 1;
+}
 static int res_threads(int M, int ept) { return ((M + ept - 1) / ept + 31) / 32 * 32; }
 static int res_kpp(int nthreads, int N) { return nthreads >= 4 * N ? 4 : (nthreads >= 2 * N ? 2 : 1); }
 // rows of the transposed gather list from the valences (any order): row[j] (maxval + 1 entries); returns the padded total.
@@ -123,7 +128,7 @@ static bool resident_fits(const gs_model_desc *d) {
     const std::vector<int> val = res_valences(d);
     const int maxval = *std::max_element(val.begin(), val.end());
     const int Ltot = res_rows(val, res_kpp(nthreads, d->n_particles), nullptr);
-    const int nthreads_f = res_threads(d->n_tets, res_ept_fwd(d->n_tets, d->n_particles));
+    const int nthreads_f = res_threads(d->n_tets, res_ept_fwd(d->n_tets, d->n_particles, d->n_envs));
     const int Ltot_f = res_rows(val, res_kpp(nthreads_f, d->n_particles), nullptr);
     if (Ltot > 65535 || Ltot_f > 65535) return false;
     return res_smem(d->n_particles + 24, d->n_particles, Ltot, maxval, 2, true) <= 200 * 1024 &&
@@ -673,7 +678,7 @@ int resident_prepare(gs_model *m, const gs_model_desc *d, void *d_workspace, siz
     };
     ResHost *rh = new ResHost();
     rh->ept = res_ept(M);
-    rh->ept_fwd = res_ept_fwd(M, N);
+    rh->ept_fwd = res_ept_fwd(M, N, d->n_envs);
     build_layout(res_threads(M, rh->ept), rh->rd);
     if (rh->ept_fwd == rh->ept) rh->rd_fwd = rh->rd;
     else build_layout(res_threads(M, rh->ept_fwd), rh->rd_fwd);

@@ -143,6 +143,34 @@ def test_resident_plan_rollout_and_gradients(config):
         assert rel_inf(got[k], ref[k]) <= TOL_GRAD, k
 
 
+def test_resident_plan_large_batch_uses_the_two_tets_per_thread_forward_layout():
+    """A batch that fills the GPU (more than two CTAs per SM) switches the resident forward kernel to its own layout (two
+    tets per thread, 160-thread CTAs, its own gather list); the adjoint keeps one tet per thread.  304 deformed environments,
+    airborne for 96 substeps; sampled environments against the oracle run on each alone, element by element, and the whole
+    batch against the streaming plan."""
+    sc = scenes.batched_sysid_scene(n_envs=304, n_substeps=96, y0=0.02)
+    sc.x0, sc.v0 = scenes.perturbed_state(sc, amp_x=0.08, amp_v=0.4, seed=5)
+    tgt = orc.truth_targets(sc)
+    got = gpu_run_scene(sc, tgt, plan=gs.GS_PLAN_RESIDENT)
+    assert got["model"].plan == gs.GS_PLAN_RESIDENT and got["bad"] == -1
+    ext = sc.extent()
+    for e in (0, 1, 157, 295, 296, 303):
+        s1 = copy.copy(sc)
+        s1.n_envs = 1
+        for k in ("x0", "v0", "mass", "tet_mu", "tet_lambda", "tet_damp", "tri_mu", "tri_lambda", "tri_damp", "ke", "kd", "kf", "mu_c", "k_drag", "k_lift"):
+            setattr(s1, k, getattr(sc, k)[e:e + 1])
+        s1.truth = {k: v[e:e + 1] for k, v in sc.truth.items()}
+        ref = orc.run_scene(s1, target=tgt[:, e:e + 1])
+        assert np.abs(got["xT"][e] - ref["xT"][0]).max() <= TOL_ROLLOUT * ext
+        for k in ("adj_x0", "adj_v0", "g_tet_mu", "g_tet_lambda", "g_tet_damp", "g_mass"):
+            assert np.abs(ref[k]).max() > 0, k
+            assert rel_inf(got[k][e], ref[k][0]) <= TOL_GRAD, (e, k)
+    stream = gpu_run_scene(sc, tgt, plan=gs.GS_PLAN_STREAMING)
+    assert np.abs(got["xT"] - stream["xT"]).max() <= 1e-4 * ext
+    for k in ("adj_x0", "g_tet_mu", "g_mass"):
+        assert rel_inf(got[k], stream[k]) <= 1e-3, k
+
+
 def test_resident_plan_edge_cases():
     x = np.array([[0, 0.01, 0], [0.1, 0.01, 0], [0, 0.11, 0], [0, 0.01, 0.1]], float)
     # a single tet (4 particles, one warp) rolls out resident and matches the oracle
