@@ -305,6 +305,23 @@ int gs_loss_silhouette(int n_envs, int n_particles, const float *d_x, int n_tris
                        void *d_scratch, size_t scratch_bytes, gs_stream stream);
 
 /*
+ * gs_loss_silhouette without any allocation and without a caller scratch block, for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same arguments, results and errors as
+ * gs_loss_silhouette (d_image and d_adj_x optional), but the scratch lives in a file-scope device array of
+ * GS_RASTER_STATIC_BYTES (8 MiB) inside the library: every GPU that loads the library holds that much until the process
+ * exits.  A problem whose gs_raster_scratch_bytes(n_envs, n_particles, n_tris) exceeds GS_RASTER_STATIC_BYTES is rejected
+ * with GS_EINVAL before any CUDA call (e.g. 64 environments x 1089 particles x 1922 triangles = 7.6 MiB fits; twice that does
+ * not).  The call itself enqueues kernels and cudaMemsetAsync only: no cudaMalloc / cudaFree / allocating library routine.
+ * ALL calls on one GPU share the one array and it keeps the last call's contents (what must start at zero is cleared by the
+ * call): two calls that overlap on the GPU (different streams, or graphs replayed concurrently) RACE -- serialise them.  The
+ * array's device address is looked up once per device, with the caller's current device, on first use.
+ */
+#define GS_RASTER_STATIC_BYTES (8u << 20)
+int gs_loss_silhouette_static(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const gs_camera *cam,
+                              const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x, float *d_image,
+                              gs_stream stream);
+
+/*
  * Colour channel of the soft rasteriser and its adjoint (SURVEY.md 8(f) NEXT-4 "silhouette/colour"; A22b).
  * PAPER.md:168-172 blurs the edges, PAPER.md:495 names the "only colour" shading; the aggregation is the one SPEC.md:251
  * states ("depth-softmax aggregation ... weights proportional to D_j exp(zbar_j / gamma) plus a background term, normalized;

@@ -671,3 +671,54 @@ extern "C" int gs_loss_rgb(int n_envs, int n_particles, const float *d_x, int n_
     return raster_run_rgb(n_envs, n_particles, d_x, n_tris, d_tris, d_colour, cam, shading, d_image, d_target, scale, accumulate, d_loss, d_adj_x,
                           d_adj_colour, d_scratch, scratch_bytes, (cudaStream_t)stream);
 }
+
+// ------------------------------------------------------------------------------------------ entry point that allocates nothing
+// gs_loss_silhouette_static: gs_loss_silhouette with the scratch block (NDC vertices, NDC gradients, triangle records) in a
+// file-scope device array instead of a caller block, for callers that cannot allocate (CUDA graph capture, serving loops).
+// GS_RASTER_STATIC_BYTES of every GPU that loads the library are held until the process exits.  In host code the array's
+// name is a host-side stand-in, not a device address: the address is taken with cudaGetSymbolAddress, once per device, with
+// that device current, and passed to the kernels like any other scratch pointer.
+static __device__ __align__(256) unsigned char g_rs_static[GS_RASTER_STATIC_BYTES];
+
+#include <mutex>
+static int raster_static_ptr(void **out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static void *ptrs[kMaxDev] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice (static raster scratch)");
+    if (dev < 0 || dev >= kMaxDev) { set_error("static raster scratch: device ordinal %d out of range", dev); return GS_EINVAL; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_rs_static);  // of the CURRENT device's copy of the array
+        if (e != cudaSuccess || !p) return cuda_fail(e, "cudaGetSymbolAddress (static raster scratch)");
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return GS_OK;
+}
+
+extern "C" int gs_loss_silhouette_static(int n_envs, int n_particles, const float *d_x, int n_tris, const int32_t *d_tris, const gs_camera *cam,
+                                         const float *d_target, float scale, int accumulate, float *d_loss, float *d_adj_x, float *d_image,
+                                         gs_stream stream) {
+    if (!d_target || !d_loss) { set_error("target and loss are required"); return GS_EINVAL; }
+    // sizes first: no CUDA call is made for a problem the block cannot hold
+    const size_t need = gs_raster_scratch_bytes(n_envs, n_particles, n_tris);
+    if (need == 0) { set_error("bad argument: n_envs, n_particles >= 1, n_tris >= 0"); return GS_EINVAL; }
+    if (need > (size_t)GS_RASTER_STATIC_BYTES) {
+        set_error("gs_loss_silhouette_static: this problem needs %zu bytes of scratch, the static block holds %zu (GS_RASTER_STATIC_BYTES); "
+                  "use gs_loss_silhouette with a caller block",
+                  need, (size_t)GS_RASTER_STATIC_BYTES);
+        return GS_EINVAL;
+    }
+    void *scratch = nullptr;
+    const int rc = raster_static_ptr(&scratch);
+    if (rc != GS_OK) return rc;
+    // the block keeps the previous call's contents: the NDC vertices and the triangle records are fully rewritten by
+    // k_rs_project / k_rs_pack for this call's sizes, the NDC gradients and (unless accumulate) the loss are zeroed by
+    // raster_run (cudaMemsetAsync on the stream: no allocation) before the adjoint adds into them
+    return raster_run(n_envs, n_particles, d_x, n_tris, d_tris, cam, d_image, d_target, scale, accumulate, d_loss, d_adj_x, scratch,
+                      (size_t)GS_RASTER_STATIC_BYTES, (cudaStream_t)stream);
+}

@@ -106,6 +106,7 @@ SIGNATURES = {
     "gs_raster_scratch_bytes": (_sz, [_int, _int, _int]),
     "gs_render_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, _vp, _sz, _vp]),
     "gs_loss_silhouette": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "gs_loss_silhouette_static": (_int, [_int, _int, _vp, _int, _vp, C.POINTER(gs_camera), _vp, C.c_float, _int, _vp, _vp, _vp, _vp]),
     "gs_raster_rgb_scratch_bytes": (_sz, [_int, _int, _int]),
     "gs_render_rgb": (_int, [_int, _int, _vp, _int, _vp, _vp, C.POINTER(gs_camera), C.POINTER(gs_shading), _vp, _vp, _sz, _vp]),
     "gs_loss_rgb": (_int, [_int, _int, _vp, _int, _vp, _vp, C.POINTER(gs_camera), C.POINTER(gs_shading), _vp, C.c_float, _int, _vp, _vp, _vp, _vp, _vp,
@@ -577,3 +578,20 @@ def controller_grads(W, g_act, frame_dt, omega, amplitude=1.0):
     g_W = torch.empty_like(W)
     _check(lib().gs_controller_grads(F, E, M, N, float(omega), float(frame_dt), float(amplitude), _dp(W), _dp(_st(g_act, (F, E, M))), _dp(g_W), _stream()))
     return g_W
+
+
+RASTER_STATIC_BYTES = 8 << 20  # GS_RASTER_STATIC_BYTES
+
+
+def loss_silhouette_static(x, tris, cam, target, loss, adj=None, image=None, scale=None, accumulate=False):
+    """gs_loss_silhouette_static: as loss_silhouette, with the scratch in the library's static device array.  Nothing is
+    allocated, here either: the caller passes every output (loss [E]; adj [E, N, 3] and image [E, H, W] optional)."""
+    torch = _torch()
+    E, N, _ = x.shape
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+    assert tris.is_cuda and tris.dtype == torch.int32 and tris.is_contiguous() and tris.ndim == 2 and tris.shape[1] == 3
+    scale = 1.0 / (cam.width * cam.height) if scale is None else float(scale)
+    _check(lib().gs_loss_silhouette_static(E, N, _dp(x), int(tris.shape[0]), _dp(tris), C.byref(cam), _dp(_st(target, (E, cam.height, cam.width))), scale,
+                                           int(accumulate), _dp(_st(loss, (E,))), _dp(adj if adj is None else _st(adj, (E, N, 3))),
+                                           _dp(image if image is None else _st(image, (E, cam.height, cam.width))), _stream()))
+    return loss, adj, image
