@@ -114,6 +114,21 @@ def hinges_from_tris(tris: np.ndarray) -> np.ndarray:
     return np.asarray(out, dtype=np.int32).reshape(-1, 4)
 
 
+
+def boundary_faces(tets: np.ndarray) -> np.ndarray:
+    """Triangles of a tet mesh that belong to exactly one tet: the surface the rasteriser draws for a solid
+    (include/gradsim.h, gs_render_silhouette: "the boundary faces of a tet mesh").  Topology only; [F,3] int32, in the
+    order of first appearance, each face in the vertex order of its tet."""
+    count, faces = {}, []
+    for a, b, c, d in np.asarray(tets).tolist():
+        for f in ((b, c, d), (a, d, c), (a, b, d), (a, c, b)):
+            key = tuple(sorted(f))
+            if key not in count:
+                count[key] = 0
+                faces.append((key, f))
+            count[key] += 1
+    return np.asarray([f for key, f in faces if count[key] == 1], dtype=np.int32).reshape(-1, 3)
+
 # ----------------------------------------------------------------------------
 # scene container
 # ----------------------------------------------------------------------------

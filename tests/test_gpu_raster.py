@@ -206,3 +206,39 @@ def test_colour_pixels_to_parameters_gradient_through_the_rollout():
     assert rel_inf(host(adj_c), gc[None]) <= 2e-3
     assert rel_inf(host(av0g), av0) <= 2e-3 and rel_inf(host(ax0g), ax0) <= 2e-3
     assert rel_inf(host(m.param_grads("tri_mu")), o.grads("tri_mu")) <= 2e-3
+
+
+@pytest.mark.parametrize("plan", [gs.GS_PLAN_RESIDENT, gs.GS_PLAN_STREAMING])
+def test_solid_pixels_to_parameters_gradient_through_the_rollout(plan):
+    """The deformable-solid loop of the paper (material parameters and masses of an FEM solid from images):
+    unroll the falling, bouncing box of config 0 (small), draw the BOUNDARY FACES of its tet mesh at x_T, pixelwise MSE against
+    a target silhouette, and back through rasteriser and physics: dL/dmu, dL/dlambda, dL/dk_damp per tet, dL/dm per particle,
+    dL/dx0, dL/dv0 against the two oracles chained the same way, on both plans."""
+    sc = scenes.make_scene(0, small=True)
+    T = sc.n_substeps
+    faces = scenes.boundary_faces(sc.tets)
+    th = 0.5
+    R = np.array([[np.cos(th), 0, np.sin(th)], [0, 1, 0], [-np.sin(th), 0, np.cos(th)]])
+    cam_args = (R, -R @ sc.x0[0].astype(np.float64).mean(0) + np.array([0.0, 0.05, 1.2]), 2.0, 2.0, 96, 80, 1e-3)
+    co, cg = ro.Camera(*cam_args), gs.make_camera(*cam_args)
+    o = orc.Oracle(sc)
+    rollo = o.rollout(sc.x0, sc.v0, T, rec_times=[T])
+    xT = rollo["xT"]
+    target = ro.silhouette(xT[0] * np.array([1.05, 0.9, 1.0]) + np.array([0.02, 0.0, 0.01]), faces, co).astype(np.float32)[None]
+    L, gx = ro.silhouette_loss_and_grad(xT[0], faces, co, target[0].astype(np.float64))
+    assert L > 1e-4 and np.abs(gx).max() > 0
+    o.zero_grads()
+    ax0, av0 = o.rollout_backward(rollo, [T], gx[None, None])
+    m = gs.Model(sc, plan=plan)
+    assert m.plan == plan
+    tape = m.tape(T)
+    m.zero_grads()
+    xTg, _ = tape.rollout(dev(sc.x0), dev(sc.v0))
+    loss, adj, _ = gs.loss_silhouette(xTg, _itris(faces), cg, dev(target))
+    ax0g, av0g = tape.backward(adj_x_T=adj)
+    assert m.check_finite() == -1
+    assert rel_inf(host(loss), np.array([L])) <= 1e-3
+    assert rel_inf(host(av0g), av0) <= 2e-3 and rel_inf(host(ax0g), ax0) <= 2e-3
+    for g in ("tet_mu", "tet_lambda", "tet_damp", "mass"):
+        assert np.abs(o.grads(g)).max() > 0
+        assert rel_inf(host(m.param_grads(g)), o.grads(g)) <= 2e-3, g

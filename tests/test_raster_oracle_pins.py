@@ -3,6 +3,7 @@ SPEC.md:240-251 and the mathematics fix.  No GPU."""
 import numpy as np
 
 from oracle import raster_oracle as ro
+from paper_2104_02646_b200 import scenes
 
 
 def _cam(W=32, H=24, sigma=1e-3, fx=1.0, fy=1.0, t=(0.0, 0.0, 5.0)):
@@ -205,3 +206,28 @@ def test_rgb_slivers_and_hidden_triangles_are_skipped():
     assert np.abs(base - _sh().background[:, None, None]).max() > 0.1
     x[3] = 0.25 * x[0] + 0.75 * x[1]  # on the segment 0-1, hence collinear in the image too
     assert np.array_equal(ro.rgb(x, [[0, 1, 2], [0, 3, 1], [0, 1, 4]], col, cam, _sh()), base)
+
+
+def test_boundary_faces_of_a_tet_mesh_and_its_silhouette():
+    """scenes.boundary_faces (topology only): one tet -> its four faces; the 4 x 4 x 4-cell box -> 6 x 16 x 2 = 192 triangles
+    forming a closed surface (every edge in exactly two faces), all on the box's boundary; and the silhouette drawn from them is
+    that of ALL tet faces (interior faces project inside the outline: same hard silhouette as sigma -> 0)."""
+    assert sorted(map(sorted, scenes.boundary_faces(np.array([[0, 1, 2, 3]])).tolist())) == [[0, 1, 2], [0, 1, 3], [0, 2, 3], [1, 2, 3]]
+    sc = scenes.make_scene(0, small=True)
+    f = scenes.boundary_faces(sc.tets)
+    assert f.shape == (192, 3)
+    edges = {}
+    for t in f.tolist():
+        for a, b in ((t[0], t[1]), (t[1], t[2]), (t[2], t[0])):
+            edges[tuple(sorted((a, b)))] = edges.get(tuple(sorted((a, b))), 0) + 1
+    assert set(edges.values()) == {2}
+    x = sc.x_rest.astype(np.float64)
+    lo, hi = x.min(0), x.max(0)
+    on_boundary = (np.isclose(x, lo) | np.isclose(x, hi)).any(1)
+    assert on_boundary[f].all() and not on_boundary.all()
+    all_faces = np.array([[t[i] for i in idx] for t in sc.tets.tolist() for idx in ((1, 2, 3), (0, 3, 2), (0, 1, 3), (0, 2, 1))])
+    th = 0.5
+    R = np.array([[np.cos(th), 0, np.sin(th)], [0, 1, 0], [-np.sin(th), 0, np.cos(th)]])
+    cam = ro.Camera(R, -R @ x.mean(0) + np.array([0.0, 0.0, 1.5]), 2.0, 2.0, 40, 40, 1e-7)
+    assert np.array_equal(ro.hard_silhouette(x, f, cam), ro.hard_silhouette(x, all_faces, cam))
+    assert 0.1 < ro.hard_silhouette(x, f, cam).mean() < 0.9
