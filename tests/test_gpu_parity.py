@@ -780,3 +780,35 @@ def test_deterministic_mode_is_bitwise_reproducible(config):
     m.set_deterministic(True)
     gpu_run_scene(sc, ref["target"], model=m)
     assert L.gs_launch_count() - n1 > n1 - n0  # one element launch per colour class and substep
+
+
+def test_gradient_descent_on_the_gradients_lowers_the_system_identification_loss():
+    """What the gradients are for (guess -> unroll -> compare -> update): config 3 (small) starts from its guess
+    parameters; six steps of sign-scaled multiplicative descent on per-tet mu, lambda and the per-particle masses, each from one
+    rollout + backward of the CUDA path through its own loss call, must lower every environment's centroid-trajectory loss
+    against the truth trajectory -- a wrong sign or a gradient of the wrong parameter would raise it."""
+    sc = scenes.make_scene(3, small=True)
+    tgt = dev(orc.truth_targets(sc))
+    m = gs.Model(sc)
+    tape = m.tape(sc.n_substeps)
+    s, E, N = sc.frame_stride, sc.n_envs, sc.n_particles
+    n_t = sc.n_substeps // s
+    p = {g: dev(getattr(sc, a)).clone() for g, a in (("tet_mu", "tet_mu"), ("tet_lambda", "tet_lambda"), ("mass", "mass"))}
+    assert tuple(tgt.shape) == (n_t, E, 3) and N > 0
+    losses = []
+    for it in range(7):
+        m.zero_grads()
+        tape.rollout(dev(sc.x0), dev(sc.v0))
+        loss, cot = tape.loss_centroid_traj(s, tgt.float())
+        losses.append(host(loss).copy())
+        tape.backward(adj_x_frames=cot, frame_stride=s)
+        assert m.check_finite() == -1
+        for g in p:
+            gr = m.param_grads(g)
+            step = gr * p[g]  # dL/dlog p
+            p[g] = p[g] * torch.exp(-0.03 * step / step.abs().amax(dim=1, keepdim=True).clamp_min(1e-30))
+            m.set_params(g, p[g].contiguous())
+    losses = np.stack(losses)
+    assert (losses[0] > 0).all()
+    assert (losses[-1] < 0.9 * losses[0]).all(), losses
+    assert (np.diff(losses, axis=0) < 0).mean() >= 0.8  # nearly monotone: the steps are small
