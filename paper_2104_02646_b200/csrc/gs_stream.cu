@@ -875,6 +875,14 @@ static inline int grid_for(size_t n, int block = 256) {
     return (int)(g < 1 ? 1 : (g > cap ? cap : g));
 }
 
+// particle kernels: at most ONE resident wave (8 CTAs of 256 threads per SM), the rest by the grid-stride loop -- a partial
+// second wave costs a whole wave's latency
+static inline int grid_particles(size_t n) {
+    size_t g = (n + 255) / 256;
+    const size_t cap = 148 * 8;  // measured on config 4 (476 k particles): caps of 4, 6, 12, 16 per SM are 0.1-0.4 ms per step slower
+    return (int)(g < 1 ? 1 : (g > cap ? cap : g));
+}
+
 // launch with programmatic stream serialization (see grid_dep_wait)
 template <class... KArgs, class... Args>
 static cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
@@ -978,7 +986,7 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
         auto kern = act ? (me ? k_elements_fwd<true, true> : k_elements_fwd<true, false>) : (me ? k_elements_fwd<false, true> : k_elements_fwd<false, false>);
         GS_TIMED(m, GS_K_ELEMENTS_FWD, st, "k_elements_fwd", launch_pdl(m->pdl, kern, tile_grid(m, m->occ_fwd), kTileElems, m->smem_fwd, st, m->dev, ad, x, v, m->d_f));
     }
-    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, bad_idx));
+    GS_TIMED(m, GS_K_PARTICLES_FWD, st, "k_particles_fwd", launch_pdl(m->pdl, k_particles_fwd, grid_particles((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, m->d_f, xo, vo, bad_idx));
     return GS_OK;
 }
 
@@ -987,7 +995,7 @@ int stream_step_forward(gs_model *m, const float4 *x, const float4 *v, float4 *x
 int stream_step_adjoint(gs_model *m, const float4 *x, const float4 *v, const float4 *v_next, long long frame_off, int substep, cudaStream_t st) {
     const ActDev ad = m->act_for(substep < 0 ? m->act_cur * m->act_stride : substep);
     GS_TIMED(m, GS_K_PARTICLES_ADJ, st, "k_particles_adj",
-             launch_pdl(m->pdl, k_particles_adj, grid_for((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
+             launch_pdl(m->pdl, k_particles_adj, grid_particles((size_t)m->E * m->N), 256, 0, st, m->dev, x, v, v_next, frame_off, m->d_adjx, m->d_adjv, m->d_adjf));
     if (m->elem_items > 0 && m->det) {
         auto kern = m->E > 1 ? k_elements_adj<true, true> : k_elements_adj<true, false>;
         for (int c = 0; c < m->det_colours; c++) {
